@@ -1,0 +1,228 @@
+/*
+ * srp_oracle_trace.c -- TEST INFRASTRUCTURE ONLY.  CPU oracle, part 2 of 2:
+ * the forward photon tracer for the solar-radiation-pressure force
+ *     F(omega, theta) = int_M f(x, omega, theta) dx            (Eq. 3)
+ * with the light-to-force map l2f = L <n,w_in>+ (-w_in - w_out f_r) / c
+ * (Eq. 2), estimated by Monte-Carlo path tracing with BRDF
+ * importance sampling, next-event estimation and multiple bounces
+ * (PAPER.md:146-159), every ray tested against ALL triangles.
+ *
+ * Forward form (R1-R16): a parallel photon bundle of
+ * pressure P = L/c leaves an emitter rectangle perpendicular to the sun
+ * direction; momentum is deposited at every hit.  The steps below are numbered
+ * as in DESIGN.md "O-steps".  fp64, single thread, no acceleration structure,
+ * no blocking or reordering.  Only the facet-material lobe thresholds are
+ * taken in fp32 (they decide an integer: which lobe) -- DESIGN.md R17.
+ *
+ * Pins (tests/test_oracle_*.py): Philox KAT, flat plate, convex polyhedron,
+ * cannonball limit, occlusion, V-groove, perpendicular-plate form factor,
+ * conservation, symmetries, N^-1/2 decay, estimator agreement.
+ */
+#include <stdlib.h>
+#include <string.h>
+#include "srp_oracle_common.h"
+
+typedef struct {
+    unsigned long long launched, primary_miss, absorbed, escaped, capped, segments;
+    unsigned long long hits_at_depth[16];
+} orc_stats;
+
+typedef struct {
+    double solar_pressure;   /* P, N/m^2 */
+    int sampler;             /* 0 stratified-jittered Morton grid, 1 i.i.d. */
+    int deposit;             /* 0 expected-value, 1 analog */
+} orc_options;
+
+/* O-step 4: closest hit over ALL triangles with index != src.
+ * Moller-Trumbore on (v0, e1, e2); accept det != 0, u >= 0, v >= 0, u+v <= 1,
+ * t > 0; smallest t wins, ties -> smallest index (strict <). */
+static long closest_hit(const double *v0, const double *e1, const double *e2, long T,
+                        orc_v3 o, orc_v3 d, long src, double *t_out)
+{
+    long best = -1; double tbest = INFINITY;
+    for (long f = 0; f < T; ++f) {
+        if (f == src) continue;
+        orc_v3 E1 = orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]);
+        orc_v3 E2 = orc_mk(e2[3 * f], e2[3 * f + 1], e2[3 * f + 2]);
+        orc_v3 pv = orc_cross(d, E2);
+        double det = orc_dot(E1, pv);
+        if (det == 0.0) continue;
+        double inv = 1.0 / det;
+        orc_v3 tv = orc_sub(o, orc_mk(v0[3 * f], v0[3 * f + 1], v0[3 * f + 2]));
+        double u = orc_dot(tv, pv) * inv;
+        if (!(u >= 0.0)) continue;
+        orc_v3 qv = orc_cross(tv, E1);
+        double v = orc_dot(d, qv) * inv;
+        if (!(v >= 0.0) || !(u + v <= 1.0)) continue;
+        double t = orc_dot(E2, qv) * inv;
+        if (!(t > 0.0)) continue;
+        if (t < tbest) { tbest = t; best = f; }
+    }
+    *t_out = tbest;
+    return best;
+}
+
+static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
+{
+    uint32_t x = 0, y = 0;
+    for (int b = 0; b < 32; ++b) {
+        x |= (uint32_t)((i >> (2 * b)) & 1u) << b;
+        y |= (uint32_t)((i >> (2 * b + 1)) & 1u) << b;
+    }
+    *cx = x; *cy = y;
+}
+
+/*
+ * Forces of ONE design (index k in its batch -- k enters the Philox counter)
+ * for S sun directions.
+ *   verts float[T][3][3], mats float[T][3] = (alpha, rho_s, rho_d)
+ *   sun_dirs float[S][3]: body -> sun (the paper's omega); any length > 0
+ *   j0: global direction index of sun_dirs[0] (enters the Philox counter), so a
+ *       caller can split the directions of a pair list over processes
+ *   F double[S][3] newtons; sumsq double[S][3] = sum over photons of the squared
+ *       per-photon momentum total (for the MC standard error), may be NULL
+ *   stats accumulated over all S (zeroed here), may be NULL
+ *   first_hit int32[S][N] primary-hit triangle (-1 miss), may be NULL
+ * Returns 0, or -1 on invalid arguments.
+ */
+int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
+                      const float *sun_dirs, int S, int j0, long long N, int B,
+                      unsigned long long seed, const orc_options *opt,
+                      double *F, double *sumsq, orc_stats *stats, int *first_hit)
+{
+    if (!verts || !mats || !sun_dirs || !F || !opt || T <= 0 || S <= 0 || N <= 0 || B < 0 || B > 15)
+        return -1;
+    int m = 0;
+    if (opt->sampler == 0) {
+        while ((1LL << m) < N) ++m;
+        if ((1LL << m) != N) return -1;          /* stratified grid needs N = 2^m */
+    }
+    const double nx = (double)(1LL << ((m + 1) / 2)), ny = (double)(1LL << (m / 2));
+    const double P = opt->solar_pressure;
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+
+    double *v0 = malloc(sizeof(double) * 3 * T), *e1 = malloc(sizeof(double) * 3 * T),
+           *e2 = malloc(sizeof(double) * 3 * T), *nrm = malloc(sizeof(double) * 3 * T);
+    double lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
+    for (long f = 0; f < T; ++f) {
+        for (int c = 0; c < 3; ++c) {
+            double a = verts[9 * f + c], b = verts[9 * f + 3 + c], cc = verts[9 * f + 6 + c];
+            v0[3 * f + c] = a; e1[3 * f + c] = b - a; e2[3 * f + c] = cc - a;
+            double mn = fmin(a, fmin(b, cc)), mx = fmax(a, fmax(b, cc));
+            if (mn < lo[c]) lo[c] = mn;
+            if (mx > hi[c]) hi[c] = mx;
+        }
+        orc_v3 n = orc_cross(orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]),
+                             orc_mk(e2[3 * f], e2[3 * f + 1], e2[3 * f + 2]));
+        double len = sqrt(orc_dot(n, n));
+        nrm[3 * f] = n.x / len; nrm[3 * f + 1] = n.y / len; nrm[3 * f + 2] = n.z / len;
+    }
+    orc_stats st; memset(&st, 0, sizeof st);
+
+    for (int jj = 0; jj < S; ++jj) {
+        const uint32_t j = (uint32_t)(j0 + jj);
+        /* O-step 1: photon travel direction s = -normalize(omega), basis (u, v). */
+        orc_v3 om = orc_mk(sun_dirs[3 * jj], sun_dirs[3 * jj + 1], sun_dirs[3 * jj + 2]);
+        orc_v3 s = orc_scale(orc_normalize(om), -1.0), bu, bv;
+        orc_basis(s, &bu, &bv);
+        /* O-step 2: emitter rectangle = projected AABB corners; photon weight. */
+        double u0 = INFINITY, u1 = -INFINITY, vv0 = INFINITY, vv1 = -INFINITY, w0 = INFINITY;
+        for (int c = 0; c < 8; ++c) {
+            orc_v3 p = orc_mk((c & 1) ? hi[0] : lo[0], (c & 2) ? hi[1] : lo[1], (c & 4) ? hi[2] : lo[2]);
+            double pu = orc_dot(p, bu), pv = orc_dot(p, bv), pw = orc_dot(p, s);
+            u0 = fmin(u0, pu); u1 = fmax(u1, pu);
+            vv0 = fmin(vv0, pv); vv1 = fmax(vv1, pv);
+            w0 = fmin(w0, pw);
+        }
+        const double Ae = (u1 - u0) * (vv1 - vv0);
+        const double wph = P * Ae / (double)N;
+        double Fj[3] = { 0, 0, 0 }, Qj[3] = { 0, 0, 0 };
+
+        for (long long i = 0; i < N && Ae > 0.0; ++i) {
+            /* O-step 3: ray i. */
+            uint32_t ctr[4] = { (uint32_t)i, j, (uint32_t)k, 0u }, r[4];
+            orc_philox4x32_10(ctr, key, r);
+            double pu, pv;
+            if (opt->sampler == 0) {
+                uint32_t cx, cy;
+                deinterleave((uint64_t)i, &cx, &cy);
+                pu = u0 + ((double)cx + orc_u24(r[0])) / nx * (u1 - u0);
+                pv = vv0 + ((double)cy + orc_u24(r[1])) / ny * (vv1 - vv0);
+            } else {
+                pu = u0 + orc_u24(r[0]) * (u1 - u0);
+                pv = vv0 + orc_u24(r[1]) * (vv1 - vv0);
+            }
+            orc_v3 o = orc_add(orc_add(orc_scale(bu, pu), orc_scale(bv, pv)), orc_scale(s, w0 - 1.0));
+            orc_v3 d = s;
+            long src = -1;
+            int depth = 0;
+            double dp[3] = { 0, 0, 0 };
+            st.launched++;
+            for (;;) {
+                /* O-step 4 */
+                double t;
+                st.segments++;
+                long f = closest_hit(v0, e1, e2, T, o, d, src, &t);
+                if (depth == 0 && first_hit) first_hit[(long long)jj * N + i] = (int)f;
+                if (f < 0) {
+                    if (depth == 0) st.primary_miss++; else st.escaped++;
+                    break;
+                }
+                st.hits_at_depth[depth]++;
+                /* O-step 5: facing normal, mirror direction, deposit. */
+                orc_v3 n = orc_mk(nrm[3 * f], nrm[3 * f + 1], nrm[3 * f + 2]);
+                orc_v3 nf = (orc_dot(n, d) > 0.0) ? orc_scale(n, -1.0) : n;
+                double cost = -orc_dot(d, nf);
+                orc_v3 refl = orc_add(d, orc_scale(nf, 2.0 * cost));
+                orc_v3 x = orc_add(o, orc_scale(d, t));
+                const double al = mats[3 * f], rs = mats[3 * f + 1], rd = mats[3 * f + 2];
+                if (opt->deposit == 0) {
+                    double a = al + rs + rd;
+                    dp[0] += wph * (a * d.x - rs * refl.x - (2.0 / 3.0) * rd * nf.x);
+                    dp[1] += wph * (a * d.y - rs * refl.y - (2.0 / 3.0) * rd * nf.y);
+                    dp[2] += wph * (a * d.z - rs * refl.z - (2.0 / 3.0) * rd * nf.z);
+                }
+                /* O-step 6: lobe selection (thresholds in fp32, R17). */
+                uint32_t c2[4] = { (uint32_t)i, j, (uint32_t)k, (uint32_t)(depth + 1) }, y[4];
+                orc_philox4x32_10(c2, key, y);
+                const double z0 = orc_u24(y[0]), z1 = orc_u24(y[1]), z2 = orc_u24(y[2]);
+                const float th1 = mats[3 * f];
+                const float th2 = mats[3 * f] + mats[3 * f + 1];
+                orc_v3 dnew;
+                if (z0 < (double)th1) {
+                    if (opt->deposit == 1) { dp[0] += wph * d.x; dp[1] += wph * d.y; dp[2] += wph * d.z; }
+                    st.absorbed++;
+                    break;
+                } else if (z0 < (double)th2) {
+                    dnew = refl;
+                } else {
+                    double phi = 6.283185307179586476925286766559 * z1, rho = sqrt(z2);
+                    double lx = rho * cos(phi), ly = rho * sin(phi), lz = sqrt(1.0 - z2);
+                    orc_v3 tu, tv;
+                    orc_basis(nf, &tu, &tv);
+                    dnew = orc_add(orc_add(orc_scale(tu, lx), orc_scale(tv, ly)), orc_scale(nf, lz));
+                }
+                if (opt->deposit == 1) {
+                    dp[0] += wph * (d.x - dnew.x); dp[1] += wph * (d.y - dnew.y); dp[2] += wph * (d.z - dnew.z);
+                }
+                /* O-step 7: depth cap. */
+                if (depth == B) { st.capped++; break; }
+                o = x; d = dnew; src = f; depth += 1;
+            }
+            for (int c = 0; c < 3; ++c) { Fj[c] += dp[c]; Qj[c] += dp[c] * dp[c]; }
+        }
+        if (!(Ae > 0.0) && first_hit)
+            for (long long i = 0; i < N; ++i) first_hit[(long long)jj * N + i] = -1;
+        for (int c = 0; c < 3; ++c) { F[3 * jj + c] = Fj[c]; if (sumsq) sumsq[3 * jj + c] = Qj[c]; }
+    }
+    if (stats) *stats = st;
+    free(v0); free(e1); free(e2); free(nrm);
+    return 0;
+}
+
+/* Philox and the uniform map exposed for the known-answer tests. */
+void srp_oracle_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    orc_philox4x32_10(ctr, key, out);
+}
+double srp_oracle_u24(uint32_t x) { return orc_u24(x); }
