@@ -1,0 +1,155 @@
+/*
+ * srp.h -- C ABI of libsrp_b200: batched Monte-Carlo solar-radiation-pressure (SRP) forces
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * The library computes, for every (design k, sun direction j) pair, the force
+ *     F(omega_j, theta_k) = int_{M(theta_k)} f(x, omega_j, theta_k) dx      PAPER.md:131 (Eq. 3)
+ * with f given by the light-to-force map of PAPER.md:125 (Eq. 2), by forward Monte-Carlo photon
+ * tracing with multiple bounces (Sec. 3.2 "Estimation"), the reading of the paper
+ * written out in DESIGN.md ("O-steps", R1-R17).  "takes design parameters and the light direction,
+ * returns 3-D force": srp_build_designs is the "design parameters -> triangle mesh
+ * with per-face material" map of PAPER.md:148 plus a per-design LBVH (Karras-style linear BVH, the
+ * structure the paper builds for its Fig. 8); srp_forces is the estimator.
+ *
+ * Conventions
+ *  - Every function returns srp_status; outputs are untouched unless SRP_OK.  No exceptions cross
+ *    the boundary.  srp_last_error(ctx) gives the text of the last failure of that context.
+ *  - Pointers marked DEVICE are CUDA device pointers on the context's device (e.g. a torch tensor's
+ *    data_ptr()); pointers marked HOST are ordinary host memory.  The caller owns every buffer it
+ *    passes; the library owns the opaque handles and an internal workspace (cudaMalloc'ed lazily).
+ *  - srp_build_designs* and srp_forces only ENQUEUE work on the context's stream; the caller
+ *    synchronises that stream.  Functions documented "syncs" wait for the stream.
+ *  - Same inputs + same seed => bit-identical output (integer fixed-point accumulation).
+ *  - One context per host thread.  No CPU fallback exists: without a CUDA device every call fails.
+ */
+#ifndef SRP_B200_H
+#define SRP_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct srp_context srp_context;   /* opaque: device, stream, options, workspace, last error */
+typedef struct srp_designs srp_designs;   /* opaque: device meshes + BVHs of D designs              */
+
+typedef enum {
+    SRP_OK = 0,
+    SRP_ERR_INVALID = -1,       /* bad argument, detected on the host before any launch */
+    SRP_ERR_CUDA = -2,          /* a CUDA runtime call failed; text in srp_last_error    */
+    SRP_ERR_OOM = -3,           /* device allocation failed                              */
+    SRP_ERR_UNSUPPORTED = -4
+} srp_status;
+
+/* Mesh families (BASELINE.json configs 1-5).  theta layout per family:
+ *   PLATE    n_params 3: (alpha, rho_s, rho_d) of the 1 m x 1 m plate            T = 2
+ *   BOXWING  n_params 2: (panel length L [m], panel angle phi [rad])             T = 16
+ *   DETAILED n_params 2: (dish tilt theta_dish, panel angle phi_pan) [rad]       T = 49840
+ *   BOXWING6 n_params 6: (phi1, phi2, L, bus aspect a, rho_s panel, rho_d bus)   T = 16
+ *   SAIL     n_params 1: (height-field amplitude [m], 0.05 in config 5)          T = 1019698 */
+typedef enum {
+    SRP_FAMILY_PLATE = 0,
+    SRP_FAMILY_BOXWING = 1,
+    SRP_FAMILY_DETAILED = 2,
+    SRP_FAMILY_BOXWING6 = 3,
+    SRP_FAMILY_SAIL = 4
+} srp_family;
+
+typedef struct {
+    double solar_pressure;  /* P = L/c of Eq. 2 [N/m^2]; default 4.56e-6 (1 AU)                    */
+    int sampler;            /* 0 = stratified jittered grid in Morton order (default),
+                               1 = i.i.d. uniform over the emitter rectangle                        */
+    int deposit;            /* 0 = expected-value deposit (default), 1 = analog (sampled path only) */
+    int force_brute;        /* 1 = ignore the BVH and test every triangle; test use   */
+} srp_options;
+
+/* Photon bookkeeping of the last srp_forces call (DESIGN.md "Pins" P8).
+ * launched = primary_miss + absorbed + escaped + capped; segments = every ray cast.
+ * box_tests / tri_tests are filled only by the instrumented kernels (srp_forces_instrumented). */
+typedef struct {
+    unsigned long long launched, primary_miss, absorbed, escaped, capped, segments;
+    unsigned long long hits_at_depth[16];
+    unsigned long long box_tests, tri_tests;
+} srp_stats;
+
+/* Creates a context on CUDA device `cuda_device`; `cuda_stream` is a cudaStream_t (may be NULL =
+ * the legacy default stream) that all work of this context is enqueued on. */
+srp_status srp_create(srp_context **ctx, int cuda_device, void *cuda_stream);
+srp_status srp_destroy(srp_context *ctx);                       /* syncs; frees the workspace */
+srp_status srp_set_options(srp_context *ctx, const srp_options *opt);
+srp_status srp_get_options(const srp_context *ctx, srp_options *opt);
+const char *srp_last_error(const srp_context *ctx);
+
+/* Number of parameters / triangles of a family (host-side constants; -1 for an unknown family). */
+int srp_family_n_params(srp_family family);
+long long srp_family_tri_count(srp_family family);
+
+/* S0 + S1: theta DEVICE float[D, n_params] row-major -> meshes (fp64 evaluation rounded once to fp32)
+ * and per-design LBVHs.  mesh_seed keys the per-facet Dirichlet(2,2,2) material draws and the sail's
+ * noise.  n_params must equal srp_family_n_params(family).  Enqueues only. */
+srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *theta, int D,
+                             int n_params, unsigned long long mesh_seed, srp_designs **out);
+
+/* User-supplied meshes (the paper's general design->mesh map):
+ * verts DEVICE float[sumT,3,3] (v0,v1,v2), mats DEVICE float[sumT,3] = (alpha, rho_s, rho_d),
+ * tri_offsets HOST long long[D+1], tri_offsets[0] = 0, strictly increasing.  Enqueues only. */
+srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, const float *mats,
+                                         const long long *tri_offsets, int D, srp_designs **out);
+
+/* D and the triangle offsets (HOST long long[D+1], may be NULL). */
+srp_status srp_designs_info(const srp_designs *designs, int *D, long long *tri_offsets_host);
+
+/* Reads back design `design`'s mesh in ORIGINAL triangle order: verts_host HOST float[T,3,3],
+ * mats_host HOST float[T,3].  Either may be NULL.  Syncs; test use. */
+srp_status srp_designs_read_mesh(srp_context *ctx, const srp_designs *designs, int design,
+                                 float *verts_host, float *mats_host);
+
+/* Reads back design `design`'s BVH for structural tests.  Syncs.
+ *   n_nodes out: number of node records (0 if the design has no hierarchy -- brute-force leaf).
+ *   nodes_host HOST float[n_nodes,16] (may be NULL): per node
+ *     [0..5] child-0 box (lo xyz, hi xyz), [6..11] child-1 box, [12],[13] child links as int bits,
+ *     [14],[15] unused.  A link >= 0 is a node index; a link < 0 encodes a leaf: u = ~link,
+ *     first = u >> 3 (sorted triangle index within the design), count = (u & 7) + 1.
+ *   perm_host HOST int[T] (may be NULL): sorted position -> original triangle index. */
+srp_status srp_designs_read_bvh(srp_context *ctx, const srp_designs *designs, int design,
+                                long long *n_nodes, float *nodes_host, int *perm_host);
+
+srp_status srp_free_designs(srp_context *ctx, srp_designs *designs);   /* syncs */
+
+/* S2-S7: sun_dirs DEVICE float[S,3], body->sun (the paper's omega), any non-zero
+ * length; rays_per_dir N > 0 (a power of two when sampler = 0); 0 <= max_bounces <= 15 reflections
+ * followed (R5); seed keys Philox4x32-10 with counter (ray, direction, design, depth).
+ * out_forces DEVICE float[D,S,3], newtons, body frame.  Enqueues only. */
+srp_status srp_forces(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                      long long rays_per_dir, int max_bounces, unsigned long long seed,
+                      float *out_forces);
+
+/* Same, restricted to an explicit list of pairs: pairs DEVICE int[n_pairs,2] = (design k,
+ * direction j); out_forces DEVICE float[n_pairs,3].  The Philox counters use (k, j), so the result
+ * of a pair equals the corresponding entry of the full srp_forces call bit for bit. */
+srp_status srp_forces_pairs(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                            const int *pairs, long long n_pairs, long long rays_per_dir,
+                            int max_bounces, unsigned long long seed, float *out_forces);
+
+/* Host-buffer convenience (the end-to-end call): theta-independent; sun_dirs_host HOST float[S,3],
+ * out_forces_host HOST float[D,S,3].  Copies in, runs srp_forces, copies out, syncs. */
+srp_status srp_forces_host(srp_context *ctx, const srp_designs *designs, const float *sun_dirs_host,
+                           int S, long long rays_per_dir, int max_bounces, unsigned long long seed,
+                           float *out_forces_host);
+
+/* Debug: primary-hit triangle (ORIGINAL index, -1 = miss) of every ray of the listed pairs:
+ * out_prim DEVICE int[n_pairs, rays_per_dir].  method 0 = BVH traversal, 1 = brute force. */
+srp_status srp_first_hits(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                          const int *pairs, long long n_pairs, long long rays_per_dir,
+                          unsigned long long seed, int method, int *out_prim);
+
+/* Counters of the last srp_forces* call on this context.  Syncs. */
+srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out);
+
+/* Micro-benchmarks for the roofline denominators: register-resident FP32
+ * FMA chains, and an L2-resident 16-byte-load sweep.  Syncs; results in TFLOP/s and GB/s. */
+srp_status srp_probe_peaks(srp_context *ctx, double *fp32_tflops, double *l2_read_gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SRP_B200_H */

@@ -75,8 +75,8 @@ def lib():
             ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats), ctypes.c_void_p]
         L.srp_oracle_philox.restype = None
         L.srp_oracle_philox.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
-        L.srp_oracle_u24.restype = ctypes.c_double
-        L.srp_oracle_u24.argtypes = [ctypes.c_uint32]
+        L.srp_oracle_uniform.restype = ctypes.c_double
+        L.srp_oracle_uniform.argtypes = [ctypes.c_uint32]
         _lib = L
     return _lib
 
@@ -89,8 +89,8 @@ def philox(ctr, key):
     return out
 
 
-def u24(x):
-    return lib().srp_oracle_u24(int(x) & 0xFFFFFFFF)
+def uniform(x):
+    return lib().srp_oracle_uniform(int(x) & 0xFFFFFFFF)
 
 
 def n_params(family):

@@ -6,7 +6,7 @@
  * this file includes nothing from there: the oracle and the CUDA path share no
  * code.  Plain C99, fp64, single-threaded.
  *
- * Contents: Philox4x32-10 (counter-based RNG), the 24-bit
+ * Contents: Philox4x32-10 (counter-based RNG), the 23-bit
  * uniform mapping (reading R4), small fp64 vector helpers and the branch-free
  * orthonormal basis (O-step 1; Duff et al. 2017 "Building an orthonormal
  * basis, revisited").
@@ -41,11 +41,12 @@ static inline void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* Reading R4: xi = ((x >> 8) + 0.5) * 2^-24, strictly inside (0,1), exact in
- * fp32 and fp64 alike. */
-static inline double orc_u24(uint32_t x)
+/* Reading R4: xi = ((x >> 9) + 0.5) * 2^-23 = (2m+1) * 2^-24 with m < 2^23:
+ * strictly inside (0,1) and an odd 24-bit integer times 2^-24, hence exactly
+ * representable in fp32 and fp64 alike (a 24-bit m would need 25 bits). */
+static inline double orc_uniform(uint32_t x)
 {
-    return ((double)(x >> 8) + 0.5) * (1.0 / 16777216.0);
+    return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0);
 }
 
 typedef struct { double x, y, z; } orc_v3;

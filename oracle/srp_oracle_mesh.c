@@ -197,7 +197,7 @@ static double lattice_angle(int ix, int iy, int oct, uint64_t mesh_seed)
     uint32_t ctr[4] = { (uint32_t)ix, (uint32_t)iy, (uint32_t)oct, 0xC0u };
     uint32_t key[2] = { (uint32_t)mesh_seed, (uint32_t)(mesh_seed >> 32) }, r[4];
     orc_philox4x32_10(ctr, key, r);
-    return ORC_TWO_PI * orc_u24(r[0]);
+    return ORC_TWO_PI * orc_uniform(r[0]);
 }
 static double fade5(double t) { return t * t * t * (t * (t * 6.0 - 15.0) + 10.0); }
 static double corner_dot(int ix, int iy, int oct, uint64_t seed, double dx, double dy)
@@ -296,9 +296,9 @@ static void dirichlet222(long f, int k, uint64_t mesh_seed, double m[3])
     uint32_t r0[4], r1[4];
     orc_philox4x32_10(c0, key, r0);
     orc_philox4x32_10(c1, key, r1);
-    double g0 = -log(orc_u24(r0[0]) * orc_u24(r0[1]));
-    double g1 = -log(orc_u24(r0[2]) * orc_u24(r0[3]));
-    double g2 = -log(orc_u24(r1[0]) * orc_u24(r1[1]));
+    double g0 = -log(orc_uniform(r0[0]) * orc_uniform(r0[1]));
+    double g1 = -log(orc_uniform(r0[2]) * orc_uniform(r0[3]));
+    double g2 = -log(orc_uniform(r1[0]) * orc_uniform(r1[1]));
     double s = g0 + g1 + g2;
     m[0] = g0 / s; m[1] = g1 / s; m[2] = g2 / s;
 }

@@ -146,11 +146,11 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
             if (opt->sampler == 0) {
                 uint32_t cx, cy;
                 deinterleave((uint64_t)i, &cx, &cy);
-                pu = u0 + ((double)cx + orc_u24(r[0])) / nx * (u1 - u0);
-                pv = vv0 + ((double)cy + orc_u24(r[1])) / ny * (vv1 - vv0);
+                pu = u0 + ((double)cx + orc_uniform(r[0])) / nx * (u1 - u0);
+                pv = vv0 + ((double)cy + orc_uniform(r[1])) / ny * (vv1 - vv0);
             } else {
-                pu = u0 + orc_u24(r[0]) * (u1 - u0);
-                pv = vv0 + orc_u24(r[1]) * (vv1 - vv0);
+                pu = u0 + orc_uniform(r[0]) * (u1 - u0);
+                pv = vv0 + orc_uniform(r[1]) * (vv1 - vv0);
             }
             orc_v3 o = orc_add(orc_add(orc_scale(bu, pu), orc_scale(bv, pv)), orc_scale(s, w0 - 1.0));
             orc_v3 d = s;
@@ -185,7 +185,7 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                 /* O-step 6: lobe selection (thresholds in fp32, R17). */
                 uint32_t c2[4] = { (uint32_t)i, j, (uint32_t)k, (uint32_t)(depth + 1) }, y[4];
                 orc_philox4x32_10(c2, key, y);
-                const double z0 = orc_u24(y[0]), z1 = orc_u24(y[1]), z2 = orc_u24(y[2]);
+                const double z0 = orc_uniform(y[0]), z1 = orc_uniform(y[1]), z2 = orc_uniform(y[2]);
                 const float th1 = mats[3 * f];
                 const float th2 = mats[3 * f] + mats[3 * f + 1];
                 orc_v3 dnew;
@@ -225,4 +225,4 @@ void srp_oracle_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 {
     orc_philox4x32_10(ctr, key, out);
 }
-double srp_oracle_u24(uint32_t x) { return orc_u24(x); }
+double srp_oracle_uniform(uint32_t x) { return orc_uniform(x); }

@@ -1,0 +1,103 @@
+// srp_internal.cuh -- shared declarations of libsrp_b200's translation units (CUDA path only;
+// nothing under oracle/ includes this file).  See include/srp.h for the public C ABI and
+// DESIGN.md for the data layout.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "srp.h"
+
+#define SRP_BRUTE_MAX_TRIS 64      // designs with T <= this are traced without a hierarchy (one leaf)
+#define SRP_LEAF_MAX 4             // LBVH subtrees with <= this many triangles become one leaf
+#define SRP_ACC_SCALE 4294967296.0 // fixed-point scale (2^32) of the dimensionless force accumulators
+
+// Packed, BVH-sorted triangle: 3 x float4 = 48 B, fetched as three 16-byte loads.
+//   q0 = (v0.x, v0.y, v0.z, alpha)   q1 = (e1.x, e1.y, e1.z, rho_s)   q2 = (e2.x, e2.y, e2.z, rho_d)
+// BVH2 node: 4 x float4 = 64 B.
+//   q0 = (lo0.x, lo0.y, lo0.z, hi0.x)  q1 = (hi0.y, hi0.z, lo1.x, lo1.y)
+//   q2 = (lo1.z, hi1.x, hi1.y, hi1.z)  q3 = (link0, link1, -, -) as int bits
+// link >= 0: node index (relative to the design's node base); link < 0: leaf, u = ~link,
+// first = u >> 3 (sorted triangle index relative to the design's triangle base), count = (u & 7) + 1.
+struct DesignsDev {
+    const float4 *tri;        // [sumT * 3]
+    const float4 *nodes;      // [sumT * 4]; node base of design k == tri_off[k]
+    const long long *tri_off; // [D + 1]
+    const float4 *box;        // [D * 2]: (lo, -), (hi, -)
+    const int *perm;          // [sumT]: sorted position -> original index within the design
+    int D;
+    int has_bvh;
+};
+
+struct srp_designs {
+    int D = 0;
+    int family = -1;
+    long long sumT = 0, maxT = 0;
+    std::vector<long long> tri_off;     // host copy [D+1]
+    float *verts_orig = nullptr;        // [sumT*9] original order (device)
+    float *mats_orig = nullptr;         // [sumT*3]
+    float4 *tri = nullptr;
+    float4 *nodes = nullptr;
+    long long *tri_off_dev = nullptr;
+    float4 *box = nullptr;
+    int *perm = nullptr;
+    bool has_bvh = false;
+    DesignsDev dev() const {
+        DesignsDev d;
+        d.tri = tri; d.nodes = nodes; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.D = D;
+        d.has_bvh = has_bvh ? 1 : 0;
+        return d;
+    }
+};
+
+struct DevStats {           // device mirror of srp_stats
+    unsigned long long launched, primary_miss, absorbed, escaped, capped, segments;
+    unsigned long long hits_at_depth[16];
+    unsigned long long box_tests, tri_tests;
+};
+
+struct srp_context {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    srp_options opt;
+    std::string last_error;
+    int num_sms = 148;
+    // workspace (grown on demand, never shrunk)
+    long long *accum = nullptr;   size_t accum_items = 0;     // int64 fixed-point [pairs*3]
+    DevStats *stats = nullptr;
+    unsigned long long *work_counter = nullptr;
+    float *stage_dirs = nullptr;  size_t stage_dirs_items = 0; // srp_forces_host staging
+    float *stage_out = nullptr;   size_t stage_out_items = 0;
+};
+
+struct TraceArgs {
+    DesignsDev dz;
+    const float *sun_dirs;   // [S,3]
+    const int *pairs;        // [n_pairs,2] or nullptr (then pair p = (p / S, p % S))
+    long long n_pairs;
+    int S;
+    long long N;             // rays per direction
+    int log2N;               // valid when sampler == 0
+    int B;
+    uint32_t key0, key1;
+    int sampler, deposit;
+    double P;
+    long long *accum;        // [n_pairs*3]
+    DevStats *stats;
+    unsigned long long *work_counter;
+    long long tiles_per_pair;
+    int tile_rays;
+};
+
+// ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----
+cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_params,
+                                unsigned long long mesh_seed, long long T, float *verts, float *mats,
+                                cudaStream_t stream);
+cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream);
+cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms,
+                             cudaStream_t stream);
+cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, cudaStream_t stream);
+cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream);
+cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
+
+long long srp_family_tris_host(int family);

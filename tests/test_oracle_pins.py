@@ -21,12 +21,13 @@ def test_p1_philox_known_answers(oracle):
 
 
 def test_p1_uniform_map_is_exact_and_open(oracle):
-    assert oracle.u24(0) == 0.5 / 2 ** 24
-    assert oracle.u24(0xFFFFFFFF) == 1.0 - 0.5 / 2 ** 24
-    assert oracle.u24(0x000000FF) == oracle.u24(0)               # low 8 bits dropped
-    for x in (0x12345678, 0x80000000, 0xDEADBEEF):
-        u = oracle.u24(x)
-        assert np.float32(u) == u                                 # exact in fp32
+    assert oracle.uniform(0) == 0.5 / 2 ** 23
+    assert oracle.uniform(0xFFFFFFFF) == 1.0 - 0.5 / 2 ** 23
+    assert oracle.uniform(0x000001FF) == oracle.uniform(0)       # low 9 bits dropped
+    for x in (0x12345678, 0x80000000, 0xDEADBEEF, 0xFFFFFFFF, 0x7FFFFE00):
+        u = oracle.uniform(x)
+        assert float(np.float32(u)) == u                          # exact in fp32 (R4)
+        assert u == ((x >> 9) + 0.5) / 2 ** 23
 
 
 @pytest.mark.parametrize("sampler", [0, 1])
