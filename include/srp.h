@@ -60,11 +60,12 @@ typedef struct {
                                1 = i.i.d. uniform over the emitter rectangle                        */
     int deposit;            /* 0 = expected-value deposit (default), 1 = analog (sampled path only) */
     int force_brute;        /* 1 = ignore the BVH and test every triangle; test use   */
+    int instrumented;       /* 1 = also count ray-box and ray-triangle tests (slower kernels)        */
 } srp_options;
 
 /* Photon bookkeeping of the last srp_forces call (DESIGN.md "Pins" P8).
  * launched = primary_miss + absorbed + escaped + capped; segments = every ray cast.
- * box_tests / tri_tests are filled only by the instrumented kernels (srp_forces_instrumented). */
+ * box_tests / tri_tests are filled only when srp_options.instrumented = 1. */
 typedef struct {
     unsigned long long launched, primary_miss, absorbed, escaped, capped, segments;
     unsigned long long hits_at_depth[16];

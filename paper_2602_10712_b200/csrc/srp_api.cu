@@ -1,0 +1,370 @@
+// srp_api.cu -- the extern "C" boundary of libsrp_b200 (include/srp.h): argument validation,
+// handle ownership, workspace, and the enqueue order of the kernels in mesh_gen.cu / lbvh.cu /
+// trace.cu.  No arithmetic of the method lives here.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "srp_internal.cuh"
+
+namespace {
+
+srp_status fail(srp_context *ctx, srp_status st, const char *what, cudaError_t e = cudaSuccess)
+{
+    if (ctx) {
+        ctx->last_error = what;
+        if (e != cudaSuccess) { ctx->last_error += ": "; ctx->last_error += cudaGetErrorString(e); }
+    }
+    return st;
+}
+
+srp_status cuda_fail(srp_context *ctx, const char *what, cudaError_t e)
+{
+    return fail(ctx, e == cudaErrorMemoryAllocation ? SRP_ERR_OOM : SRP_ERR_CUDA, what, e);
+}
+
+#define TRY_CUDA(ctx, call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, what, e_); } while (0)
+
+void free_designs_mem(srp_designs *d)
+{
+    cudaFree(d->verts_orig); cudaFree(d->mats_orig); cudaFree(d->tri); cudaFree(d->nodes);
+    cudaFree(d->tri_off_dev); cudaFree(d->box); cudaFree(d->perm);
+}
+
+// allocates everything that depends on tri_off / sumT
+srp_status alloc_designs(srp_context *ctx, srp_designs *d)
+{
+    const long long sumT = d->sumT;
+    TRY_CUDA(ctx, cudaMalloc(&d->verts_orig, sizeof(float) * 9 * sumT), "alloc verts");
+    TRY_CUDA(ctx, cudaMalloc(&d->mats_orig, sizeof(float) * 3 * sumT), "alloc mats");
+    TRY_CUDA(ctx, cudaMalloc(&d->tri, sizeof(float4) * 3 * sumT), "alloc packed triangles");
+    if (d->has_bvh) TRY_CUDA(ctx, cudaMalloc(&d->nodes, sizeof(float4) * 4 * sumT), "alloc nodes");
+    TRY_CUDA(ctx, cudaMalloc(&d->tri_off_dev, sizeof(long long) * (d->D + 1)), "alloc offsets");
+    TRY_CUDA(ctx, cudaMalloc(&d->box, sizeof(float4) * 2 * d->D), "alloc boxes");
+    TRY_CUDA(ctx, cudaMalloc(&d->perm, sizeof(int) * sumT), "alloc perm");
+    TRY_CUDA(ctx, cudaMemcpyAsync(d->tri_off_dev, d->tri_off.data(), sizeof(long long) * (d->D + 1),
+                                  cudaMemcpyHostToDevice, ctx->stream), "copy offsets");
+    // the pageable host vector must outlive the async copy
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync offsets");
+    return SRP_OK;
+}
+
+srp_status ensure_workspace(srp_context *ctx, size_t accum_items)
+{
+    if (!ctx->stats) TRY_CUDA(ctx, cudaMalloc(&ctx->stats, sizeof(DevStats)), "alloc stats");
+    if (!ctx->work_counter) TRY_CUDA(ctx, cudaMalloc(&ctx->work_counter, sizeof(unsigned long long)), "alloc counter");
+    if (ctx->accum_items < accum_items) {
+        TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before workspace growth");
+        cudaFree(ctx->accum); ctx->accum = nullptr; ctx->accum_items = 0;
+        TRY_CUDA(ctx, cudaMalloc(&ctx->accum, sizeof(long long) * accum_items), "alloc accumulators");
+        ctx->accum_items = accum_items;
+    }
+    return SRP_OK;
+}
+
+srp_status check_trace_args(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S,
+                            long long N, int B, const void *out)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!dz || !sun_dirs || !out) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    if (S <= 0) return fail(ctx, SRP_ERR_INVALID, "S must be positive");
+    if (N <= 0 || N > (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "rays_per_dir must be in [1, 2^31]");
+    if (B < 0 || B > 15) return fail(ctx, SRP_ERR_INVALID, "max_bounces must be in [0, 15]");
+    if (ctx->opt.sampler == 0 && (N & (N - 1)) != 0)
+        return fail(ctx, SRP_ERR_INVALID, "stratified sampler needs rays_per_dir to be a power of two");
+    return SRP_OK;
+}
+
+TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
+                    long long n_pairs, long long N, int B, unsigned long long seed)
+{
+    TraceArgs a;
+    memset(&a, 0, sizeof a);
+    a.dz = dz->dev();
+    a.sun_dirs = sun_dirs; a.pairs = pairs; a.n_pairs = n_pairs; a.S = S; a.N = N; a.B = B;
+    a.log2N = 0;
+    while ((1LL << a.log2N) < N) ++a.log2N;
+    a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
+    a.sampler = ctx->opt.sampler; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
+    a.accum = ctx->accum; a.stats = ctx->stats; a.work_counter = ctx->work_counter;
+    // tile size: large tiles amortise the per-item set-up and the drain at the end of a tile; shrink
+    // them only when there would be too few items to occupy every resident warp several times
+    const bool brute = !dz->has_bvh;
+    const long long warps = (long long)ctx->num_sms * srp_trace_blocks_per_sm(brute);
+    long long tile = 8192;
+    if (tile > N) tile = N;
+    while (tile > 256 && n_pairs * ((N + tile - 1) / tile) < 8 * warps) tile >>= 1;
+    a.tile_rays = (int)tile;
+    a.tiles_per_pair = (N + tile - 1) / tile;
+    return a;
+}
+
+srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
+                      long long n_pairs, long long N, int B, unsigned long long seed, float *out)
+{
+    srp_status st = ensure_workspace(ctx, (size_t)n_pairs * 3);
+    if (st != SRP_OK) return st;
+    TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * n_pairs, ctx->stream), "zero accumulators");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
+    const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
+    TRY_CUDA(ctx, srp_launch_trace(a, brute, ctx->opt.instrumented != 0, ctx->num_sms, ctx->stream), "trace launch");
+    TRY_CUDA(ctx, srp_launch_finalize(a, out, ctx->stream), "finalize launch");
+    return SRP_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
+{
+    if (!out) return SRP_ERR_INVALID;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || cuda_device < 0 || cuda_device >= count)
+        return SRP_ERR_CUDA;                      // no device: there is no CPU fallback
+    if (cudaSetDevice(cuda_device) != cudaSuccess) return SRP_ERR_CUDA;
+    srp_context *ctx = new (std::nothrow) srp_context();
+    if (!ctx) return SRP_ERR_OOM;
+    ctx->device = cuda_device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->opt.solar_pressure = 4.56e-6; ctx->opt.sampler = 0; ctx->opt.deposit = 0;
+    ctx->opt.force_brute = 0; ctx->opt.instrumented = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
+    *out = ctx;
+    return SRP_OK;
+}
+
+srp_status srp_destroy(srp_context *ctx)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter);
+    cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);
+    delete ctx;
+    return SRP_OK;
+}
+
+srp_status srp_set_options(srp_context *ctx, const srp_options *opt)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!opt) return fail(ctx, SRP_ERR_INVALID, "null options");
+    if (!(opt->solar_pressure > 0.0) || opt->sampler < 0 || opt->sampler > 1 || opt->deposit < 0 || opt->deposit > 1)
+        return fail(ctx, SRP_ERR_INVALID, "option out of range");
+    ctx->opt = *opt;
+    return SRP_OK;
+}
+
+srp_status srp_get_options(const srp_context *ctx, srp_options *opt)
+{
+    if (!ctx || !opt) return SRP_ERR_INVALID;
+    *opt = ctx->opt;
+    return SRP_OK;
+}
+
+const char *srp_last_error(const srp_context *ctx) { return ctx ? ctx->last_error.c_str() : "null context"; }
+
+int srp_family_n_params(srp_family family)
+{
+    switch (family) {
+    case SRP_FAMILY_PLATE: return 3; case SRP_FAMILY_BOXWING: return 2; case SRP_FAMILY_DETAILED: return 2;
+    case SRP_FAMILY_BOXWING6: return 6; case SRP_FAMILY_SAIL: return 1; default: return -1;
+    }
+}
+
+long long srp_family_tri_count(srp_family family) { return srp_family_tris_host((int)family); }
+
+srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *theta, int D, int n_params,
+                             unsigned long long mesh_seed, srp_designs **out)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!out) return fail(ctx, SRP_ERR_INVALID, "null output handle");
+    *out = nullptr;
+    const long long T = srp_family_tris_host((int)family);
+    if (T < 0) return fail(ctx, SRP_ERR_INVALID, "unknown family");
+    if (!theta) return fail(ctx, SRP_ERR_INVALID, "null theta");
+    if (D <= 0 || D > 65535) return fail(ctx, SRP_ERR_INVALID, "D must be in [1, 65535]");
+    if (n_params != srp_family_n_params(family)) return fail(ctx, SRP_ERR_INVALID, "wrong n_params for this family");
+    if ((long long)D * T >= (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "too many triangles in one batch");
+    cudaSetDevice(ctx->device);
+    srp_designs *d = new (std::nothrow) srp_designs();
+    if (!d) return fail(ctx, SRP_ERR_OOM, "host allocation");
+    d->D = D; d->family = (int)family; d->sumT = (long long)D * T; d->maxT = T;
+    d->tri_off.resize(D + 1);
+    for (int k = 0; k <= D; ++k) d->tri_off[k] = (long long)k * T;
+    d->has_bvh = T > SRP_BRUTE_MAX_TRIS;
+    srp_status st = alloc_designs(ctx, d);
+    if (st != SRP_OK) { free_designs_mem(d); delete d; return st; }
+    cudaError_t e = srp_launch_mesh_gen((int)family, theta, D, n_params, mesh_seed, T, d->verts_orig,
+                                        d->mats_orig, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->stream);
+    if (e != cudaSuccess) { free_designs_mem(d); delete d; return cuda_fail(ctx, "design build", e); }
+    *out = d;
+    return SRP_OK;
+}
+
+srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, const float *mats,
+                                         const long long *tri_offsets, int D, srp_designs **out)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!out) return fail(ctx, SRP_ERR_INVALID, "null output handle");
+    *out = nullptr;
+    if (!verts || !mats || !tri_offsets) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    if (D <= 0 || D > 65535) return fail(ctx, SRP_ERR_INVALID, "D must be in [1, 65535]");
+    if (tri_offsets[0] != 0) return fail(ctx, SRP_ERR_INVALID, "tri_offsets[0] must be 0");
+    long long maxT = 0;
+    for (int k = 0; k < D; ++k) {
+        const long long t = tri_offsets[k + 1] - tri_offsets[k];
+        if (t <= 0) return fail(ctx, SRP_ERR_INVALID, "tri_offsets must be strictly increasing");
+        if (t >= (1LL << 28)) return fail(ctx, SRP_ERR_INVALID, "design too large");
+        if (t > maxT) maxT = t;
+    }
+    if (tri_offsets[D] >= (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "too many triangles in one batch");
+    cudaSetDevice(ctx->device);
+    srp_designs *d = new (std::nothrow) srp_designs();
+    if (!d) return fail(ctx, SRP_ERR_OOM, "host allocation");
+    d->D = D; d->family = -1; d->sumT = tri_offsets[D]; d->maxT = maxT;
+    d->tri_off.assign(tri_offsets, tri_offsets + D + 1);
+    d->has_bvh = maxT > SRP_BRUTE_MAX_TRIS;
+    srp_status st = alloc_designs(ctx, d);
+    if (st != SRP_OK) { free_designs_mem(d); delete d; return st; }
+    cudaError_t e = cudaMemcpyAsync(d->verts_orig, verts, sizeof(float) * 9 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(d->mats_orig, mats, sizeof(float) * 3 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->stream);
+    if (e != cudaSuccess) { free_designs_mem(d); delete d; return cuda_fail(ctx, "design build", e); }
+    *out = d;
+    return SRP_OK;
+}
+
+srp_status srp_designs_info(const srp_designs *dz, int *D, long long *tri_offsets_host)
+{
+    if (!dz) return SRP_ERR_INVALID;
+    if (D) *D = dz->D;
+    if (tri_offsets_host) memcpy(tri_offsets_host, dz->tri_off.data(), sizeof(long long) * (dz->D + 1));
+    return SRP_OK;
+}
+
+srp_status srp_designs_read_mesh(srp_context *ctx, const srp_designs *dz, int design, float *verts_host,
+                                 float *mats_host)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!dz || design < 0 || design >= dz->D) return fail(ctx, SRP_ERR_INVALID, "bad design index");
+    cudaSetDevice(ctx->device);
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
+    const long long b = dz->tri_off[design], T = dz->tri_off[design + 1] - b;
+    if (verts_host) TRY_CUDA(ctx, cudaMemcpy(verts_host, dz->verts_orig + 9 * b, sizeof(float) * 9 * T, cudaMemcpyDeviceToHost), "read verts");
+    if (mats_host) TRY_CUDA(ctx, cudaMemcpy(mats_host, dz->mats_orig + 3 * b, sizeof(float) * 3 * T, cudaMemcpyDeviceToHost), "read mats");
+    return SRP_OK;
+}
+
+srp_status srp_designs_read_bvh(srp_context *ctx, const srp_designs *dz, int design, long long *n_nodes,
+                                float *nodes_host, int *perm_host)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!dz || design < 0 || design >= dz->D) return fail(ctx, SRP_ERR_INVALID, "bad design index");
+    cudaSetDevice(ctx->device);
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
+    const long long b = dz->tri_off[design], T = dz->tri_off[design + 1] - b;
+    const long long nn = dz->has_bvh ? (T > 1 ? T - 1 : 1) : 0;
+    if (n_nodes) *n_nodes = nn;
+    if (nodes_host && nn > 0)
+        TRY_CUDA(ctx, cudaMemcpy(nodes_host, dz->nodes + 4 * b, sizeof(float4) * 4 * nn, cudaMemcpyDeviceToHost), "read nodes");
+    if (perm_host) TRY_CUDA(ctx, cudaMemcpy(perm_host, dz->perm + b, sizeof(int) * T, cudaMemcpyDeviceToHost), "read perm");
+    return SRP_OK;
+}
+
+srp_status srp_free_designs(srp_context *ctx, srp_designs *dz)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!dz) return SRP_OK;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    free_designs_mem(dz);
+    delete dz;
+    return SRP_OK;
+}
+
+srp_status srp_forces(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, long long N, int B,
+                      unsigned long long seed, float *out)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out);
+    if (st != SRP_OK) return st;
+    cudaSetDevice(ctx->device);
+    return run_forces(ctx, dz, sun_dirs, S, nullptr, (long long)dz->D * S, N, B, seed, out);
+}
+
+srp_status srp_forces_pairs(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
+                            long long n_pairs, long long N, int B, unsigned long long seed, float *out)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out);
+    if (st != SRP_OK) return st;
+    if (!pairs || n_pairs <= 0) return fail(ctx, SRP_ERR_INVALID, "bad pair list");
+    cudaSetDevice(ctx->device);
+    return run_forces(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed, out);
+}
+
+srp_status srp_forces_host(srp_context *ctx, const srp_designs *dz, const float *sun_dirs_host, int S, long long N,
+                           int B, unsigned long long seed, float *out_host)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs_host, S, N, B, out_host);
+    if (st != SRP_OK) return st;
+    cudaSetDevice(ctx->device);
+    const size_t n_dirs = (size_t)S * 3, n_out = (size_t)dz->D * S * 3;
+    if (ctx->stage_dirs_items < n_dirs) {
+        cudaFree(ctx->stage_dirs); ctx->stage_dirs = nullptr; ctx->stage_dirs_items = 0;
+        TRY_CUDA(ctx, cudaMalloc(&ctx->stage_dirs, sizeof(float) * n_dirs), "alloc staging");
+        ctx->stage_dirs_items = n_dirs;
+    }
+    if (ctx->stage_out_items < n_out) {
+        cudaFree(ctx->stage_out); ctx->stage_out = nullptr; ctx->stage_out_items = 0;
+        TRY_CUDA(ctx, cudaMalloc(&ctx->stage_out, sizeof(float) * n_out), "alloc staging");
+        ctx->stage_out_items = n_out;
+    }
+    TRY_CUDA(ctx, cudaMemcpyAsync(ctx->stage_dirs, sun_dirs_host, sizeof(float) * n_dirs, cudaMemcpyHostToDevice, ctx->stream), "h2d sun_dirs");
+    st = run_forces(ctx, dz, ctx->stage_dirs, S, nullptr, (long long)dz->D * S, N, B, seed, ctx->stage_out);
+    if (st != SRP_OK) return st;
+    TRY_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->stage_out, sizeof(float) * n_out, cudaMemcpyDeviceToHost, ctx->stream), "d2h forces");
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
+    return SRP_OK;
+}
+
+srp_status srp_first_hits(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
+                          long long n_pairs, long long N, unsigned long long seed, int method, int *out_prim)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, 0, out_prim);
+    if (st != SRP_OK) return st;
+    if (!pairs || n_pairs <= 0 || method < 0 || method > 1) return fail(ctx, SRP_ERR_INVALID, "bad pair list or method");
+    cudaSetDevice(ctx->device);
+    st = ensure_workspace(ctx, 3);
+    if (st != SRP_OK) return st;
+    TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, 0, seed);
+    TRY_CUDA(ctx, srp_launch_first_hits(a, method, out_prim, ctx->stream), "first-hit launch");
+    return SRP_OK;
+}
+
+srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!host_out) return fail(ctx, SRP_ERR_INVALID, "null output");
+    cudaSetDevice(ctx->device);
+    if (!ctx->stats) { memset(host_out, 0, sizeof *host_out); return SRP_OK; }
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
+    static_assert(sizeof(DevStats) == sizeof(srp_stats), "stats layout");
+    TRY_CUDA(ctx, cudaMemcpy(host_out, ctx->stats, sizeof(DevStats), cudaMemcpyDeviceToHost), "read stats");
+    return SRP_OK;
+}
+
+srp_status srp_probe_peaks(srp_context *ctx, double *fp32_tflops, double *l2_read_gbs)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!fp32_tflops || !l2_read_gbs) return fail(ctx, SRP_ERR_INVALID, "null output");
+    cudaSetDevice(ctx->device);
+    TRY_CUDA(ctx, srp_run_probes(ctx->num_sms, ctx->stream, fp32_tflops, l2_read_gbs), "probes");
+    return SRP_OK;
+}
+
+} // extern "C"

@@ -101,3 +101,4 @@ cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim,
 cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
 
 long long srp_family_tris_host(int family);
+int srp_trace_blocks_per_sm(bool brute);

@@ -1,0 +1,554 @@
+// trace.cu -- S2..S7 of the hot path: emitter set-up, Philox ray generation, closest-hit search
+// (BVH traversal, or all triangles of a small design from shared memory -- PAPER.md:159), material
+// lobe shading / momentum deposit (Eq. 2; 152,157), bounce loop with lane refill, and
+// the force reduction (Eq. 3).  DESIGN.md "O-steps" numbers the algorithm; the same
+// numbers appear in the comments below.
+//
+// One persistent kernel.  A WARP is the scheduling unit: it pulls (pair, ray tile) work items from
+// a global atomic counter, keeps one photon per lane, and after every segment replaces finished
+// photons by fresh rays of the tile (ballot + prefix popcount), so lanes stay busy across bounces.
+// Deposits are summed per lane in fp32 (dimensionless, <= a few hundred terms), per warp in fp64 by
+// shuffles, and added to a 2^-32 fixed-point int64 accumulator per pair -- integer adds commute,
+// so the result is bit-reproducible whatever the scheduling.
+#include <cfloat>
+#include "srp_internal.cuh"
+
+namespace {
+
+constexpr int TRACE_THREADS = 128;
+constexpr int TRACE_WARPS = TRACE_THREADS / 32;
+constexpr int STACK_SMEM = 24;       // traversal stack entries per thread kept in shared memory
+constexpr int STACK_OVF = 80;        // deeper entries spill to local memory (degenerate trees only)
+constexpr unsigned FULL = 0xffffffffu;
+
+enum { MODE_BRUTE_SMEM = 0, MODE_BVH = 1, MODE_BRUTE_GLOBAL = 2 };
+
+__device__ __forceinline__ float3 f3(float x, float y, float z) { return make_float3(x, y, z); }
+__device__ __forceinline__ float dot3(float3 a, float3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
+__device__ __forceinline__ float3 cross3(float3 a, float3 b)
+{
+    return f3(a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x);
+}
+
+__device__ __forceinline__ void philox4(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                        uint32_t k1, uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+// R4: ((x >> 9) + 0.5) * 2^-23 -- exact in fp32
+__device__ __forceinline__ float uniform23(uint32_t x) { return ((float)(x >> 9) + 0.5f) * (1.0f / 8388608.0f); }
+
+// O-step 1: orthonormal basis perpendicular to unit s (Duff et al. 2017)
+__device__ __forceinline__ void basis3(float3 s, float3 &u, float3 &v)
+{
+    const float sign = copysignf(1.0f, s.z);
+    const float a = -1.0f / (sign + s.z);
+    const float b = s.x * s.y * a;
+    u = f3(1.0f + sign * s.x * s.x * a, sign * b, -sign * s.x);
+    v = f3(b, sign + s.y * s.y * a, -s.y);
+}
+
+struct Emitter {
+    float3 s, u, v;
+    float u0, v0, du, dv, worg, Ae;
+};
+
+// O-steps 1-2: travel direction, basis, rectangle of the projected AABB corners, origin plane.
+__device__ inline Emitter make_emitter(const float *sun_dirs, int j, float4 lo, float4 hi)
+{
+    Emitter e;
+    const float wx = sun_dirs[3 * j], wy = sun_dirs[3 * j + 1], wz = sun_dirs[3 * j + 2];
+    const float len = sqrtf(wx * wx + wy * wy + wz * wz);
+    e.s = f3(-wx / len, -wy / len, -wz / len);
+    basis3(e.s, e.u, e.v);
+    float u0 = FLT_MAX, u1 = -FLT_MAX, v0 = FLT_MAX, v1 = -FLT_MAX, w0 = FLT_MAX;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const float3 p = f3((c & 1) ? hi.x : lo.x, (c & 2) ? hi.y : lo.y, (c & 4) ? hi.z : lo.z);
+        const float pu = dot3(p, e.u), pv = dot3(p, e.v), pw = dot3(p, e.s);
+        u0 = fminf(u0, pu); u1 = fmaxf(u1, pu);
+        v0 = fminf(v0, pv); v1 = fmaxf(v1, pv);
+        w0 = fminf(w0, pw);
+    }
+    e.u0 = u0; e.v0 = v0; e.du = u1 - u0; e.dv = v1 - v0;
+    e.worg = w0 - 1.0f;
+    e.Ae = e.du * e.dv;
+    return e;
+}
+
+__device__ __forceinline__ uint32_t compact_even_bits(uint32_t x)
+{
+    x &= 0x55555555u;
+    x = (x | (x >> 1)) & 0x33333333u;
+    x = (x | (x >> 2)) & 0x0F0F0F0Fu;
+    x = (x | (x >> 4)) & 0x00FF00FFu;
+    x = (x | (x >> 8)) & 0x0000FFFFu;
+    return x;
+}
+
+struct RayGen {            // warp-uniform per work item
+    uint32_t j, k, key0, key1;
+    int sampler;
+    float inv_nx, inv_ny;
+};
+
+// O-step 3: ray i of the pair.
+__device__ __forceinline__ void make_ray(const Emitter &e, const RayGen &g, uint32_t i, float3 &o)
+{
+    uint32_t r0, r1, r2, r3;
+    philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
+    float fu, fv;
+    if (g.sampler == 0) {
+        const float cx = (float)compact_even_bits(i), cy = (float)compact_even_bits(i >> 1);
+        fu = (cx + uniform23(r0)) * g.inv_nx;
+        fv = (cy + uniform23(r1)) * g.inv_ny;
+    } else {
+        fu = uniform23(r0); fv = uniform23(r1);
+    }
+    const float pu = fmaf(fu, e.du, e.u0), pv = fmaf(fv, e.dv, e.v0);
+    o = f3(fmaf(pu, e.u.x, fmaf(pv, e.v.x, e.worg * e.s.x)),
+           fmaf(pu, e.u.y, fmaf(pv, e.v.y, e.worg * e.s.y)),
+           fmaf(pu, e.u.z, fmaf(pv, e.v.z, e.worg * e.s.z)));
+}
+
+// O-step 4, one triangle: Moller-Trumbore on (v0, e1, e2) in the division-free sign-normalised
+// form: accept det != 0, u >= 0, v >= 0, u+v <= 1, t > 0; t = T/|det| only for accepted hits.
+__device__ __forceinline__ void tri_test(const float4 q0, const float4 q1, const float4 q2, const float3 o,
+                                         const float3 d, const int f, float &tbest, int &best)
+{
+    const float3 e1 = f3(q1.x, q1.y, q1.z), e2 = f3(q2.x, q2.y, q2.z);
+    const float3 pv = cross3(d, e2);
+    const float det = dot3(e1, pv);
+    const float3 tv = f3(o.x - q0.x, o.y - q0.y, o.z - q0.z);
+    const float3 qv = cross3(tv, e1);
+    const uint32_t sb = __float_as_uint(det) & 0x80000000u;
+    const float U = __uint_as_float(__float_as_uint(dot3(tv, pv)) ^ sb);
+    const float V = __uint_as_float(__float_as_uint(dot3(d, qv)) ^ sb);
+    const float Tn = __uint_as_float(__float_as_uint(dot3(e2, qv)) ^ sb);
+    const float adet = fabsf(det);
+    if (U >= 0.0f && V >= 0.0f && U + V <= adet && Tn > 0.0f && adet > 0.0f) {
+        const float t = Tn / adet;
+        if (t < tbest) { tbest = t; best = f; }
+    }
+}
+
+// All triangles of a design, in index order (ties -> smallest index), source excluded (R10).
+template <bool INSTR>
+__device__ __forceinline__ void closest_brute(const float4 *__restrict__ tp, const int T, const float3 o,
+                                              const float3 d, const int src, float &tbest, int &best,
+                                              unsigned &n_tri)
+{
+    for (int f = 0; f < T; ++f) {
+        if (f == src) continue;
+        tri_test(tp[3 * f], tp[3 * f + 1], tp[3 * f + 2], o, d, f, tbest, best);
+    }
+    if (INSTR) n_tri += (unsigned)(T - (src >= 0 ? 1 : 0));
+}
+
+__device__ __forceinline__ float safe_rcp(float x)
+{
+    return 1.0f / (fabsf(x) < 1e-30f ? copysignf(1e-30f, x) : x);
+}
+
+// Stack-based BVH2 descent, nearer child first.  Stack: STACK_SMEM entries per thread in shared
+// memory (thread-interleaved, conflict-free), deeper levels in a local array.
+template <bool INSTR>
+__device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, const float4 *__restrict__ tri,
+                                            const float3 o, const float3 d, const int src, float &tbest,
+                                            int &best, int *s_stack, unsigned &n_box, unsigned &n_tri)
+{
+    const float idx = safe_rcp(d.x), idy = safe_rcp(d.y), idz = safe_rcp(d.z);
+    const float oxi = o.x * idx, oyi = o.y * idy, ozi = o.z * idz;
+    int ovf[STACK_OVF];
+    int sp = 0;
+    int cur = 0;
+    for (;;) {
+        if (cur >= 0) {
+            const float4 n0 = __ldg(nodes + 4 * cur), n1 = __ldg(nodes + 4 * cur + 1),
+                         n2 = __ldg(nodes + 4 * cur + 2), n3 = __ldg(nodes + 4 * cur + 3);
+            if (INSTR) n_box += 2;
+            float a0 = fmaf(n0.x, idx, -oxi), a1 = fmaf(n0.w, idx, -oxi);
+            float b0 = fmaf(n0.y, idy, -oyi), b1 = fmaf(n1.x, idy, -oyi);
+            float c0 = fmaf(n0.z, idz, -ozi), c1 = fmaf(n1.y, idz, -ozi);
+            const float tmin0 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
+            const float tmax0 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
+            a0 = fmaf(n1.z, idx, -oxi); a1 = fmaf(n2.y, idx, -oxi);
+            b0 = fmaf(n1.w, idy, -oyi); b1 = fmaf(n2.z, idy, -oyi);
+            c0 = fmaf(n2.x, idz, -ozi); c1 = fmaf(n2.w, idz, -ozi);
+            const float tmin1 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
+            const float tmax1 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
+            const bool h0 = tmin0 <= tmax0 * 1.0000004f, h1 = tmin1 <= tmax1 * 1.0000004f;
+            int l0 = __float_as_int(n3.x), l1 = __float_as_int(n3.y);
+            if (h0 && h1) {
+                if (tmin1 < tmin0) { const int t = l0; l0 = l1; l1 = t; }
+                if (sp < STACK_SMEM) s_stack[sp * TRACE_THREADS] = l1; else ovf[sp - STACK_SMEM] = l1;
+                ++sp;
+                cur = l0;
+                continue;
+            }
+            if (h0) { cur = l0; continue; }
+            if (h1) { cur = l1; continue; }
+        } else {
+            const unsigned u = (unsigned)~cur;
+            const int first = (int)(u >> 3), cnt = (int)(u & 7u) + 1;
+            for (int f = first; f < first + cnt; ++f) {
+                if (f == src) continue;
+                tri_test(__ldg(tri + 3 * f), __ldg(tri + 3 * f + 1), __ldg(tri + 3 * f + 2), o, d, f, tbest, best);
+            }
+            if (INSTR) n_tri += (unsigned)cnt;
+        }
+        if (sp == 0) break;
+        --sp;
+        cur = sp < STACK_SMEM ? s_stack[sp * TRACE_THREADS] : ovf[sp - STACK_SMEM];
+    }
+}
+
+struct LaneCounters {
+    unsigned launched, pmiss, absorbed, escaped, capped, segments, n_box, n_tri;
+};
+
+// O-steps 5-7 at a hit: deposit, lobe selection, continuation.  Returns true if the photon goes on.
+__device__ __forceinline__ bool shade(const float4 q0, const float4 q1, const float4 q2, const float t,
+                                      const int f, const RayGen &g, const uint32_t i, const int B,
+                                      const int deposit, float3 &o, float3 &d, int &src, int &depth,
+                                      float3 &acc, LaneCounters &cn)
+{
+    (void)q0;
+    const float al = q0.w, rs = q1.w, rd = q2.w;
+    float3 n = cross3(f3(q1.x, q1.y, q1.z), f3(q2.x, q2.y, q2.z));
+    const float inv_len = 1.0f / sqrtf(dot3(n, n));
+    n = f3(n.x * inv_len, n.y * inv_len, n.z * inv_len);
+    const float nd = dot3(n, d);
+    const float3 nf = nd > 0.0f ? f3(-n.x, -n.y, -n.z) : n;      // facets are two-sided (R6)
+    const float cost = fabsf(nd);
+    const float3 refl = f3(fmaf(2.0f * cost, nf.x, d.x), fmaf(2.0f * cost, nf.y, d.y), fmaf(2.0f * cost, nf.z, d.z));
+    if (deposit == 0) {                                           // expected-value deposit
+        const float a = al + rs + rd, c = (2.0f / 3.0f) * rd;
+        acc.x += a * d.x - rs * refl.x - c * nf.x;
+        acc.y += a * d.y - rs * refl.y - c * nf.y;
+        acc.z += a * d.z - rs * refl.z - c * nf.z;
+    }
+    uint32_t y0, y1, y2, y3;
+    philox4(i, g.j, g.k, (uint32_t)(depth + 1), g.key0, g.key1, y0, y1, y2, y3);
+    const float z0 = uniform23(y0);
+    float3 dn;
+    if (z0 < al) {                                                // absorbed
+        if (deposit == 1) { acc.x += d.x; acc.y += d.y; acc.z += d.z; }
+        cn.absorbed++;
+        return false;
+    } else if (z0 < al + rs) {                                    // ideal mirror (R3)
+        dn = refl;
+    } else {                                                      // Lambertian: cosine-weighted about nf
+        const float z1 = uniform23(y1), z2 = uniform23(y2);
+        float sn, cs;
+        sincospif(2.0f * z1, &sn, &cs);
+        const float rho = sqrtf(z2), lz = sqrtf(1.0f - z2);
+        float3 tu, tv;
+        basis3(nf, tu, tv);
+        const float lx = rho * cs, ly = rho * sn;
+        dn = f3(fmaf(lx, tu.x, fmaf(ly, tv.x, lz * nf.x)), fmaf(lx, tu.y, fmaf(ly, tv.y, lz * nf.y)),
+                fmaf(lx, tu.z, fmaf(ly, tv.z, lz * nf.z)));
+    }
+    if (deposit == 1) { acc.x += d.x - dn.x; acc.y += d.y - dn.y; acc.z += d.z - dn.z; }
+    if (depth == B) { cn.capped++; return false; }               // R5: B reflections followed
+    o = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
+    d = dn; src = f; depth += 1;
+    return true;
+}
+
+__device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k, int &j)
+{
+    if (a.pairs) { k = a.pairs[2 * p]; j = a.pairs[2 * p + 1]; }
+    else { k = (int)(p / a.S); j = (int)(p - (long long)k * a.S); }
+}
+
+// ---- the persistent trace kernel ----
+template <int MODE, bool INSTR>
+__global__ void __launch_bounds__(TRACE_THREADS, MODE == MODE_BVH ? 4 : 5)
+trace_kernel(const TraceArgs a)
+{
+    __shared__ int s_stack[MODE == MODE_BVH ? STACK_SMEM * TRACE_THREADS : 1];
+    __shared__ float4 s_tri[MODE == MODE_BRUTE_SMEM ? TRACE_WARPS * SRP_BRUTE_MAX_TRIS * 3 : 1];
+    __shared__ unsigned s_hist[TRACE_WARPS][16];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    if (lane < 16) s_hist[warp][lane] = 0;
+    __syncwarp();
+    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
+    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
+    int loaded_k = -1;
+    float4 *my_tri = s_tri + (MODE == MODE_BRUTE_SMEM ? warp * SRP_BRUTE_MAX_TRIS * 3 : 0);
+
+    for (;;) {
+        unsigned long long tile = 0;
+        if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
+        tile = __shfl_sync(FULL, tile, 0);
+        if (tile >= total_tiles) break;
+        const long long p = (long long)(tile / a.tiles_per_pair);
+        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
+        int k, j;
+        pair_of(a, p, k, j);
+        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
+        if (!(em.Ae > 0.0f)) continue;                      // edge-on flat design: F = 0, nothing launched
+        const long long tbase = a.dz.tri_off[k];
+        const int T = (int)(a.dz.tri_off[k + 1] - tbase);
+        const float4 *gtri = a.dz.tri + 3 * tbase;
+        const float4 *gnodes = a.dz.nodes + 4 * tbase;
+        if (MODE == MODE_BRUTE_SMEM && loaded_k != k) {
+            __syncwarp();
+            for (int x = lane; x < 3 * T; x += 32) my_tri[x] = gtri[x];
+            __syncwarp();
+            loaded_k = k;
+        }
+        RayGen g;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler;
+        g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
+        g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
+        uint32_t next = (uint32_t)(q * a.tile_rays);
+        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
+
+        bool alive = false;
+        uint32_t i = 0;
+        float3 o = f3(0, 0, 0), d = em.s, acc = f3(0, 0, 0);
+        int src = -1, depth = 0;
+        for (;;) {
+            // S6: lanes whose photon ended take the next rays of the tile
+            const unsigned need = __ballot_sync(FULL, !alive);
+            if (need) {
+                const uint32_t mine = next + __popc(need & lt_mask);
+                if (!alive && mine < end) {
+                    i = mine; make_ray(em, g, i, o); d = em.s; src = -1; depth = 0; alive = true;
+                    cn.launched++;
+                }
+                const uint32_t room = end - next, want = __popc(need);
+                next += want < room ? want : room;
+            }
+            if (!__any_sync(FULL, alive)) break;
+            if (alive) {
+                float tbest = FLT_MAX; int best = -1;
+                cn.segments++;
+                if (MODE == MODE_BVH)
+                    closest_bvh<INSTR>(gnodes, gtri, o, d, src, tbest, best, s_stack + threadIdx.x, cn.n_box, cn.n_tri);
+                else if (MODE == MODE_BRUTE_SMEM)
+                    closest_brute<INSTR>(my_tri, T, o, d, src, tbest, best, cn.n_tri);
+                else
+                    closest_brute<INSTR>(gtri, T, o, d, src, tbest, best, cn.n_tri);
+                if (best < 0) {
+                    if (depth == 0) cn.pmiss++; else cn.escaped++;
+                    alive = false;
+                } else {
+                    atomicAdd(&s_hist[warp][depth], 1u);
+                    const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
+                    alive = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, cn);
+                }
+            }
+        }
+        // S7: warp reduction in fp64, then one fixed-point atomic per component
+        double sx = acc.x, sy = acc.y, sz = acc.z;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            sx += __shfl_xor_sync(FULL, sx, off);
+            sy += __shfl_xor_sync(FULL, sy, off);
+            sz += __shfl_xor_sync(FULL, sz, off);
+        }
+        if (lane == 0) {
+            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
+            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
+            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
+            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
+        }
+    }
+    // counters: warp sums, one global atomic each
+    unsigned long long *st = (unsigned long long *)a.stats;
+    const unsigned vals[8] = { cn.launched, cn.pmiss, cn.absorbed, cn.escaped, cn.capped, cn.segments, cn.n_box, cn.n_tri };
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        if (!INSTR && c >= 6) break;
+        unsigned long long v = vals[c];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+        if (lane == 0 && v) atomicAdd(st + (c < 6 ? c : 22 + (c - 6)), v);
+    }
+    __syncwarp();
+    if (lane < 16 && s_hist[warp][lane]) atomicAdd(st + 6 + lane, (unsigned long long)s_hist[warp][lane]);
+}
+
+// F[p] = accum[p] * 2^-32 * P * A_e / N
+__global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float *out)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= a.n_pairs) return;
+    int k, j;
+    pair_of(a, p, k, j);
+    const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
+    const double w = em.Ae > 0.0f ? a.P * (double)em.Ae / (double)a.N / SRP_ACC_SCALE : 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) out[3 * p + c] = (float)((double)a.accum[3 * p + c] * w);
+}
+
+// debug: primary-hit triangle (original index) of every ray of the listed pairs
+template <int MODE>
+__global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArgs a, int *out_prim)
+{
+    __shared__ int s_stack[MODE == MODE_BVH ? STACK_SMEM * TRACE_THREADS : 1];
+    const long long total = a.n_pairs * a.N;
+    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < total;
+         r += (long long)gridDim.x * blockDim.x) {
+        const long long p = r / a.N;
+        const uint32_t i = (uint32_t)(r - p * a.N);
+        int k, j;
+        pair_of(a, p, k, j);
+        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
+        int best = -1;
+        if (em.Ae > 0.0f) {
+            const long long tbase = a.dz.tri_off[k];
+            const int T = (int)(a.dz.tri_off[k + 1] - tbase);
+            RayGen g;
+            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler;
+            g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
+            g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
+            float3 o;
+            make_ray(em, g, i, o);
+            float tbest = FLT_MAX;
+            unsigned nb = 0, nt = 0;
+            if (MODE == MODE_BVH)
+                closest_bvh<false>(a.dz.nodes + 4 * tbase, a.dz.tri + 3 * tbase, o, em.s, -1, tbest, best,
+                                   s_stack + threadIdx.x, nb, nt);
+            else
+                closest_brute<false>(a.dz.tri + 3 * tbase, T, o, em.s, -1, tbest, best, nt);
+            if (best >= 0) best = a.dz.perm[tbase + best];
+        }
+        out_prim[r] = best;
+    }
+}
+
+} // namespace
+
+// ---- roofline probes ----
+namespace {
+__global__ void __launch_bounds__(256) fma_probe_kernel(float *out, int iters, float a, float b)
+{
+    float x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
+            x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
+        }
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+}
+__global__ void __launch_bounds__(256) l2_probe_kernel(const float4 *buf, size_t n_vec, int passes, float *out)
+{
+    float s = 0.f;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (int p = 0; p < passes; ++p)
+        for (size_t x = (size_t)blockIdx.x * blockDim.x + threadIdx.x; x < n_vec; x += stride) {
+            const float4 v = __ldcg(buf + x);
+            s += v.x + v.y + v.z + v.w;
+        }
+    if (s == 12345.678f) out[0] = s;
+}
+} // namespace
+
+cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs)
+{
+    float *out = nullptr; float4 *buf = nullptr;
+    const int blocks = num_sms * 8, iters = 4096;
+    const size_t n_vec = (size_t)32 << 20 >> 4;           // 32 MiB, well inside L2
+    cudaError_t e = cudaMalloc(&out, sizeof(float) * blocks * 256);
+    if (e != cudaSuccess) return e;
+    e = cudaMalloc(&buf, n_vec * sizeof(float4));
+    if (e != cudaSuccess) { cudaFree(out); return e; }
+    cudaMemsetAsync(buf, 0, n_vec * sizeof(float4), stream);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best_f = 0, best_l = 0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, stream);
+        fma_probe_kernel<<<blocks, 256, 0, stream>>>(out, iters, 0.999f, 0.001f);
+        cudaEventRecord(e1, stream);
+        cudaEventSynchronize(e1);
+        float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+        double tf = 2.0 * 64.0 * iters * blocks * 256.0 / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best_f) best_f = tf;
+        const int passes = 20;
+        cudaEventRecord(e0, stream);
+        l2_probe_kernel<<<num_sms * 8, 256, 0, stream>>>(buf, n_vec, passes, out);
+        cudaEventRecord(e1, stream);
+        cudaEventSynchronize(e1);
+        cudaEventElapsedTime(&ms, e0, e1);
+        double gb = (double)passes * n_vec * 16.0 / (ms * 1e-3) / 1e9;
+        if (rep > 0 && gb > best_l) best_l = gb;
+    }
+    e = cudaGetLastError();
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out); cudaFree(buf);
+    *fp32_tflops = best_f; *l2_gbs = best_l;
+    return e;
+}
+
+// ---- launchers ----
+template <int MODE, bool INSTR>
+static cudaError_t launch_trace_t(const TraceArgs &a, int num_sms, cudaStream_t stream)
+{
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE, INSTR>,
+                                                                  TRACE_THREADS, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
+    unsigned long long blocks = (unsigned long long)num_sms * per_sm;       // persistent: fill the machine once
+    const unsigned long long needed = (total_tiles + TRACE_WARPS - 1) / TRACE_WARPS;
+    if (blocks > needed) blocks = needed;
+    if (blocks < 1) blocks = 1;
+    trace_kernel<MODE, INSTR><<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a);
+    return cudaGetLastError();
+}
+
+int srp_trace_blocks_per_sm(bool brute)
+{
+    int per_sm = 0;
+    if (brute) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BRUTE_SMEM, false>, TRACE_THREADS, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BVH, false>, TRACE_THREADS, 0);
+    return per_sm * TRACE_WARPS;
+}
+
+cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms, cudaStream_t stream)
+{
+    if (brute) {
+        if (a.dz.has_bvh)       // forced brute force over a design that also has a hierarchy (test use)
+            return instrumented ? launch_trace_t<MODE_BRUTE_GLOBAL, true>(a, num_sms, stream)
+                                : launch_trace_t<MODE_BRUTE_GLOBAL, false>(a, num_sms, stream);
+        return instrumented ? launch_trace_t<MODE_BRUTE_SMEM, true>(a, num_sms, stream)
+                            : launch_trace_t<MODE_BRUTE_SMEM, false>(a, num_sms, stream);
+    }
+    return instrumented ? launch_trace_t<MODE_BVH, true>(a, num_sms, stream)
+                        : launch_trace_t<MODE_BVH, false>(a, num_sms, stream);
+}
+
+cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, cudaStream_t stream)
+{
+    finalize_kernel<<<(unsigned)((a.n_pairs + 255) / 256), 256, 0, stream>>>(a, out_forces);
+    return cudaGetLastError();
+}
+
+cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream)
+{
+    const long long total = a.n_pairs * a.N;
+    long long blocks = (total + TRACE_THREADS - 1) / TRACE_THREADS;
+    if (blocks > 148 * 64) blocks = 148 * 64;
+    if (method == 0 && a.dz.has_bvh)
+        first_hit_kernel<MODE_BVH><<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a, out_prim);
+    else
+        first_hit_kernel<MODE_BRUTE_GLOBAL><<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a, out_prim);
+    return cudaGetLastError();
+}
