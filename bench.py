@@ -1,0 +1,306 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3_detailed] [--impl ours|reference]
+
+A step = one pass of the whole hot path over one batch of synthetic input: srp_build_designs
+(mesh generation + LBVH build, S0-S1) followed by srp_forces (S2-S7) for every (design, direction)
+pair of the workload.  metric = photon-bounce segments per second (every ray cast, hit or miss),
+whole job; forces/s is reported beside it.  N > 1 (torchrun): designs are replicated, each rank takes
+its own S directions of an N*S-direction Fibonacci sphere (weak scaling, no data-path collective).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2602_10712_b200 import workloads as W          # noqa: E402
+
+METRIC = "photon-bounce segments/s"
+UNIT = "segments/s"
+# FP32 peak the ALU roofline is quoted against: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
+# (B200_PROFILING.md unit counts and max SM clock); the probed FMA-chain figure is printed beside it.
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# algorithmic work per unit: 12 flop per ray-box test, 44 per ray-triangle test,
+# 80 per shaded hit; 64 B per node visited (2 boxes), 48 B per triangle tested.
+FLOP_BOX, FLOP_TRI, FLOP_HIT = 12.0, 44.0, 80.0
+BYTES_NODE, BYTES_TRI = 64.0, 48.0
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3_detailed", choices=sorted(W.CONFIGS))
+    ap.add_argument("--scale", type=float, default=1.0,
+                    help="fraction of the workload's sun directions (debug; < 1 marks the line invalid)")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=5)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, n_pairs, N, seed=0):
+    """Times the oracle, as it stands, on n_pairs pairs of the workload at N rays, one single-threaded
+    oracle call per pair spread over the host cores.  Returns (segments, seconds, threads used)."""
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import srp_oracle as O
+    O.build()
+    th, sun = cfg.params(), cfg.sun_dirs()
+    rng = np.random.default_rng(123)
+    pairs = [(int(rng.integers(0, cfg.D)), int(rng.integers(0, cfg.S))) for _ in range(n_pairs)]
+    meshes = {k: O.build_mesh(cfg.family, th[k], k=k) for k in sorted({p[0] for p in pairs})}
+    threads = min(os.cpu_count() or 1, n_pairs)
+
+    def one(p):
+        v, m = meshes[p[0]]
+        return O.forces(v, m, sun[p[1]:p[1] + 1], N, cfg.B, seed=seed, k=p[0], j0=p[1])["stats"]["segments"]
+
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(threads) as ex:
+        segs = sum(ex.map(one, pairs))
+    return segs, time.perf_counter() - t0, threads
+
+
+# bounded oracle samples per workload: (pairs per host core, rays per pair) ~ 10-30 s of CPU work
+ORACLE_SAMPLE = {"cfg1_plate": (8, 1 << 16), "cfg2_boxwing": (8, 1 << 18), "cfg3_detailed": (2, 1 << 11),
+                 "cfg4_sweep": (16, 1 << 16), "cfg5_sail": (1, 1 << 8)}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle (oracle/, fp64, brute force, one thread per call) on the host cores,
+    each step a bounded sample of the workload.  Rank 0 only."""
+    if rank != 0:
+        return
+    cfg = W.CONFIGS[args.workload]
+    per_core, N = ORACLE_SAMPLE[args.workload]
+    cores = os.cpu_count() or 1
+    n_pairs = per_core * cores
+    for _ in range(args.warmup):
+        oracle_sample(cfg, min(n_pairs, cores), max(N >> 4, 1))
+    segs = secs = 0.0
+    for s in range(args.steps):
+        a, b, threads = oracle_sample(cfg, n_pairs, N, seed=s)
+        segs += a; secs += b
+    value = segs / secs
+    sample = "%d random pairs x N=%d rays per step, %d steps" % (n_pairs, N, args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": args.workload, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2602_10712_b200.binding import Context
+    from paper_2602_10712_b200 import sharding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = W.CONFIGS[args.workload]
+    S = max(1, int(round(cfg.S * args.scale)))
+    sun_np = sharding.weak_scaling_directions(S, rank, world, cfg.front_hemisphere)
+    theta_np = cfg.params()
+    ctx = Context(local_rank)
+    theta = torch.from_numpy(theta_np).to(dev)
+    sun = torch.from_numpy(sun_np).to(dev)
+    out = torch.empty((cfg.D, S, 3), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    peaks = ctx.srp_probe_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(seed):
+        dz = ctx.srp_build_designs(cfg.family, theta, W.MESH_SEED)
+        ctx.srp_forces(dz, sun, cfg.N, cfg.B, seed, out=out)
+        return dz
+
+    for s in range(args.warmup):
+        dz = step(1000 + s)
+        torch.cuda.synchronize()
+        dz.free()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    t_total = 0.0
+    segs = 0
+    hits = launched = pmiss = 0
+    for s in range(args.steps):
+        flush.zero_()                                                   # L2 flush between timed steps
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        dz = step(s)
+        e1.record()
+        torch.cuda.synchronize()
+        t_total += e0.elapsed_time(e1) * 1e-3
+        st = ctx.srp_get_stats()
+        segs += st["segments"]; hits += sum(st["hits_at_depth"]); launched += st["launched"]
+        pmiss += st["primary_miss"]
+        dz.free()
+    barrier()
+    clocks = sampler.stop()
+    t_max, segs_all = sharding.combine_timing(t_total, segs, dev)
+
+    # dominant kernel alone (trace_kernel): CUDA events around srp_forces only, designs resident
+    dz = ctx.srp_build_designs(cfg.family, theta, W.MESH_SEED)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    flush.zero_()
+    e0.record()
+    ctx.srp_forces(dz, sun, cfg.N, cfg.B, 0, out=out)
+    e1.record()
+    torch.cuda.synchronize()
+    t_kernel = e0.elapsed_time(e1) * 1e-3
+    st_k = ctx.srp_get_stats()
+    # algorithmic work per segment from the instrumented kernel on every 64th direction
+    ctx.srp_set_options(instrumented=1)
+    sub = sun[::64].contiguous() if S >= 64 else sun
+    ctx.srp_forces(dz, sub, cfg.N, cfg.B, 0)
+    st_i = ctx.srp_get_stats()
+    ctx.srp_set_options()
+    seg_i = max(st_i["segments"], 1)
+    box_ps, tri_ps = st_i["box_tests"] / seg_i, st_i["tri_tests"] / seg_i
+    hit_ps = sum(st_i["hits_at_depth"]) / seg_i
+    flop_ps = FLOP_BOX * box_ps + FLOP_TRI * tri_ps + FLOP_HIT * hit_ps
+    bytes_ps = BYTES_NODE * box_ps / 2.0 + BYTES_TRI * tri_ps
+    ach_tflops = flop_ps * st_k["segments"] / t_kernel / 1e12
+    roofline = {"bound": "alu", "kernel": "trace_kernel", "achieved": ach_tflops, "peak": FP32_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": ach_tflops / FP32_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz; probed FMA chain %.1f TFLOP/s" % peaks["fp32_tflops"],
+                "flop_per_segment": flop_ps, "box_tests_per_segment": box_ps, "tri_tests_per_segment": tri_ps,
+                "l2": {"achieved_gbs": bytes_ps * st_k["segments"] / t_kernel / 1e9, "probed_peak_gbs": peaks["l2_read_gbs"],
+                       "bytes_per_segment": bytes_ps},
+                "kernel_ms": 1e3 * t_kernel, "kernel_segments": st_k["segments"]}
+
+    # end to end through the host-buffer entry point: theta, sun_dirs from pinned host memory, forces back
+    theta_h = torch.from_numpy(theta_np).pin_memory()
+    sun_h = torch.from_numpy(sun_np).pin_memory()
+    out_h = torch.empty((cfg.D, S, 3), dtype=torch.float32).pin_memory()
+    dz.free()
+    barrier()
+    e2e_steps = max(1, min(args.steps, 2))
+    t_e2e = 0.0
+    seg_e2e = 0
+    for s in range(e2e_steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        dz = ctx.srp_build_designs(cfg.family, theta_h.to(dev, non_blocking=True), W.MESH_SEED)
+        ctx.srp_forces_host(dz, sun_h, cfg.N, cfg.B, s, out_host=out_h)
+        checksum = float(out_h.sum())                                     # the result is read on the host
+        t_e2e += time.perf_counter() - t0
+        seg_e2e += ctx.srp_get_stats()["segments"]
+        dz.free()
+    t_e2e_max, seg_e2e_all = sharding.combine_timing(t_e2e, seg_e2e, dev)
+    e2e = {"value": seg_e2e_all / t_e2e_max, "unit": UNIT,
+           "h2d_bytes_per_step": int(theta_np.nbytes + sun_np.nbytes), "d2h_bytes_per_step": int(out_h.numel() * 4),
+           "steps": e2e_steps, "checksum": checksum}
+
+    cpu = None
+    if rank == 0 and world == 1:
+        per_core, N_o = ORACLE_SAMPLE[args.workload]
+        n_pairs = per_core * (os.cpu_count() or 1)
+        a, b, threads = oracle_sample(cfg, n_pairs, N_o)
+        cpu = {"value": a / b, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": "%d random pairs x N=%d rays (fp64, brute force over all %d triangles)" % (n_pairs, N_o, W.TRI_COUNT[cfg.family]),
+               "per_core": a / b / threads}
+    if rank == 0:
+        pairs_all = cfg.D * S * world
+        line = {"metric": METRIC, "value": segs_all / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": args.workload, "designs": cfg.D, "directions_per_gpu": S, "rays_per_dir": cfg.N,
+                           "max_bounces": cfg.B, "triangles_per_design": W.TRI_COUNT[cfg.family],
+                           "l2": "256 MiB buffer written between timed steps", "parallelism": "dp%d" % world,
+                           "valid": args.scale == 1.0},
+                "forces_per_s": pairs_all * args.steps / t_max,
+                "primary_hit_fraction": 1.0 - pmiss / max(launched, 1), "hits_per_photon": hits / max(launched, 1),
+                "segments_per_photon": segs / max(launched, 1),
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": (10 if W.TRI_COUNT[cfg.family] > 64 else 6) * args.steps,
+                "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -143,6 +143,14 @@ srp_status srp_first_hits(srp_context *ctx, const srp_designs *designs, const fl
                           const int *pairs, long long n_pairs, long long rays_per_dir,
                           unsigned long long seed, int method, int *out_prim);
 
+/* Debug: path signature of every photon of the listed pairs: out_sig DEVICE unsigned long long
+ * [n_pairs, rays_per_dir]; sig = 0, then sig = sig * 1000003 + (ORIGINAL triangle index + 1) at every
+ * hit (mod 2^64).  Two tracers took the same path through the mesh iff the signatures agree, so the
+ * harness counts divergent rays with it.  Runs the instrumented kernel.  Enqueues only. */
+srp_status srp_path_signatures(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                               const int *pairs, long long n_pairs, long long rays_per_dir,
+                               int max_bounces, unsigned long long seed, unsigned long long *out_sig);
+
 /* Counters of the last srp_forces* call on this context.  Syncs. */
 srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out);
 

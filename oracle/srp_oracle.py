@@ -72,7 +72,7 @@ def lib():
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int,
             ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int,
             ctypes.c_ulonglong, ctypes.POINTER(Options),
-            ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats), ctypes.c_void_p]
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats), ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_philox.restype = None
         L.srp_oracle_philox.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_uniform.restype = ctypes.c_double
@@ -117,7 +117,7 @@ def build_mesh(family, theta, k=0, mesh_seed=2):
 
 
 def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sampler=0,
-           deposit=0, want_first_hit=False):
+           deposit=0, want_first_hit=False, want_path_sig=False):
     """Forces of ONE design for the given sun directions.
 
     Returns dict(F f64[S,3], sumsq f64[S,3], sigma f64[S] (i.i.d. standard error of |F|,
@@ -131,13 +131,15 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
     F = np.zeros((S, 3)); Q = np.zeros((S, 3))
     st = Stats()
     fh = np.empty((S, N), dtype=np.int32) if want_first_hit else None
+    ps = np.empty((S, N), dtype=np.uint64) if want_path_sig else None
     opt = Options(float(P), int(sampler), int(deposit))
     rc = lib().srp_oracle_forces(verts.ctypes.data, mats.ctypes.data, T, int(k), sun.ctypes.data,
                                  S, int(j0), int(N), int(B), int(seed), ctypes.byref(opt),
                                  F.ctypes.data, Q.ctypes.data, ctypes.byref(st),
-                                 fh.ctypes.data if fh is not None else None)
+                                 fh.ctypes.data if fh is not None else None,
+                                 ps.ctypes.data if ps is not None else None)
     if rc != 0:
         raise ValueError("srp_oracle_forces: invalid arguments")
     var = np.maximum(Q - F * F / float(N), 0.0)     # N * sample variance of the photon totals
     sigma = np.sqrt(var.sum(axis=1))
-    return {"F": F, "sumsq": Q, "sigma": sigma, "stats": st.as_dict(), "first_hit": fh}
+    return {"F": F, "sumsq": Q, "sigma": sigma, "stats": st.as_dict(), "first_hit": fh, "path_sig": ps}

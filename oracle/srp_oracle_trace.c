@@ -83,12 +83,15 @@ static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
  *       per-photon momentum total (for the MC standard error), may be NULL
  *   stats accumulated over all S (zeroed here), may be NULL
  *   first_hit int32[S][N] primary-hit triangle (-1 miss), may be NULL
+ *   path_sig uint64[S][N] bookkeeping for the divergent-ray count, may be NULL: sig = 0, then
+ *       sig = sig*1000003 + (triangle index + 1) at every hit (mod 2^64)
  * Returns 0, or -1 on invalid arguments.
  */
 int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                       const float *sun_dirs, int S, int j0, long long N, int B,
                       unsigned long long seed, const orc_options *opt,
-                      double *F, double *sumsq, orc_stats *stats, int *first_hit)
+                      double *F, double *sumsq, orc_stats *stats, int *first_hit,
+                      unsigned long long *path_sig)
 {
     if (!verts || !mats || !sun_dirs || !F || !opt || T <= 0 || S <= 0 || N <= 0 || B < 0 || B > 15)
         return -1;
@@ -157,6 +160,7 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
             long src = -1;
             int depth = 0;
             double dp[3] = { 0, 0, 0 };
+            unsigned long long sig = 0;
             st.launched++;
             for (;;) {
                 /* O-step 4 */
@@ -169,6 +173,7 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                     break;
                 }
                 st.hits_at_depth[depth]++;
+                sig = sig * 1000003ULL + (unsigned long long)(f + 1);
                 /* O-step 5: facing normal, mirror direction, deposit. */
                 orc_v3 n = orc_mk(nrm[3 * f], nrm[3 * f + 1], nrm[3 * f + 2]);
                 orc_v3 nf = (orc_dot(n, d) > 0.0) ? orc_scale(n, -1.0) : n;
@@ -198,8 +203,11 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                 } else {
                     double phi = 6.283185307179586476925286766559 * z1, rho = sqrt(z2);
                     double lx = rho * cos(phi), ly = rho * sin(phi), lz = sqrt(1.0 - z2);
-                    orc_v3 tu, tv;
-                    orc_basis(nf, &tu, &tv);
+                    /* tangent frame (R18): first edge of the facet and nf x edge -- defined by the
+                     * mesh itself, so it has no discontinuity that rounding noise in nf could trip
+                     * (the step-1 rule flips across nf.z = 0, where axis-aligned facets sit) */
+                    orc_v3 tu = orc_normalize(orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]));
+                    orc_v3 tv = orc_cross(nf, tu);
                     dnew = orc_add(orc_add(orc_scale(tu, lx), orc_scale(tv, ly)), orc_scale(nf, lz));
                 }
                 if (opt->deposit == 1) {
@@ -210,9 +218,12 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                 o = x; d = dnew; src = f; depth += 1;
             }
             for (int c = 0; c < 3; ++c) { Fj[c] += dp[c]; Qj[c] += dp[c] * dp[c]; }
+            if (path_sig) path_sig[(long long)jj * N + i] = sig;
         }
         if (!(Ae > 0.0) && first_hit)
             for (long long i = 0; i < N; ++i) first_hit[(long long)jj * N + i] = -1;
+        if (!(Ae > 0.0) && path_sig)
+            for (long long i = 0; i < N; ++i) path_sig[(long long)jj * N + i] = 0;
         for (int c = 0; c < 3; ++c) { F[3 * jj + c] = Fj[c]; if (sumsq) sumsq[3 * jj + c] = Qj[c]; }
     }
     if (stats) *stats = st;

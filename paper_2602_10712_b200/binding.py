@@ -47,7 +47,7 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_family_n_params", "srp_family_tri_count", "srp_build_designs",
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
-           "srp_first_hits", "srp_get_stats", "srp_probe_peaks"]
+           "srp_first_hits", "srp_path_signatures", "srp_get_stats", "srp_probe_peaks"]
 
 _lib = None
 
@@ -81,6 +81,7 @@ def load_library():
     L.srp_forces_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_forces_host.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
     L.srp_first_hits.argtypes = [vp, vp, vp, ci, vp, ll, ll, ull, ci, vp]
+    L.srp_path_signatures.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_get_stats.argtypes = [vp, ctypes.POINTER(srp_stats)]
     L.srp_probe_peaks.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     for name in EXPORTS:
@@ -222,6 +223,15 @@ class Context:
         self._check(self.lib.srp_first_hits(self.handle, designs.handle, sun_dirs.data_ptr(), sun_dirs.shape[0],
                                             pairs.data_ptr(), pairs.shape[0], rays_per_dir, seed, method,
                                             out.data_ptr()))
+        self.stream.synchronize()
+        return out
+
+    def srp_path_signatures(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0):
+        pairs = torch.as_tensor(pairs).to(device=self.device, dtype=torch.int32).contiguous()
+        out = torch.empty((pairs.shape[0], rays_per_dir), dtype=torch.int64, device=self.device)
+        self._check(self.lib.srp_path_signatures(self.handle, designs.handle, sun_dirs.data_ptr(), sun_dirs.shape[0],
+                                                 pairs.data_ptr(), pairs.shape[0], rays_per_dir, max_bounces, seed,
+                                                 out.data_ptr()))
         self.stream.synchronize()
         return out
 

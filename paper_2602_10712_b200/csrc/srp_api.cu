@@ -346,6 +346,27 @@ srp_status srp_first_hits(srp_context *ctx, const srp_designs *dz, const float *
     return SRP_OK;
 }
 
+srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S,
+                               const int *pairs, long long n_pairs, long long N, int B,
+                               unsigned long long seed, unsigned long long *out_sig)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out_sig);
+    if (st != SRP_OK) return st;
+    if (!pairs || n_pairs <= 0) return fail(ctx, SRP_ERR_INVALID, "bad pair list");
+    cudaSetDevice(ctx->device);
+    st = ensure_workspace(ctx, (size_t)n_pairs * 3);
+    if (st != SRP_OK) return st;
+    TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
+    a.sig_out = out_sig;
+    TRY_CUDA(ctx, cudaMemsetAsync(out_sig, 0, sizeof(unsigned long long) * n_pairs * N, ctx->stream), "zero signatures");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * n_pairs, ctx->stream), "zero accumulators");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
+    const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
+    TRY_CUDA(ctx, srp_launch_trace(a, brute, true, ctx->num_sms, ctx->stream), "trace launch");
+    return SRP_OK;
+}
+
 srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out)
 {
     if (!ctx) return SRP_ERR_INVALID;

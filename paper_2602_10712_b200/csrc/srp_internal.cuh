@@ -87,6 +87,7 @@ struct TraceArgs {
     unsigned long long *work_counter;
     long long tiles_per_pair;
     int tile_rays;
+    unsigned long long *sig_out;   // debug (instrumented kernels): [n_pairs, N] path signatures, or nullptr
 };
 
 // ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----

@@ -250,15 +250,24 @@ __device__ __forceinline__ bool shade(const float4 q0, const float4 q1, const fl
         float sn, cs;
         sincospif(2.0f * z1, &sn, &cs);
         const float rho = sqrtf(z2), lz = sqrtf(1.0f - z2);
-        float3 tu, tv;
-        basis3(nf, tu, tv);
+        // tangent frame (R18): first edge of the facet and nf x edge (no discontinuity in nf)
+        const float ie = rsqrtf(q1.x * q1.x + q1.y * q1.y + q1.z * q1.z);
+        const float3 tu = f3(q1.x * ie, q1.y * ie, q1.z * ie);
+        const float3 tv = cross3(nf, tu);
         const float lx = rho * cs, ly = rho * sn;
         dn = f3(fmaf(lx, tu.x, fmaf(ly, tv.x, lz * nf.x)), fmaf(lx, tu.y, fmaf(ly, tv.y, lz * nf.y)),
                 fmaf(lx, tu.z, fmaf(ly, tv.z, lz * nf.z)));
     }
     if (deposit == 1) { acc.x += d.x - dn.x; acc.y += d.y - dn.y; acc.z += d.z - dn.z; }
     if (depth == B) { cn.capped++; return false; }               // R5: B reflections followed
-    o = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
+    // Hit point in fp32 is off the facet's plane by a few ulp of |x| + t (micrometres here).  An origin
+    // that ends up BELOW the plane lets the outgoing ray hit a coplanar or convex neighbour from
+    // behind -- a path the exact arithmetic of the definition never takes.  Lift the origin along the
+    // facing normal by more than that error (R10: "exclude the source triangle, t > 0, no
+    // epsilon" is the definition; this is the fp32 guard that keeps the CUDA path on it).
+    const float3 x = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
+    const float lift = 1.0e-6f * (fabsf(x.x) + fabsf(x.y) + fabsf(x.z) + t);
+    o = f3(fmaf(lift, nf.x, x.x), fmaf(lift, nf.y, x.y), fmaf(lift, nf.z, x.z));
     d = dn; src = f; depth += 1;
     return true;
 }
@@ -317,6 +326,7 @@ trace_kernel(const TraceArgs a)
 
         bool alive = false;
         uint32_t i = 0;
+        unsigned long long sig = 0;                         // debug: hash of the hit-triangle sequence
         float3 o = f3(0, 0, 0), d = em.s, acc = f3(0, 0, 0);
         int src = -1, depth = 0;
         for (;;) {
@@ -327,6 +337,7 @@ trace_kernel(const TraceArgs a)
                 if (!alive && mine < end) {
                     i = mine; make_ray(em, g, i, o); d = em.s; src = -1; depth = 0; alive = true;
                     cn.launched++;
+                    if (INSTR) sig = 0;
                 }
                 const uint32_t room = end - next, want = __popc(need);
                 next += want < room ? want : room;
@@ -347,8 +358,10 @@ trace_kernel(const TraceArgs a)
                 } else {
                     atomicAdd(&s_hist[warp][depth], 1u);
                     const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
+                    if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
                     alive = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, cn);
                 }
+                if (INSTR && !alive && a.sig_out) a.sig_out[p * a.N + i] = sig;
             }
         }
         // S7: warp reduction in fp64, then one fixed-point atomic per component

@@ -59,3 +59,53 @@ def rel_l2(a, b):
     a = np.asarray(a, float)
     b = np.asarray(b, float)
     return np.linalg.norm(a - b, axis=-1) / np.linalg.norm(b, axis=-1)
+
+
+def oracle_pairs(oracle, meshes, pairs, sun, N, B, seed=0, workers=None, **kw):
+    """Oracle forces for a list of (design k, direction j) pairs, one oracle call per pair, spread
+    over host threads (the oracle itself is single-threaded; ctypes releases the GIL).
+    meshes: dict k -> (verts, mats).  Returns (F f64[n,3], sigma f64[n], summed stats dict)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+
+    def one(kj):
+        k, j = int(kj[0]), int(kj[1])
+        v, m = meshes[k]
+        return oracle.forces(v, m, sun[j:j + 1], N, B, seed=seed, k=k, j0=j, **kw)
+
+    with ThreadPoolExecutor(workers or min(32, os.cpu_count() or 1)) as ex:
+        res = list(ex.map(one, pairs))
+    F = np.stack([r["F"][0] for r in res])
+    sig = np.array([r["sigma"][0] for r in res])
+    tot = None
+    for r in res:
+        s = r["stats"]
+        if tot is None:
+            tot = {a: (list(b) if isinstance(b, list) else b) for a, b in s.items()}
+        else:
+            for a, b in s.items():
+                tot[a] = [x + y for x, y in zip(tot[a], b)] if isinstance(b, list) else tot[a] + b
+    if kw.get("want_path_sig"):
+        return F, sig, tot, np.stack([r["path_sig"][0] for r in res])
+    return F, sig, tot
+
+
+def assert_parity(F_gpu, F_orc, sigma, tol_vec=1e-4, tol_agg=1e-3, diverged=None):
+    """BASELINE.json acceptance: per-vector relative L2 <= 1e-4 where no ray diverged; vectors above
+    that (a ray took another path at a grazing edge) must lie within 4 sigma, and the aggregate
+    relative L2 over all vectors must be <= 1e-3.  `diverged` (bool per vector, from the path
+    signatures) makes the first clause exact: a vector with no divergent ray MUST be within 1e-4.
+    Returns the number of vectors above 1e-4."""
+    F_gpu = np.asarray(F_gpu, float).reshape(-1, 3)
+    F_orc = np.asarray(F_orc, float).reshape(-1, 3)
+    sigma = np.asarray(sigma, float).reshape(-1)
+    err = np.linalg.norm(F_gpu - F_orc, axis=1)
+    nrm = np.linalg.norm(F_orc, axis=1)
+    ok = err <= tol_vec * nrm + 1e-30
+    bad = ~ok
+    if diverged is not None:
+        assert not np.any(bad & ~np.asarray(diverged, bool)), "vector off by > 1e-4 although no ray diverged"
+    assert np.all(err[bad] <= 4.0 * sigma[bad] + 1e-30), "vector beyond 1e-4 AND beyond 4 sigma: %s" % err[bad]
+    agg = np.linalg.norm(F_gpu - F_orc) / np.linalg.norm(F_orc)
+    assert agg <= tol_agg, agg
+    return int(bad.sum())
