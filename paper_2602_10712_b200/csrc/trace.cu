@@ -17,7 +17,7 @@ namespace {
 
 constexpr int TRACE_THREADS = 128;
 constexpr int TRACE_WARPS = TRACE_THREADS / 32;
-constexpr int STACK_SMEM = 24;       // traversal stack entries per thread kept in shared memory
+constexpr int STACK_SMEM = 20;       // traversal stack entries per thread kept in shared memory
 constexpr int STACK_OVF = 80;        // deeper entries spill to local memory (degenerate trees only)
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -157,8 +157,20 @@ __device__ __forceinline__ float safe_rcp(float x)
     return 1.0f / (fabsf(x) < 1e-30f ? copysignf(1e-30f, x) : x);
 }
 
-// Stack-based BVH2 descent, nearer child first.  Stack: STACK_SMEM entries per thread in shared
-// memory (thread-interleaved, conflict-free), deeper levels in a local array.
+// Stack-based BVH2 descent, nearer child first, in "while-while" form: a lane stays in the node
+// loop until it lands on a leaf (or runs out of nodes); the warp reconverges after the node loop, so
+// the triangle tests of all lanes that hold a leaf run together (in the single-loop form they ran
+// with ~4 of 32 lanes active and took a third of the issue slots -- profiles/ round 1).
+// Stack: STACK_SMEM entries per thread in shared memory (thread-interleaved, conflict-free), deeper
+// levels in a local array.
+constexpr int CUR_DONE = 0x7fffffff;
+
+#define SRP_POP(cur_)                                                                     \
+    do {                                                                                  \
+        if (sp == 0) cur_ = CUR_DONE;                                                     \
+        else { --sp; cur_ = sp < STACK_SMEM ? s_stack[sp * TRACE_THREADS] : ovf[sp - STACK_SMEM]; } \
+    } while (0)
+
 template <bool INSTR>
 __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, const float4 *__restrict__ tri,
                                             const float3 o, const float3 d, const int src, float &tbest,
@@ -169,8 +181,8 @@ __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, co
     int ovf[STACK_OVF];
     int sp = 0;
     int cur = 0;
-    for (;;) {
-        if (cur >= 0) {
+    while (cur != CUR_DONE) {
+        while ((unsigned)cur < (unsigned)CUR_DONE) {                 // internal nodes
             const float4 n0 = __ldg(nodes + 4 * cur), n1 = __ldg(nodes + 4 * cur + 1),
                          n2 = __ldg(nodes + 4 * cur + 2), n3 = __ldg(nodes + 4 * cur + 3);
             if (INSTR) n_box += 2;
@@ -191,11 +203,11 @@ __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, co
                 if (sp < STACK_SMEM) s_stack[sp * TRACE_THREADS] = l1; else ovf[sp - STACK_SMEM] = l1;
                 ++sp;
                 cur = l0;
-                continue;
-            }
-            if (h0) { cur = l0; continue; }
-            if (h1) { cur = l1; continue; }
-        } else {
+            } else if (h0) cur = l0;
+            else if (h1) cur = l1;
+            else SRP_POP(cur);
+        }
+        if (cur < 0) {                                               // leaf: all lanes that hold one, together
             const unsigned u = (unsigned)~cur;
             const int first = (int)(u >> 3), cnt = (int)(u & 7u) + 1;
             for (int f = first; f < first + cnt; ++f) {
@@ -203,10 +215,8 @@ __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, co
                 tri_test(__ldg(tri + 3 * f), __ldg(tri + 3 * f + 1), __ldg(tri + 3 * f + 2), o, d, f, tbest, best);
             }
             if (INSTR) n_tri += (unsigned)cnt;
+            SRP_POP(cur);
         }
-        if (sp == 0) break;
-        --sp;
-        cur = sp < STACK_SMEM ? s_stack[sp * TRACE_THREADS] : ovf[sp - STACK_SMEM];
     }
 }
 
@@ -214,11 +224,13 @@ struct LaneCounters {
     unsigned launched, pmiss, absorbed, escaped, capped, segments, n_box, n_tri;
 };
 
-// O-steps 5-7 at a hit: deposit, lobe selection, continuation.  Returns true if the photon goes on.
-__device__ __forceinline__ bool shade(const float4 q0, const float4 q1, const float4 q2, const float t,
+// O-steps 5-7 at a hit: deposit, lobe selection, continuation.
+// Returns SHADE_CONTINUE if the photon goes on (o, d, src, depth updated), else how it ended.
+enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2 };
+__device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
                                       const int deposit, float3 &o, float3 &d, int &src, int &depth,
-                                      float3 &acc, LaneCounters &cn)
+                                      float3 &acc)
 {
     (void)q0;
     const float al = q0.w, rs = q1.w, rd = q2.w;
@@ -241,8 +253,7 @@ __device__ __forceinline__ bool shade(const float4 q0, const float4 q1, const fl
     float3 dn;
     if (z0 < al) {                                                // absorbed
         if (deposit == 1) { acc.x += d.x; acc.y += d.y; acc.z += d.z; }
-        cn.absorbed++;
-        return false;
+        return SHADE_ABSORBED;
     } else if (z0 < al + rs) {                                    // ideal mirror (R3)
         dn = refl;
     } else {                                                      // Lambertian: cosine-weighted about nf
@@ -259,7 +270,7 @@ __device__ __forceinline__ bool shade(const float4 q0, const float4 q1, const fl
                 fmaf(lx, tu.z, fmaf(ly, tv.z, lz * nf.z)));
     }
     if (deposit == 1) { acc.x += d.x - dn.x; acc.y += d.y - dn.y; acc.z += d.z - dn.z; }
-    if (depth == B) { cn.capped++; return false; }               // R5: B reflections followed
+    if (depth == B) return SHADE_CAPPED;                         // R5: B reflections followed
     // Hit point in fp32 is off the facet's plane by a few ulp of |x| + t (micrometres here).  An origin
     // that ends up BELOW the plane lets the outgoing ray hit a coplanar or convex neighbour from
     // behind -- a path the exact arithmetic of the definition never takes.  Lift the origin along the
@@ -269,7 +280,7 @@ __device__ __forceinline__ bool shade(const float4 q0, const float4 q1, const fl
     const float lift = 1.0e-6f * (fabsf(x.x) + fabsf(x.y) + fabsf(x.z) + t);
     o = f3(fmaf(lift, nf.x, x.x), fmaf(lift, nf.y, x.y), fmaf(lift, nf.z, x.z));
     d = dn; src = f; depth += 1;
-    return true;
+    return SHADE_CONTINUE;
 }
 
 __device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k, int &j)
@@ -359,7 +370,10 @@ trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    alive = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, cn);
+                    const int fate = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc);
+                    if (fate == SHADE_ABSORBED) cn.absorbed++;
+                    if (fate == SHADE_CAPPED) cn.capped++;
+                    alive = fate == SHADE_CONTINUE;
                 }
                 if (INSTR && !alive && a.sig_out) a.sig_out[p * a.N + i] = sig;
             }
@@ -510,12 +524,11 @@ cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops
 }
 
 // ---- launchers ----
-template <int MODE, bool INSTR>
-static cudaError_t launch_trace_t(const TraceArgs &a, int num_sms, cudaStream_t stream)
+template <typename K>
+static cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStream_t stream)
 {
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE, INSTR>,
-                                                                  TRACE_THREADS, 0);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
@@ -523,7 +536,7 @@ static cudaError_t launch_trace_t(const TraceArgs &a, int num_sms, cudaStream_t 
     const unsigned long long needed = (total_tiles + TRACE_WARPS - 1) / TRACE_WARPS;
     if (blocks > needed) blocks = needed;
     if (blocks < 1) blocks = 1;
-    trace_kernel<MODE, INSTR><<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a);
+    kernel<<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -539,13 +552,13 @@ cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, 
 {
     if (brute) {
         if (a.dz.has_bvh)       // forced brute force over a design that also has a hierarchy (test use)
-            return instrumented ? launch_trace_t<MODE_BRUTE_GLOBAL, true>(a, num_sms, stream)
-                                : launch_trace_t<MODE_BRUTE_GLOBAL, false>(a, num_sms, stream);
-        return instrumented ? launch_trace_t<MODE_BRUTE_SMEM, true>(a, num_sms, stream)
-                            : launch_trace_t<MODE_BRUTE_SMEM, false>(a, num_sms, stream);
+            return instrumented ? launch_persistent(trace_kernel<MODE_BRUTE_GLOBAL, true>, a, num_sms, stream)
+                                : launch_persistent(trace_kernel<MODE_BRUTE_GLOBAL, false>, a, num_sms, stream);
+        return instrumented ? launch_persistent(trace_kernel<MODE_BRUTE_SMEM, true>, a, num_sms, stream)
+                            : launch_persistent(trace_kernel<MODE_BRUTE_SMEM, false>, a, num_sms, stream);
     }
-    return instrumented ? launch_trace_t<MODE_BVH, true>(a, num_sms, stream)
-                        : launch_trace_t<MODE_BVH, false>(a, num_sms, stream);
+    return instrumented ? launch_persistent(trace_kernel<MODE_BVH, true>, a, num_sms, stream)
+                        : launch_persistent(trace_kernel<MODE_BVH, false>, a, num_sms, stream);
 }
 
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, cudaStream_t stream)
