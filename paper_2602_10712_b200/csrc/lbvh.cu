@@ -78,11 +78,13 @@ morton_kernel(const float *verts, const long long *off, int D, long long sumT, c
     const float *v = verts + g * 9;
     float c[3], l[3] = { lo.x, lo.y, lo.z }, h[3] = { hi.x, hi.y, hi.z };
     unsigned q[3];
+    // one scale for all axes (cubic cells): an elongated design (19 m of wings, 1.6 m wide) is then
+    // split along its long axis first instead of alternating x, y, z halves of a flat box
+    const float ext = fmaxf(h[0] - l[0], fmaxf(h[1] - l[1], h[2] - l[2]));
+    const float s = ext > 0.f ? 65535.0f / ext : 0.f;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         c[a] = (v[a] + v[3 + a] + v[6 + a]) * (1.0f / 3.0f);
-        float ext = h[a] - l[a];
-        float s = ext > 0.f ? 65535.0f / ext : 0.f;
         q[a] = (unsigned)fminf(fmaxf((c[a] - l[a]) * s, 0.f), 65535.f);
     }
     u64 code = (spread16(q[0]) << 2) | (spread16(q[1]) << 1) | spread16(q[2]);

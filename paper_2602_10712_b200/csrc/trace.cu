@@ -289,6 +289,24 @@ __device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k,
     else { k = (int)(p / a.S); j = (int)(p - (long long)k * a.S); }
 }
 
+// counters: warp sums, one global atomic each
+template <bool INSTR>
+__device__ __forceinline__ void flush_counters(const TraceArgs &a, const LaneCounters &cn, const unsigned *hist, int lane)
+{
+    unsigned long long *st = (unsigned long long *)a.stats;
+    const unsigned vals[8] = { cn.launched, cn.pmiss, cn.absorbed, cn.escaped, cn.capped, cn.segments, cn.n_box, cn.n_tri };
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        if (!INSTR && c >= 6) break;
+        unsigned long long v = vals[c];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+        if (lane == 0 && v) atomicAdd(st + (c < 6 ? c : 22 + (c - 6)), v);
+    }
+    __syncwarp();
+    if (lane < 16 && hist[lane]) atomicAdd(st + 6 + lane, (unsigned long long)hist[lane]);
+}
+
 // ---- the persistent trace kernel ----
 template <int MODE, bool INSTR>
 __global__ void __launch_bounds__(TRACE_THREADS, MODE == MODE_BVH ? 4 : 5)
@@ -393,19 +411,129 @@ trace_kernel(const TraceArgs a)
             atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
         }
     }
-    // counters: warp sums, one global atomic each
-    unsigned long long *st = (unsigned long long *)a.stats;
-    const unsigned vals[8] = { cn.launched, cn.pmiss, cn.absorbed, cn.escaped, cn.capped, cn.segments, cn.n_box, cn.n_tri };
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        if (!INSTR && c >= 6) break;
-        unsigned long long v = vals[c];
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
-        if (lane == 0 && v) atomicAdd(st + (c < 6 ? c : 22 + (c - 6)), v);
-    }
+    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
+}
+
+// ---- the BVH trace kernel: persistent warps with a per-warp queue of bounce rays ----
+// A warp traces 32 rays of ONE kind per pass: either 32 fresh primaries of its tile (parallel, in
+// Morton order, so they walk the same part of the tree) or 32 queued secondary rays (incoherent, and
+// mostly gone after a few nodes).  Photons that survive shading are pushed to the warp's queue in
+// shared memory (ballot + prefix popcount, so the order is deterministic) and popped 32 at a time.
+// Mixing the two kinds in one pass left the short secondaries waiting for the long primaries
+// (14 of 32 lanes active, profiles/ round 1); this is S6's "compaction between bounces".
+constexpr int QCAP = 64;
+struct WarpQueue {
+    float ox[QCAP], oy[QCAP], oz[QCAP], dx[QCAP], dy[QCAP], dz[QCAP];
+    uint32_t i[QCAP];
+    int src_depth[QCAP];                 // (depth << 27) | src
+};
+
+template <bool INSTR>
+__global__ void __launch_bounds__(TRACE_THREADS, 5)
+bvh_trace_kernel(const TraceArgs a)
+{
+    __shared__ int s_stack[STACK_SMEM * TRACE_THREADS];
+    __shared__ WarpQueue s_q[TRACE_WARPS];
+    __shared__ unsigned long long s_qsig[INSTR ? TRACE_WARPS * QCAP : 1];
+    __shared__ unsigned s_hist[TRACE_WARPS][16];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    if (lane < 16) s_hist[warp][lane] = 0;
     __syncwarp();
-    if (lane < 16 && s_hist[warp][lane]) atomicAdd(st + 6 + lane, (unsigned long long)s_hist[warp][lane]);
+    WarpQueue &Q = s_q[warp];
+    unsigned long long *qsig = s_qsig + (INSTR ? warp * QCAP : 0);
+    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
+    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
+
+    for (;;) {
+        unsigned long long tile = 0;
+        if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
+        tile = __shfl_sync(FULL, tile, 0);
+        if (tile >= total_tiles) break;
+        const long long p = (long long)(tile / a.tiles_per_pair);
+        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
+        int k, j;
+        pair_of(a, p, k, j);
+        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
+        if (!(em.Ae > 0.0f)) continue;
+        const long long tbase = a.dz.tri_off[k];
+        const float4 *gtri = a.dz.tri + 3 * tbase;
+        const float4 *gnodes = a.dz.nodes + 4 * tbase;
+        RayGen g;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler;
+        g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
+        g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
+        uint32_t next = (uint32_t)(q * a.tile_rays);
+        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
+        int qcount = 0;                                   // warp-uniform
+        float3 acc = f3(0, 0, 0);
+
+        for (;;) {
+            bool alive = false;
+            uint32_t i = 0;
+            float3 o = f3(0, 0, 0), d = em.s;
+            int src = -1, depth = 0;
+            unsigned long long sig = 0;
+            if (qcount >= 32 || (next >= end && qcount > 0)) {          // a pass of secondary rays
+                const int take = qcount < 32 ? qcount : 32;
+                if (lane < take) {
+                    const int e = qcount - take + lane;
+                    o = f3(Q.ox[e], Q.oy[e], Q.oz[e]); d = f3(Q.dx[e], Q.dy[e], Q.dz[e]);
+                    i = Q.i[e]; src = Q.src_depth[e] & 0x07ffffff; depth = (int)((unsigned)Q.src_depth[e] >> 27);
+                    if (INSTR) sig = qsig[e];
+                    alive = true;
+                }
+                qcount -= take;
+            } else if (next < end) {                                     // a pass of primaries
+                const uint32_t mine = next + lane;
+                if (mine < end) { i = mine; make_ray(em, g, i, o); alive = true; cn.launched++; }
+                next = (end - next) < 32u ? end : next + 32u;
+            } else break;                                                // tile exhausted, queue empty
+            __syncwarp();
+            int fate = -1;                                               // -1: no hit / no photon
+            if (alive) {
+                float tbest = FLT_MAX; int best = -1;
+                cn.segments++;
+                closest_bvh<INSTR>(gnodes, gtri, o, d, src, tbest, best, s_stack + threadIdx.x, cn.n_box, cn.n_tri);
+                if (best < 0) {
+                    if (depth == 0) cn.pmiss++; else cn.escaped++;
+                } else {
+                    atomicAdd(&s_hist[warp][depth], 1u);
+                    if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
+                    fate = shade(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
+                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc);
+                    if (fate == SHADE_ABSORBED) cn.absorbed++;
+                    if (fate == SHADE_CAPPED) cn.capped++;
+                }
+                if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
+            }
+            const unsigned cont = __ballot_sync(FULL, fate == SHADE_CONTINUE);
+            if (fate == SHADE_CONTINUE) {
+                const int e = qcount + __popc(cont & lt_mask);
+                Q.ox[e] = o.x; Q.oy[e] = o.y; Q.oz[e] = o.z; Q.dx[e] = d.x; Q.dy[e] = d.y; Q.dz[e] = d.z;
+                Q.i[e] = i; Q.src_depth[e] = (depth << 27) | src;
+                if (INSTR) qsig[e] = sig;
+            }
+            qcount += __popc(cont);
+            __syncwarp();
+        }
+        // S7: warp reduction in fp64, then one fixed-point atomic per component
+        double sx = acc.x, sy = acc.y, sz = acc.z;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            sx += __shfl_xor_sync(FULL, sx, off);
+            sy += __shfl_xor_sync(FULL, sy, off);
+            sz += __shfl_xor_sync(FULL, sz, off);
+        }
+        if (lane == 0) {
+            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
+            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
+            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
+            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
+        }
+    }
+    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
 }
 
 // F[p] = accum[p] * 2^-32 * P * A_e / N
@@ -544,7 +672,7 @@ int srp_trace_blocks_per_sm(bool brute)
 {
     int per_sm = 0;
     if (brute) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BRUTE_SMEM, false>, TRACE_THREADS, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BVH, false>, TRACE_THREADS, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bvh_trace_kernel<false>, TRACE_THREADS, 0);
     return per_sm * TRACE_WARPS;
 }
 
@@ -557,8 +685,8 @@ cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, 
         return instrumented ? launch_persistent(trace_kernel<MODE_BRUTE_SMEM, true>, a, num_sms, stream)
                             : launch_persistent(trace_kernel<MODE_BRUTE_SMEM, false>, a, num_sms, stream);
     }
-    return instrumented ? launch_persistent(trace_kernel<MODE_BVH, true>, a, num_sms, stream)
-                        : launch_persistent(trace_kernel<MODE_BVH, false>, a, num_sms, stream);
+    return instrumented ? launch_persistent(bvh_trace_kernel<true>, a, num_sms, stream)
+                        : launch_persistent(bvh_trace_kernel<false>, a, num_sms, stream);
 }
 
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, cudaStream_t stream)
