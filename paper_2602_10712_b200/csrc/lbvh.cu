@@ -9,6 +9,7 @@
 // hierarchy: the tracer tests all their triangles (the paper's own method).
 #include <cub/device/device_radix_sort.cuh>
 #include <cfloat>
+#include <cstdlib>
 #include "srp_internal.cuh"
 
 namespace {
@@ -204,7 +205,7 @@ refit_kernel(const float4 *tri, const long long *off, int D, long long sumT, con
 __global__ void __launch_bounds__(256)
 emit_kernel(const unsigned long long *keys_all, const long long *off, long long sumT, const int *left,
             const int *right, const int *range_first, const int *range_count, const float4 *lbox,
-            const float4 *nbox, float4 *nodes)
+            const float4 *nbox, float4 *nodes, int leaf_max)
 {
     long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= sumT) return;
@@ -230,7 +231,7 @@ emit_kernel(const unsigned long long *keys_all, const long long *off, long long 
             } else {
                 lo[side] = nbox[2 * (base + c)]; hi[side] = nbox[2 * (base + c) + 1];
                 const int cnt = range_count[base + c];
-                link[side] = cnt <= SRP_LEAF_MAX ? ~((range_first[base + c] << 3) | (cnt - 1)) : c;
+                link[side] = cnt <= leaf_max ? ~((range_first[base + c] << 3) | (cnt - 1)) : c;
             }
         }
     }
@@ -286,8 +287,10 @@ cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream)
                                                  pleaf, rfirst, rcount);
     refit_kernel<<<blocks, 256, 0, stream>>>(dz->tri, dz->tri_off_dev, D, sumT, left, right, pnode, pleaf,
                                              flags, lbox, nbox);
+    int leaf_max = SRP_LEAF_MAX;
+    if (const char *e = getenv("SRP_LEAF_MAX")) { int v = atoi(e); if (v >= 1 && v <= 8) leaf_max = v; }   // tuning aid
     emit_kernel<<<blocks, 256, 0, stream>>>(keys_out, dz->tri_off_dev, sumT, left, right, rfirst, rcount,
-                                            lbox, nbox, dz->nodes);
+                                            lbox, nbox, dz->nodes, leaf_max);
     cudaError_t e = cudaGetLastError();
     cudaFreeAsync(keys, stream); cudaFreeAsync(keys_out, stream); cudaFreeAsync(vals, stream);
     cudaFreeAsync(vals_out, stream); cudaFreeAsync(ibuf, stream); cudaFreeAsync(lbox, stream);

@@ -9,7 +9,7 @@
 #include "srp.h"
 
 #define SRP_BRUTE_MAX_TRIS 64      // designs with T <= this are traced without a hierarchy (one leaf)
-#define SRP_LEAF_MAX 4             // LBVH subtrees with <= this many triangles become one leaf
+#define SRP_LEAF_MAX 3             // LBVH subtrees with <= this many triangles become one leaf
 #define SRP_ACC_SCALE 4294967296.0 // fixed-point scale (2^32) of the dimensionless force accumulators
 
 // Packed, BVH-sorted triangle: 3 x float4 = 48 B, fetched as three 16-byte loads.

@@ -429,7 +429,7 @@ struct WarpQueue {
 };
 
 template <bool INSTR>
-__global__ void __launch_bounds__(TRACE_THREADS, 5)
+__global__ void __launch_bounds__(TRACE_THREADS, 8)
 bvh_trace_kernel(const TraceArgs a)
 {
     __shared__ int s_stack[STACK_SMEM * TRACE_THREADS];
