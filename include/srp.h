@@ -61,6 +61,10 @@ typedef struct {
     int deposit;            /* 0 = expected-value deposit (default), 1 = analog (sampled path only) */
     int force_brute;        /* 1 = ignore the BVH and test every triangle; test use   */
     int instrumented;       /* 1 = also count ray-box and ray-triangle tests (slower kernels)        */
+    int primary_mode;       /* how the primaries of designs with a BVH are traced (stratified sampler):
+                               0 = auto: as beams (blocks of rays share one BVH descent) when
+                                   rays_per_dir >= 8 x the largest design's triangle count, else one by one,
+                               1 = every primary walks the BVH on its own, 2 = beams always; test use   */
 } srp_options;
 
 /* Photon bookkeeping of the last srp_forces call (DESIGN.md "Pins" P8).
@@ -70,6 +74,9 @@ typedef struct {
     unsigned long long launched, primary_miss, absorbed, escaped, capped, segments;
     unsigned long long hits_at_depth[16];
     unsigned long long box_tests, tri_tests;
+    /* beam tracing of primaries: rays resolved as misses by a whole tile / sub-block / group of 32,
+       and primaries that fell back to per-ray traversal because a beam list overflowed */
+    unsigned long long beam_tile_miss, beam_block_miss, beam_group_miss, beam_fallback;
 } srp_stats;
 
 /* Creates a context on CUDA device `cuda_device`; `cuda_stream` is a cudaStream_t (may be NULL =

@@ -61,6 +61,37 @@ srp_status ensure_workspace(srp_context *ctx, size_t accum_items)
     return SRP_OK;
 }
 
+// Beam tracing of the primaries (trace.cu, beam_trace_kernel) pays when many rays share a triangle: a
+// beam's candidate list is then short and serves many rays.  With about one ray per triangle (the
+// 1M-triangle sail at N = 2^20) every beam overflows its lists, so primaries walk the BVH one by one.
+bool want_beams(const srp_context *ctx, bool brute, long long max_tris, long long N, long long n_pairs)
+{
+    if (brute || ctx->opt.sampler != 0 || n_pairs >= (1LL << 32)) return false;   // pool entries hold p in 32 bits
+    if (ctx->opt.primary_mode == 1) return false;
+    if (ctx->opt.primary_mode == 2) return true;
+    return N >= 8 * max_tris;
+}
+
+// The beam kernel's per-warp ray pools; grown on demand.
+srp_status ensure_pool(srp_context *ctx, TraceArgs &a, bool brute, bool instrumented)
+{
+    a.pool = nullptr; a.pool_cap = 0;
+    if (!want_beams(ctx, brute, a.max_tris, a.N, a.n_pairs)) return SRP_OK;
+    int cap = 0;
+    const size_t words = srp_beam_pool_words(ctx->num_sms, instrumented, a.tile_rays, &cap);
+    if (ctx->pool_words < words) {
+        TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before pool growth");
+        cudaFree(ctx->pool); ctx->pool = nullptr; ctx->pool_words = 0;
+        if (cudaMalloc(&ctx->pool, sizeof(unsigned) * words) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(ctx, SRP_ERR_OOM, "ray pool allocation failed");
+        }
+        ctx->pool_words = words;
+    }
+    a.pool = ctx->pool; a.pool_cap = cap;
+    return SRP_OK;
+}
+
 srp_status check_trace_args(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S,
                             long long N, int B, const void *out)
 {
@@ -89,7 +120,9 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     // tile size: large tiles amortise the per-item set-up and the drain at the end of a tile; shrink
     // them only when there would be too few items to occupy every resident warp several times
     const bool brute = !dz->has_bvh;
-    const long long warps = (long long)ctx->num_sms * srp_trace_blocks_per_sm(brute);
+    a.max_tris = dz->maxT;
+    const bool beam = want_beams(ctx, brute || ctx->opt.force_brute != 0, a.max_tris, N, n_pairs);
+    const long long warps = (long long)ctx->num_sms * srp_trace_blocks_per_sm(brute, beam);
     long long tile = 8192;
     if (tile > N) tile = N;
     while (tile > 256 && n_pairs * ((N + tile - 1) / tile) < 8 * warps) tile >>= 1;
@@ -108,6 +141,8 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
+    st = ensure_pool(ctx, a, brute, ctx->opt.instrumented != 0);
+    if (st != SRP_OK) return st;
     TRY_CUDA(ctx, srp_launch_trace(a, brute, ctx->opt.instrumented != 0, ctx->num_sms, ctx->stream), "trace launch");
     TRY_CUDA(ctx, srp_launch_finalize(a, out, ctx->stream), "finalize launch");
     return SRP_OK;
@@ -130,7 +165,7 @@ srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
     ctx->device = cuda_device;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt.solar_pressure = 4.56e-6; ctx->opt.sampler = 0; ctx->opt.deposit = 0;
-    ctx->opt.force_brute = 0; ctx->opt.instrumented = 0;
+    ctx->opt.force_brute = 0; ctx->opt.instrumented = 0; ctx->opt.primary_mode = 0;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
     *out = ctx;
@@ -142,7 +177,7 @@ srp_status srp_destroy(srp_context *ctx)
     if (!ctx) return SRP_ERR_INVALID;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter);
+    cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->pool);
     cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);
     delete ctx;
     return SRP_OK;
@@ -152,7 +187,8 @@ srp_status srp_set_options(srp_context *ctx, const srp_options *opt)
 {
     if (!ctx) return SRP_ERR_INVALID;
     if (!opt) return fail(ctx, SRP_ERR_INVALID, "null options");
-    if (!(opt->solar_pressure > 0.0) || opt->sampler < 0 || opt->sampler > 1 || opt->deposit < 0 || opt->deposit > 1)
+    if (!(opt->solar_pressure > 0.0) || opt->sampler < 0 || opt->sampler > 1 || opt->deposit < 0 || opt->deposit > 1 ||
+        opt->primary_mode < 0 || opt->primary_mode > 2)
         return fail(ctx, SRP_ERR_INVALID, "option out of range");
     ctx->opt = *opt;
     return SRP_OK;
@@ -363,6 +399,8 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const fl
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
+    st = ensure_pool(ctx, a, brute, true);
+    if (st != SRP_OK) return st;
     TRY_CUDA(ctx, srp_launch_trace(a, brute, true, ctx->num_sms, ctx->stream), "trace launch");
     return SRP_OK;
 }

@@ -54,6 +54,7 @@ struct DevStats {           // device mirror of srp_stats
     unsigned long long launched, primary_miss, absorbed, escaped, capped, segments;
     unsigned long long hits_at_depth[16];
     unsigned long long box_tests, tri_tests;
+    unsigned long long beam_tile_miss, beam_block_miss, beam_group_miss, beam_fallback;
 };
 
 struct srp_context {
@@ -66,6 +67,7 @@ struct srp_context {
     long long *accum = nullptr;   size_t accum_items = 0;     // int64 fixed-point [pairs*3]
     DevStats *stats = nullptr;
     unsigned long long *work_counter = nullptr;
+    unsigned *pool = nullptr;     size_t pool_words = 0;      // beam kernel's ray pools
     float *stage_dirs = nullptr;  size_t stage_dirs_items = 0; // srp_forces_host staging
     float *stage_out = nullptr;   size_t stage_out_items = 0;
 };
@@ -88,6 +90,9 @@ struct TraceArgs {
     long long tiles_per_pair;
     int tile_rays;
     unsigned long long *sig_out;   // debug (instrumented kernels): [n_pairs, N] path signatures, or nullptr
+    unsigned *pool;                // beam kernel: per-warp ray pools (srp_beam_pool_words), or nullptr
+    int pool_cap;                  // rays per pool (a power of two)
+    long long max_tris;            // largest design of the batch
 };
 
 // ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----
@@ -102,4 +107,5 @@ cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim,
 cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
 
 long long srp_family_tris_host(int family);
-int srp_trace_blocks_per_sm(bool brute);
+int srp_trace_blocks_per_sm(bool brute, bool beam);
+size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *cap_out);

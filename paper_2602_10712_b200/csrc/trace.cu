@@ -168,10 +168,66 @@ constexpr int CUR_DONE = 0x7fffffff;
 #define SRP_POP(cur_)                                                                     \
     do {                                                                                  \
         if (sp == 0) cur_ = CUR_DONE;                                                     \
-        else { --sp; cur_ = sp < STACK_SMEM ? s_stack[sp * TRACE_THREADS] : ovf[sp - STACK_SMEM]; } \
+        else { --sp; cur_ = sp < NSMEM ? s_stack[sp * STRIDE] : ovf[sp - NSMEM]; }        \
     } while (0)
 
-template <bool INSTR>
+// STRIDE: distance in ints between consecutive stack entries of one thread (thread-interleaved
+// layout); NSMEM: entries kept in shared memory.
+// One internal node for one lane: both child boxes against the ray, nearer child next, farther child
+// pushed.  Returns the next value of `cur` (node index, leaf link < 0, or CUR_DONE).
+template <int STRIDE, int NSMEM>
+__device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, int cur, int &sp, int *s_stack, int *ovf,
+                                             float idx, float idy, float idz, float oxi, float oyi, float ozi, float tbest)
+{
+    const float4 n0 = __ldg(nodes + 4 * cur), n1 = __ldg(nodes + 4 * cur + 1),
+                 n2 = __ldg(nodes + 4 * cur + 2), n3 = __ldg(nodes + 4 * cur + 3);
+    float a0 = fmaf(n0.x, idx, -oxi), a1 = fmaf(n0.w, idx, -oxi);
+    float b0 = fmaf(n0.y, idy, -oyi), b1 = fmaf(n1.x, idy, -oyi);
+    float c0 = fmaf(n0.z, idz, -ozi), c1 = fmaf(n1.y, idz, -ozi);
+    const float tmin0 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
+    const float tmax0 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
+    a0 = fmaf(n1.z, idx, -oxi); a1 = fmaf(n2.y, idx, -oxi);
+    b0 = fmaf(n1.w, idy, -oyi); b1 = fmaf(n2.z, idy, -oyi);
+    c0 = fmaf(n2.x, idz, -ozi); c1 = fmaf(n2.w, idz, -ozi);
+    const float tmin1 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
+    const float tmax1 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
+    const bool h0 = tmin0 <= tmax0 * 1.0000004f, h1 = tmin1 <= tmax1 * 1.0000004f;
+    int l0 = __float_as_int(n3.x), l1 = __float_as_int(n3.y);
+    if (h0 && h1) {
+        if (tmin1 < tmin0) { const int t = l0; l0 = l1; l1 = t; }
+        if (sp < NSMEM) s_stack[sp * STRIDE] = l1; else ovf[sp - NSMEM] = l1;
+        ++sp;
+#ifdef SRP_PREFETCH_PUSH
+        if (l1 >= 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(nodes + 4 * l1));
+#endif
+        return l0;
+    }
+    if (h0) return l0;
+    if (h1) return l1;
+    SRP_POP(cur);
+    return cur;
+}
+
+// One leaf for one lane: its triangles (source excluded, R10), then the next stack entry.
+template <int STRIDE, int NSMEM>
+__device__ __forceinline__ int bvh_leaf_step(const float4 *__restrict__ tri, int cur, int &sp, int *s_stack, int *ovf,
+                                             const float3 o, const float3 d, const int src, float &tbest, int &best,
+                                             unsigned &n_tri)
+{
+    const unsigned u = (unsigned)~cur;
+    const int first = (int)(u >> 3), cnt = (int)(u & 7u) + 1;
+    for (int f = first; f < first + cnt; ++f) {
+        if (f == src) continue;
+        tri_test(__ldg(tri + 3 * f), __ldg(tri + 3 * f + 1), __ldg(tri + 3 * f + 2), o, d, f, tbest, best);
+    }
+    n_tri += (unsigned)cnt;
+    SRP_POP(cur);
+    return cur;
+}
+
+// STRIDE: distance in ints between consecutive stack entries of one thread (thread-interleaved
+// layout); NSMEM: entries kept in shared memory.
+template <bool INSTR, int STRIDE = TRACE_THREADS, int NSMEM = STACK_SMEM>
 __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, const float4 *__restrict__ tri,
                                             const float3 o, const float3 d, const int src, float &tbest,
                                             int &best, int *s_stack, unsigned &n_box, unsigned &n_tri)
@@ -181,47 +237,23 @@ __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, co
     int ovf[STACK_OVF];
     int sp = 0;
     int cur = 0;
+    unsigned nt = 0;
     while (cur != CUR_DONE) {
         while ((unsigned)cur < (unsigned)CUR_DONE) {                 // internal nodes
-            const float4 n0 = __ldg(nodes + 4 * cur), n1 = __ldg(nodes + 4 * cur + 1),
-                         n2 = __ldg(nodes + 4 * cur + 2), n3 = __ldg(nodes + 4 * cur + 3);
             if (INSTR) n_box += 2;
-            float a0 = fmaf(n0.x, idx, -oxi), a1 = fmaf(n0.w, idx, -oxi);
-            float b0 = fmaf(n0.y, idy, -oyi), b1 = fmaf(n1.x, idy, -oyi);
-            float c0 = fmaf(n0.z, idz, -ozi), c1 = fmaf(n1.y, idz, -ozi);
-            const float tmin0 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
-            const float tmax0 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
-            a0 = fmaf(n1.z, idx, -oxi); a1 = fmaf(n2.y, idx, -oxi);
-            b0 = fmaf(n1.w, idy, -oyi); b1 = fmaf(n2.z, idy, -oyi);
-            c0 = fmaf(n2.x, idz, -ozi); c1 = fmaf(n2.w, idz, -ozi);
-            const float tmin1 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
-            const float tmax1 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
-            const bool h0 = tmin0 <= tmax0 * 1.0000004f, h1 = tmin1 <= tmax1 * 1.0000004f;
-            int l0 = __float_as_int(n3.x), l1 = __float_as_int(n3.y);
-            if (h0 && h1) {
-                if (tmin1 < tmin0) { const int t = l0; l0 = l1; l1 = t; }
-                if (sp < STACK_SMEM) s_stack[sp * TRACE_THREADS] = l1; else ovf[sp - STACK_SMEM] = l1;
-                ++sp;
-                cur = l0;
-            } else if (h0) cur = l0;
-            else if (h1) cur = l1;
-            else SRP_POP(cur);
+            cur = bvh_node_step<STRIDE, NSMEM>(nodes, cur, sp, s_stack, ovf, idx, idy, idz, oxi, oyi, ozi, tbest);
         }
-        if (cur < 0) {                                               // leaf: all lanes that hold one, together
-            const unsigned u = (unsigned)~cur;
-            const int first = (int)(u >> 3), cnt = (int)(u & 7u) + 1;
-            for (int f = first; f < first + cnt; ++f) {
-                if (f == src) continue;
-                tri_test(__ldg(tri + 3 * f), __ldg(tri + 3 * f + 1), __ldg(tri + 3 * f + 2), o, d, f, tbest, best);
-            }
-            if (INSTR) n_tri += (unsigned)cnt;
-            SRP_POP(cur);
-        }
+        if (cur < 0)                                                 // leaf: all lanes that hold one, together
+            cur = bvh_leaf_step<STRIDE, NSMEM>(tri, cur, sp, s_stack, ovf, o, d, src, tbest, best, nt);
     }
+    if (INSTR) n_tri += nt;
 }
 
 struct LaneCounters {
     unsigned launched, pmiss, absorbed, escaped, capped, segments, n_box, n_tri;
+};
+struct BeamCounters {       // rays resolved per beam level (lane-distributed counts)
+    unsigned tile_miss, block_miss, group_miss, fallback;
 };
 
 // O-steps 5-7 at a hit: deposit, lobe selection, continuation.
@@ -283,6 +315,12 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     return SHADE_CONTINUE;
 }
 
+// same for a pair index known to fit 32 bits (rays of the beam kernel's pool)
+__device__ __forceinline__ void pair_of32(const TraceArgs &a, uint32_t p, int &k, int &j)
+{
+    if (a.pairs) { k = a.pairs[2 * (size_t)p]; j = a.pairs[2 * (size_t)p + 1]; }
+    else { const uint32_t kk = p / (uint32_t)a.S; k = (int)kk; j = (int)(p - kk * (uint32_t)a.S); }
+}
 __device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k, int &j)
 {
     if (a.pairs) { k = a.pairs[2 * p]; j = a.pairs[2 * p + 1]; }
@@ -536,6 +574,591 @@ bvh_trace_kernel(const TraceArgs a)
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
 }
 
+// ---- the beam trace kernel: coherent primaries as beams, bounce rays one by one ----
+// The primaries of a pair are parallel and, in the stratified sampler, ray i sits in cell
+// Morton(i) of the emitter grid, so every aligned block of 2^b consecutive rays is a rectangle of
+// cells -- a BEAM with a rectangular cross-section.  A warp walks the BVH once per beam instead of
+// once per ray (BVH "packet"/beam traversal; the tree and the hit definition are unchanged):
+//   tile      (<= 8192 rays): frontier descent from the root, all lanes testing different nodes
+//             against the tile's rectangle, until the frontier holds > 32 nodes -> entry list.
+//             Nothing overlaps: the whole tile is primary misses, no ray is generated.
+//   sub-block (256 rays, 16 x 16 cells): descent from the entry list to the leaves -> candidate
+//             triangles (<= BEAM_CMAX), each set up ONCE as three 2-D edge functions and a depth
+//             plane in the emitter frame (the ray-triangle test of a ray parallel to the frame's
+//             axis: inside <=> the three edge functions are >= 0, same inclusive rule as O-step 4).
+//   group     (32 rays, 8 x 4 cells, one per lane): the candidates whose edge functions admit the
+//             group's rectangle are listed; an empty list resolves 32 misses without Philox;
+//             otherwise every lane tests ITS ray against the same short list, all 32 lanes
+//             converged, operands broadcast from shared memory.
+// Bounce rays are incoherent: they go to the warp's ray pool and through per-ray stack traversal
+// (drain(), below).  A sub-block whose lists overflow is halved; a single group that still
+// overflows (a beam along an edge-on panel, a bundle of thin facets) sends its 32 primaries to the
+// pool as well, so any input is handled.
+#ifndef BEAM_BLOCKS_PER_SM
+#define BEAM_BLOCKS_PER_SM 4
+#endif
+constexpr int BEAM_SB = 256;        // rays per sub-block
+#ifndef BEAM_CMAX_DEF
+#define BEAM_CMAX_DEF 128
+#endif
+constexpr int BEAM_CMAX = BEAM_CMAX_DEF;      // candidate triangles per sub-block
+constexpr int BEAM_QN = 160;        // node queue of the sub-block descent
+constexpr int BEAM_EN = 64;         // tile entry list: internal nodes
+constexpr int BEAM_EL = 64;         // tile entry list: leaf links
+constexpr int BEAM_STACK = 16;      // per-thread stack entries in shared memory (bounce rays)
+
+struct BeamFrame {                  // warp-uniform per pair
+    float3 uh, vh, auh, avh;        // u/2, v/2 and their absolute values
+    float csu, csv;                 // cell size along u and v
+    float margin;                   // bound of the fp32 projection error of a box
+};
+
+// Does the box's projection on the emitter plane meet the rectangle [0,wu] x [0,wv] of the local
+// frame whose origin projects to (offu, offv)?  NaN (the empty-box sentinel) compares false.
+__device__ __forceinline__ bool beam_box(const BeamFrame &f, float offu, float offv, float wu, float wv,
+                                         float lox, float loy, float loz, float hix, float hiy, float hiz)
+{
+    const float sx = lox + hix, sy = loy + hiy, sz = loz + hiz;
+    const float dx = hix - lox, dy = hiy - loy, dz = hiz - loz;
+    const float pu = fmaf(sx, f.uh.x, fmaf(sy, f.uh.y, sz * f.uh.z)) - offu;
+    const float pv = fmaf(sx, f.vh.x, fmaf(sy, f.vh.y, sz * f.vh.z)) - offv;
+    const float ru = fmaf(dx, f.auh.x, fmaf(dy, f.auh.y, dz * f.auh.z)) + f.margin;
+    const float rv = fmaf(dx, f.avh.x, fmaf(dy, f.avh.y, dz * f.avh.z)) + f.margin;
+    return (pu + ru >= 0.0f) && (pu - ru <= wu) && (pv + rv >= 0.0f) && (pv - rv <= wv);
+}
+
+// One node against a beam: which children overlap, and their links.
+template <bool INSTR>
+__device__ __forceinline__ void beam_node(const float4 *__restrict__ nodes, int node, const BeamFrame &f, float offu,
+                                          float offv, float wu, float wv, bool &h0, bool &h1, int &l0, int &l1,
+                                          unsigned &n_box)
+{
+    h0 = h1 = false; l0 = l1 = 0;
+    if (node < 0) return;
+    const float4 n0 = __ldg(nodes + 4 * node), n1 = __ldg(nodes + 4 * node + 1), n2 = __ldg(nodes + 4 * node + 2),
+                 n3 = __ldg(nodes + 4 * node + 3);
+    h0 = beam_box(f, offu, offv, wu, wv, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y);
+    h1 = beam_box(f, offu, offv, wu, wv, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w);
+    l0 = __float_as_int(n3.x); l1 = __float_as_int(n3.y);
+    if (INSTR) n_box += 2;
+}
+
+// Appends the triangles of up to two leaves per lane to the candidate list (warp scan of the
+// counts, so the order is deterministic).  Returns false if the list would overflow.
+__device__ __forceinline__ bool beam_push_tris(int *cid, int &ncand, int first0, int cnt0, int first1, int cnt1,
+                                               int lane)
+{
+    const int c = cnt0 + cnt1;
+    int incl = c;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const int t = __shfl_up_sync(FULL, incl, off);
+        if (lane >= off) incl += t;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    if (ncand + total > BEAM_CMAX) return false;
+    int pos = ncand + incl - c;
+    for (int t = 0; t < cnt0; ++t) cid[pos++] = first0 + t;
+    for (int t = 0; t < cnt1; ++t) cid[pos++] = first1 + t;
+    ncand += total;
+    return true;
+}
+
+// Candidate set-up: triangle -> sign-normalised edge functions E_i(x) = A_i x_u + B_i x_v + C_i
+// (inside <=> all >= 0) and the depth plane t(x) = Wu x_u + Wv x_v + Wc, in the sub-block's local
+// emitter frame (origin at the sub-block's corner, t measured from the ray-origin plane).
+__device__ __forceinline__ void beam_setup(const float4 *__restrict__ tri, int f, const Emitter &em, float offu,
+                                           float offv, float4 *eq)
+{
+    const float4 q0 = __ldg(tri + 3 * f), q1 = __ldg(tri + 3 * f + 1), q2 = __ldg(tri + 3 * f + 2);
+    const float3 a = f3(q0.x, q0.y, q0.z);
+    const float3 b = f3(q0.x + q1.x, q0.y + q1.y, q0.z + q1.z);
+    const float3 c = f3(q0.x + q2.x, q0.y + q2.y, q0.z + q2.z);
+    const float au = dot3(a, em.u) - offu, av = dot3(a, em.v) - offv, aw = dot3(a, em.s) - em.worg;
+    const float bu = dot3(b, em.u) - offu, bv = dot3(b, em.v) - offv, bw = dot3(b, em.s) - em.worg;
+    const float cu = dot3(c, em.u) - offu, cv = dot3(c, em.v) - offv, cw = dot3(c, em.s) - em.worg;
+    // E_pq(x) = (q_u - p_u)(x_v - p_v) - (q_v - p_v)(x_u - p_u)
+    float A0 = -(bv - av), B0 = bu - au, C0 = -fmaf(A0, au, B0 * av);       // edge a -> b
+    float A1 = -(cv - bv), B1 = cu - bu, C1 = -fmaf(A1, bu, B1 * bv);       // edge b -> c
+    float A2 = -(av - cv), B2 = au - cu, C2 = -fmaf(A2, cu, B2 * cv);       // edge c -> a
+    const float area2 = fmaf(A0, cu, fmaf(B0, cv, C0));                     // E_ab(c)
+    if (area2 == 0.0f || !(fabsf(area2) < FLT_MAX)) {                       // edge-on or degenerate: never hit
+        eq[0] = make_float4(0.f, 0.f, -1.f, 0.f); eq[1] = eq[0]; eq[2] = eq[0];
+        return;
+    }
+    if (area2 < 0.0f) { A0 = -A0; B0 = -B0; C0 = -C0; A1 = -A1; B1 = -B1; C1 = -C1; A2 = -A2; B2 = -B2; C2 = -C2; }
+    const float ia = 1.0f / area2;
+    const float Wu = ((cv - av) * (bw - aw) - (bv - av) * (cw - aw)) * ia;
+    const float Wv = ((bu - au) * (cw - aw) - (cu - au) * (bw - aw)) * ia;
+    const float Wc = aw - fmaf(Wu, au, Wv * av);
+    eq[0] = make_float4(A0, B0, C0, Wu);
+    eq[1] = make_float4(A1, B1, C1, Wv);
+    eq[2] = make_float4(A2, B2, C2, Wc);
+}
+
+// ---- per-warp ray pool (global memory ring) ----
+// Rays that are not resolved by a beam -- bounce rays, and primaries of a group whose lists
+// overflowed -- are appended to the warp's private ring in global memory (L2-resident) and traced
+// later, many tiles' worth at a time, by the per-ray traversal loop of drain(): a lane whose ray
+// has ended takes the next ray of the pool at once, so lanes stay busy although path lengths
+// differ widely (persistent "while-while" traversal with dynamic fetch).  Hits are not shaded where
+// they are found: they are queued in shared memory and shaded 32 at a time, converged.
+// Entry = 9 words (origin, direction, ray index i, pair index p, src | depth << 27), plus the
+// 64-bit path signature in the instrumented build; field-major so appends and fetches coalesce.
+constexpr int POOL_FIELDS = 9;
+constexpr int POOL_FIELDS_INSTR = 11;
+constexpr int POOL_HIGH = 4096;          // drain when the pool holds at least this many rays
+constexpr int HITQ = 64;                 // queued hits per warp
+constexpr int DRAIN_ACTIVE_MIN = 24;     // leave the traversal loop to refill when fewer lanes are busy
+constexpr uint32_t SRC_NONE = 0x07ffffffu;
+
+struct Pool {
+    unsigned *base;
+    uint32_t cap, mask, head, tail;      // head/tail count rays; position = counter & mask
+};
+__device__ __forceinline__ void pool_st(const Pool &q, int field, uint32_t pos, uint32_t v)
+{
+    __stcg(q.base + (size_t)field * q.cap + (pos & q.mask), v);
+}
+__device__ __forceinline__ uint32_t pool_ld(const Pool &q, int field, uint32_t pos)
+{
+    return __ldcg(q.base + (size_t)field * q.cap + (pos & q.mask));
+}
+
+struct BeamSmem {                   // per warp; beam structures and drain structures are never live together
+    union {
+        struct {
+            float4 eq[3 * BEAM_CMAX];       // (A0,B0,C0,Wu) (A1,B1,C1,Wv) (A2,B2,C2,Wc) per candidate
+            int cid[BEAM_CMAX];             // candidate -> sorted triangle index
+            int enode[BEAM_EN];
+            int eleaf[BEAM_EL];
+            int nq[BEAM_QN];
+            unsigned char glist[BEAM_CMAX];
+        } b;
+        struct {
+            int stack[BEAM_STACK * 32];     // per-thread traversal stacks, thread-interleaved
+            uint32_t hq[11][HITQ];          // queued hits: o, d, i, p, sd, triangle, t
+        } s;
+    } u;
+};
+
+template <bool INSTR>
+__global__ void __launch_bounds__(TRACE_THREADS, BEAM_BLOCKS_PER_SM)
+beam_trace_kernel(const TraceArgs a)
+{
+    __shared__ BeamSmem s_w[TRACE_WARPS];
+    __shared__ unsigned long long s_hsig[INSTR ? TRACE_WARPS * HITQ : 1];
+    __shared__ unsigned s_hist[TRACE_WARPS][16];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    if (lane < 16) s_hist[warp][lane] = 0;
+    __syncwarp();
+    BeamSmem &W = s_w[warp];
+    unsigned long long *hsig = s_hsig + (INSTR ? warp * HITQ : 0);
+    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
+    BeamCounters bc = { 0, 0, 0, 0 };
+    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
+    const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
+    const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
+    Pool pool;
+    pool.cap = (uint32_t)a.pool_cap; pool.mask = pool.cap - 1u; pool.head = pool.tail = 0u;
+    pool.base = a.pool + (size_t)(blockIdx.x * TRACE_WARPS + warp) * (size_t)(INSTR ? POOL_FIELDS_INSTR : POOL_FIELDS) * pool.cap;
+
+    // Appends this lane's ray (if `push`) to the pool; warp-wide call.
+    auto pool_push = [&](bool push, const float3 &o, const float3 &d, uint32_t i, uint32_t p, uint32_t sd,
+                         unsigned long long sig) {
+        const unsigned m = __ballot_sync(FULL, push);
+        if (push) {
+            const uint32_t pos = pool.tail + (uint32_t)__popc(m & lt_mask);
+            pool_st(pool, 0, pos, __float_as_uint(o.x)); pool_st(pool, 1, pos, __float_as_uint(o.y));
+            pool_st(pool, 2, pos, __float_as_uint(o.z)); pool_st(pool, 3, pos, __float_as_uint(d.x));
+            pool_st(pool, 4, pos, __float_as_uint(d.y)); pool_st(pool, 5, pos, __float_as_uint(d.z));
+            pool_st(pool, 6, pos, i); pool_st(pool, 7, pos, p); pool_st(pool, 8, pos, sd);
+            if (INSTR) { pool_st(pool, 9, pos, (uint32_t)sig); pool_st(pool, 10, pos, (uint32_t)(sig >> 32)); }
+        }
+        pool.tail += (uint32_t)__popc(m);
+    };
+
+    // ---- S5-S7 for <= 32 queued hits, converged; survivors go back to the pool ----
+    int nhit = 0;                                                  // warp-uniform
+    auto shade_batch = [&]() {
+        const int take = nhit < 32 ? nhit : 32;
+        int fate = -1, src = -1, depth = 0;
+        float3 o = f3(0, 0, 0), d = f3(0, 0, 1);
+        uint32_t i = 0, p = 0;
+        unsigned long long sig = 0;
+        if (lane < take) {
+            const int e = nhit - take + lane;
+            o = f3(__uint_as_float(W.u.s.hq[0][e]), __uint_as_float(W.u.s.hq[1][e]), __uint_as_float(W.u.s.hq[2][e]));
+            d = f3(__uint_as_float(W.u.s.hq[3][e]), __uint_as_float(W.u.s.hq[4][e]), __uint_as_float(W.u.s.hq[5][e]));
+            i = W.u.s.hq[6][e]; p = W.u.s.hq[7][e];
+            depth = (int)(W.u.s.hq[8][e] >> 27);
+            const int best = (int)W.u.s.hq[9][e];
+            const float t = __uint_as_float(W.u.s.hq[10][e]);
+            int k, j;
+            pair_of32(a, p, k, j);
+            const long long tb = a.dz.tri_off[k];
+            const float4 *lt = a.dz.tri + 3 * tb;
+            RayGen g;
+            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0;
+            g.inv_nx = inv_nx; g.inv_ny = inv_ny;
+            atomicAdd(&s_hist[warp][depth], 1u);
+            if (INSTR) sig = hsig[e] * 1000003ULL + (unsigned long long)(a.dz.perm[tb + best] + 1);
+            float3 dep = f3(0, 0, 0);
+            fate = shade(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
+                         a.deposit, o, d, src, depth, dep);
+            if (fate == SHADE_ABSORBED) cn.absorbed++;
+            if (fate == SHADE_CAPPED) cn.capped++;
+            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * (long long)p);
+            if (dep.x != 0.0f) atomicAdd(dst + 0, (unsigned long long)__double2ll_rn((double)dep.x * SRP_ACC_SCALE));
+            if (dep.y != 0.0f) atomicAdd(dst + 1, (unsigned long long)__double2ll_rn((double)dep.y * SRP_ACC_SCALE));
+            if (dep.z != 0.0f) atomicAdd(dst + 2, (unsigned long long)__double2ll_rn((double)dep.z * SRP_ACC_SCALE));
+            if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[(long long)p * a.N + i] = sig;
+        }
+        nhit -= take;
+        __syncwarp();
+        pool_push(fate == SHADE_CONTINUE, o, d, i, p, ((uint32_t)depth << 27) | (uint32_t)src, sig);
+    };
+
+    // ---- per-ray traversal of everything in the pool (S4 for incoherent rays, S6) ----
+    auto drain = [&]() {
+        constexpr int STRIDE = 32, NSMEM = BEAM_STACK;
+        int *s_stack = W.u.s.stack + lane;
+        int ovf[STACK_OVF];
+        bool has = false;
+        int cur = CUR_DONE, sp = 0, best = -1, src = -1;
+        float tbest = FLT_MAX;
+        float3 o = f3(0, 0, 0), d = f3(0, 0, 1);
+        float idx = 0.f, idy = 0.f, idz = 0.f, oxi = 0.f, oyi = 0.f, ozi = 0.f;
+        uint32_t ri = 0, rp = 0, rsd = 0;
+        unsigned long long rsig = 0;
+        const float4 *ln = a.dz.nodes, *lt = a.dz.tri;
+        unsigned nt = 0;
+        for (;;) {
+            // lanes without a ray take the next rays of the pool
+            const unsigned idle = __ballot_sync(FULL, !has);
+            uint32_t navail = pool.tail - pool.head;
+            if (idle != 0u && navail != 0u) {
+                const uint32_t rank = (uint32_t)__popc(idle & lt_mask);
+                if (!has && rank < navail) {
+                    const uint32_t pos = pool.head + rank;
+                    o = f3(__uint_as_float(pool_ld(pool, 0, pos)), __uint_as_float(pool_ld(pool, 1, pos)),
+                           __uint_as_float(pool_ld(pool, 2, pos)));
+                    d = f3(__uint_as_float(pool_ld(pool, 3, pos)), __uint_as_float(pool_ld(pool, 4, pos)),
+                           __uint_as_float(pool_ld(pool, 5, pos)));
+                    ri = pool_ld(pool, 6, pos); rp = pool_ld(pool, 7, pos); rsd = pool_ld(pool, 8, pos);
+                    if (INSTR) rsig = (unsigned long long)pool_ld(pool, 9, pos) | ((unsigned long long)pool_ld(pool, 10, pos) << 32);
+                    int k, j;
+                    pair_of32(a, rp, k, j);
+                    const long long tb = a.dz.tri_off[k];
+                    ln = a.dz.nodes + 4 * tb; lt = a.dz.tri + 3 * tb;
+                    const uint32_t s27 = rsd & SRC_NONE;
+                    src = s27 == SRC_NONE ? -1 : (int)s27;
+                    idx = safe_rcp(d.x); idy = safe_rcp(d.y); idz = safe_rcp(d.z);
+                    oxi = o.x * idx; oyi = o.y * idy; ozi = o.z * idz;
+                    has = true; cur = 0; sp = 0; tbest = FLT_MAX; best = -1;
+                    if ((rsd >> 27) != 0u) cn.segments++;            // primaries were counted when generated
+                }
+                const uint32_t want = (uint32_t)__popc(idle);
+                pool.head += want < navail ? want : navail;
+                navail = pool.tail - pool.head;
+            }
+            if (!__any_sync(FULL, has)) {
+                if (nhit > 0) { shade_batch(); continue; }          // shading may put rays back
+                break;
+            }
+            // traverse until every lane is done, or enough lanes are free and rays are waiting
+            // traverse until every lane is done, or enough lanes are free and rays are waiting
+            for (;;) {
+                while ((unsigned)cur < (unsigned)CUR_DONE) {
+                    if (INSTR) cn.n_box += 2;
+                    cur = bvh_node_step<STRIDE, NSMEM>(ln, cur, sp, s_stack, ovf, idx, idy, idz, oxi, oyi, ozi, tbest);
+                }
+                if (cur < 0) cur = bvh_leaf_step<STRIDE, NSMEM>(lt, cur, sp, s_stack, ovf, o, d, src, tbest, best, nt);
+                const unsigned act = __ballot_sync(FULL, cur != CUR_DONE);
+                if (act == 0u || (navail != 0u && __popc(act) < DRAIN_ACTIVE_MIN)) break;
+            }
+            // retire the rays that ended
+            const bool fin = has && cur == CUR_DONE;
+            const bool hit = fin && best >= 0;
+            if (fin && !hit) {
+                if ((rsd >> 27) == 0u) cn.pmiss++; else cn.escaped++;
+                if (INSTR && a.sig_out) a.sig_out[(long long)rp * a.N + ri] = rsig;
+            }
+            const unsigned mh = __ballot_sync(FULL, hit);
+            if (hit) {
+                const int e = nhit + __popc(mh & lt_mask);
+                W.u.s.hq[0][e] = __float_as_uint(o.x); W.u.s.hq[1][e] = __float_as_uint(o.y); W.u.s.hq[2][e] = __float_as_uint(o.z);
+                W.u.s.hq[3][e] = __float_as_uint(d.x); W.u.s.hq[4][e] = __float_as_uint(d.y); W.u.s.hq[5][e] = __float_as_uint(d.z);
+                W.u.s.hq[6][e] = ri; W.u.s.hq[7][e] = rp; W.u.s.hq[8][e] = rsd;
+                W.u.s.hq[9][e] = (uint32_t)best; W.u.s.hq[10][e] = __float_as_uint(tbest);
+                if (INSTR) hsig[e] = rsig;
+            }
+            nhit += __popc(mh);
+            if (fin) has = false;
+            __syncwarp();
+            if (nhit >= 32) shade_batch();
+        }
+        if (INSTR) cn.n_tri += nt;
+    };
+
+    // ---- S2-S5 for the primaries of one tile, as beams ----
+    auto process_tile = [&](unsigned long long tile) {
+        const long long p = (long long)(tile / a.tiles_per_pair);
+        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
+        int k, j;
+        pair_of(a, p, k, j);
+        const float4 blo = a.dz.box[2 * k], bhi = a.dz.box[2 * k + 1];
+        const Emitter em = make_emitter(a.sun_dirs, j, blo, bhi);
+        if (!(em.Ae > 0.0f)) return;                              // edge-on flat design: F = 0, nothing launched
+        const long long tbase = a.dz.tri_off[k];
+        const float4 *gtri = a.dz.tri + 3 * tbase;
+        const float4 *gnodes = a.dz.nodes + 4 * tbase;
+        RayGen g;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0;
+        g.inv_nx = inv_nx; g.inv_ny = inv_ny;
+        BeamFrame bf;
+        bf.uh = f3(0.5f * em.u.x, 0.5f * em.u.y, 0.5f * em.u.z);
+        bf.vh = f3(0.5f * em.v.x, 0.5f * em.v.y, 0.5f * em.v.z);
+        bf.auh = f3(fabsf(bf.uh.x), fabsf(bf.uh.y), fabsf(bf.uh.z));
+        bf.avh = f3(fabsf(bf.vh.x), fabsf(bf.vh.y), fabsf(bf.vh.z));
+        bf.csu = em.du * inv_nx; bf.csv = em.dv * inv_ny;
+        {   // fp32 projections of points of this design are off by < 1e-6 of this scale; 10x that
+            const float L = fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
+                            fmaxf(fabsf(blo.z), fabsf(bhi.z));
+            bf.margin = 1.0e-5f * L;
+        }
+        const uint32_t start = (uint32_t)(q * a.tile_rays);
+        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
+        const uint32_t nt = end - start;                          // a power of two
+        const int tbits = 31 - __clz((int)nt);
+        float3 acc = f3(0, 0, 0);
+
+        // tile level: frontier descent to an entry list
+        const uint32_t tcx0 = compact_even_bits(start), tcy0 = compact_even_bits(start >> 1);
+        const float t_offu = fmaf((float)tcx0 * inv_nx, em.du, em.u0), t_offv = fmaf((float)tcy0 * inv_ny, em.dv, em.v0);
+        const float t_wu = (float)(1u << ((tbits + 1) >> 1)) * bf.csu, t_wv = (float)(1u << (tbits >> 1)) * bf.csv;
+        int n_en = 1, n_el = 0;
+        if (lane == 0) W.u.b.enode[0] = 0;
+        __syncwarp();
+        for (int lvl = 0; lvl < 24 && n_en > 0 && n_en <= 32 && n_el <= 32; ++lvl) {
+            const int node = lane < n_en ? W.u.b.enode[lane] : -1;
+            __syncwarp();
+            bool h0, h1; int l0, l1;
+            beam_node<INSTR>(gnodes, node, bf, t_offu, t_offv, t_wu, t_wv, h0, h1, l0, l1, cn.n_box);
+            const bool p0 = h0 && l0 >= 0, p1 = h1 && l1 >= 0, f0 = h0 && l0 < 0, f1 = h1 && l1 < 0;
+            const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
+            const unsigned mf0 = __ballot_sync(FULL, f0), mf1 = __ballot_sync(FULL, f1);
+            const int np0 = __popc(mp0), nf0 = __popc(mf0), nf1 = __popc(mf1);
+            if (p0) W.u.b.enode[__popc(mp0 & lt_mask)] = l0;
+            if (p1) W.u.b.enode[np0 + __popc(mp1 & lt_mask)] = l1;
+            if (f0) W.u.b.eleaf[n_el + __popc(mf0 & lt_mask)] = l0;
+            if (f1) W.u.b.eleaf[n_el + nf0 + __popc(mf1 & lt_mask)] = l1;
+            n_en = np0 + __popc(mp1); n_el += nf0 + nf1;
+            __syncwarp();
+        }
+        if (n_en == 0 && n_el == 0) {                             // the tile's beam meets nothing: nt primary misses
+            const unsigned c = nt >= 32u ? nt >> 5 : (unsigned)(lane < (int)nt);
+            cn.launched += c; cn.pmiss += c; cn.segments += c; bc.tile_miss += c;
+            return;
+        }
+
+        // Sub-blocks are adaptive: a block whose lists overflow is halved (down to one group of 32 rays, whose
+        // rays then go to the pool for per-ray traversal); the size grows back at the next aligned position.
+        const uint32_t nb_max = nt < (uint32_t)BEAM_SB ? nt : (uint32_t)BEAM_SB;
+        uint32_t nb = nb_max;                                     // rays in the current sub-block
+        for (uint32_t sb = start; sb < end;) {
+            const int sbits = 31 - __clz((int)nb);
+            const uint32_t s_wx = 1u << ((sbits + 1) >> 1), s_wy = 1u << (sbits >> 1);
+            const uint32_t g_wx = nb >= 32u ? 8u : s_wx, g_wy = nb >= 32u ? 4u : s_wy;
+            const float s_wu = (float)s_wx * bf.csu, s_wv = (float)s_wy * bf.csv;
+            const uint32_t scx0 = compact_even_bits(sb), scy0 = compact_even_bits(sb >> 1);
+            const float s_offu = fmaf((float)scx0 * inv_nx, em.du, em.u0), s_offv = fmaf((float)scy0 * inv_ny, em.dv, em.v0);
+            bool ovf = false;
+            int ncand = 0;
+            {
+                // sub-block level: descent from the entry list to candidate triangles
+                for (int x = lane; x < n_en; x += 32) W.u.b.nq[x] = W.u.b.enode[x];
+                int qn = n_en;
+                for (int base = 0; base < n_el && !ovf; base += 32) {
+                    const int x = base + lane;
+                    int first = 0, cnt = 0;
+                    if (x < n_el) { const unsigned u = (unsigned)~W.u.b.eleaf[x]; first = (int)(u >> 3); cnt = (int)(u & 7u) + 1; }
+                    if (!beam_push_tris(W.u.b.cid, ncand, first, cnt, 0, 0, lane)) ovf = true;
+                }
+                __syncwarp();
+                while (qn > 0 && !ovf) {
+                    const int take = qn < 32 ? qn : 32;
+                    const int node = lane < take ? W.u.b.nq[qn - take + lane] : -1;
+                    qn -= take;
+                    __syncwarp();
+                    bool h0, h1; int l0, l1;
+                    beam_node<INSTR>(gnodes, node, bf, s_offu, s_offv, s_wu, s_wv, h0, h1, l0, l1, cn.n_box);
+                    const bool p0 = h0 && l0 >= 0, p1 = h1 && l1 >= 0, f0 = h0 && l0 < 0, f1 = h1 && l1 < 0;
+                    const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
+                    const int np0 = __popc(mp0), np1 = __popc(mp1);
+                    if (qn + np0 + np1 > BEAM_QN) { ovf = true; break; }
+                    if (p0) W.u.b.nq[qn + __popc(mp0 & lt_mask)] = l0;
+                    if (p1) W.u.b.nq[qn + np0 + __popc(mp1 & lt_mask)] = l1;
+                    qn += np0 + np1;
+                    if (__any_sync(FULL, f0 || f1)) {
+                        const unsigned u0 = (unsigned)~l0, u1 = (unsigned)~l1;
+                        if (!beam_push_tris(W.u.b.cid, ncand, (int)(u0 >> 3), f0 ? (int)(u0 & 7u) + 1 : 0, (int)(u1 >> 3),
+                                            f1 ? (int)(u1 & 7u) + 1 : 0, lane))
+                            ovf = true;
+                    }
+                    __syncwarp();
+                }
+                if (!ovf && ncand == 0) {                        // empty sub-block
+                    const unsigned c = nb >= 32u ? nb >> 5 : (unsigned)(lane < (int)nb);
+                    cn.launched += c; cn.pmiss += c; cn.segments += c; bc.block_miss += c;
+                    sb += nb;
+                    if (nb < nb_max && (sb & (2u * nb - 1u)) == 0u) nb <<= 1;
+                    continue;
+                }
+                if (ovf && nb > 32u) { nb >>= 1; continue; }     // retry this position with half the rays
+                if (!ovf) {
+                    __syncwarp();
+                    for (int c = lane; c < ncand; c += 32) beam_setup(gtri, W.u.b.cid[c], em, s_offu, s_offv, W.u.b.eq + 3 * c);
+                    __syncwarp();
+                }
+            }
+
+            // groups of 32 rays
+            for (uint32_t gs = sb; gs < sb + nb; gs += 32) {
+                const uint32_t gcx = compact_even_bits(gs) - scx0, gcy = compact_even_bits(gs >> 1) - scy0;
+                int ng = 0;
+                if (!ovf) {
+                    const float gu0 = (float)gcx * bf.csu, gu1 = (float)(gcx + g_wx) * bf.csu;
+                    const float gv0 = (float)gcy * bf.csv, gv1 = (float)(gcy + g_wy) * bf.csv;
+                    for (int base = 0; base < ncand; base += 32) {
+                        const int c = base + lane;
+                        bool keep = false;
+                        if (c < ncand) {
+                            const float4 E0 = W.u.b.eq[3 * c], E1 = W.u.b.eq[3 * c + 1], E2 = W.u.b.eq[3 * c + 2];
+                            // largest value of each edge function over the rectangle (monotone in fp32 too)
+                            const float m0 = fmaf(E0.x, E0.x >= 0.f ? gu1 : gu0, fmaf(E0.y, E0.y >= 0.f ? gv1 : gv0, E0.z));
+                            const float m1 = fmaf(E1.x, E1.x >= 0.f ? gu1 : gu0, fmaf(E1.y, E1.y >= 0.f ? gv1 : gv0, E1.z));
+                            const float m2 = fmaf(E2.x, E2.x >= 0.f ? gu1 : gu0, fmaf(E2.y, E2.y >= 0.f ? gv1 : gv0, E2.z));
+                            keep = fminf(m0, fminf(m1, m2)) >= 0.0f;
+                        }
+                        const unsigned m = __ballot_sync(FULL, keep);
+                        if (keep) W.u.b.glist[ng + __popc(m & lt_mask)] = (unsigned char)c;
+                        ng += __popc(m);
+                    }
+                    __syncwarp();
+                    if (ng == 0) {                               // 32 primary misses, no ray generated
+                        const unsigned c = (unsigned)(lane < (int)nb);
+                        cn.launched += c; cn.pmiss += c; cn.segments += c; bc.group_miss += c;
+                        continue;
+                    }
+                }
+                // O-step 3 for this lane's ray
+                const bool on = lane < (int)nb;
+                const uint32_t i = gs + (uint32_t)lane;
+                float3 o = f3(0, 0, 0), d = em.s;
+                float lu = 0.f, lv = 0.f;
+                if (on) {
+                    uint32_t r0, r1, r2, r3;
+                    philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
+                    const float xi0 = uniform23(r0), xi1 = uniform23(r1);
+                    const uint32_t cx = nb >= 32u ? scx0 + gcx + ldx : compact_even_bits(i);
+                    const uint32_t cy = nb >= 32u ? scy0 + gcy + ldy : compact_even_bits(i >> 1);
+                    const float fu = ((float)cx + xi0) * inv_nx, fv = ((float)cy + xi1) * inv_ny;
+                    const float pu = fmaf(fu, em.du, em.u0), pv = fmaf(fv, em.dv, em.v0);
+                    o = f3(fmaf(pu, em.u.x, fmaf(pv, em.v.x, em.worg * em.s.x)),
+                           fmaf(pu, em.u.y, fmaf(pv, em.v.y, em.worg * em.s.y)),
+                           fmaf(pu, em.u.z, fmaf(pv, em.v.z, em.worg * em.s.z)));
+                    lu = ((float)(cx - scx0) + xi0) * bf.csu;
+                    lv = ((float)(cy - scy0) + xi1) * bf.csv;
+                    cn.launched++; cn.segments++;
+                }
+                if (ovf) {                                       // too much geometry behind this group: per-ray traversal
+                    if (on) bc.fallback++;
+                    pool_push(on, o, d, i, (uint32_t)p, SRC_NONE, 0ULL);
+                    continue;
+                }
+                // O-step 4 against the shared list: all lanes converged, operands broadcast
+                float tbest = FLT_MAX;
+                int best = -1;
+                for (int e = 0; e < ng; ++e) {
+                    const int c = W.u.b.glist[e];
+                    const float4 E0 = W.u.b.eq[3 * c], E1 = W.u.b.eq[3 * c + 1], E2 = W.u.b.eq[3 * c + 2];
+                    const float e0 = fmaf(E0.x, lu, fmaf(E0.y, lv, E0.z));
+                    const float e1 = fmaf(E1.x, lu, fmaf(E1.y, lv, E1.z));
+                    const float e2 = fmaf(E2.x, lu, fmaf(E2.y, lv, E2.z));
+                    const float t = fmaf(E0.w, lu, fmaf(E1.w, lv, E2.w));
+                    if (fminf(e0, fminf(e1, e2)) >= 0.0f && t < tbest) { tbest = t; best = c; }
+                }
+                if (INSTR && on) cn.n_tri += (unsigned)ng;
+                if (best >= 0) best = W.u.b.cid[best];
+                if (!on) best = -1;
+                int fate = -1, src = -1, depth = 0;
+                unsigned long long sig = 0;
+                if (on) {
+                    if (best < 0) cn.pmiss++;
+                    else {
+                        atomicAdd(&s_hist[warp][0], 1u);
+                        if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
+                        fate = shade(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
+                                     best, g, i, a.B, a.deposit, o, d, src, depth, acc);
+                        if (fate == SHADE_ABSORBED) cn.absorbed++;
+                        if (fate == SHADE_CAPPED) cn.capped++;
+                    }
+                    if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
+                }
+                pool_push(fate == SHADE_CONTINUE, o, d, i, (uint32_t)p, ((uint32_t)depth << 27) | (uint32_t)src, sig);
+            }
+            sb += nb;
+            if (nb < nb_max && (sb & (2u * nb - 1u)) == 0u) nb <<= 1;
+        }
+
+        // S7 for the tile's primaries: warp reduction in fp64, then one fixed-point atomic per component
+        double sx = acc.x, sy = acc.y, sz = acc.z;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            sx += __shfl_xor_sync(FULL, sx, off);
+            sy += __shfl_xor_sync(FULL, sy, off);
+            sz += __shfl_xor_sync(FULL, sz, off);
+        }
+        if (lane == 0) {
+            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
+            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
+            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
+            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
+        }
+    };
+
+    // ---- persistent loop: tiles until the pool is worth draining ----
+    bool more = true;
+    for (;;) {
+        if (more) {
+            unsigned long long tile = 0;
+            if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
+            tile = __shfl_sync(FULL, tile, 0);
+            if (tile >= total_tiles) more = false;
+            else process_tile(tile);
+        }
+        __syncwarp();
+        const uint32_t cnt = pool.tail - pool.head;
+        if (cnt >= (uint32_t)POOL_HIGH || (!more && cnt != 0u)) { drain(); __syncwarp(); }
+        if (!more && pool.tail == pool.head) break;
+    }
+    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
+    {
+        unsigned long long *st = (unsigned long long *)a.stats;
+        const unsigned vals[4] = { bc.tile_miss, bc.block_miss, bc.group_miss, bc.fallback };
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            unsigned long long v = vals[c];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+            if (lane == 0 && v) atomicAdd(st + 24 + c, v);
+        }
+    }
+}
+
 // F[p] = accum[p] * 2^-32 * P * A_e / N
 __global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float *out)
 {
@@ -668,12 +1291,26 @@ static cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, 
     return cudaGetLastError();
 }
 
-int srp_trace_blocks_per_sm(bool brute)
+int srp_trace_blocks_per_sm(bool brute, bool beam)
 {
     int per_sm = 0;
     if (brute) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BRUTE_SMEM, false>, TRACE_THREADS, 0);
+    else if (beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false>, TRACE_THREADS, 0);
     else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bvh_trace_kernel<false>, TRACE_THREADS, 0);
     return per_sm * TRACE_WARPS;
+}
+
+// Words of global memory the beam kernel's per-warp ray pools need, and the ring capacity per warp.
+size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *cap_out)
+{
+    int per_sm = 0;
+    if (instrumented) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<true>, TRACE_THREADS, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false>, TRACE_THREADS, 0);
+    if (per_sm < 1) per_sm = 1;
+    int cap = 64;
+    while (cap < POOL_HIGH + tile_rays + 64) cap <<= 1;
+    *cap_out = cap;
+    return (size_t)num_sms * per_sm * TRACE_WARPS * (instrumented ? POOL_FIELDS_INSTR : POOL_FIELDS) * (size_t)cap;
 }
 
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms, cudaStream_t stream)
@@ -685,6 +1322,9 @@ cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, 
         return instrumented ? launch_persistent(trace_kernel<MODE_BRUTE_SMEM, true>, a, num_sms, stream)
                             : launch_persistent(trace_kernel<MODE_BRUTE_SMEM, false>, a, num_sms, stream);
     }
+    if (a.sampler == 0 && a.pool != nullptr)          // beams chosen by the caller (srp_api.cu, want_beams)
+        return instrumented ? launch_persistent(beam_trace_kernel<true>, a, num_sms, stream)
+                            : launch_persistent(beam_trace_kernel<false>, a, num_sms, stream);
     return instrumented ? launch_persistent(bvh_trace_kernel<true>, a, num_sms, stream)
                         : launch_persistent(bvh_trace_kernel<false>, a, num_sms, stream);
 }

@@ -186,15 +186,24 @@ def test_small_design_configs_full_N(ctx, oracle, name, n_pairs):
     dz.free()
 
 
-def test_cfg3_detailed_reduced_N(ctx, oracle):
+@pytest.mark.parametrize("primary_mode", [1, 2])          # primaries one by one / as beams (auto picks by N / T)
+def test_cfg3_detailed_reduced_N(ctx, oracle, primary_mode):
     cfg = W.CONFIGS["cfg3_detailed"]
     th, sun = cfg.params(), cfg.sun_dirs()
     dz = ctx.srp_build_designs(cfg.family, th)
     N = 1 << 12
     rng = np.random.default_rng(6)
     pairs = np.stack([np.arange(cfg.D), rng.integers(0, cfg.S, cfg.D)], 1).astype(np.int32)   # one per design
-    F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
-    psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
+    ctx.srp_set_options(primary_mode=primary_mode)
+    try:
+        F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
+        psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
+    finally:
+        ctx.srp_set_options()
+    if primary_mode == 2:
+        assert st["beam_tile_miss"] + st["beam_block_miss"] + st["beam_group_miss"] > 0.5 * st["launched"]
+    else:
+        assert st["beam_tile_miss"] + st["beam_block_miss"] + st["beam_group_miss"] + st["beam_fallback"] == 0
     meshes = {k: oracle.build_mesh(cfg.family, th[k], k=k) for k in range(cfg.D)}
     Fo, sig, ost, osig = oracle_pairs(oracle, meshes, pairs, sun, N, cfg.B, seed=cfg.seed, want_path_sig=True)
     n_div = (psig != osig).sum(axis=1)                     # divergent rays per pair
@@ -212,7 +221,8 @@ def test_cfg3_detailed_reduced_N(ctx, oracle):
     dz.free()
 
 
-def test_cfg5_sail_reduced_N(ctx, oracle):
+@pytest.mark.parametrize("primary_mode", [1, 2])
+def test_cfg5_sail_reduced_N(ctx, oracle, primary_mode):
     cfg = W.CONFIGS["cfg5_sail"]
     th = cfg.params()
     dz = ctx.srp_build_designs(cfg.family, th)
@@ -221,8 +231,12 @@ def test_cfg5_sail_reduced_N(ctx, oracle):
     sun = np.array([[1, 0.2, 0.02], [0.3, -1, -0.03], [0.5, 0.4, 0.7], [-0.2, 0.6, -0.6],
                     [0.05, 0.02, 1], [0.01, -0.03, -1]], np.float32)
     pairs = np.stack([np.zeros(len(sun)), np.arange(len(sun))], 1).astype(np.int32)
-    F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
-    psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
+    ctx.srp_set_options(primary_mode=primary_mode)       # 2: ~1000 triangles per ray, every beam list overflows
+    try:
+        F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
+        psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
+    finally:
+        ctx.srp_set_options()
     meshes = {0: oracle.build_mesh(cfg.family, th[0], k=0)}
     Fo, sig, ost, osig = oracle_pairs(oracle, meshes, pairs, sun, N, cfg.B, seed=cfg.seed, want_path_sig=True)
     n_div = (psig != osig).sum(axis=1)
@@ -363,6 +377,53 @@ def test_edge_cases(ctx, oracle):
     ov, omat = oracle.build_mesh(W.FAMILY_PLATE, th[0])
     r = oracle.forces(ov, omat, np.array([[0, 0, 2.5]], np.float32), 1000, 1, j0=1, sampler=1)
     assert rel_l2(Fi[1], r["F"][0]) < 1e-5
+    dz.free()
+
+
+def test_beams_equal_per_ray_primaries(ctx):
+    """The beam tracer (shared BVH descent per block of rays, 2-D edge-function tests in the emitter frame,
+    pooled bounce rays) follows the same photons as per-ray traversal: identical path signatures up to a
+    handful of rays on facet edges, identical counters up to those, forces to 1e-6, on N from 1 ray
+    (one lane) over ragged sub-blocks to several tiles, and on a sphere seen from 12 sides."""
+    th = W.draw_params(W.FAMILY_DETAILED, 2)
+    dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    sun = W.fibonacci_sphere(6)
+    pairs = np.array([[k, j] for k in range(2) for j in range(6)], np.int32)
+    for N, B in ((1, 2), (8, 2), (1 << 6, 3), (1 << 9, 8), (1 << 15, 8)):
+        res = {}
+        for mode in (1, 2):
+            ctx.srp_set_options(primary_mode=mode)
+            try:
+                F, st = run_pairs(ctx, dz, sun, pairs, N, B, seed=5)
+                sg = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, B, 5).cpu().numpy().astype(np.uint64)
+            finally:
+                ctx.srp_set_options()
+            res[mode] = (F, st, sg)
+        n_div = int((res[1][2] != res[2][2]).sum())
+        assert n_div <= max(2, N * len(pairs) // 100000), (N, n_div)
+        for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments"):
+            assert abs(res[1][1][key] - res[2][1][key]) <= 4 * n_div, (N, key)
+        assert res[2][1]["launched"] == N * len(pairs)
+        if n_div == 0 and N >= 64:
+            assert rel_l2(res[2][0], res[1][0]).max() < 1e-5
+    dz.free()
+
+
+def test_beam_auto_mode_and_determinism(ctx):
+    """auto: beams when rays_per_dir >= 8 x triangles.  Beam results are bit-reproducible (integer
+    accumulation; the pool order does not matter)."""
+    verts = W.icosphere(3, 1.3)                                           # 1280 facets
+    mats = W.dirichlet_materials(len(verts), 7)
+    dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
+    sun = cuda(W.fibonacci_sphere(5))
+    a = ctx.srp_forces(dz, sun, 1 << 14, 3, 1).cpu().numpy()
+    st = ctx.srp_get_stats()
+    assert st["beam_tile_miss"] + st["beam_block_miss"] + st["beam_group_miss"] > 0       # 16384 >= 8 * 1280
+    b = ctx.srp_forces(dz, sun, 1 << 14, 3, 1).cpu().numpy()
+    assert np.array_equal(a, b)
+    ctx.srp_forces(dz, sun, 1 << 12, 3, 1)
+    st = ctx.srp_get_stats()
+    assert st["beam_tile_miss"] + st["beam_block_miss"] + st["beam_group_miss"] + st["beam_fallback"] == 0
     dz.free()
 
 
