@@ -121,7 +121,9 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     // them only when there would be too few items to occupy every resident warp several times
     const bool brute = !dz->has_bvh;
     a.max_tris = dz->maxT;
-    const bool beam = want_beams(ctx, brute || ctx->opt.force_brute != 0, a.max_tris, N, n_pairs);
+    a.primary_mode = ctx->opt.primary_mode;
+    const bool beam = brute ? (ctx->opt.sampler == 0 && ctx->opt.primary_mode != 1)
+                            : want_beams(ctx, ctx->opt.force_brute != 0, a.max_tris, N, n_pairs);
     const long long warps = (long long)ctx->num_sms * srp_trace_blocks_per_sm(brute, beam);
     long long tile = 8192;
     if (tile > N) tile = N;

@@ -93,6 +93,7 @@ struct TraceArgs {
     unsigned *pool;                // beam kernel: per-warp ray pools (srp_beam_pool_words), or nullptr
     int pool_cap;                  // rays per pool (a power of two)
     long long max_tris;            // largest design of the batch
+    int primary_mode;              // srp_options.primary_mode
 };
 
 // ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----

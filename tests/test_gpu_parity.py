@@ -409,6 +409,38 @@ def test_beams_equal_per_ray_primaries(ctx):
     dz.free()
 
 
+@pytest.mark.parametrize("family,D,S,N,B", [(W.FAMILY_BOXWING, 8, 12, 1 << 14, 4), (W.FAMILY_BOXWING6, 8, 12, 1 << 16, 4),
+                                            (W.FAMILY_PLATE, 1, 12, 1 << 10, 1), (W.FAMILY_BOXWING, 2, 5, 1, 4),
+                                            (W.FAMILY_BOXWING, 2, 5, 16, 4)])
+def test_small_design_beams_equal_brute_force(ctx, family, D, S, N, B):
+    """Designs without a hierarchy: the tile / sub-block / group culling and the 2-D edge-function test of the
+    primaries (small_beam_kernel) against Moller-Trumbore over all triangles for every segment (primary_mode 1)."""
+    th = W.draw_params(family, D)
+    sun = W.fibonacci_sphere(S)
+    dz = ctx.srp_build_designs(family, th)
+    pairs = np.array([[k, j] for k in range(D) for j in range(S)], np.int32)
+    res = {}
+    for mode in (0, 1):
+        ctx.srp_set_options(primary_mode=mode)
+        try:
+            F, st = run_pairs(ctx, dz, sun, pairs, N, B, seed=4)
+            sg = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, B, 4).cpu().numpy().astype(np.uint64)
+        finally:
+            ctx.srp_set_options()
+        res[mode] = (F, st, sg)
+    n_div = int((res[0][2] != res[1][2]).sum())
+    assert n_div <= max(1, N * len(pairs) // 1000000), n_div
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments"):
+        assert abs(res[0][1][key] - res[1][1][key]) <= 4 * n_div, key
+    assert res[1][1]["beam_tile_miss"] + res[1][1]["beam_block_miss"] + res[1][1]["beam_group_miss"] == 0
+    if N >= 1 << 10:
+        assert res[0][1]["beam_tile_miss"] + res[0][1]["beam_block_miss"] + res[0][1]["beam_group_miss"] > 0
+        nrm = np.linalg.norm(res[1][0], axis=1)
+        err = np.linalg.norm(res[0][0] - res[1][0], axis=1)
+        assert np.all(err <= 1e-4 * nrm + 1e-30) or n_div > 0
+    dz.free()
+
+
 def test_beam_auto_mode_and_determinism(ctx):
     """auto: beams when rays_per_dir >= 8 x triangles.  Beam results are bit-reproducible (integer
     accumulation; the pool order does not matter)."""
