@@ -29,9 +29,13 @@ UNIT = "segments/s"
 # FP32 peak the ALU roofline is quoted against: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
 # (B200_PROFILING.md unit counts and max SM clock); the probed FMA-chain figure is printed beside it.
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# algorithmic work per unit: 12 flop per ray-box test, 44 per ray-triangle test,
-# 80 per shaded hit; 64 B per node visited (2 boxes), 48 B per triangle tested.
-FLOP_BOX, FLOP_TRI, FLOP_HIT = 12.0, 44.0, 80.0
+# algorithmic work per unit: 12 flop per ray-box slab test, 44 per Moller-Trumbore
+# ray-triangle test, 20 per ray-triangle test in the emitter frame (three 2-D edge functions + depth),
+# 80 per shaded hit; 64 B per node visited (2 boxes), 48 B per triangle fetched.  Beam work (DESIGN.md
+# "Kernels"): 32 flop per beam-box test (12 FMA + 8 add), 14 per rectangle-triangle culling test
+# (6 FMA + 2 min), 110 per triangle set-up (9 dot products, 3 edge functions, depth plane).
+FLOP_BOX, FLOP_TRI, FLOP_TRI2D, FLOP_HIT = 12.0, 44.0, 20.0, 80.0
+FLOP_BEAM_BOX, FLOP_RECT, FLOP_SETUP = 32.0, 14.0, 110.0
 BYTES_NODE, BYTES_TRI = 64.0, 48.0
 
 
@@ -226,15 +230,24 @@ def run_ours(args, rank, world, local_rank):
     st_i = ctx.srp_get_stats()
     ctx.srp_set_options()
     seg_i = max(st_i["segments"], 1)
-    box_ps, tri_ps = st_i["box_tests"] / seg_i, st_i["tri_tests"] / seg_i
+    per = {k: st_i[k] / seg_i for k in ("box_tests", "tri_tests", "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests")}
     hit_ps = sum(st_i["hits_at_depth"]) / seg_i
-    flop_ps = FLOP_BOX * box_ps + FLOP_TRI * tri_ps + FLOP_HIT * hit_ps
-    bytes_ps = BYTES_NODE * box_ps / 2.0 + BYTES_TRI * tri_ps
+    flop_ps = (FLOP_BOX * per["box_tests"] + FLOP_TRI * per["tri_tests"] + FLOP_TRI2D * per["tri2d_tests"] +
+               FLOP_BEAM_BOX * per["beam_box_tests"] + FLOP_RECT * per["rect_tests"] + FLOP_SETUP * per["tri_setups"] +
+               FLOP_HIT * hit_ps)
+    # node and triangle bytes the tests above read (beam descents and set-ups fetch each node / triangle once)
+    bytes_ps = (BYTES_NODE * (per["box_tests"] + per["beam_box_tests"]) / 2.0 +
+                BYTES_TRI * (per["tri_tests"] + per["tri_setups"]))
     ach_tflops = flop_ps * st_k["segments"] / t_kernel / 1e12
-    roofline = {"bound": "alu", "kernel": "trace_kernel", "achieved": ach_tflops, "peak": FP32_PEAK_TFLOPS,
+    big = W.TRI_COUNT[cfg.family] > 64
+    beams = st_i["beam_tile_miss"] + st_i["beam_block_miss"] + st_i["beam_group_miss"] + st_i["tri2d_tests"] > 0
+    kernel = ("beam_trace_kernel" if beams else "bvh_trace_kernel") if big else ("small_beam_kernel" if beams else "trace_kernel")
+    roofline = {"bound": "alu", "kernel": kernel, "achieved": ach_tflops, "peak": FP32_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": ach_tflops / FP32_PEAK_TFLOPS, "traffic": None,
                 "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz; probed FMA chain %.1f TFLOP/s" % peaks["fp32_tflops"],
-                "flop_per_segment": flop_ps, "box_tests_per_segment": box_ps, "tri_tests_per_segment": tri_ps,
+                "flop_per_segment": flop_ps, "tests_per_segment": per, "hits_per_segment": hit_ps,
+                "beam_resolved": {k: st_k[k] / max(st_k["launched"], 1) for k in
+                                  ("beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback")},
                 "l2": {"achieved_gbs": bytes_ps * st_k["segments"] / t_kernel / 1e9, "probed_peak_gbs": peaks["l2_read_gbs"],
                        "bytes_per_segment": bytes_ps},
                 "kernel_ms": 1e3 * t_kernel, "kernel_segments": st_k["segments"]}

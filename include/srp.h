@@ -77,6 +77,11 @@ typedef struct {
     /* beam tracing of primaries: rays resolved as misses by a whole tile / sub-block / group of 32,
        and primaries that fell back to per-ray traversal because a beam list overflowed */
     unsigned long long beam_tile_miss, beam_block_miss, beam_group_miss, beam_fallback;
+    /* instrumented only: work of the beam path -- beam-vs-box tests of the cooperative descents, 2-D
+       (emitter-frame) ray-triangle tests, triangle set-ups (edge functions + depth plane), and
+       rectangle-vs-triangle culling tests.  box_tests / tri_tests count per-ray slab tests and
+       Moller-Trumbore tests only. */
+    unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
 } srp_stats;
 
 /* Creates a context on CUDA device `cuda_device`; `cuda_stream` is a cudaStream_t (may be NULL =

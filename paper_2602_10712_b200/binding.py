@@ -35,12 +35,14 @@ class srp_stats(ctypes.Structure):
                 ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments")] + \
                [("hits_at_depth", ctypes.c_ulonglong * 16), ("box_tests", ctypes.c_ulonglong),
                 ("tri_tests", ctypes.c_ulonglong)] + \
-               [(n, ctypes.c_ulonglong) for n in ("beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback")]
+               [(n, ctypes.c_ulonglong) for n in ("beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback",
+                                                  "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests")]
 
     def as_dict(self):
         d = {n: int(getattr(self, n)) for n in
              ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "box_tests", "tri_tests",
-              "beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback")}
+              "beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback",
+              "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests")}
         d["hits_at_depth"] = [int(x) for x in self.hits_at_depth]
         return d
 

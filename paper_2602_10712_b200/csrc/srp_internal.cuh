@@ -55,6 +55,7 @@ struct DevStats {           // device mirror of srp_stats
     unsigned long long hits_at_depth[16];
     unsigned long long box_tests, tri_tests;
     unsigned long long beam_tile_miss, beam_block_miss, beam_group_miss, beam_fallback;
+    unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
 };
 
 struct srp_context {

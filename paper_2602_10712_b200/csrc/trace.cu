@@ -252,8 +252,9 @@ __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, co
 struct LaneCounters {
     unsigned launched, pmiss, absorbed, escaped, capped, segments, n_box, n_tri;
 };
-struct BeamCounters {       // rays resolved per beam level (lane-distributed counts)
+struct BeamCounters {       // rays resolved per beam level (lane-distributed counts); instrumented: beam work
     unsigned tile_miss, block_miss, group_miss, fallback;
+    unsigned beam_box, tri2d, setups, rect;     // beam-box tests, 2-D ray-triangle tests, triangle set-ups, rectangle-triangle tests
 };
 
 // O-steps 5-7 at a hit: deposit, lobe selection, continuation.
@@ -577,9 +578,9 @@ bvh_trace_kernel(const TraceArgs a)
 __device__ __forceinline__ void flush_beam_counters(const TraceArgs &a, const BeamCounters &bc, int lane)
 {
     unsigned long long *st = (unsigned long long *)a.stats;
-    const unsigned vals[4] = { bc.tile_miss, bc.block_miss, bc.group_miss, bc.fallback };
+    const unsigned vals[8] = { bc.tile_miss, bc.block_miss, bc.group_miss, bc.fallback, bc.beam_box, bc.tri2d, bc.setups, bc.rect };
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < 8; ++c) {
         unsigned long long v = vals[c];
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
@@ -769,7 +770,7 @@ beam_trace_kernel(const TraceArgs a)
     BeamSmem &W = s_w[warp];
     unsigned long long *hsig = s_hsig + (INSTR ? warp * HITQ : 0);
     LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    BeamCounters bc = { 0, 0, 0, 0 };
+    BeamCounters bc = { 0, 0, 0, 0, 0, 0, 0, 0 };
     const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
     const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
     const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
@@ -958,7 +959,7 @@ beam_trace_kernel(const TraceArgs a)
             const int node = lane < n_en ? W.u.b.enode[lane] : -1;
             __syncwarp();
             bool h0, h1; int l0, l1;
-            beam_node<INSTR>(gnodes, node, bf, t_offu, t_offv, t_wu, t_wv, h0, h1, l0, l1, cn.n_box);
+            beam_node<INSTR>(gnodes, node, bf, t_offu, t_offv, t_wu, t_wv, h0, h1, l0, l1, bc.beam_box);
             const bool p0 = h0 && l0 >= 0, p1 = h1 && l1 >= 0, f0 = h0 && l0 < 0, f1 = h1 && l1 < 0;
             const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
             const unsigned mf0 = __ballot_sync(FULL, f0), mf1 = __ballot_sync(FULL, f1);
@@ -1006,7 +1007,7 @@ beam_trace_kernel(const TraceArgs a)
                     qn -= take;
                     __syncwarp();
                     bool h0, h1; int l0, l1;
-                    beam_node<INSTR>(gnodes, node, bf, s_offu, s_offv, s_wu, s_wv, h0, h1, l0, l1, cn.n_box);
+                    beam_node<INSTR>(gnodes, node, bf, s_offu, s_offv, s_wu, s_wv, h0, h1, l0, l1, bc.beam_box);
                     const bool p0 = h0 && l0 >= 0, p1 = h1 && l1 >= 0, f0 = h0 && l0 < 0, f1 = h1 && l1 < 0;
                     const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
                     const int np0 = __popc(mp0), np1 = __popc(mp1);
@@ -1034,6 +1035,7 @@ beam_trace_kernel(const TraceArgs a)
                     __syncwarp();
                     for (int c = lane; c < ncand; c += 32) {
                         const int f = W.u.b.cid[c];
+                        if (INSTR) bc.setups++;
                         beam_setup(__ldg(gtri + 3 * f), __ldg(gtri + 3 * f + 1), __ldg(gtri + 3 * f + 2), em, s_offu, s_offv,
                                    W.u.b.eq + 3 * c);
                     }
@@ -1052,6 +1054,7 @@ beam_trace_kernel(const TraceArgs a)
                         const int c = base + lane;
                         bool keep = false;
                         if (c < ncand) {
+                            if (INSTR) bc.rect++;
                             const float4 E0 = W.u.b.eq[3 * c], E1 = W.u.b.eq[3 * c + 1], E2 = W.u.b.eq[3 * c + 2];
                             // largest value of each edge function over the rectangle (monotone in fp32 too)
                             const float m0 = fmaf(E0.x, E0.x >= 0.f ? gu1 : gu0, fmaf(E0.y, E0.y >= 0.f ? gv1 : gv0, E0.z));
@@ -1107,7 +1110,7 @@ beam_trace_kernel(const TraceArgs a)
                     const float t = fmaf(E0.w, lu, fmaf(E1.w, lv, E2.w));
                     if (fminf(e0, fminf(e1, e2)) >= 0.0f && t < tbest) { tbest = t; best = c; }
                 }
-                if (INSTR && on) cn.n_tri += (unsigned)ng;
+                if (INSTR && on) bc.tri2d += (unsigned)ng;
                 if (best >= 0) best = W.u.b.cid[best];
                 if (!on) best = -1;
                 int fate = -1, src = -1, depth = 0;
@@ -1182,8 +1185,10 @@ struct SmallSmem {                  // per warp
 
 // Candidates of `in` (n_in of them; nullptr = all triangles 0..n_in-1) whose edge functions admit the
 // rectangle [u0,u1] x [v0,v1] -> out; returns how many.  Warp-wide call.
+template <bool INSTR>
 __device__ __forceinline__ int small_filter(const float4 *eq, const unsigned char *in, int n_in, float u0, float u1,
-                                            float v0, float v1, unsigned char *out, int lane, unsigned lt_mask)
+                                            float v0, float v1, unsigned char *out, int lane, unsigned lt_mask,
+                                            unsigned &n_rect)
 {
     int n = 0;
     for (int base = 0; base < n_in; base += 32) {
@@ -1191,6 +1196,7 @@ __device__ __forceinline__ int small_filter(const float4 *eq, const unsigned cha
         bool keep = false;
         int c = 0;
         if (x < n_in) {
+            if (INSTR) ++n_rect;
             c = in ? (int)in[x] : x;
             const float4 E0 = eq[3 * c], E1 = eq[3 * c + 1], E2 = eq[3 * c + 2];
             const float m0 = fmaf(E0.x, E0.x >= 0.f ? u1 : u0, fmaf(E0.y, E0.y >= 0.f ? v1 : v0, E0.z));
@@ -1222,7 +1228,7 @@ small_beam_kernel(const TraceArgs a)
     WarpQueue &Q = W.q;
     unsigned long long *qsig = s_qsig + (INSTR ? warp * QCAP : 0);
     LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    BeamCounters bc = { 0, 0, 0, 0 };
+    BeamCounters bc = { 0, 0, 0, 0, 0, 0, 0, 0 };
     const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
     const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
     const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
@@ -1306,10 +1312,13 @@ small_beam_kernel(const TraceArgs a)
         // tile level: set every triangle up in the tile's local emitter frame; which ones touch the tile?
         const uint32_t tcx0 = compact_even_bits(start), tcy0 = compact_even_bits(start >> 1);
         const float offu = fmaf((float)tcx0 * inv_nx, em.du, em.u0), offv = fmaf((float)tcy0 * inv_ny, em.dv, em.v0);
-        for (int c = lane; c < T; c += 32) beam_setup(W.tri[3 * c], W.tri[3 * c + 1], W.tri[3 * c + 2], em, offu, offv, W.eq + 3 * c);
+        for (int c = lane; c < T; c += 32) {
+            if (INSTR) bc.setups++;
+            beam_setup(W.tri[3 * c], W.tri[3 * c + 1], W.tri[3 * c + 2], em, offu, offv, W.eq + 3 * c);
+        }
         __syncwarp();
         const float t_wu = (float)(1u << ((tbits + 1) >> 1)) * csu, t_wv = (float)(1u << (tbits >> 1)) * csv;
-        const int n_tl = small_filter(W.eq, nullptr, T, 0.0f, t_wu, 0.0f, t_wv, W.tl, lane, lt_mask);
+        const int n_tl = small_filter<INSTR>(W.eq, nullptr, T, 0.0f, t_wu, 0.0f, t_wv, W.tl, lane, lt_mask, bc.rect);
         if (n_tl == 0) {
             const unsigned c = nt >= 32u ? nt >> 5 : (unsigned)(lane < (int)nt);
             cn.launched += c; cn.pmiss += c; cn.segments += c; bc.tile_miss += c;
@@ -1321,8 +1330,8 @@ small_beam_kernel(const TraceArgs a)
         const uint32_t g_wx = nb >= 32u ? 8u : s_wx, g_wy = nb >= 32u ? 4u : s_wy;
         for (uint32_t sb = start; sb < end; sb += nb) {
             const uint32_t scx = compact_even_bits(sb) - tcx0, scy = compact_even_bits(sb >> 1) - tcy0;   // cells from the tile corner
-            const int n_sl = small_filter(W.eq, W.tl, n_tl, (float)scx * csu, (float)(scx + s_wx) * csu, (float)scy * csv,
-                                          (float)(scy + s_wy) * csv, W.sl, lane, lt_mask);
+            const int n_sl = small_filter<INSTR>(W.eq, W.tl, n_tl, (float)scx * csu, (float)(scx + s_wx) * csu, (float)scy * csv,
+                                          (float)(scy + s_wy) * csv, W.sl, lane, lt_mask, bc.rect);
             if (n_sl == 0) {
                 const unsigned c = nb >= 32u ? nb >> 5 : (unsigned)(lane < (int)nb);
                 cn.launched += c; cn.pmiss += c; cn.segments += c; bc.block_miss += c;
@@ -1330,8 +1339,8 @@ small_beam_kernel(const TraceArgs a)
             }
             for (uint32_t gs = sb; gs < sb + nb; gs += 32) {
                 const uint32_t gcx = compact_even_bits(gs) - tcx0, gcy = compact_even_bits(gs >> 1) - tcy0;
-                const int ng = small_filter(W.eq, W.sl, n_sl, (float)gcx * csu, (float)(gcx + g_wx) * csu, (float)gcy * csv,
-                                            (float)(gcy + g_wy) * csv, W.gl, lane, lt_mask);
+                const int ng = small_filter<INSTR>(W.eq, W.sl, n_sl, (float)gcx * csu, (float)(gcx + g_wx) * csu, (float)gcy * csv,
+                                            (float)(gcy + g_wy) * csv, W.gl, lane, lt_mask, bc.rect);
                 if (ng == 0) {
                     const unsigned c = (unsigned)(lane < (int)nb);
                     cn.launched += c; cn.pmiss += c; cn.segments += c; bc.group_miss += c;
@@ -1370,7 +1379,7 @@ small_beam_kernel(const TraceArgs a)
                     // ties -> smallest index, as O-step 4 (the list is in index order)
                     if (fminf(e0, fminf(e1, e2)) >= 0.0f && t < tbest) { tbest = t; best = c; }
                 }
-                if (INSTR && on) cn.n_tri += (unsigned)ng;
+                if (INSTR && on) bc.tri2d += (unsigned)ng;
                 if (!on) best = -1;
                 int fate = -1, src = -1, depth = 0;
                 unsigned long long sig = 0;
