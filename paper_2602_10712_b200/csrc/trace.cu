@@ -882,7 +882,6 @@ beam_trace_kernel(const TraceArgs a)
                 break;
             }
             // traverse until every lane is done, or enough lanes are free and rays are waiting
-            // traverse until every lane is done, or enough lanes are free and rays are waiting
             for (;;) {
                 while ((unsigned)cur < (unsigned)CUR_DONE) {
                     if (INSTR) cn.n_box += 2;
