@@ -883,7 +883,15 @@ beam_trace_kernel(const TraceArgs a)
             }
             // traverse until every lane is done, or enough lanes are free and rays are waiting
             for (;;) {
+#ifndef NODE_RUN_CAP
+#define NODE_RUN_CAP 8
+#endif
+#if NODE_RUN_CAP > 0
+#pragma unroll 1
+                for (int steps = 0; steps < NODE_RUN_CAP && (unsigned)cur < (unsigned)CUR_DONE; ++steps) {
+#else
                 while ((unsigned)cur < (unsigned)CUR_DONE) {
+#endif
                     if (INSTR) cn.n_box += 2;
                     cur = bvh_node_step<STRIDE, NSMEM>(ln, cur, sp, s_stack, ovf, idx, idy, idz, oxi, oyi, ozi, tbest);
                 }
