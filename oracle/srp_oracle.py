@@ -73,6 +73,8 @@ def lib():
             ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int,
             ctypes.c_ulonglong, ctypes.POINTER(Options),
             ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats), ctypes.c_void_p, ctypes.c_void_p]
+        L.srp_oracle_forces_torques.restype = ctypes.c_int
+        L.srp_oracle_forces_torques.argtypes = L.srp_oracle_forces.argtypes + [ctypes.c_void_p] * 3
         L.srp_oracle_philox.restype = None
         L.srp_oracle_philox.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_uniform.restype = ctypes.c_double
@@ -117,11 +119,13 @@ def build_mesh(family, theta, k=0, mesh_seed=2):
 
 
 def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sampler=0,
-           deposit=0, want_first_hit=False, want_path_sig=False):
+           deposit=0, want_first_hit=False, want_path_sig=False, x_com=None):
     """Forces of ONE design for the given sun directions.
 
     Returns dict(F f64[S,3], sumsq f64[S,3], sigma f64[S] (i.i.d. standard error of |F|,
     conservative for the stratified sampler), stats dict, first_hit int32[S,N] or None).
+    With x_com (3 floats, the centre of mass of PAPER.md:136 Eq. 4) also T f64[S,3] (torque, N m)
+    and sigma_T f64[S].
     """
     verts = np.ascontiguousarray(verts, dtype=np.float32).reshape(-1, 3, 3)
     mats = np.ascontiguousarray(mats, dtype=np.float32).reshape(-1, 3)
@@ -133,13 +137,24 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
     fh = np.empty((S, N), dtype=np.int32) if want_first_hit else None
     ps = np.empty((S, N), dtype=np.uint64) if want_path_sig else None
     opt = Options(float(P), int(sampler), int(deposit))
-    rc = lib().srp_oracle_forces(verts.ctypes.data, mats.ctypes.data, T, int(k), sun.ctypes.data,
-                                 S, int(j0), int(N), int(B), int(seed), ctypes.byref(opt),
-                                 F.ctypes.data, Q.ctypes.data, ctypes.byref(st),
-                                 fh.ctypes.data if fh is not None else None,
-                                 ps.ctypes.data if ps is not None else None)
+    args = (verts.ctypes.data, mats.ctypes.data, T, int(k), sun.ctypes.data,
+            S, int(j0), int(N), int(B), int(seed), ctypes.byref(opt),
+            F.ctypes.data, Q.ctypes.data, ctypes.byref(st),
+            fh.ctypes.data if fh is not None else None,
+            ps.ctypes.data if ps is not None else None)
+    Tq = TQ = None
+    if x_com is None:
+        rc = lib().srp_oracle_forces(*args)
+    else:
+        xc = np.ascontiguousarray(x_com, dtype=np.float64).reshape(3)
+        Tq = np.zeros((S, 3)); TQ = np.zeros((S, 3))
+        rc = lib().srp_oracle_forces_torques(*args, xc.ctypes.data, Tq.ctypes.data, TQ.ctypes.data)
     if rc != 0:
         raise ValueError("srp_oracle_forces: invalid arguments")
     var = np.maximum(Q - F * F / float(N), 0.0)     # N * sample variance of the photon totals
     sigma = np.sqrt(var.sum(axis=1))
-    return {"F": F, "sumsq": Q, "sigma": sigma, "stats": st.as_dict(), "first_hit": fh, "path_sig": ps}
+    out = {"F": F, "sumsq": Q, "sigma": sigma, "stats": st.as_dict(), "first_hit": fh, "path_sig": ps}
+    if Tq is not None:
+        out["T"] = Tq
+        out["sigma_T"] = np.sqrt(np.maximum(TQ - Tq * Tq / float(N), 0.0).sum(axis=1))
+    return out

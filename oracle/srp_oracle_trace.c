@@ -14,9 +14,13 @@
  * no blocking or reordering.  Only the facet-material lobe thresholds are
  * taken in fp32 (they decide an integer: which lobe) -- DESIGN.md R17.
  *
+ * Torque (Eq. 4): tau = int_M (x - x_COM) x f(x) dx -- every
+ * momentum deposit, made at hit point x, also contributes (x - x_COM) x deposit.
+ *
  * Pins (tests/test_oracle_*.py): Philox KAT, flat plate, convex polyhedron,
  * cannonball limit, occlusion, V-groove, perpendicular-plate form factor,
- * conservation, symmetries, N^-1/2 decay, estimator agreement.
+ * conservation, symmetries, N^-1/2 decay, estimator agreement; torque: off-centre
+ * plate, two-plate windmill, centre-of-mass shift identity, centred sphere.
  */
 #include <stdlib.h>
 #include <string.h>
@@ -62,6 +66,16 @@ static long closest_hit(const double *v0, const double *e1, const double *e2, lo
     return best;
 }
 
+/* A momentum deposit dd made at point x: force total dp += dd, torque total dq += (x - xc) x dd (Eq. 4). */
+static void orc_deposit(const double dd[3], orc_v3 x, orc_v3 xc, double dp[3], double dq[3])
+{
+    const orc_v3 r = orc_sub(x, xc);
+    dp[0] += dd[0]; dp[1] += dd[1]; dp[2] += dd[2];
+    dq[0] += r.y * dd[2] - r.z * dd[1];
+    dq[1] += r.z * dd[0] - r.x * dd[2];
+    dq[2] += r.x * dd[1] - r.y * dd[0];
+}
+
 static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
 {
     uint32_t x = 0, y = 0;
@@ -85,13 +99,16 @@ static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
  *   first_hit int32[S][N] primary-hit triangle (-1 miss), may be NULL
  *   path_sig uint64[S][N] bookkeeping for the divergent-ray count, may be NULL: sig = 0, then
  *       sig = sig*1000003 + (triangle index + 1) at every hit (mod 2^64)
+ *   x_com double[3] centre of mass (Eq. 4), Tq double[S][3] torque in N m, tq_sumsq double[S][3]
+ *       sum of squared per-photon torque totals: all three may be NULL (no torque)
  * Returns 0, or -1 on invalid arguments.
  */
-int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
-                      const float *sun_dirs, int S, int j0, long long N, int B,
-                      unsigned long long seed, const orc_options *opt,
-                      double *F, double *sumsq, orc_stats *stats, int *first_hit,
-                      unsigned long long *path_sig)
+int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int k,
+                              const float *sun_dirs, int S, int j0, long long N, int B,
+                              unsigned long long seed, const orc_options *opt,
+                              double *F, double *sumsq, orc_stats *stats, int *first_hit,
+                              unsigned long long *path_sig, const double *x_com, double *Tq,
+                              double *tq_sumsq)
 {
     if (!verts || !mats || !sun_dirs || !F || !opt || T <= 0 || S <= 0 || N <= 0 || B < 0 || B > 15)
         return -1;
@@ -139,7 +156,8 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
         }
         const double Ae = (u1 - u0) * (vv1 - vv0);
         const double wph = P * Ae / (double)N;
-        double Fj[3] = { 0, 0, 0 }, Qj[3] = { 0, 0, 0 };
+        double Fj[3] = { 0, 0, 0 }, Qj[3] = { 0, 0, 0 }, Tj[3] = { 0, 0, 0 }, TQj[3] = { 0, 0, 0 };
+        const orc_v3 xc = x_com ? orc_mk(x_com[0], x_com[1], x_com[2]) : orc_mk(0.0, 0.0, 0.0);
 
         for (long long i = 0; i < N && Ae > 0.0; ++i) {
             /* O-step 3: ray i. */
@@ -159,7 +177,7 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
             orc_v3 d = s;
             long src = -1;
             int depth = 0;
-            double dp[3] = { 0, 0, 0 };
+            double dp[3] = { 0, 0, 0 }, dq[3] = { 0, 0, 0 };
             unsigned long long sig = 0;
             st.launched++;
             for (;;) {
@@ -181,11 +199,13 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                 orc_v3 refl = orc_add(d, orc_scale(nf, 2.0 * cost));
                 orc_v3 x = orc_add(o, orc_scale(d, t));
                 const double al = mats[3 * f], rs = mats[3 * f + 1], rd = mats[3 * f + 2];
+                /* dd = this hit's momentum deposit, made at x; Eq. 4: torque += (x - x_COM) x dd */
+                double dd[3] = { 0, 0, 0 };
                 if (opt->deposit == 0) {
                     double a = al + rs + rd;
-                    dp[0] += wph * (a * d.x - rs * refl.x - (2.0 / 3.0) * rd * nf.x);
-                    dp[1] += wph * (a * d.y - rs * refl.y - (2.0 / 3.0) * rd * nf.y);
-                    dp[2] += wph * (a * d.z - rs * refl.z - (2.0 / 3.0) * rd * nf.z);
+                    dd[0] = wph * (a * d.x - rs * refl.x - (2.0 / 3.0) * rd * nf.x);
+                    dd[1] = wph * (a * d.y - rs * refl.y - (2.0 / 3.0) * rd * nf.y);
+                    dd[2] = wph * (a * d.z - rs * refl.z - (2.0 / 3.0) * rd * nf.z);
                 }
                 /* O-step 6: lobe selection (thresholds in fp32, R17). */
                 uint32_t c2[4] = { (uint32_t)i, j, (uint32_t)k, (uint32_t)(depth + 1) }, y[4];
@@ -195,7 +215,8 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                 const float th2 = mats[3 * f] + mats[3 * f + 1];
                 orc_v3 dnew;
                 if (z0 < (double)th1) {
-                    if (opt->deposit == 1) { dp[0] += wph * d.x; dp[1] += wph * d.y; dp[2] += wph * d.z; }
+                    if (opt->deposit == 1) { dd[0] = wph * d.x; dd[1] = wph * d.y; dd[2] = wph * d.z; }
+                    orc_deposit(dd, x, xc, dp, dq);
                     st.absorbed++;
                     break;
                 } else if (z0 < (double)th2) {
@@ -211,24 +232,44 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                     dnew = orc_add(orc_add(orc_scale(tu, lx), orc_scale(tv, ly)), orc_scale(nf, lz));
                 }
                 if (opt->deposit == 1) {
-                    dp[0] += wph * (d.x - dnew.x); dp[1] += wph * (d.y - dnew.y); dp[2] += wph * (d.z - dnew.z);
+                    dd[0] = wph * (d.x - dnew.x); dd[1] = wph * (d.y - dnew.y); dd[2] = wph * (d.z - dnew.z);
                 }
+                orc_deposit(dd, x, xc, dp, dq);
                 /* O-step 7: depth cap. */
                 if (depth == B) { st.capped++; break; }
                 o = x; d = dnew; src = f; depth += 1;
             }
-            for (int c = 0; c < 3; ++c) { Fj[c] += dp[c]; Qj[c] += dp[c] * dp[c]; }
+            for (int c = 0; c < 3; ++c) {
+                Fj[c] += dp[c]; Qj[c] += dp[c] * dp[c];
+                Tj[c] += dq[c]; TQj[c] += dq[c] * dq[c];
+            }
             if (path_sig) path_sig[(long long)jj * N + i] = sig;
         }
         if (!(Ae > 0.0) && first_hit)
             for (long long i = 0; i < N; ++i) first_hit[(long long)jj * N + i] = -1;
         if (!(Ae > 0.0) && path_sig)
             for (long long i = 0; i < N; ++i) path_sig[(long long)jj * N + i] = 0;
-        for (int c = 0; c < 3; ++c) { F[3 * jj + c] = Fj[c]; if (sumsq) sumsq[3 * jj + c] = Qj[c]; }
+        for (int c = 0; c < 3; ++c) {
+            F[3 * jj + c] = Fj[c];
+            if (sumsq) sumsq[3 * jj + c] = Qj[c];
+            if (Tq) Tq[3 * jj + c] = Tj[c];
+            if (tq_sumsq) tq_sumsq[3 * jj + c] = TQj[c];
+        }
     }
     if (stats) *stats = st;
     free(v0); free(e1); free(e2); free(nrm);
     return 0;
+}
+
+/* Forces only (the call the force tests and timings use). */
+int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
+                      const float *sun_dirs, int S, int j0, long long N, int B,
+                      unsigned long long seed, const orc_options *opt,
+                      double *F, double *sumsq, orc_stats *stats, int *first_hit,
+                      unsigned long long *path_sig)
+{
+    return srp_oracle_forces_torques(verts, mats, T, k, sun_dirs, S, j0, N, B, seed, opt, F, sumsq, stats,
+                                     first_hit, path_sig, NULL, NULL, NULL);
 }
 
 /* Philox and the uniform map exposed for the known-answer tests. */
