@@ -143,6 +143,19 @@ srp_status srp_forces_pairs(srp_context *ctx, const srp_designs *designs, const 
                             const int *pairs, long long n_pairs, long long rays_per_dir,
                             int max_bounces, unsigned long long seed, float *out_forces);
 
+/* Forces AND torques (Eq. 4: tau = int (x - x_COM) x f(x) dx; the paper's simulator
+ * returns both).  x_com DEVICE float[D,3]: centre of mass of each design in the body frame, or
+ * NULL for the origin.  out_torques DEVICE float[D,S,3] (or [n_pairs,3]) in N m.  Every momentum deposit of
+ * srp_forces, made at hit point x, also adds (x - x_COM) x deposit; out_forces is what srp_forces returns
+ * (same photons; sums may differ in the last bits).  Enqueues only. */
+srp_status srp_forces_torques(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                              long long rays_per_dir, int max_bounces, unsigned long long seed,
+                              const float *x_com, float *out_forces, float *out_torques);
+srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                                    const int *pairs, long long n_pairs, long long rays_per_dir, int max_bounces,
+                                    unsigned long long seed, const float *x_com, float *out_forces,
+                                    float *out_torques);
+
 /* Host-buffer convenience (the end-to-end call): theta-independent; sun_dirs_host HOST float[S,3],
  * out_forces_host HOST float[D,S,3].  Copies in, runs srp_forces, copies out, syncs. */
 srp_status srp_forces_host(srp_context *ctx, const srp_designs *designs, const float *sun_dirs_host,

@@ -51,6 +51,7 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_family_n_params", "srp_family_tri_count", "srp_build_designs",
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
+           "srp_forces_torques", "srp_forces_torques_pairs",
            "srp_first_hits", "srp_path_signatures", "srp_get_stats", "srp_probe_peaks"]
 
 _lib = None
@@ -84,6 +85,8 @@ def load_library():
     L.srp_forces.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
     L.srp_forces_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_forces_host.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
+    L.srp_forces_torques.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp, vp]
+    L.srp_forces_torques_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp, vp]
     L.srp_first_hits.argtypes = [vp, vp, vp, ci, vp, ll, ll, ull, ci, vp]
     L.srp_path_signatures.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_get_stats.argtypes = [vp, ctypes.POINTER(srp_stats)]
@@ -210,6 +213,41 @@ class Context:
                                               out.data_ptr()))
         self.stream.synchronize()
         return out
+
+    def _xcom(self, designs, x_com):
+        if x_com is None:
+            return None
+        x = torch.as_tensor(x_com).to(device=self.device, dtype=torch.float32).contiguous()
+        if tuple(x.shape) != (designs.D, 3):
+            raise ValueError("x_com must be [D, 3]")
+        return x
+
+    def srp_forces_torques(self, designs, sun_dirs, rays_per_dir, max_bounces, seed=0, x_com=None):
+        """Forces and torques about x_com ([D,3], None = origin): two CUDA float32 [D,S,3] tensors."""
+        if not (sun_dirs.is_cuda and sun_dirs.dtype == torch.float32 and sun_dirs.is_contiguous()):
+            raise ValueError("sun_dirs must be a contiguous CUDA float32 tensor")
+        S = sun_dirs.shape[0]
+        x = self._xcom(designs, x_com)
+        F = torch.empty((designs.D, S, 3), dtype=torch.float32, device=self.device)
+        T = torch.empty((designs.D, S, 3), dtype=torch.float32, device=self.device)
+        self._check(self.lib.srp_forces_torques(self.handle, designs.handle, sun_dirs.data_ptr(), S, rays_per_dir,
+                                                max_bounces, seed, x.data_ptr() if x is not None else None,
+                                                F.data_ptr(), T.data_ptr()))
+        self.stream.synchronize()
+        return F, T
+
+    def srp_forces_torques_pairs(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0, x_com=None):
+        pairs = torch.as_tensor(pairs).to(device=self.device, dtype=torch.int32).contiguous()
+        x = self._xcom(designs, x_com)
+        F = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
+        T = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
+        self._check(self.lib.srp_forces_torques_pairs(self.handle, designs.handle, sun_dirs.data_ptr(),
+                                                      sun_dirs.shape[0], pairs.data_ptr(), pairs.shape[0],
+                                                      rays_per_dir, max_bounces, seed,
+                                                      x.data_ptr() if x is not None else None, F.data_ptr(),
+                                                      T.data_ptr()))
+        self.stream.synchronize()
+        return F, T
 
     def srp_forces_host(self, designs, sun_dirs_host, rays_per_dir, max_bounces, seed=0, out_host=None):
         """Host buffers in and out (numpy float32 or pinned CPU tensors); synchronous."""

@@ -116,7 +116,8 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     while ((1LL << a.log2N) < N) ++a.log2N;
     a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
     a.sampler = ctx->opt.sampler; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
-    a.accum = ctx->accum; a.stats = ctx->stats; a.work_counter = ctx->work_counter;
+    a.accum = ctx->accum; a.acc_stride = 3; a.torque = 0; a.xcom = nullptr;
+    a.stats = ctx->stats; a.work_counter = ctx->work_counter;
     // tile size: large tiles amortise the per-item set-up and the drain at the end of a tile; shrink
     // them only when there would be too few items to occupy every resident warp several times
     const bool brute = !dz->has_bvh;
@@ -133,20 +134,24 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     return a;
 }
 
+// out_torques != nullptr: also the torque about x_com (DEVICE float[D,3], or nullptr = the origin), Eq. 4.
 srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
-                      long long n_pairs, long long N, int B, unsigned long long seed, float *out)
+                      long long n_pairs, long long N, int B, unsigned long long seed, float *out,
+                      const float *x_com = nullptr, float *out_torques = nullptr)
 {
-    srp_status st = ensure_workspace(ctx, (size_t)n_pairs * 3);
+    const int stride = out_torques ? 6 : 3;
+    srp_status st = ensure_workspace(ctx, (size_t)n_pairs * stride);
     if (st != SRP_OK) return st;
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
-    TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * n_pairs, ctx->stream), "zero accumulators");
+    a.accum = ctx->accum; a.acc_stride = stride; a.torque = out_torques ? 1 : 0; a.xcom = x_com;
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * stride * n_pairs, ctx->stream), "zero accumulators");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
     st = ensure_pool(ctx, a, brute, ctx->opt.instrumented != 0);
     if (st != SRP_OK) return st;
     TRY_CUDA(ctx, srp_launch_trace(a, brute, ctx->opt.instrumented != 0, ctx->num_sms, ctx->stream), "trace launch");
-    TRY_CUDA(ctx, srp_launch_finalize(a, out, ctx->stream), "finalize launch");
+    TRY_CUDA(ctx, srp_launch_finalize(a, out, out_torques, ctx->stream), "finalize launch");
     return SRP_OK;
 }
 
@@ -335,6 +340,28 @@ srp_status srp_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
     return run_forces(ctx, dz, sun_dirs, S, nullptr, (long long)dz->D * S, N, B, seed, out);
 }
 
+srp_status srp_forces_torques(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, long long N, int B,
+                              unsigned long long seed, const float *x_com, float *out_forces, float *out_torques)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out_forces);
+    if (st != SRP_OK) return st;
+    if (!out_torques) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    cudaSetDevice(ctx->device);
+    return run_forces(ctx, dz, sun_dirs, S, nullptr, (long long)dz->D * S, N, B, seed, out_forces, x_com, out_torques);
+}
+
+srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S,
+                                    const int *pairs, long long n_pairs, long long N, int B, unsigned long long seed,
+                                    const float *x_com, float *out_forces, float *out_torques)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out_forces);
+    if (st != SRP_OK) return st;
+    if (!out_torques) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    if (!pairs || n_pairs <= 0) return fail(ctx, SRP_ERR_INVALID, "bad pair list");
+    cudaSetDevice(ctx->device);
+    return run_forces(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed, out_forces, x_com, out_torques);
+}
+
 srp_status srp_forces_pairs(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
                             long long n_pairs, long long N, int B, unsigned long long seed, float *out)
 {
@@ -395,6 +422,7 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const fl
     st = ensure_workspace(ctx, (size_t)n_pairs * 3);
     if (st != SRP_OK) return st;
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
+    a.accum = ctx->accum;
     a.sig_out = out_sig;
     TRY_CUDA(ctx, cudaMemsetAsync(out_sig, 0, sizeof(unsigned long long) * n_pairs * N, ctx->stream), "zero signatures");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * n_pairs, ctx->stream), "zero accumulators");

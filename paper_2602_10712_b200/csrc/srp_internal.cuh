@@ -85,7 +85,10 @@ struct TraceArgs {
     uint32_t key0, key1;
     int sampler, deposit;
     double P;
-    long long *accum;        // [n_pairs*3]
+    long long *accum;        // [n_pairs*acc_stride]: force (and torque) sums in 2^-32 fixed point
+    int acc_stride;          // 3, or 6 with torque
+    int torque;              // 1: also accumulate torque about xcom
+    const float *xcom;       // [D,3] centres of mass, or nullptr (origin)
     DevStats *stats;
     unsigned long long *work_counter;
     long long tiles_per_pair;
@@ -104,7 +107,7 @@ cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_par
 cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream);
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms,
                              cudaStream_t stream);
-cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, cudaStream_t stream);
+cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream);
 cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream);
 cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
 

@@ -97,6 +97,8 @@ struct RayGen {            // warp-uniform per work item
     uint32_t j, k, key0, key1;
     int sampler;
     float inv_nx, inv_ny;
+    int torque;            // also accumulate (x - x_COM) x deposit (Eq. 4)
+    float3 xc;             // the design's centre of mass
 };
 
 // O-step 3: ray i of the pair.
@@ -268,9 +270,18 @@ enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2 };
 __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
                                       const int deposit, float3 &o, float3 &d, int &src, int &depth,
-                                      float3 &acc)
+                                      float3 &acc, float3 &acc_t)
 {
     (void)q0;
+    // every deposit of this hit is made at the hit point x; Eq. 4: torque += (x - x_COM) x deposit
+    const float3 x = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
+    auto put = [&](const float3 dd) {
+        acc.x += dd.x; acc.y += dd.y; acc.z += dd.z;
+        if (g.torque) {
+            const float3 r = f3(x.x - g.xc.x, x.y - g.xc.y, x.z - g.xc.z), m = cross3(r, dd);
+            acc_t.x += m.x; acc_t.y += m.y; acc_t.z += m.z;
+        }
+    };
     const float al = q0.w, rs = q1.w, rd = q2.w;
     float3 n = cross3(f3(q1.x, q1.y, q1.z), f3(q2.x, q2.y, q2.z));
     const float inv_len = 1.0f / sqrtf(dot3(n, n));
@@ -281,16 +292,14 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     const float3 refl = f3(fmaf(2.0f * cost, nf.x, d.x), fmaf(2.0f * cost, nf.y, d.y), fmaf(2.0f * cost, nf.z, d.z));
     if (deposit == 0) {                                           // expected-value deposit
         const float a = al + rs + rd, c = (2.0f / 3.0f) * rd;
-        acc.x += a * d.x - rs * refl.x - c * nf.x;
-        acc.y += a * d.y - rs * refl.y - c * nf.y;
-        acc.z += a * d.z - rs * refl.z - c * nf.z;
+        put(f3(a * d.x - rs * refl.x - c * nf.x, a * d.y - rs * refl.y - c * nf.y, a * d.z - rs * refl.z - c * nf.z));
     }
     uint32_t y0, y1, y2, y3;
     philox4(i, g.j, g.k, (uint32_t)(depth + 1), g.key0, g.key1, y0, y1, y2, y3);
     const float z0 = uniform23(y0);
     float3 dn;
     if (z0 < al) {                                                // absorbed
-        if (deposit == 1) { acc.x += d.x; acc.y += d.y; acc.z += d.z; }
+        if (deposit == 1) put(d);
         return SHADE_ABSORBED;
     } else if (z0 < al + rs) {                                    // ideal mirror (R3)
         dn = refl;
@@ -307,14 +316,13 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
         dn = f3(fmaf(lx, tu.x, fmaf(ly, tv.x, lz * nf.x)), fmaf(lx, tu.y, fmaf(ly, tv.y, lz * nf.y)),
                 fmaf(lx, tu.z, fmaf(ly, tv.z, lz * nf.z)));
     }
-    if (deposit == 1) { acc.x += d.x - dn.x; acc.y += d.y - dn.y; acc.z += d.z - dn.z; }
+    if (deposit == 1) put(f3(d.x - dn.x, d.y - dn.y, d.z - dn.z));
     if (depth == B) return SHADE_CAPPED;                         // R5: B reflections followed
     // Hit point in fp32 is off the facet's plane by a few ulp of |x| + t (micrometres here).  An origin
     // that ends up BELOW the plane lets the outgoing ray hit a coplanar or convex neighbour from
     // behind -- a path the exact arithmetic of the definition never takes.  Lift the origin along the
     // facing normal by more than that error (R10: "exclude the source triangle, t > 0, no
     // epsilon" is the definition; this is the fp32 guard that keeps the CUDA path on it).
-    const float3 x = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
     const float lift = 1.0e-6f * (fabsf(x.x) + fabsf(x.y) + fabsf(x.z) + t);
     o = f3(fmaf(lift, nf.x, x.x), fmaf(lift, nf.y, x.y), fmaf(lift, nf.z, x.z));
     d = dn; src = f; depth += 1;
@@ -331,6 +339,29 @@ __device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k,
 {
     if (a.pairs) { k = a.pairs[2 * p]; j = a.pairs[2 * p + 1]; }
     else { k = (int)(p / a.S); j = (int)(p - (long long)k * a.S); }
+}
+
+__device__ __forceinline__ void set_torque(RayGen &g, const TraceArgs &a, int k)
+{
+    g.torque = a.torque;
+    g.xc = (a.torque && a.xcom) ? f3(a.xcom[3 * k], a.xcom[3 * k + 1], a.xcom[3 * k + 2]) : f3(0.f, 0.f, 0.f);
+}
+
+// S7 for one work item: per-lane fp32 sums -> fp64 warp shuffle tree -> one fixed-point atomic per component.
+// accum holds acc_stride (3, or 6 with torque) int64 per pair.
+__device__ __forceinline__ void flush_tile_acc(const TraceArgs &a, long long p, const float3 acc, const float3 acc_t, int lane)
+{
+    double s[6] = { acc.x, acc.y, acc.z, acc_t.x, acc_t.y, acc_t.z };
+    const int nc = a.torque ? 6 : 3;
+    for (int c = 0; c < nc; ++c) {
+        double v = s[c];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+        if (lane == 0) {
+            unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * p);
+            atomicAdd(dst + c, (unsigned long long)__double2ll_rn(v * SRP_ACC_SCALE));
+        }
+    }
 }
 
 // counters: warp sums, one global atomic each
@@ -391,7 +422,7 @@ trace_kernel(const TraceArgs a)
             loaded_k = k;
         }
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque(g, a, k);
         g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
         g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
         uint32_t next = (uint32_t)(q * a.tile_rays);
@@ -400,7 +431,7 @@ trace_kernel(const TraceArgs a)
         bool alive = false;
         uint32_t i = 0;
         unsigned long long sig = 0;                         // debug: hash of the hit-triangle sequence
-        float3 o = f3(0, 0, 0), d = em.s, acc = f3(0, 0, 0);
+        float3 o = f3(0, 0, 0), d = em.s, acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
         int src = -1, depth = 0;
         for (;;) {
             // S6: lanes whose photon ended take the next rays of the tile
@@ -432,7 +463,7 @@ trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    const int fate = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc);
+                    const int fate = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                     alive = fate == SHADE_CONTINUE;
@@ -441,19 +472,7 @@ trace_kernel(const TraceArgs a)
             }
         }
         // S7: warp reduction in fp64, then one fixed-point atomic per component
-        double sx = acc.x, sy = acc.y, sz = acc.z;
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            sx += __shfl_xor_sync(FULL, sx, off);
-            sy += __shfl_xor_sync(FULL, sy, off);
-            sz += __shfl_xor_sync(FULL, sz, off);
-        }
-        if (lane == 0) {
-            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
-            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
-            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
-            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
-        }
+        flush_tile_acc(a, p, acc, acc_t, lane);
     }
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
 }
@@ -505,13 +524,13 @@ bvh_trace_kernel(const TraceArgs a)
         const float4 *gtri = a.dz.tri + 3 * tbase;
         const float4 *gnodes = a.dz.nodes + 4 * tbase;
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque(g, a, k);
         g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
         g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
         uint32_t next = (uint32_t)(q * a.tile_rays);
         const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
         int qcount = 0;                                   // warp-uniform
-        float3 acc = f3(0, 0, 0);
+        float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
 
         for (;;) {
             bool alive = false;
@@ -546,7 +565,7 @@ bvh_trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
                     fate = shade(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc);
+                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                 }
@@ -563,19 +582,7 @@ bvh_trace_kernel(const TraceArgs a)
             __syncwarp();
         }
         // S7: warp reduction in fp64, then one fixed-point atomic per component
-        double sx = acc.x, sy = acc.y, sz = acc.z;
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            sx += __shfl_xor_sync(FULL, sx, off);
-            sy += __shfl_xor_sync(FULL, sy, off);
-            sz += __shfl_xor_sync(FULL, sz, off);
-        }
-        if (lane == 0) {
-            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
-            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
-            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
-            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
-        }
+        flush_tile_acc(a, p, acc, acc_t, lane);
     }
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
 }
@@ -825,19 +832,24 @@ beam_trace_kernel(const TraceArgs a)
             const long long tb = a.dz.tri_off[k];
             const float4 *lt = a.dz.tri + 3 * tb;
             RayGen g;
-            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0;
+            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque(g, a, k);
             g.inv_nx = inv_nx; g.inv_ny = inv_ny;
             atomicAdd(&s_hist[warp][depth], 1u);
             if (INSTR) sig = hsig[e] * 1000003ULL + (unsigned long long)(a.dz.perm[tb + best] + 1);
-            float3 dep = f3(0, 0, 0);
+            float3 dep = f3(0, 0, 0), dep_t = f3(0, 0, 0);
             fate = shade(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
-                         a.deposit, o, d, src, depth, dep);
+                         a.deposit, o, d, src, depth, dep, dep_t);
             if (fate == SHADE_ABSORBED) cn.absorbed++;
             if (fate == SHADE_CAPPED) cn.capped++;
-            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * (long long)p);
+            unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * (long long)p);
             if (dep.x != 0.0f) atomicAdd(dst + 0, (unsigned long long)__double2ll_rn((double)dep.x * SRP_ACC_SCALE));
             if (dep.y != 0.0f) atomicAdd(dst + 1, (unsigned long long)__double2ll_rn((double)dep.y * SRP_ACC_SCALE));
             if (dep.z != 0.0f) atomicAdd(dst + 2, (unsigned long long)__double2ll_rn((double)dep.z * SRP_ACC_SCALE));
+            if (a.torque) {
+                if (dep_t.x != 0.0f) atomicAdd(dst + 3, (unsigned long long)__double2ll_rn((double)dep_t.x * SRP_ACC_SCALE));
+                if (dep_t.y != 0.0f) atomicAdd(dst + 4, (unsigned long long)__double2ll_rn((double)dep_t.y * SRP_ACC_SCALE));
+                if (dep_t.z != 0.0f) atomicAdd(dst + 5, (unsigned long long)__double2ll_rn((double)dep_t.z * SRP_ACC_SCALE));
+            }
             if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[(long long)p * a.N + i] = sig;
         }
         nhit -= take;
@@ -940,7 +952,7 @@ beam_trace_kernel(const TraceArgs a)
         const float4 *gtri = a.dz.tri + 3 * tbase;
         const float4 *gnodes = a.dz.nodes + 4 * tbase;
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque(g, a, k);
         g.inv_nx = inv_nx; g.inv_ny = inv_ny;
         BeamFrame bf;
         bf.uh = f3(0.5f * em.u.x, 0.5f * em.u.y, 0.5f * em.u.z);
@@ -957,7 +969,7 @@ beam_trace_kernel(const TraceArgs a)
         const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
         const uint32_t nt = end - start;                          // a power of two
         const int tbits = 31 - __clz((int)nt);
-        float3 acc = f3(0, 0, 0);
+        float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
 
         // tile level: frontier descent to an entry list
         const uint32_t tcx0 = compact_even_bits(start), tcy0 = compact_even_bits(start >> 1);
@@ -1132,7 +1144,7 @@ beam_trace_kernel(const TraceArgs a)
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
                         fate = shade(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                     best, g, i, a.B, a.deposit, o, d, src, depth, acc);
+                                     best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
                         if (fate == SHADE_CAPPED) cn.capped++;
                     }
@@ -1145,19 +1157,7 @@ beam_trace_kernel(const TraceArgs a)
         }
 
         // S7 for the tile's primaries: warp reduction in fp64, then one fixed-point atomic per component
-        double sx = acc.x, sy = acc.y, sz = acc.z;
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            sx += __shfl_xor_sync(FULL, sx, off);
-            sy += __shfl_xor_sync(FULL, sy, off);
-            sz += __shfl_xor_sync(FULL, sz, off);
-        }
-        if (lane == 0) {
-            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
-            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
-            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
-            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
-        }
+        flush_tile_acc(a, p, acc, acc_t, lane);
     };
 
     // ---- persistent loop: tiles until the pool is worth draining ----
@@ -1266,7 +1266,7 @@ small_beam_kernel(const TraceArgs a)
         }
         __syncwarp();
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0;
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque(g, a, k);
         g.inv_nx = inv_nx; g.inv_ny = inv_ny;
         const float csu = em.du * inv_nx, csv = em.dv * inv_ny;
         const uint32_t start = (uint32_t)(q * a.tile_rays);
@@ -1274,7 +1274,7 @@ small_beam_kernel(const TraceArgs a)
         const uint32_t nt = end - start;                          // a power of two
         const int tbits = 31 - __clz((int)nt);
         int qcount = 0;                                           // warp-uniform
-        float3 acc = f3(0, 0, 0);
+        float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
 
         // a pass of <= 32 queued bounce rays against all triangles (S4, S6)
         auto secondary_pass = [&]() {
@@ -1303,7 +1303,7 @@ small_beam_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
                     fate = shade(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
-                                 a.deposit, o, d, src, depth, acc);
+                                 a.deposit, o, d, src, depth, acc, acc_t);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                 }
@@ -1400,7 +1400,7 @@ small_beam_kernel(const TraceArgs a)
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
                         fate = shade(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
-                                     a.deposit, o, d, src, depth, acc);
+                                     a.deposit, o, d, src, depth, acc, acc_t);
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
                         if (fate == SHADE_CAPPED) cn.capped++;
                     }
@@ -1421,26 +1421,14 @@ small_beam_kernel(const TraceArgs a)
         while (qcount > 0) secondary_pass();
 
         // S7: warp reduction in fp64, then one fixed-point atomic per component
-        double sx = acc.x, sy = acc.y, sz = acc.z;
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            sx += __shfl_xor_sync(FULL, sx, off);
-            sy += __shfl_xor_sync(FULL, sy, off);
-            sz += __shfl_xor_sync(FULL, sz, off);
-        }
-        if (lane == 0) {
-            unsigned long long *dst = (unsigned long long *)(a.accum + 3 * p);
-            atomicAdd(dst + 0, (unsigned long long)__double2ll_rn(sx * SRP_ACC_SCALE));
-            atomicAdd(dst + 1, (unsigned long long)__double2ll_rn(sy * SRP_ACC_SCALE));
-            atomicAdd(dst + 2, (unsigned long long)__double2ll_rn(sz * SRP_ACC_SCALE));
-        }
+        flush_tile_acc(a, p, acc, acc_t, lane);
     }
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
     flush_beam_counters(a, bc, lane);
 }
 
 // F[p] = accum[p] * 2^-32 * P * A_e / N
-__global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float *out)
+__global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float *out, float *out_torque)
 {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= a.n_pairs) return;
@@ -1449,7 +1437,10 @@ __global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float 
     const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
     const double w = em.Ae > 0.0f ? a.P * (double)em.Ae / (double)a.N / SRP_ACC_SCALE : 0.0;
 #pragma unroll
-    for (int c = 0; c < 3; ++c) out[3 * p + c] = (float)((double)a.accum[3 * p + c] * w);
+    for (int c = 0; c < 3; ++c) out[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + c] * w);
+    if (a.torque && out_torque)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) out_torque[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + 3 + c] * w);
 }
 
 // debug: primary-hit triangle (original index) of every ray of the listed pairs
@@ -1470,7 +1461,7 @@ __global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArg
             const long long tbase = a.dz.tri_off[k];
             const int T = (int)(a.dz.tri_off[k + 1] - tbase);
             RayGen g;
-            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler;
+            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque(g, a, k);
             g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
             g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
             float3 o;
@@ -1613,9 +1604,9 @@ cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, 
                         : launch_persistent(bvh_trace_kernel<false>, a, num_sms, stream);
 }
 
-cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, cudaStream_t stream)
+cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream)
 {
-    finalize_kernel<<<(unsigned)((a.n_pairs + 255) / 256), 256, 0, stream>>>(a, out_forces);
+    finalize_kernel<<<(unsigned)((a.n_pairs + 255) / 256), 256, 0, stream>>>(a, out_forces, out_torques);
     return cudaGetLastError();
 }
 

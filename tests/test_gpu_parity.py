@@ -459,6 +459,69 @@ def test_beam_auto_mode_and_determinism(ctx):
     dz.free()
 
 
+# ---------------------------------------------------------------- torque (Eq. 4)
+@pytest.mark.parametrize("family,D,S,N,B,mode", [
+    (W.FAMILY_BOXWING, 3, 6, 1 << 14, 4, 0),        # small_beam_kernel
+    (W.FAMILY_BOXWING6, 3, 6, 1 << 12, 4, 1),       # trace_kernel (all triangles, every segment)
+    (W.FAMILY_DETAILED, 2, 3, 1 << 12, 8, 1),       # bvh_trace_kernel
+    (W.FAMILY_DETAILED, 2, 3, 1 << 12, 8, 2),       # beam_trace_kernel: tile sums + pooled hits
+])
+def test_torque_matches_oracle(ctx, oracle, family, D, S, N, B, mode):
+    """srp_forces_torques against the oracle's Eq. 4 on the same photons, off-origin centres of mass;
+    the forces it returns are those of srp_forces."""
+    th = W.draw_params(family, D)
+    sun = W.fibonacci_sphere(S)
+    x_com = np.array([[0.3, -0.2, 0.5], [-0.4, 0.1, 0.0], [0.0, 0.6, -0.7]], np.float32)[:D]
+    dz = ctx.srp_build_designs(family, th)
+    ctx.srp_set_options(primary_mode=mode)
+    try:
+        F, T = ctx.srp_forces_torques(dz, cuda(sun), N, B, seed=9, x_com=x_com)
+        F0 = ctx.srp_forces(dz, cuda(sun), N, B, 9).cpu().numpy()
+        pairs = np.array([[D - 1, 1], [0, S - 1]], np.int32)
+        Fp, Tp = ctx.srp_forces_torques_pairs(dz, cuda(sun), pairs, N, B, seed=9, x_com=x_com)
+    finally:
+        ctx.srp_set_options()
+    F, T = F.cpu().numpy(), T.cpu().numpy()
+    assert rel_l2(F.reshape(-1, 3), F0.reshape(-1, 3)).max() < 1e-6
+    assert np.array_equal(Tp.cpu().numpy(), T[pairs[:, 0], pairs[:, 1]])
+    assert np.array_equal(Fp.cpu().numpy(), F[pairs[:, 0], pairs[:, 1]])
+    for k in range(D):
+        v, m = oracle.build_mesh(family, th[k], k=k)
+        r = oracle.forces(v, m, sun, N, B, seed=9, k=k, x_com=x_com[k])
+        assert_parity(F[k], r["F"], r["sigma"], tol_agg=3e-3)
+        # same acceptance for the torque vectors, with their own standard error
+        assert_parity(T[k], r["T"], r["sigma_T"], tol_agg=3e-3)
+    dz.free()
+
+
+def test_torque_closed_forms_on_gpu(ctx):
+    """Off-centre plate: tau = (centroid - x_COM) x F; two-plate windmill: sign and lever arms; NULL x_com = origin."""
+    p0 = np.array([1.5, -1.75, 0.5]); eu = np.array([1.0, 0, 0]); ev = np.array([0, 1.5, 0.3])
+    verts = quad(p0, eu, ev)
+    centroid = p0 + 0.5 * eu + 0.5 * ev
+    normal = np.cross(eu, ev); area = np.linalg.norm(normal); normal /= area
+    dz = ctx.srp_build_designs_from_meshes(verts, const_mats(2, 0.3, 0.5, 0.2), [0, 2])
+    om = np.array([[0.3, 0.2, 0.8], [-0.5, 0.1, 0.6]], np.float32)
+    xc = np.array([[0.2, 0.1, -0.4]], np.float32)
+    F, T = ctx.srp_forces_torques(dz, cuda(om), 1 << 16, 1, seed=3, x_com=xc)
+    F0, T0 = ctx.srp_forces_torques(dz, cuda(om), 1 << 16, 1, seed=3)
+    F, T, T0 = F.cpu().numpy()[0], T.cpu().numpy()[0], T0.cpu().numpy()[0]
+    for j in range(2):
+        Fc = flat_plate_force(om[j], normal, area, 0.3, 0.5, 0.2)
+        assert np.linalg.norm(T[j] - np.cross(centroid - xc[0], Fc)) < 5e-3 * np.linalg.norm(np.cross(centroid - xc[0], Fc))
+        assert np.linalg.norm(T0[j] - np.cross(centroid, Fc)) < 5e-3 * np.linalg.norm(np.cross(centroid, Fc))
+        np.testing.assert_allclose(T[j], T0[j] - np.cross(xc[0], F[j]), rtol=0, atol=2e-6 * np.linalg.norm(T0[j]))
+    dz.free()
+    black = quad([1.5, -0.5, 0.0], [1, 0, 0], [0, 1, 0])
+    mirror = quad([-2.5, -0.5, 0.0], [1, 0, 0], [0, 1, 0])
+    dz = ctx.srp_build_designs_from_meshes(np.concatenate([black, mirror]),
+                                           np.concatenate([const_mats(2, 1, 0, 0), const_mats(2, 0, 1, 0)]), [0, 4])
+    F, T = ctx.srp_forces_torques(dz, cuda(np.array([[0, 0, 1]], np.float32)), 1 << 16, 2, seed=1)
+    T = T.cpu().numpy()[0, 0]
+    assert np.linalg.norm(T - np.array([0, -2 * P0, 0])) < 5e-3 * 2 * P0
+    dz.free()
+
+
 # ---------------------------------------------------------------- full sizes, in bench.py's launch configuration
 def test_cfg2_full_size_sampled_against_oracle(ctx, oracle):
     """The whole 256 x 1024 x 2^18 job in one srp_forces call (as bench.py launches it); 24 sampled
