@@ -140,6 +140,8 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
                       const float *x_com = nullptr, float *out_torques = nullptr)
 {
     const int stride = out_torques ? 6 : 3;
+    if (out_torques && ctx->opt.instrumented)
+        return fail(ctx, SRP_ERR_UNSUPPORTED, "torques are not available from the instrumented kernels");
     srp_status st = ensure_workspace(ctx, (size_t)n_pairs * stride);
     if (st != SRP_OK) return st;
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);

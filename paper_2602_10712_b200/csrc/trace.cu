@@ -97,8 +97,7 @@ struct RayGen {            // warp-uniform per work item
     uint32_t j, k, key0, key1;
     int sampler;
     float inv_nx, inv_ny;
-    int torque;            // also accumulate (x - x_COM) x deposit (Eq. 4)
-    float3 xc;             // the design's centre of mass
+    float3 xc;             // the design's centre of mass (TORQUE kernels: Eq. 4)
 };
 
 // O-step 3: ray i of the pair.
@@ -267,6 +266,7 @@ struct BeamCounters {       // rays resolved per beam level (lane-distributed co
 // O-steps 5-7 at a hit: deposit, lobe selection, continuation.
 // Returns SHADE_CONTINUE if the photon goes on (o, d, src, depth updated), else how it ended.
 enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2 };
+template <bool TORQUE>
 __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
                                       const int deposit, float3 &o, float3 &d, int &src, int &depth,
@@ -277,7 +277,7 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     const float3 x = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
     auto put = [&](const float3 dd) {
         acc.x += dd.x; acc.y += dd.y; acc.z += dd.z;
-        if (g.torque) {
+        if (TORQUE) {
             const float3 r = f3(x.x - g.xc.x, x.y - g.xc.y, x.z - g.xc.z), m = cross3(r, dd);
             acc_t.x += m.x; acc_t.y += m.y; acc_t.z += m.z;
         }
@@ -341,19 +341,20 @@ __device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k,
     else { k = (int)(p / a.S); j = (int)(p - (long long)k * a.S); }
 }
 
+template <bool TORQUE>
 __device__ __forceinline__ void set_torque(RayGen &g, const TraceArgs &a, int k)
 {
-    g.torque = a.torque;
-    g.xc = (a.torque && a.xcom) ? f3(a.xcom[3 * k], a.xcom[3 * k + 1], a.xcom[3 * k + 2]) : f3(0.f, 0.f, 0.f);
+    g.xc = (TORQUE && a.xcom) ? f3(a.xcom[3 * k], a.xcom[3 * k + 1], a.xcom[3 * k + 2]) : f3(0.f, 0.f, 0.f);
 }
 
 // S7 for one work item: per-lane fp32 sums -> fp64 warp shuffle tree -> one fixed-point atomic per component.
 // accum holds acc_stride (3, or 6 with torque) int64 per pair.
+template <bool TORQUE>
 __device__ __forceinline__ void flush_tile_acc(const TraceArgs &a, long long p, const float3 acc, const float3 acc_t, int lane)
 {
-    double s[6] = { acc.x, acc.y, acc.z, acc_t.x, acc_t.y, acc_t.z };
-    const int nc = a.torque ? 6 : 3;
-    for (int c = 0; c < nc; ++c) {
+    const double s[6] = { acc.x, acc.y, acc.z, acc_t.x, acc_t.y, acc_t.z };
+#pragma unroll
+    for (int c = 0; c < (TORQUE ? 6 : 3); ++c) {
         double v = s[c];
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
@@ -383,7 +384,7 @@ __device__ __forceinline__ void flush_counters(const TraceArgs &a, const LaneCou
 }
 
 // ---- the persistent trace kernel ----
-template <int MODE, bool INSTR>
+template <int MODE, bool INSTR, bool TORQUE>
 __global__ void __launch_bounds__(TRACE_THREADS, MODE == MODE_BVH ? 4 : 5)
 trace_kernel(const TraceArgs a)
 {
@@ -422,7 +423,7 @@ trace_kernel(const TraceArgs a)
             loaded_k = k;
         }
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque(g, a, k);
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque<TORQUE>(g, a, k);
         g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
         g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
         uint32_t next = (uint32_t)(q * a.tile_rays);
@@ -463,7 +464,7 @@ trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    const int fate = shade(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
+                    const int fate = shade<TORQUE>(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                     alive = fate == SHADE_CONTINUE;
@@ -472,7 +473,7 @@ trace_kernel(const TraceArgs a)
             }
         }
         // S7: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc(a, p, acc, acc_t, lane);
+        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
     }
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
 }
@@ -491,7 +492,7 @@ struct WarpQueue {
     int src_depth[QCAP];                 // (depth << 27) | src
 };
 
-template <bool INSTR>
+template <bool INSTR, bool TORQUE>
 __global__ void __launch_bounds__(TRACE_THREADS, 8)
 bvh_trace_kernel(const TraceArgs a)
 {
@@ -524,7 +525,7 @@ bvh_trace_kernel(const TraceArgs a)
         const float4 *gtri = a.dz.tri + 3 * tbase;
         const float4 *gnodes = a.dz.nodes + 4 * tbase;
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque(g, a, k);
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque<TORQUE>(g, a, k);
         g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
         g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
         uint32_t next = (uint32_t)(q * a.tile_rays);
@@ -564,7 +565,7 @@ bvh_trace_kernel(const TraceArgs a)
                 } else {
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    fate = shade(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
+                    fate = shade<TORQUE>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
                                  best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
@@ -582,7 +583,7 @@ bvh_trace_kernel(const TraceArgs a)
             __syncwarp();
         }
         // S7: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc(a, p, acc, acc_t, lane);
+        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
     }
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
 }
@@ -773,7 +774,7 @@ struct BeamSmem {                   // per warp; beam structures and drain struc
     } u;
 };
 
-template <bool INSTR>
+template <bool INSTR, bool TORQUE>
 __global__ void __launch_bounds__(TRACE_THREADS, BEAM_BLOCKS_PER_SM)
 beam_trace_kernel(const TraceArgs a)
 {
@@ -832,12 +833,12 @@ beam_trace_kernel(const TraceArgs a)
             const long long tb = a.dz.tri_off[k];
             const float4 *lt = a.dz.tri + 3 * tb;
             RayGen g;
-            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque(g, a, k);
+            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque<TORQUE>(g, a, k);
             g.inv_nx = inv_nx; g.inv_ny = inv_ny;
             atomicAdd(&s_hist[warp][depth], 1u);
             if (INSTR) sig = hsig[e] * 1000003ULL + (unsigned long long)(a.dz.perm[tb + best] + 1);
             float3 dep = f3(0, 0, 0), dep_t = f3(0, 0, 0);
-            fate = shade(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
+            fate = shade<TORQUE>(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
                          a.deposit, o, d, src, depth, dep, dep_t);
             if (fate == SHADE_ABSORBED) cn.absorbed++;
             if (fate == SHADE_CAPPED) cn.capped++;
@@ -845,7 +846,7 @@ beam_trace_kernel(const TraceArgs a)
             if (dep.x != 0.0f) atomicAdd(dst + 0, (unsigned long long)__double2ll_rn((double)dep.x * SRP_ACC_SCALE));
             if (dep.y != 0.0f) atomicAdd(dst + 1, (unsigned long long)__double2ll_rn((double)dep.y * SRP_ACC_SCALE));
             if (dep.z != 0.0f) atomicAdd(dst + 2, (unsigned long long)__double2ll_rn((double)dep.z * SRP_ACC_SCALE));
-            if (a.torque) {
+            if (TORQUE) {
                 if (dep_t.x != 0.0f) atomicAdd(dst + 3, (unsigned long long)__double2ll_rn((double)dep_t.x * SRP_ACC_SCALE));
                 if (dep_t.y != 0.0f) atomicAdd(dst + 4, (unsigned long long)__double2ll_rn((double)dep_t.y * SRP_ACC_SCALE));
                 if (dep_t.z != 0.0f) atomicAdd(dst + 5, (unsigned long long)__double2ll_rn((double)dep_t.z * SRP_ACC_SCALE));
@@ -952,7 +953,7 @@ beam_trace_kernel(const TraceArgs a)
         const float4 *gtri = a.dz.tri + 3 * tbase;
         const float4 *gnodes = a.dz.nodes + 4 * tbase;
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque(g, a, k);
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque<TORQUE>(g, a, k);
         g.inv_nx = inv_nx; g.inv_ny = inv_ny;
         BeamFrame bf;
         bf.uh = f3(0.5f * em.u.x, 0.5f * em.u.y, 0.5f * em.u.z);
@@ -1143,7 +1144,7 @@ beam_trace_kernel(const TraceArgs a)
                     else {
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                        fate = shade(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
+                        fate = shade<TORQUE>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
                                      best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
                         if (fate == SHADE_CAPPED) cn.capped++;
@@ -1157,7 +1158,7 @@ beam_trace_kernel(const TraceArgs a)
         }
 
         // S7 for the tile's primaries: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc(a, p, acc, acc_t, lane);
+        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
     };
 
     // ---- persistent loop: tiles until the pool is worth draining ----
@@ -1223,7 +1224,7 @@ __device__ __forceinline__ int small_filter(const float4 *eq, const unsigned cha
     return n;
 }
 
-template <bool INSTR>
+template <bool INSTR, bool TORQUE>
 __global__ void __launch_bounds__(TRACE_THREADS, 6)
 small_beam_kernel(const TraceArgs a)
 {
@@ -1266,7 +1267,7 @@ small_beam_kernel(const TraceArgs a)
         }
         __syncwarp();
         RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque(g, a, k);
+        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque<TORQUE>(g, a, k);
         g.inv_nx = inv_nx; g.inv_ny = inv_ny;
         const float csu = em.du * inv_nx, csv = em.dv * inv_ny;
         const uint32_t start = (uint32_t)(q * a.tile_rays);
@@ -1302,7 +1303,7 @@ small_beam_kernel(const TraceArgs a)
                 else {
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    fate = shade(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
+                    fate = shade<TORQUE>(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
                                  a.deposit, o, d, src, depth, acc, acc_t);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
@@ -1399,7 +1400,7 @@ small_beam_kernel(const TraceArgs a)
                     else {
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                        fate = shade(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
+                        fate = shade<TORQUE>(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
                                      a.deposit, o, d, src, depth, acc, acc_t);
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
                         if (fate == SHADE_CAPPED) cn.capped++;
@@ -1421,7 +1422,7 @@ small_beam_kernel(const TraceArgs a)
         while (qcount > 0) secondary_pass();
 
         // S7: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc(a, p, acc, acc_t, lane);
+        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
     }
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
     flush_beam_counters(a, bc, lane);
@@ -1461,7 +1462,7 @@ __global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArg
             const long long tbase = a.dz.tri_off[k];
             const int T = (int)(a.dz.tri_off[k + 1] - tbase);
             RayGen g;
-            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque(g, a, k);
+            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; g.xc = f3(0.f, 0.f, 0.f);
             g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
             g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
             float3 o;
@@ -1565,19 +1566,23 @@ static cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, 
 int srp_trace_blocks_per_sm(bool brute, bool beam)
 {
     int per_sm = 0;
-    if (brute && beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_beam_kernel<false>, TRACE_THREADS, 0);
-    else if (brute) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BRUTE_SMEM, false>, TRACE_THREADS, 0);
-    else if (beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false>, TRACE_THREADS, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bvh_trace_kernel<false>, TRACE_THREADS, 0);
+    if (brute && beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_beam_kernel<false, false>, TRACE_THREADS, 0);
+    else if (brute) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BRUTE_SMEM, false, false>, TRACE_THREADS, 0);
+    else if (beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false, false>, TRACE_THREADS, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bvh_trace_kernel<false, false>, TRACE_THREADS, 0);
     return per_sm * TRACE_WARPS;
 }
 
 // Words of global memory the beam kernel's per-warp ray pools need, and the ring capacity per warp.
 size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *cap_out)
 {
-    int per_sm = 0;
-    if (instrumented) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<true>, TRACE_THREADS, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false>, TRACE_THREADS, 0);
+    int per_sm = 0, per_sm_t = 0;
+    if (instrumented) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<true, false>, TRACE_THREADS, 0);
+    else {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false, false>, TRACE_THREADS, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_t, beam_trace_kernel<false, true>, TRACE_THREADS, 0);
+        if (per_sm_t > per_sm) per_sm = per_sm_t;
+    }
     if (per_sm < 1) per_sm = 1;
     int cap = 64;
     while (cap < POOL_HIGH + tile_rays + 64) cap <<= 1;
@@ -1585,23 +1590,24 @@ size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *c
     return (size_t)num_sms * per_sm * TRACE_WARPS * (instrumented ? POOL_FIELDS_INSTR : POOL_FIELDS) * (size_t)cap;
 }
 
+// Three builds of each trace kernel: plain, instrumented (test counters, path signatures), and with torque
+// accumulation.  Instrumented torque runs are refused by the caller (srp_api.cu).
+#define SRP_LAUNCH3(K_, ...)                                                                              \
+    (instrumented ? launch_persistent(K_<__VA_ARGS__ true, false>, a, num_sms, stream)                       \
+                  : a.torque ? launch_persistent(K_<__VA_ARGS__ false, true>, a, num_sms, stream)            \
+                             : launch_persistent(K_<__VA_ARGS__ false, false>, a, num_sms, stream))
+
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms, cudaStream_t stream)
 {
     if (brute) {
         if (a.dz.has_bvh)       // forced brute force over a design that also has a hierarchy (test use)
-            return instrumented ? launch_persistent(trace_kernel<MODE_BRUTE_GLOBAL, true>, a, num_sms, stream)
-                                : launch_persistent(trace_kernel<MODE_BRUTE_GLOBAL, false>, a, num_sms, stream);
-        if (a.sampler == 0 && a.primary_mode != 1)
-            return instrumented ? launch_persistent(small_beam_kernel<true>, a, num_sms, stream)
-                                : launch_persistent(small_beam_kernel<false>, a, num_sms, stream);
-        return instrumented ? launch_persistent(trace_kernel<MODE_BRUTE_SMEM, true>, a, num_sms, stream)
-                            : launch_persistent(trace_kernel<MODE_BRUTE_SMEM, false>, a, num_sms, stream);
+            return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_GLOBAL,);
+        if (a.sampler == 0 && a.primary_mode != 1) return SRP_LAUNCH3(small_beam_kernel);
+        return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_SMEM,);
     }
     if (a.sampler == 0 && a.pool != nullptr)          // beams chosen by the caller (srp_api.cu, want_beams)
-        return instrumented ? launch_persistent(beam_trace_kernel<true>, a, num_sms, stream)
-                            : launch_persistent(beam_trace_kernel<false>, a, num_sms, stream);
-    return instrumented ? launch_persistent(bvh_trace_kernel<true>, a, num_sms, stream)
-                        : launch_persistent(bvh_trace_kernel<false>, a, num_sms, stream);
+        return SRP_LAUNCH3(beam_trace_kernel);
+    return SRP_LAUNCH3(bvh_trace_kernel);
 }
 
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream)
