@@ -634,7 +634,7 @@ constexpr int BEAM_SB = BEAM_SB_DEF;        // rays per sub-block
 constexpr int BEAM_CMAX = BEAM_CMAX_DEF;      // candidate triangles per sub-block
 constexpr int BEAM_QN = 160;        // node queue of the sub-block descent
 constexpr int BEAM_EN = 64;         // tile entry list: internal nodes
-constexpr int BEAM_EL = 64;         // tile entry list: leaf links
+constexpr int BEAM_EL = 96;         // tile entry list: leaf links (<= 32 when a level starts, + 2 x 32 in that level)
 constexpr int BEAM_STACK = 16;      // per-thread stack entries in shared memory (bounce rays)
 
 struct BeamFrame {                  // warp-uniform per pair

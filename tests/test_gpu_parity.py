@@ -441,6 +441,32 @@ def test_small_design_beams_equal_brute_force(ctx, family, D, S, N, B):
     dz.free()
 
 
+@pytest.mark.parametrize("leaf_max", [1, 8])
+def test_beams_with_other_leaf_sizes(ctx, leaf_max, monkeypatch):
+    """Single-triangle leaves fill the beam's leaf lists (a tile-level frontier of 32 nodes can add 64 leaves at
+    once -- the list once held 64 and overflowed), 8-triangle leaves its candidate list: same photons either way."""
+    monkeypatch.setenv("SRP_LEAF_MAX", str(leaf_max))            # read by srp_build_designs (tuning aid)
+    th = W.draw_params(W.FAMILY_DETAILED, 1)
+    dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    monkeypatch.delenv("SRP_LEAF_MAX")
+    sun = W.fibonacci_sphere(4)
+    pairs = np.array([[0, j] for j in range(4)], np.int32)
+    res = {}
+    for mode in (1, 2):
+        ctx.srp_set_options(primary_mode=mode)
+        try:
+            F, st = run_pairs(ctx, dz, sun, pairs, 1 << 16, 8, seed=0)
+            sg = ctx.srp_path_signatures(dz, cuda(sun), pairs, 1 << 16, 8, 0).cpu().numpy().astype(np.uint64)
+        finally:
+            ctx.srp_set_options()
+        res[mode] = (F, st, sg)
+    n_div = int((res[1][2] != res[2][2]).sum())
+    assert n_div <= 3, n_div
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments"):
+        assert abs(res[1][1][key] - res[2][1][key]) <= 4 * n_div, key
+    dz.free()
+
+
 def test_beam_auto_mode_and_determinism(ctx):
     """auto: beams when rays_per_dir >= 8 x triangles.  Beam results are bit-reproducible (integer
     accumulation; the pool order does not matter)."""
