@@ -1,6 +1,10 @@
 """Builds the C-ABI library ``libsrp_b200.so`` in-tree with nvcc for sm_100a.
 
-    python -m paper_2602_10712_b200.build [--force]
+    python -m paper_2602_10712_b200.build [--force] [--bounds-check]
+
+``--bounds-check`` builds ``libsrp_b200_chk.so`` instead, with -DSRP_BOUNDS_CHECK: every write into a
+fixed-capacity list of the trace kernels traps with a message when out of range (debug aid; load it by
+setting ``paper_2602_10712_b200.binding.LIB_PATH`` before the first call).
 
 No GPU is needed to build (nvcc cross-compiles).  The library is git-ignored but travels to the
 GPU box with the working tree.
@@ -40,8 +44,14 @@ def _stale(target, deps):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force=False, verbose=False):
+def build_library(force=False, verbose=False, bounds_check=False):
     """Compile csrc/*.cu -> build/*.o -> libsrp_b200.so.  Returns the library path."""
+    global OBJ_DIR, LIB_PATH
+    extra_all = []
+    if bounds_check:
+        OBJ_DIR = os.path.join(HERE, "build_chk")
+        LIB_PATH = os.path.join(HERE, "libsrp_b200_chk.so")
+        extra_all = ["-DSRP_BOUNDS_CHECK"]
     os.makedirs(OBJ_DIR, exist_ok=True)
     headers = [os.path.join(CSRC, "srp_internal.cuh"), os.path.join(INCLUDE, "srp.h"), os.path.abspath(__file__)]
     nvcc = _nvcc()
@@ -51,7 +61,7 @@ def build_library(force=False, verbose=False):
         o = os.path.join(OBJ_DIR, src.replace(".cu", ".o"))
         objs.append(o)
         if force or _stale(o, [s] + headers):
-            cmd = [nvcc, *ARCH, *COMMON, *extra, "-c", s, "-o", o]
+            cmd = [nvcc, *ARCH, *COMMON, *extra, *extra_all, "-c", s, "-o", o]
             if verbose:
                 print(" ".join(cmd))
             procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)))
@@ -70,4 +80,4 @@ def build_library(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose=True))
+    print(build_library(force="--force" in sys.argv, verbose=True, bounds_check="--bounds-check" in sys.argv))

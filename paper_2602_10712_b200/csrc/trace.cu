@@ -13,6 +13,15 @@
 #include <cfloat>
 #include "srp_internal.cuh"
 
+// Debug build (nvcc -DSRP_BOUNDS_CHECK): every write into a fixed-capacity shared-memory list, stack or ray pool
+// checks its index and traps with a message.  compute-sanitizer is not available on the target pool.
+#ifdef SRP_BOUNDS_CHECK
+#include <cstdio>
+#define SRP_CHECK(cond, tag) do { if (!(cond)) { printf("SRP_CHECK failed: %s (trace.cu:%d)\n", tag, __LINE__); __trap(); } } while (0)
+#else
+#define SRP_CHECK(cond, tag) do { } while (0)
+#endif
+
 namespace {
 
 constexpr int TRACE_THREADS = 128;
@@ -199,6 +208,7 @@ __device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, i
     int l0 = __float_as_int(n3.x), l1 = __float_as_int(n3.y);
     if (h0 && h1) {
         if (tmin1 < tmin0) { const int t = l0; l0 = l1; l1 = t; }
+        SRP_CHECK(sp < NSMEM + STACK_OVF, "traversal stack");
         if (sp < NSMEM) s_stack[sp * STRIDE] = l1; else ovf[sp - NSMEM] = l1;
         ++sp;
 #ifdef SRP_PREFETCH_PUSH
@@ -810,6 +820,7 @@ beam_trace_kernel(const TraceArgs a)
             if (INSTR) { pool_st(pool, 9, pos, (uint32_t)sig); pool_st(pool, 10, pos, (uint32_t)(sig >> 32)); }
         }
         pool.tail += (uint32_t)__popc(m);
+        SRP_CHECK(pool.tail - pool.head <= pool.cap, "ray pool");
     };
 
     // ---- S5-S7 for <= 32 queued hits, converged; survivors go back to the pool ----
@@ -924,6 +935,7 @@ beam_trace_kernel(const TraceArgs a)
                 if (INSTR && a.sig_out) a.sig_out[(long long)rp * a.N + ri] = rsig;
             }
             const unsigned mh = __ballot_sync(FULL, hit);
+            SRP_CHECK(nhit + __popc(mh) <= HITQ, "hit queue");
             if (hit) {
                 const int e = nhit + __popc(mh & lt_mask);
                 W.u.s.hq[0][e] = __float_as_uint(o.x); W.u.s.hq[1][e] = __float_as_uint(o.y); W.u.s.hq[2][e] = __float_as_uint(o.z);
@@ -988,6 +1000,7 @@ beam_trace_kernel(const TraceArgs a)
             const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
             const unsigned mf0 = __ballot_sync(FULL, f0), mf1 = __ballot_sync(FULL, f1);
             const int np0 = __popc(mp0), nf0 = __popc(mf0), nf1 = __popc(mf1);
+            SRP_CHECK(np0 + __popc(mp1) <= BEAM_EN, "entry nodes"); SRP_CHECK(n_el + nf0 + nf1 <= BEAM_EL, "entry leaves");
             if (p0) W.u.b.enode[__popc(mp0 & lt_mask)] = l0;
             if (p1) W.u.b.enode[np0 + __popc(mp1 & lt_mask)] = l1;
             if (f0) W.u.b.eleaf[n_el + __popc(mf0 & lt_mask)] = l0;
@@ -1087,6 +1100,7 @@ beam_trace_kernel(const TraceArgs a)
                             keep = fminf(m0, fminf(m1, m2)) >= 0.0f;
                         }
                         const unsigned m = __ballot_sync(FULL, keep);
+                        SRP_CHECK(ng + __popc(m) <= BEAM_CMAX, "group list");
                         if (keep) W.u.b.glist[ng + __popc(m & lt_mask)] = (unsigned char)c;
                         ng += __popc(m);
                     }
@@ -1217,6 +1231,7 @@ __device__ __forceinline__ int small_filter(const float4 *eq, const unsigned cha
             keep = fminf(m0, fminf(m1, m2)) >= 0.0f;
         }
         const unsigned m = __ballot_sync(FULL, keep);
+        SRP_CHECK(n + __popc(m) <= SRP_BRUTE_MAX_TRIS, "small-design list");
         if (keep) out[n + __popc(m & lt_mask)] = (unsigned char)c;
         n += __popc(m);
     }
