@@ -639,10 +639,13 @@ __device__ __forceinline__ void flush_beam_counters(const TraceArgs &a, const Be
 #endif
 constexpr int BEAM_SB = BEAM_SB_DEF;        // rays per sub-block
 #ifndef BEAM_CMAX_DEF
-#define BEAM_CMAX_DEF 128
+#define BEAM_CMAX_DEF 160
 #endif
 constexpr int BEAM_CMAX = BEAM_CMAX_DEF;      // candidate triangles per sub-block
-constexpr int BEAM_QN = 160;        // node queue of the sub-block descent
+#ifndef BEAM_QN_DEF
+#define BEAM_QN_DEF 192
+#endif
+constexpr int BEAM_QN = BEAM_QN_DEF;        // node queue of the sub-block descent
 constexpr int BEAM_EN = 64;         // tile entry list: internal nodes
 constexpr int BEAM_EL = 96;         // tile entry list: leaf links (<= 32 when a level starts, + 2 x 32 in that level)
 constexpr int BEAM_STACK = 16;      // per-thread stack entries in shared memory (bounce rays)
