@@ -249,6 +249,17 @@ class Context:
         self.stream.synchronize()
         return F, T
 
+    def force_maps(self, designs, n_lat, n_lon, rays_per_dir, max_bounces, seed=0):
+        """The paper's force-map figures (Fig. 5): forces over a latitude-longitude image of sun
+        directions, and their split into direct light (no bounce, the paper's "NB" variant) and
+        indirect light (the rest).  Two srp_forces calls; returns CUDA float32 [D, n_lat, n_lon, 3] tensors
+        (total, direct, indirect)."""
+        sun = torch.from_numpy(W.latlong_directions(n_lat, n_lon)).to(self.device)
+        total = self.srp_forces(designs, sun, rays_per_dir, max_bounces, seed)
+        direct = self.srp_forces(designs, sun, rays_per_dir, 0, seed)
+        shape = (designs.D, n_lat, n_lon, 3)
+        return total.reshape(shape), direct.reshape(shape), (total - direct).reshape(shape)
+
     def srp_forces_host(self, designs, sun_dirs_host, rays_per_dir, max_bounces, seed=0, out_host=None):
         """Host buffers in and out (numpy float32 or pinned CPU tensors); synchronous."""
         s = sun_dirs_host if isinstance(sun_dirs_host, torch.Tensor) else torch.from_numpy(

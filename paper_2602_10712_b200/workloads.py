@@ -34,6 +34,17 @@ def fibonacci_sphere(S, front_hemisphere=False):
     return np.stack([r * np.cos(phi), r * np.sin(phi), z], axis=1).astype(np.float32)
 
 
+def latlong_directions(n_lat, n_lon):
+    """Force-map layout of the paper's figures (Fig. 5/6/12): a latitude-longitude image of sun
+    directions, pixel centres, row r = polar angle theta = pi (r + 1/2) / n_lat from +z, column c = azimuth
+    phi = 2 pi (c + 1/2) / n_lon.  Returns float32[n_lat * n_lon, 3] in row-major image order."""
+    th = np.pi * (np.arange(n_lat, dtype=np.float64) + 0.5) / n_lat
+    ph = 2.0 * np.pi * (np.arange(n_lon, dtype=np.float64) + 0.5) / n_lon
+    st, ct = np.sin(th)[:, None], np.cos(th)[:, None]
+    d = np.stack([st * np.cos(ph)[None, :], st * np.sin(ph)[None, :], np.broadcast_to(ct, (n_lat, n_lon))], axis=2)
+    return np.ascontiguousarray(d.reshape(-1, 3), dtype=np.float32)
+
+
 def draw_params(family, D, seed=PARAM_SEED):
     """float32[D, n_params] design parameters, uniform over the physical ranges of each family."""
     rng = np.random.default_rng([seed, family])

@@ -84,3 +84,15 @@ def test_input_recipes():
     assert t2[:, 0].min() >= 2 and t2[:, 0].max() <= 8 and t2[:, 1].min() >= 0 and t2[:, 1].max() <= np.pi
     assert [c.primaries for c in W.CONFIGS.values()] == [1 << 22, 1 << 36, 1 << 36, 1 << 36, 1 << 32]
     assert len(W.icosphere(2)) == 320
+
+
+def test_latlong_force_map_layout():
+    """lat-long image of directions; unit vectors, rows = polar angle, north row first, and the
+    pixel solid angles sin(theta) dtheta dphi sum to 4 pi."""
+    d = W.latlong_directions(6, 12).reshape(6, 12, 3).astype(np.float64)
+    assert np.allclose(np.linalg.norm(d, axis=2), 1.0, atol=1e-6)
+    assert np.all(d[0, :, 2] > 0.9) and np.all(d[-1, :, 2] < -0.9)
+    assert np.allclose(d[:, 0, 1] / d[:, 0, 0], np.tan(np.pi / 12), atol=1e-5)       # first column: phi = pi / 12
+    assert np.allclose(d[2, :, 2], np.cos(np.pi * 2.5 / 6), atol=1e-6)
+    th = np.pi * (np.arange(400) + 0.5) / 400
+    assert abs((np.sin(th) * (np.pi / 400) * 2 * np.pi).sum() - 4 * np.pi) < 1e-4

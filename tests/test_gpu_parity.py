@@ -630,3 +630,24 @@ def test_cfg5_full_N_properties_and_reduced_N_oracle(ctx, oracle):
     err = np.linalg.norm(F[pairs[:, 1]] - Fo, axis=1)
     assert np.all(err <= 4 * sig), (err, sig)
     dz.free()
+
+
+def test_force_maps_direct_and_indirect(ctx):
+    """PAPER.md:394 force maps.  A convex body has no indirect light (its map is the closed form of P3, indirect = 0
+    up to seam rays); the box-wing has some, and total = direct + indirect by construction."""
+    verts = W.icosphere(2, 1.0)
+    mats = W.dirichlet_materials(len(verts), 3)
+    dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
+    total, direct, indirect = ctx.force_maps(dz, 4, 8, 1 << 14, 3, seed=1)
+    sun = W.latlong_directions(4, 8)
+    t = total.cpu().numpy().reshape(-1, 3)
+    for j in range(len(sun)):
+        assert rel_l2(t[j], convex_polyhedron_force(verts, mats, sun[j])) < 5e-3
+    assert float(indirect.abs().max()) <= 1e-3 * float(total.abs().max())
+    dz.free()
+    dz = ctx.srp_build_designs(W.FAMILY_BOXWING, W.draw_params(W.FAMILY_BOXWING, 2))
+    total, direct, indirect = ctx.force_maps(dz, 4, 8, 1 << 14, 4, seed=1)
+    assert tuple(total.shape) == (2, 4, 8, 3)
+    assert float(indirect.abs().max()) > 1e-3 * float(total.abs().max())
+    assert float(indirect.abs().max()) < float(direct.abs().max())
+    dz.free()
