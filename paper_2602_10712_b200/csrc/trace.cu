@@ -1209,6 +1209,7 @@ struct SmallSmem {                  // per warp
     float4 tri[3 * SRP_BRUTE_MAX_TRIS];     // the design's packed triangles (S4 for bounce rays, S5)
     float4 eq[3 * SRP_BRUTE_MAX_TRIS];      // per tile: edge functions + depth plane of every triangle
     unsigned char tl[SRP_BRUTE_MAX_TRIS], sl[SRP_BRUTE_MAX_TRIS], gl[SRP_BRUTE_MAX_TRIS];   // tile / sub-block / group lists
+    unsigned long long vis[2][SRP_BRUTE_MAX_TRIS];   // per design: triangles with a vertex in front of / behind each facet
     WarpQueue q;
 };
 
@@ -1282,6 +1283,29 @@ small_beam_kernel(const TraceArgs a)
             __syncwarp();
             for (int x = lane; x < 3 * T; x += 32) W.tri[x] = gtri[x];
             loaded_k = k;
+            __syncwarp();
+            // A ray that leaves facet f on the side of +n (or -n) can only hit triangles with a vertex on that
+            // side of f's plane: two 64-bit masks per facet, built once per design.  The margin (1e-5 of the
+            // design's extent) keeps only coplanar neighbours out, which exact arithmetic never hits.
+            const float4 blo = a.dz.box[2 * k], bhi = a.dz.box[2 * k + 1];
+            const float eps = 1.0e-5f * (fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
+                                         fmaxf(fabsf(blo.z), fabsf(bhi.z)));
+            for (int f = lane; f < T; f += 32) {
+                const float4 q0 = W.tri[3 * f], q1 = W.tri[3 * f + 1], q2 = W.tri[3 * f + 2];
+                float3 n = cross3(f3(q1.x, q1.y, q1.z), f3(q2.x, q2.y, q2.z));
+                const float il = rsqrtf(dot3(n, n));
+                n = f3(n.x * il, n.y * il, n.z * il);
+                unsigned long long front = 0, back = 0;
+                for (int t = 0; t < T; ++t) {
+                    if (t == f) continue;
+                    const float4 p0 = W.tri[3 * t], p1 = W.tri[3 * t + 1], p2 = W.tri[3 * t + 2];
+                    const float3 r = f3(p0.x - q0.x, p0.y - q0.y, p0.z - q0.z);
+                    const float d0 = dot3(n, r), d1 = d0 + dot3(n, f3(p1.x, p1.y, p1.z)), d2 = d0 + dot3(n, f3(p2.x, p2.y, p2.z));
+                    if (fmaxf(d0, fmaxf(d1, d2)) > eps) front |= 1ULL << t;
+                    if (fminf(d0, fminf(d1, d2)) < -eps) back |= 1ULL << t;
+                }
+                W.vis[0][f] = front; W.vis[1][f] = back;
+            }
         }
         __syncwarp();
         RayGen g;
@@ -1316,7 +1340,17 @@ small_beam_kernel(const TraceArgs a)
             if (alive) {
                 float tbest = FLT_MAX; int best = -1;
                 cn.segments++;
-                closest_brute<INSTR>(W.tri, T, o, d, src, tbest, best, cn.n_tri);
+                {   // only the triangles on the side of the source facet the ray leaves on, in index order
+                    const float3 ns = cross3(f3(W.tri[3 * src + 1].x, W.tri[3 * src + 1].y, W.tri[3 * src + 1].z),
+                                             f3(W.tri[3 * src + 2].x, W.tri[3 * src + 2].y, W.tri[3 * src + 2].z));
+                    unsigned long long m = W.vis[dot3(ns, d) > 0.0f ? 0 : 1][src];
+                    if (INSTR) cn.n_tri += (unsigned)__popcll(m);
+                    while (m) {
+                        const int f = __ffsll((long long)m) - 1;
+                        m &= m - 1;
+                        tri_test(W.tri[3 * f], W.tri[3 * f + 1], W.tri[3 * f + 2], o, d, f, tbest, best);
+                    }
+                }
                 if (best < 0) cn.escaped++;
                 else {
                     atomicAdd(&s_hist[warp][depth], 1u);
