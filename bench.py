@@ -38,8 +38,9 @@ FLOP_BOX, FLOP_TRI, FLOP_TRI2D, FLOP_HIT = 12.0, 44.0, 20.0, 80.0
 FLOP_BEAM_BOX, FLOP_RECT, FLOP_SETUP = 32.0, 14.0, 110.0
 BYTES_NODE, BYTES_TRI = 64.0, 48.0
 # DRAM bytes per segment of the dominant kernel from the committed `ncu --set full` captures
-# (dram__bytes_read.sum + dram__bytes_write.sum over the segments of the captured launch; profiles/r1b_*.md)
-NCU_DRAM_BYTES_PER_SEGMENT = {"cfg3_detailed": 37.0e9 / 4.72e9, "cfg2_boxwing": 0.7e6 / 5.26e9}
+# (dram__bytes_read.sum + dram__bytes_write.sum over the segments of the captured launch; profiles/r1c_final_round1.md,
+# profiles/r1b_beam_trace_cfg3.md)
+NCU_DRAM_BYTES_PER_SEGMENT = {"cfg3_detailed": 33.9e9 / 4.72e9, "cfg2_boxwing": 0.7e6 / 5.26e9}
 
 
 def parse():
@@ -249,7 +250,7 @@ def run_ours(args, rank, world, local_rank):
                 "unit": "TFLOP/s", "frac": ach_tflops / FP32_PEAK_TFLOPS,
                 "traffic": (NCU_DRAM_BYTES_PER_SEGMENT[args.workload] * st_k["segments"]
                             if args.workload in NCU_DRAM_BYTES_PER_SEGMENT else None),
-                "traffic_source": "ncu capture of a 1/16 slice (profiles/r1b_beam_trace_cfg3.md), bytes per segment x this launch's segments",
+                "traffic_source": "ncu capture of a 1/16 slice (profiles/r1c_final_round1.md), bytes per segment x this launch's segments",
                 "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz; probed FMA chain %.1f TFLOP/s" % peaks["fp32_tflops"],
                 "flop_per_segment": flop_ps, "tests_per_segment": per, "hits_per_segment": hit_ps,
                 "beam_resolved": {k: st_k[k] / max(st_k["launched"], 1) for k in
