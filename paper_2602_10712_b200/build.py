@@ -27,6 +27,9 @@ SOURCES = {
     "mesh_gen.cu": ["--fmad=false"],
     "lbvh.cu": [],
     "trace.cu": [],
+    "trace_perray.cu": [],
+    "trace_beam.cu": [],
+    "trace_small.cu": [],
 }
 
 
@@ -53,7 +56,7 @@ def build_library(force=False, verbose=False, bounds_check=False):
         LIB_PATH = os.path.join(HERE, "libsrp_b200_chk.so")
         extra_all = ["-DSRP_BOUNDS_CHECK"]
     os.makedirs(OBJ_DIR, exist_ok=True)
-    headers = [os.path.join(CSRC, "srp_internal.cuh"), os.path.join(INCLUDE, "srp.h"), os.path.abspath(__file__)]
+    headers = [os.path.join(CSRC, "srp_internal.cuh"), os.path.join(CSRC, "trace_common.cuh"), os.path.join(INCLUDE, "srp.h"), os.path.abspath(__file__)]
     nvcc = _nvcc()
     objs, procs = [], []
     for src, extra in SOURCES.items():

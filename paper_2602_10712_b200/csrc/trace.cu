@@ -1,1538 +1,37 @@
-// trace.cu -- S2..S7 of the hot path: emitter set-up, Philox ray generation, closest-hit search
-// (BVH traversal, or all triangles of a small design from shared memory -- PAPER.md:159), material
-// lobe shading / momentum deposit (Eq. 2; 152,157), bounce loop with lane refill, and
-// the force reduction (Eq. 3).  DESIGN.md "O-steps" numbers the algorithm; the same
-// numbers appear in the comments below.
-//
-// One persistent kernel.  A WARP is the scheduling unit: it pulls (pair, ray tile) work items from
-// a global atomic counter, keeps one photon per lane, and after every segment replaces finished
-// photons by fresh rays of the tile (ballot + prefix popcount), so lanes stay busy across bounces.
-// Deposits are summed per lane in fp32 (dimensionless, <= a few hundred terms), per warp in fp64 by
-// shuffles, and added to a 2^-32 fixed-point int64 accumulator per pair -- integer adds commute,
-// so the result is bit-reproducible whatever the scheduling.
-#include <cfloat>
+// trace.cu -- which trace kernel runs (S2-S7), and the roofline probes.
+//   beam_trace_kernel   (trace_beam.cu)    designs with a BVH, stratified sampler, many rays per triangle
+//   small_beam_kernel   (trace_small.cu)   designs without a hierarchy (T <= 64), stratified sampler
+//   bvh_trace_kernel    (trace_perray.cu)  designs with a BVH otherwise (about one ray per triangle, i.i.d. sampler)
+//   trace_kernel        (trace_perray.cu)  all triangles for every segment: T <= 64 with the i.i.d. sampler, force_brute
 #include "srp_internal.cuh"
 
-// Debug build (nvcc -DSRP_BOUNDS_CHECK): every write into a fixed-capacity shared-memory list, stack or ray pool
-// checks its index and traps with a message.  compute-sanitizer is not available on the target pool.
-#ifdef SRP_BOUNDS_CHECK
-#include <cstdio>
-#define SRP_CHECK(cond, tag) do { if (!(cond)) { printf("SRP_CHECK failed: %s (trace.cu:%d)\n", tag, __LINE__); __trap(); } } while (0)
-#else
-#define SRP_CHECK(cond, tag) do { } while (0)
-#endif
+int srp_perray_blocks_per_sm(bool brute);
+int srp_beam_blocks_per_sm();
+int srp_small_blocks_per_sm();
+cudaError_t srp_launch_perray(const TraceArgs &a, int mode, bool instrumented, int num_sms, cudaStream_t stream);
+cudaError_t srp_launch_beam(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream);
+cudaError_t srp_launch_small(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream);
 
-namespace {
-
-constexpr int TRACE_THREADS = 128;
-constexpr int TRACE_WARPS = TRACE_THREADS / 32;
-constexpr int STACK_SMEM = 20;       // traversal stack entries per thread kept in shared memory
-constexpr int STACK_OVF = 80;        // deeper entries spill to local memory (degenerate trees only)
-constexpr unsigned FULL = 0xffffffffu;
-
-enum { MODE_BRUTE_SMEM = 0, MODE_BVH = 1, MODE_BRUTE_GLOBAL = 2 };
-
-__device__ __forceinline__ float3 f3(float x, float y, float z) { return make_float3(x, y, z); }
-__device__ __forceinline__ float dot3(float3 a, float3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
-__device__ __forceinline__ float3 cross3(float3 a, float3 b)
+// resident warps per SM of the kernel that will run (tile sizing in srp_api.cu)
+int srp_trace_blocks_per_sm(bool brute, bool beam)
 {
-    return f3(a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x);
+    const int per_sm = brute ? (beam ? srp_small_blocks_per_sm() : srp_perray_blocks_per_sm(true))
+                             : (beam ? srp_beam_blocks_per_sm() : srp_perray_blocks_per_sm(false));
+    return per_sm * 4;
 }
 
-__device__ __forceinline__ void philox4(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
-                                        uint32_t k1, uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3)
+cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms, cudaStream_t stream)
 {
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
-        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
-        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    if (brute) {
+        if (a.dz.has_bvh)       // forced brute force over a design that also has a hierarchy (test use)
+            return srp_launch_perray(a, 2, instrumented, num_sms, stream);
+        if (a.sampler == 0 && a.primary_mode != 1) return srp_launch_small(a, instrumented, num_sms, stream);
+        return srp_launch_perray(a, 0, instrumented, num_sms, stream);
     }
-    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+    if (a.sampler == 0 && a.pool != nullptr)          // beams chosen by the caller (srp_api.cu, want_beams)
+        return srp_launch_beam(a, instrumented, num_sms, stream);
+    return srp_launch_perray(a, 1, instrumented, num_sms, stream);
 }
-// R4: ((x >> 9) + 0.5) * 2^-23 -- exact in fp32
-__device__ __forceinline__ float uniform23(uint32_t x) { return ((float)(x >> 9) + 0.5f) * (1.0f / 8388608.0f); }
-
-// O-step 1: orthonormal basis perpendicular to unit s (Duff et al. 2017)
-__device__ __forceinline__ void basis3(float3 s, float3 &u, float3 &v)
-{
-    const float sign = copysignf(1.0f, s.z);
-    const float a = -1.0f / (sign + s.z);
-    const float b = s.x * s.y * a;
-    u = f3(1.0f + sign * s.x * s.x * a, sign * b, -sign * s.x);
-    v = f3(b, sign + s.y * s.y * a, -s.y);
-}
-
-struct Emitter {
-    float3 s, u, v;
-    float u0, v0, du, dv, worg, Ae;
-};
-
-// O-steps 1-2: travel direction, basis, rectangle of the projected AABB corners, origin plane.
-__device__ inline Emitter make_emitter(const float *sun_dirs, int j, float4 lo, float4 hi)
-{
-    Emitter e;
-    const float wx = sun_dirs[3 * j], wy = sun_dirs[3 * j + 1], wz = sun_dirs[3 * j + 2];
-    const float len = sqrtf(wx * wx + wy * wy + wz * wz);
-    e.s = f3(-wx / len, -wy / len, -wz / len);
-    basis3(e.s, e.u, e.v);
-    float u0 = FLT_MAX, u1 = -FLT_MAX, v0 = FLT_MAX, v1 = -FLT_MAX, w0 = FLT_MAX;
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        const float3 p = f3((c & 1) ? hi.x : lo.x, (c & 2) ? hi.y : lo.y, (c & 4) ? hi.z : lo.z);
-        const float pu = dot3(p, e.u), pv = dot3(p, e.v), pw = dot3(p, e.s);
-        u0 = fminf(u0, pu); u1 = fmaxf(u1, pu);
-        v0 = fminf(v0, pv); v1 = fmaxf(v1, pv);
-        w0 = fminf(w0, pw);
-    }
-    e.u0 = u0; e.v0 = v0; e.du = u1 - u0; e.dv = v1 - v0;
-    e.worg = w0 - 1.0f;
-    e.Ae = e.du * e.dv;
-    return e;
-}
-
-__device__ __forceinline__ uint32_t compact_even_bits(uint32_t x)
-{
-    x &= 0x55555555u;
-    x = (x | (x >> 1)) & 0x33333333u;
-    x = (x | (x >> 2)) & 0x0F0F0F0Fu;
-    x = (x | (x >> 4)) & 0x00FF00FFu;
-    x = (x | (x >> 8)) & 0x0000FFFFu;
-    return x;
-}
-
-struct RayGen {            // warp-uniform per work item
-    uint32_t j, k, key0, key1;
-    int sampler;
-    float inv_nx, inv_ny;
-    float3 xc;             // the design's centre of mass (TORQUE kernels: Eq. 4)
-};
-
-// O-step 3: ray i of the pair.
-__device__ __forceinline__ void make_ray(const Emitter &e, const RayGen &g, uint32_t i, float3 &o)
-{
-    uint32_t r0, r1, r2, r3;
-    philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
-    float fu, fv;
-    if (g.sampler == 0) {
-        const float cx = (float)compact_even_bits(i), cy = (float)compact_even_bits(i >> 1);
-        fu = (cx + uniform23(r0)) * g.inv_nx;
-        fv = (cy + uniform23(r1)) * g.inv_ny;
-    } else {
-        fu = uniform23(r0); fv = uniform23(r1);
-    }
-    const float pu = fmaf(fu, e.du, e.u0), pv = fmaf(fv, e.dv, e.v0);
-    o = f3(fmaf(pu, e.u.x, fmaf(pv, e.v.x, e.worg * e.s.x)),
-           fmaf(pu, e.u.y, fmaf(pv, e.v.y, e.worg * e.s.y)),
-           fmaf(pu, e.u.z, fmaf(pv, e.v.z, e.worg * e.s.z)));
-}
-
-// O-step 4, one triangle: Moller-Trumbore on (v0, e1, e2) in the division-free sign-normalised
-// form: accept det != 0, u >= 0, v >= 0, u+v <= 1, t > 0; t = T/|det| only for accepted hits.
-__device__ __forceinline__ void tri_test(const float4 q0, const float4 q1, const float4 q2, const float3 o,
-                                         const float3 d, const int f, float &tbest, int &best)
-{
-    const float3 e1 = f3(q1.x, q1.y, q1.z), e2 = f3(q2.x, q2.y, q2.z);
-    const float3 pv = cross3(d, e2);
-    const float det = dot3(e1, pv);
-    const float3 tv = f3(o.x - q0.x, o.y - q0.y, o.z - q0.z);
-    const float3 qv = cross3(tv, e1);
-    const uint32_t sb = __float_as_uint(det) & 0x80000000u;
-    const float U = __uint_as_float(__float_as_uint(dot3(tv, pv)) ^ sb);
-    const float V = __uint_as_float(__float_as_uint(dot3(d, qv)) ^ sb);
-    const float Tn = __uint_as_float(__float_as_uint(dot3(e2, qv)) ^ sb);
-    const float adet = fabsf(det);
-    if (U >= 0.0f && V >= 0.0f && U + V <= adet && Tn > 0.0f && adet > 0.0f) {
-        const float t = Tn / adet;
-        if (t < tbest) { tbest = t; best = f; }
-    }
-}
-
-// All triangles of a design, in index order (ties -> smallest index), source excluded (R10).
-template <bool INSTR>
-__device__ __forceinline__ void closest_brute(const float4 *__restrict__ tp, const int T, const float3 o,
-                                              const float3 d, const int src, float &tbest, int &best,
-                                              unsigned &n_tri)
-{
-    for (int f = 0; f < T; ++f) {
-        if (f == src) continue;
-        tri_test(tp[3 * f], tp[3 * f + 1], tp[3 * f + 2], o, d, f, tbest, best);
-    }
-    if (INSTR) n_tri += (unsigned)(T - (src >= 0 ? 1 : 0));
-}
-
-__device__ __forceinline__ float safe_rcp(float x)
-{
-    return 1.0f / (fabsf(x) < 1e-30f ? copysignf(1e-30f, x) : x);
-}
-
-// Stack-based BVH2 descent, nearer child first, in "while-while" form: a lane stays in the node
-// loop until it lands on a leaf (or runs out of nodes); the warp reconverges after the node loop, so
-// the triangle tests of all lanes that hold a leaf run together (in the single-loop form they ran
-// with ~4 of 32 lanes active and took a third of the issue slots -- profiles/ round 1).
-// Stack: STACK_SMEM entries per thread in shared memory (thread-interleaved, conflict-free), deeper
-// levels in a local array.
-constexpr int CUR_DONE = 0x7fffffff;
-// "while-while" traversal lets a lane walk nodes until it reaches a leaf while the lanes that already hold one
-// wait.  Capping a node run (and not unrolling it) bounds that wait: cfg3 bounce rays +9 %, per-ray primaries +13 %.
-constexpr int NODE_RUN_CAP = 8;
-
-#define SRP_POP(cur_)                                                                     \
-    do {                                                                                  \
-        if (sp == 0) cur_ = CUR_DONE;                                                     \
-        else { --sp; cur_ = sp < NSMEM ? s_stack[sp * STRIDE] : ovf[sp - NSMEM]; }        \
-    } while (0)
-
-// STRIDE: distance in ints between consecutive stack entries of one thread (thread-interleaved
-// layout); NSMEM: entries kept in shared memory.
-// One internal node for one lane: both child boxes against the ray, nearer child next, farther child
-// pushed.  Returns the next value of `cur` (node index, leaf link < 0, or CUR_DONE).
-template <int STRIDE, int NSMEM>
-__device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, int cur, int &sp, int *s_stack, int *ovf,
-                                             float idx, float idy, float idz, float oxi, float oyi, float ozi, float tbest)
-{
-    const float4 n0 = __ldg(nodes + 4 * cur), n1 = __ldg(nodes + 4 * cur + 1),
-                 n2 = __ldg(nodes + 4 * cur + 2), n3 = __ldg(nodes + 4 * cur + 3);
-    float a0 = fmaf(n0.x, idx, -oxi), a1 = fmaf(n0.w, idx, -oxi);
-    float b0 = fmaf(n0.y, idy, -oyi), b1 = fmaf(n1.x, idy, -oyi);
-    float c0 = fmaf(n0.z, idz, -ozi), c1 = fmaf(n1.y, idz, -ozi);
-    const float tmin0 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
-    const float tmax0 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
-    a0 = fmaf(n1.z, idx, -oxi); a1 = fmaf(n2.y, idx, -oxi);
-    b0 = fmaf(n1.w, idy, -oyi); b1 = fmaf(n2.z, idy, -oyi);
-    c0 = fmaf(n2.x, idz, -ozi); c1 = fmaf(n2.w, idz, -ozi);
-    const float tmin1 = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
-    const float tmax1 = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
-    const bool h0 = tmin0 <= tmax0 * 1.0000004f, h1 = tmin1 <= tmax1 * 1.0000004f;
-    int l0 = __float_as_int(n3.x), l1 = __float_as_int(n3.y);
-    if (h0 && h1) {
-        if (tmin1 < tmin0) { const int t = l0; l0 = l1; l1 = t; }
-        SRP_CHECK(sp < NSMEM + STACK_OVF, "traversal stack");
-        if (sp < NSMEM) s_stack[sp * STRIDE] = l1; else ovf[sp - NSMEM] = l1;
-        ++sp;
-#ifdef SRP_PREFETCH_PUSH
-        if (l1 >= 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(nodes + 4 * l1));
-#endif
-        return l0;
-    }
-    if (h0) return l0;
-    if (h1) return l1;
-    SRP_POP(cur);
-    return cur;
-}
-
-// One leaf for one lane: its triangles (source excluded, R10), then the next stack entry.
-template <int STRIDE, int NSMEM>
-__device__ __forceinline__ int bvh_leaf_step(const float4 *__restrict__ tri, int cur, int &sp, int *s_stack, int *ovf,
-                                             const float3 o, const float3 d, const int src, float &tbest, int &best,
-                                             unsigned &n_tri)
-{
-    const unsigned u = (unsigned)~cur;
-    const int first = (int)(u >> 3), cnt = (int)(u & 7u) + 1;
-    for (int f = first; f < first + cnt; ++f) {
-        if (f == src) continue;
-        tri_test(__ldg(tri + 3 * f), __ldg(tri + 3 * f + 1), __ldg(tri + 3 * f + 2), o, d, f, tbest, best);
-    }
-    n_tri += (unsigned)cnt;
-    SRP_POP(cur);
-    return cur;
-}
-
-// STRIDE: distance in ints between consecutive stack entries of one thread (thread-interleaved
-// layout); NSMEM: entries kept in shared memory.
-template <bool INSTR, int STRIDE = TRACE_THREADS, int NSMEM = STACK_SMEM>
-__device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, const float4 *__restrict__ tri,
-                                            const float3 o, const float3 d, const int src, float &tbest,
-                                            int &best, int *s_stack, unsigned &n_box, unsigned &n_tri)
-{
-    const float idx = safe_rcp(d.x), idy = safe_rcp(d.y), idz = safe_rcp(d.z);
-    const float oxi = o.x * idx, oyi = o.y * idy, ozi = o.z * idz;
-    int ovf[STACK_OVF];
-    int sp = 0;
-    int cur = 0;
-    unsigned nt = 0;
-    while (cur != CUR_DONE) {
-        // internal nodes; at most NODE_RUN_CAP steps before the lanes that wait at a leaf get their turn
-#pragma unroll 1
-        for (int steps = 0; steps < NODE_RUN_CAP && (unsigned)cur < (unsigned)CUR_DONE; ++steps) {
-            if (INSTR) n_box += 2;
-            cur = bvh_node_step<STRIDE, NSMEM>(nodes, cur, sp, s_stack, ovf, idx, idy, idz, oxi, oyi, ozi, tbest);
-        }
-        if (cur < 0)                                                 // leaf: all lanes that hold one, together
-            cur = bvh_leaf_step<STRIDE, NSMEM>(tri, cur, sp, s_stack, ovf, o, d, src, tbest, best, nt);
-    }
-    if (INSTR) n_tri += nt;
-}
-
-struct LaneCounters {
-    unsigned launched, pmiss, absorbed, escaped, capped, segments, n_box, n_tri;
-};
-struct BeamCounters {       // rays resolved per beam level (lane-distributed counts); instrumented: beam work
-    unsigned tile_miss, block_miss, group_miss, fallback;
-    unsigned beam_box, tri2d, setups, rect;     // beam-box tests, 2-D ray-triangle tests, triangle set-ups, rectangle-triangle tests
-};
-
-// O-steps 5-7 at a hit: deposit, lobe selection, continuation.
-// Returns SHADE_CONTINUE if the photon goes on (o, d, src, depth updated), else how it ended.
-enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2 };
-template <bool TORQUE>
-__device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
-                                      const int f, const RayGen &g, const uint32_t i, const int B,
-                                      const int deposit, float3 &o, float3 &d, int &src, int &depth,
-                                      float3 &acc, float3 &acc_t)
-{
-    (void)q0;
-    // every deposit of this hit is made at the hit point x; Eq. 4: torque += (x - x_COM) x deposit
-    const float3 x = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
-    auto put = [&](const float3 dd) {
-        acc.x += dd.x; acc.y += dd.y; acc.z += dd.z;
-        if (TORQUE) {
-            const float3 r = f3(x.x - g.xc.x, x.y - g.xc.y, x.z - g.xc.z), m = cross3(r, dd);
-            acc_t.x += m.x; acc_t.y += m.y; acc_t.z += m.z;
-        }
-    };
-    const float al = q0.w, rs = q1.w, rd = q2.w;
-    float3 n = cross3(f3(q1.x, q1.y, q1.z), f3(q2.x, q2.y, q2.z));
-    const float inv_len = 1.0f / sqrtf(dot3(n, n));
-    n = f3(n.x * inv_len, n.y * inv_len, n.z * inv_len);
-    const float nd = dot3(n, d);
-    const float3 nf = nd > 0.0f ? f3(-n.x, -n.y, -n.z) : n;      // facets are two-sided (R6)
-    const float cost = fabsf(nd);
-    const float3 refl = f3(fmaf(2.0f * cost, nf.x, d.x), fmaf(2.0f * cost, nf.y, d.y), fmaf(2.0f * cost, nf.z, d.z));
-    if (deposit == 0) {                                           // expected-value deposit
-        const float a = al + rs + rd, c = (2.0f / 3.0f) * rd;
-        put(f3(a * d.x - rs * refl.x - c * nf.x, a * d.y - rs * refl.y - c * nf.y, a * d.z - rs * refl.z - c * nf.z));
-    }
-    uint32_t y0, y1, y2, y3;
-    philox4(i, g.j, g.k, (uint32_t)(depth + 1), g.key0, g.key1, y0, y1, y2, y3);
-    const float z0 = uniform23(y0);
-    float3 dn;
-    if (z0 < al) {                                                // absorbed
-        if (deposit == 1) put(d);
-        return SHADE_ABSORBED;
-    } else if (z0 < al + rs) {                                    // ideal mirror (R3)
-        dn = refl;
-    } else {                                                      // Lambertian: cosine-weighted about nf
-        const float z1 = uniform23(y1), z2 = uniform23(y2);
-        float sn, cs;
-        sincospif(2.0f * z1, &sn, &cs);
-        const float rho = sqrtf(z2), lz = sqrtf(1.0f - z2);
-        // tangent frame (R18): first edge of the facet and nf x edge (no discontinuity in nf)
-        const float ie = rsqrtf(q1.x * q1.x + q1.y * q1.y + q1.z * q1.z);
-        const float3 tu = f3(q1.x * ie, q1.y * ie, q1.z * ie);
-        const float3 tv = cross3(nf, tu);
-        const float lx = rho * cs, ly = rho * sn;
-        dn = f3(fmaf(lx, tu.x, fmaf(ly, tv.x, lz * nf.x)), fmaf(lx, tu.y, fmaf(ly, tv.y, lz * nf.y)),
-                fmaf(lx, tu.z, fmaf(ly, tv.z, lz * nf.z)));
-    }
-    if (deposit == 1) put(f3(d.x - dn.x, d.y - dn.y, d.z - dn.z));
-    if (depth == B) return SHADE_CAPPED;                         // R5: B reflections followed
-    // Hit point in fp32 is off the facet's plane by a few ulp of |x| + t (micrometres here).  An origin
-    // that ends up BELOW the plane lets the outgoing ray hit a coplanar or convex neighbour from
-    // behind -- a path the exact arithmetic of the definition never takes.  Lift the origin along the
-    // facing normal by more than that error (R10: "exclude the source triangle, t > 0, no
-    // epsilon" is the definition; this is the fp32 guard that keeps the CUDA path on it).
-    const float lift = 1.0e-6f * (fabsf(x.x) + fabsf(x.y) + fabsf(x.z) + t);
-    o = f3(fmaf(lift, nf.x, x.x), fmaf(lift, nf.y, x.y), fmaf(lift, nf.z, x.z));
-    d = dn; src = f; depth += 1;
-    return SHADE_CONTINUE;
-}
-
-// same for a pair index known to fit 32 bits (rays of the beam kernel's pool)
-__device__ __forceinline__ void pair_of32(const TraceArgs &a, uint32_t p, int &k, int &j)
-{
-    if (a.pairs) { k = a.pairs[2 * (size_t)p]; j = a.pairs[2 * (size_t)p + 1]; }
-    else { const uint32_t kk = p / (uint32_t)a.S; k = (int)kk; j = (int)(p - kk * (uint32_t)a.S); }
-}
-__device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k, int &j)
-{
-    if (a.pairs) { k = a.pairs[2 * p]; j = a.pairs[2 * p + 1]; }
-    else { k = (int)(p / a.S); j = (int)(p - (long long)k * a.S); }
-}
-
-template <bool TORQUE>
-__device__ __forceinline__ void set_torque(RayGen &g, const TraceArgs &a, int k)
-{
-    g.xc = (TORQUE && a.xcom) ? f3(a.xcom[3 * k], a.xcom[3 * k + 1], a.xcom[3 * k + 2]) : f3(0.f, 0.f, 0.f);
-}
-
-// S7 for one work item: per-lane fp32 sums -> fp64 warp shuffle tree -> one fixed-point atomic per component.
-// accum holds acc_stride (3, or 6 with torque) int64 per pair.
-template <bool TORQUE>
-__device__ __forceinline__ void flush_tile_acc(const TraceArgs &a, long long p, const float3 acc, const float3 acc_t, int lane)
-{
-    const double s[6] = { acc.x, acc.y, acc.z, acc_t.x, acc_t.y, acc_t.z };
-#pragma unroll
-    for (int c = 0; c < (TORQUE ? 6 : 3); ++c) {
-        double v = s[c];
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
-        if (lane == 0) {
-            unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * p);
-            atomicAdd(dst + c, (unsigned long long)__double2ll_rn(v * SRP_ACC_SCALE));
-        }
-    }
-}
-
-// counters: warp sums, one global atomic each
-template <bool INSTR>
-__device__ __forceinline__ void flush_counters(const TraceArgs &a, const LaneCounters &cn, const unsigned *hist, int lane)
-{
-    unsigned long long *st = (unsigned long long *)a.stats;
-    const unsigned vals[8] = { cn.launched, cn.pmiss, cn.absorbed, cn.escaped, cn.capped, cn.segments, cn.n_box, cn.n_tri };
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        if (!INSTR && c >= 6) break;
-        unsigned long long v = vals[c];
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
-        if (lane == 0 && v) atomicAdd(st + (c < 6 ? c : 22 + (c - 6)), v);
-    }
-    __syncwarp();
-    if (lane < 16 && hist[lane]) atomicAdd(st + 6 + lane, (unsigned long long)hist[lane]);
-}
-
-// ---- the persistent trace kernel ----
-template <int MODE, bool INSTR, bool TORQUE>
-__global__ void __launch_bounds__(TRACE_THREADS, MODE == MODE_BVH ? 4 : 5)
-trace_kernel(const TraceArgs a)
-{
-    __shared__ int s_stack[MODE == MODE_BVH ? STACK_SMEM * TRACE_THREADS : 1];
-    __shared__ float4 s_tri[MODE == MODE_BRUTE_SMEM ? TRACE_WARPS * SRP_BRUTE_MAX_TRIS * 3 : 1];
-    __shared__ unsigned s_hist[TRACE_WARPS][16];
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    if (lane < 16) s_hist[warp][lane] = 0;
-    __syncwarp();
-    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
-    int loaded_k = -1;
-    float4 *my_tri = s_tri + (MODE == MODE_BRUTE_SMEM ? warp * SRP_BRUTE_MAX_TRIS * 3 : 0);
-
-    for (;;) {
-        unsigned long long tile = 0;
-        if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
-        tile = __shfl_sync(FULL, tile, 0);
-        if (tile >= total_tiles) break;
-        const long long p = (long long)(tile / a.tiles_per_pair);
-        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
-        int k, j;
-        pair_of(a, p, k, j);
-        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
-        if (!(em.Ae > 0.0f)) continue;                      // edge-on flat design: F = 0, nothing launched
-        const long long tbase = a.dz.tri_off[k];
-        const int T = (int)(a.dz.tri_off[k + 1] - tbase);
-        const float4 *gtri = a.dz.tri + 3 * tbase;
-        const float4 *gnodes = a.dz.nodes + 4 * tbase;
-        if (MODE == MODE_BRUTE_SMEM && loaded_k != k) {
-            __syncwarp();
-            for (int x = lane; x < 3 * T; x += 32) my_tri[x] = gtri[x];
-            __syncwarp();
-            loaded_k = k;
-        }
-        RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque<TORQUE>(g, a, k);
-        g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
-        g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
-        uint32_t next = (uint32_t)(q * a.tile_rays);
-        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
-
-        bool alive = false;
-        uint32_t i = 0;
-        unsigned long long sig = 0;                         // debug: hash of the hit-triangle sequence
-        float3 o = f3(0, 0, 0), d = em.s, acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
-        int src = -1, depth = 0;
-        for (;;) {
-            // S6: lanes whose photon ended take the next rays of the tile
-            const unsigned need = __ballot_sync(FULL, !alive);
-            if (need) {
-                const uint32_t mine = next + __popc(need & lt_mask);
-                if (!alive && mine < end) {
-                    i = mine; make_ray(em, g, i, o); d = em.s; src = -1; depth = 0; alive = true;
-                    cn.launched++;
-                    if (INSTR) sig = 0;
-                }
-                const uint32_t room = end - next, want = __popc(need);
-                next += want < room ? want : room;
-            }
-            if (!__any_sync(FULL, alive)) break;
-            if (alive) {
-                float tbest = FLT_MAX; int best = -1;
-                cn.segments++;
-                if (MODE == MODE_BVH)
-                    closest_bvh<INSTR>(gnodes, gtri, o, d, src, tbest, best, s_stack + threadIdx.x, cn.n_box, cn.n_tri);
-                else if (MODE == MODE_BRUTE_SMEM)
-                    closest_brute<INSTR>(my_tri, T, o, d, src, tbest, best, cn.n_tri);
-                else
-                    closest_brute<INSTR>(gtri, T, o, d, src, tbest, best, cn.n_tri);
-                if (best < 0) {
-                    if (depth == 0) cn.pmiss++; else cn.escaped++;
-                    alive = false;
-                } else {
-                    atomicAdd(&s_hist[warp][depth], 1u);
-                    const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
-                    if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    const int fate = shade<TORQUE>(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
-                    if (fate == SHADE_ABSORBED) cn.absorbed++;
-                    if (fate == SHADE_CAPPED) cn.capped++;
-                    alive = fate == SHADE_CONTINUE;
-                }
-                if (INSTR && !alive && a.sig_out) a.sig_out[p * a.N + i] = sig;
-            }
-        }
-        // S7: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
-    }
-    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
-}
-
-// ---- the BVH trace kernel: persistent warps with a per-warp queue of bounce rays ----
-// A warp traces 32 rays of ONE kind per pass: either 32 fresh primaries of its tile (parallel, in
-// Morton order, so they walk the same part of the tree) or 32 queued secondary rays (incoherent, and
-// mostly gone after a few nodes).  Photons that survive shading are pushed to the warp's queue in
-// shared memory (ballot + prefix popcount, so the order is deterministic) and popped 32 at a time.
-// Mixing the two kinds in one pass left the short secondaries waiting for the long primaries
-// (14 of 32 lanes active, profiles/ round 1); this is S6's "compaction between bounces".
-constexpr int QCAP = 64;
-struct WarpQueue {
-    float ox[QCAP], oy[QCAP], oz[QCAP], dx[QCAP], dy[QCAP], dz[QCAP];
-    uint32_t i[QCAP];
-    int src_depth[QCAP];                 // (depth << 27) | src
-};
-
-template <bool INSTR, bool TORQUE>
-__global__ void __launch_bounds__(TRACE_THREADS, 8)
-bvh_trace_kernel(const TraceArgs a)
-{
-    __shared__ int s_stack[STACK_SMEM * TRACE_THREADS];
-    __shared__ WarpQueue s_q[TRACE_WARPS];
-    __shared__ unsigned long long s_qsig[INSTR ? TRACE_WARPS * QCAP : 1];
-    __shared__ unsigned s_hist[TRACE_WARPS][16];
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    if (lane < 16) s_hist[warp][lane] = 0;
-    __syncwarp();
-    WarpQueue &Q = s_q[warp];
-    unsigned long long *qsig = s_qsig + (INSTR ? warp * QCAP : 0);
-    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
-
-    for (;;) {
-        unsigned long long tile = 0;
-        if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
-        tile = __shfl_sync(FULL, tile, 0);
-        if (tile >= total_tiles) break;
-        const long long p = (long long)(tile / a.tiles_per_pair);
-        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
-        int k, j;
-        pair_of(a, p, k, j);
-        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
-        if (!(em.Ae > 0.0f)) continue;
-        const long long tbase = a.dz.tri_off[k];
-        const float4 *gtri = a.dz.tri + 3 * tbase;
-        const float4 *gnodes = a.dz.nodes + 4 * tbase;
-        RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque<TORQUE>(g, a, k);
-        g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
-        g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
-        uint32_t next = (uint32_t)(q * a.tile_rays);
-        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
-        int qcount = 0;                                   // warp-uniform
-        float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
-
-        for (;;) {
-            bool alive = false;
-            uint32_t i = 0;
-            float3 o = f3(0, 0, 0), d = em.s;
-            int src = -1, depth = 0;
-            unsigned long long sig = 0;
-            if (qcount >= 32 || (next >= end && qcount > 0)) {          // a pass of secondary rays
-                const int take = qcount < 32 ? qcount : 32;
-                if (lane < take) {
-                    const int e = qcount - take + lane;
-                    o = f3(Q.ox[e], Q.oy[e], Q.oz[e]); d = f3(Q.dx[e], Q.dy[e], Q.dz[e]);
-                    i = Q.i[e]; src = Q.src_depth[e] & 0x07ffffff; depth = (int)((unsigned)Q.src_depth[e] >> 27);
-                    if (INSTR) sig = qsig[e];
-                    alive = true;
-                }
-                qcount -= take;
-            } else if (next < end) {                                     // a pass of primaries
-                const uint32_t mine = next + lane;
-                if (mine < end) { i = mine; make_ray(em, g, i, o); alive = true; cn.launched++; }
-                next = (end - next) < 32u ? end : next + 32u;
-            } else break;                                                // tile exhausted, queue empty
-            __syncwarp();
-            int fate = -1;                                               // -1: no hit / no photon
-            if (alive) {
-                float tbest = FLT_MAX; int best = -1;
-                cn.segments++;
-                closest_bvh<INSTR>(gnodes, gtri, o, d, src, tbest, best, s_stack + threadIdx.x, cn.n_box, cn.n_tri);
-                if (best < 0) {
-                    if (depth == 0) cn.pmiss++; else cn.escaped++;
-                } else {
-                    atomicAdd(&s_hist[warp][depth], 1u);
-                    if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    fate = shade<TORQUE>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
-                    if (fate == SHADE_ABSORBED) cn.absorbed++;
-                    if (fate == SHADE_CAPPED) cn.capped++;
-                }
-                if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
-            }
-            const unsigned cont = __ballot_sync(FULL, fate == SHADE_CONTINUE);
-            if (fate == SHADE_CONTINUE) {
-                const int e = qcount + __popc(cont & lt_mask);
-                Q.ox[e] = o.x; Q.oy[e] = o.y; Q.oz[e] = o.z; Q.dx[e] = d.x; Q.dy[e] = d.y; Q.dz[e] = d.z;
-                Q.i[e] = i; Q.src_depth[e] = (depth << 27) | src;
-                if (INSTR) qsig[e] = sig;
-            }
-            qcount += __popc(cont);
-            __syncwarp();
-        }
-        // S7: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
-    }
-    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
-}
-
-__device__ __forceinline__ void flush_beam_counters(const TraceArgs &a, const BeamCounters &bc, int lane)
-{
-    unsigned long long *st = (unsigned long long *)a.stats;
-    const unsigned vals[8] = { bc.tile_miss, bc.block_miss, bc.group_miss, bc.fallback, bc.beam_box, bc.tri2d, bc.setups, bc.rect };
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        unsigned long long v = vals[c];
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
-        if (lane == 0 && v) atomicAdd(st + 24 + c, v);
-    }
-}
-
-// ---- the beam trace kernel: coherent primaries as beams, bounce rays one by one ----
-// The primaries of a pair are parallel and, in the stratified sampler, ray i sits in cell
-// Morton(i) of the emitter grid, so every aligned block of 2^b consecutive rays is a rectangle of
-// cells -- a BEAM with a rectangular cross-section.  A warp walks the BVH once per beam instead of
-// once per ray (BVH "packet"/beam traversal; the tree and the hit definition are unchanged):
-//   tile      (<= 8192 rays): frontier descent from the root, all lanes testing different nodes
-//             against the tile's rectangle, until the frontier holds > 32 nodes -> entry list.
-//             Nothing overlaps: the whole tile is primary misses, no ray is generated.
-//   sub-block (256 rays, 16 x 16 cells): descent from the entry list to the leaves -> candidate
-//             triangles (<= BEAM_CMAX), each set up ONCE as three 2-D edge functions and a depth
-//             plane in the emitter frame (the ray-triangle test of a ray parallel to the frame's
-//             axis: inside <=> the three edge functions are >= 0, same inclusive rule as O-step 4).
-//   group     (32 rays, 8 x 4 cells, one per lane): the candidates whose edge functions admit the
-//             group's rectangle are listed; an empty list resolves 32 misses without Philox;
-//             otherwise every lane tests ITS ray against the same short list, all 32 lanes
-//             converged, operands broadcast from shared memory.
-// Bounce rays are incoherent: they go to the warp's ray pool and through per-ray stack traversal
-// (drain(), below).  A sub-block whose lists overflow is halved; a single group that still
-// overflows (a beam along an edge-on panel, a bundle of thin facets) sends its 32 primaries to the
-// pool as well, so any input is handled.
-#ifndef BEAM_BLOCKS_PER_SM
-#define BEAM_BLOCKS_PER_SM 4
-#endif
-#ifndef BEAM_SB_DEF
-#define BEAM_SB_DEF 256
-#endif
-constexpr int BEAM_SB = BEAM_SB_DEF;        // rays per sub-block
-#ifndef BEAM_CMAX_DEF
-#define BEAM_CMAX_DEF 160
-#endif
-constexpr int BEAM_CMAX = BEAM_CMAX_DEF;      // candidate triangles per sub-block
-#ifndef BEAM_QN_DEF
-#define BEAM_QN_DEF 192
-#endif
-constexpr int BEAM_QN = BEAM_QN_DEF;        // node queue of the sub-block descent
-constexpr int BEAM_EN = 64;         // tile entry list: internal nodes
-constexpr int BEAM_EL = 96;         // tile entry list: leaf links (<= 32 when a level starts, + 2 x 32 in that level)
-constexpr int BEAM_STACK = 16;      // per-thread stack entries in shared memory (bounce rays)
-
-struct BeamFrame {                  // warp-uniform per pair
-    float3 uh, vh, auh, avh;        // u/2, v/2 and their absolute values
-    float csu, csv;                 // cell size along u and v
-    float margin;                   // bound of the fp32 projection error of a box
-};
-
-// Does the box's projection on the emitter plane meet the rectangle [0,wu] x [0,wv] of the local
-// frame whose origin projects to (offu, offv)?  NaN (the empty-box sentinel) compares false.
-__device__ __forceinline__ bool beam_box(const BeamFrame &f, float offu, float offv, float wu, float wv,
-                                         float lox, float loy, float loz, float hix, float hiy, float hiz)
-{
-    const float sx = lox + hix, sy = loy + hiy, sz = loz + hiz;
-    const float dx = hix - lox, dy = hiy - loy, dz = hiz - loz;
-    const float pu = fmaf(sx, f.uh.x, fmaf(sy, f.uh.y, sz * f.uh.z)) - offu;
-    const float pv = fmaf(sx, f.vh.x, fmaf(sy, f.vh.y, sz * f.vh.z)) - offv;
-    const float ru = fmaf(dx, f.auh.x, fmaf(dy, f.auh.y, dz * f.auh.z)) + f.margin;
-    const float rv = fmaf(dx, f.avh.x, fmaf(dy, f.avh.y, dz * f.avh.z)) + f.margin;
-    return (pu + ru >= 0.0f) && (pu - ru <= wu) && (pv + rv >= 0.0f) && (pv - rv <= wv);
-}
-
-// One node against a beam: which children overlap, and their links.
-template <bool INSTR>
-__device__ __forceinline__ void beam_node(const float4 *__restrict__ nodes, int node, const BeamFrame &f, float offu,
-                                          float offv, float wu, float wv, bool &h0, bool &h1, int &l0, int &l1,
-                                          unsigned &n_box)
-{
-    h0 = h1 = false; l0 = l1 = 0;
-    if (node < 0) return;
-    const float4 n0 = __ldg(nodes + 4 * node), n1 = __ldg(nodes + 4 * node + 1), n2 = __ldg(nodes + 4 * node + 2),
-                 n3 = __ldg(nodes + 4 * node + 3);
-    h0 = beam_box(f, offu, offv, wu, wv, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y);
-    h1 = beam_box(f, offu, offv, wu, wv, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w);
-    l0 = __float_as_int(n3.x); l1 = __float_as_int(n3.y);
-    if (INSTR) n_box += 2;
-}
-
-// Appends the triangles of up to two leaves per lane to the candidate list (warp scan of the
-// counts, so the order is deterministic).  Returns false if the list would overflow.
-__device__ __forceinline__ bool beam_push_tris(int *cid, int &ncand, int first0, int cnt0, int first1, int cnt1,
-                                               int lane)
-{
-    const int c = cnt0 + cnt1;
-    int incl = c;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-        const int t = __shfl_up_sync(FULL, incl, off);
-        if (lane >= off) incl += t;
-    }
-    const int total = __shfl_sync(FULL, incl, 31);
-    if (ncand + total > BEAM_CMAX) return false;
-    int pos = ncand + incl - c;
-    for (int t = 0; t < cnt0; ++t) cid[pos++] = first0 + t;
-    for (int t = 0; t < cnt1; ++t) cid[pos++] = first1 + t;
-    ncand += total;
-    return true;
-}
-
-// Candidate set-up: triangle -> sign-normalised edge functions E_i(x) = A_i x_u + B_i x_v + C_i
-// (inside <=> all >= 0) and the depth plane t(x) = Wu x_u + Wv x_v + Wc, in the sub-block's local
-// emitter frame (origin at the sub-block's corner, t measured from the ray-origin plane).
-__device__ __forceinline__ void beam_setup(const float4 q0, const float4 q1, const float4 q2, const Emitter &em,
-                                           float offu, float offv, float4 *eq)
-{
-    const float3 a = f3(q0.x, q0.y, q0.z);
-    const float3 b = f3(q0.x + q1.x, q0.y + q1.y, q0.z + q1.z);
-    const float3 c = f3(q0.x + q2.x, q0.y + q2.y, q0.z + q2.z);
-    const float au = dot3(a, em.u) - offu, av = dot3(a, em.v) - offv, aw = dot3(a, em.s) - em.worg;
-    const float bu = dot3(b, em.u) - offu, bv = dot3(b, em.v) - offv, bw = dot3(b, em.s) - em.worg;
-    const float cu = dot3(c, em.u) - offu, cv = dot3(c, em.v) - offv, cw = dot3(c, em.s) - em.worg;
-    // E_pq(x) = (q_u - p_u)(x_v - p_v) - (q_v - p_v)(x_u - p_u)
-    float A0 = -(bv - av), B0 = bu - au, C0 = -fmaf(A0, au, B0 * av);       // edge a -> b
-    float A1 = -(cv - bv), B1 = cu - bu, C1 = -fmaf(A1, bu, B1 * bv);       // edge b -> c
-    float A2 = -(av - cv), B2 = au - cu, C2 = -fmaf(A2, cu, B2 * cv);       // edge c -> a
-    const float area2 = fmaf(A0, cu, fmaf(B0, cv, C0));                     // E_ab(c)
-    if (area2 == 0.0f || !(fabsf(area2) < FLT_MAX)) {                       // edge-on or degenerate: never hit
-        eq[0] = make_float4(0.f, 0.f, -1.f, 0.f); eq[1] = eq[0]; eq[2] = eq[0];
-        return;
-    }
-    if (area2 < 0.0f) { A0 = -A0; B0 = -B0; C0 = -C0; A1 = -A1; B1 = -B1; C1 = -C1; A2 = -A2; B2 = -B2; C2 = -C2; }
-    const float ia = 1.0f / area2;
-    const float Wu = ((cv - av) * (bw - aw) - (bv - av) * (cw - aw)) * ia;
-    const float Wv = ((bu - au) * (cw - aw) - (cu - au) * (bw - aw)) * ia;
-    const float Wc = aw - fmaf(Wu, au, Wv * av);
-    eq[0] = make_float4(A0, B0, C0, Wu);
-    eq[1] = make_float4(A1, B1, C1, Wv);
-    eq[2] = make_float4(A2, B2, C2, Wc);
-}
-
-// ---- per-warp ray pool (global memory ring) ----
-// Rays that are not resolved by a beam -- bounce rays, and primaries of a group whose lists
-// overflowed -- are appended to the warp's private ring in global memory (L2-resident) and traced
-// later, many tiles' worth at a time, by the per-ray traversal loop of drain(): a lane whose ray
-// has ended takes the next ray of the pool at once, so lanes stay busy although path lengths
-// differ widely (persistent "while-while" traversal with dynamic fetch).  Hits are not shaded where
-// they are found: they are queued in shared memory and shaded 32 at a time, converged.
-// Entry = 9 words (origin, direction, ray index i, pair index p, src | depth << 27), plus the
-// 64-bit path signature in the instrumented build; field-major so appends and fetches coalesce.
-constexpr int POOL_FIELDS = 9;
-constexpr int POOL_FIELDS_INSTR = 11;
-#ifndef POOL_HIGH_DEF
-#define POOL_HIGH_DEF 4096
-#endif
-constexpr int POOL_HIGH = POOL_HIGH_DEF;          // drain when the pool holds at least this many rays
-constexpr int HITQ = 64;                 // queued hits per warp
-constexpr int DRAIN_ACTIVE_MIN = 24;     // leave the traversal loop to refill when fewer lanes are busy
-constexpr uint32_t SRC_NONE = 0x07ffffffu;
-
-struct Pool {
-    unsigned *base;
-    uint32_t cap, mask, head, tail;      // head/tail count rays; position = counter & mask
-};
-__device__ __forceinline__ void pool_st(const Pool &q, int field, uint32_t pos, uint32_t v)
-{
-    __stcg(q.base + (size_t)field * q.cap + (pos & q.mask), v);
-}
-__device__ __forceinline__ uint32_t pool_ld(const Pool &q, int field, uint32_t pos)
-{
-    return __ldcg(q.base + (size_t)field * q.cap + (pos & q.mask));
-}
-
-struct BeamSmem {                   // per warp; beam structures and drain structures are never live together
-    union {
-        struct {
-            float4 eq[3 * BEAM_CMAX];       // (A0,B0,C0,Wu) (A1,B1,C1,Wv) (A2,B2,C2,Wc) per candidate
-            int cid[BEAM_CMAX];             // candidate -> sorted triangle index
-            int enode[BEAM_EN];
-            int eleaf[BEAM_EL];
-            int nq[BEAM_QN];
-            unsigned char glist[BEAM_CMAX];
-        } b;
-        struct {
-            int stack[BEAM_STACK * 32];     // per-thread traversal stacks, thread-interleaved
-            uint32_t hq[11][HITQ];          // queued hits: o, d, i, p, sd, triangle, t
-        } s;
-    } u;
-};
-
-template <bool INSTR, bool TORQUE>
-__global__ void __launch_bounds__(TRACE_THREADS, BEAM_BLOCKS_PER_SM)
-beam_trace_kernel(const TraceArgs a)
-{
-    __shared__ BeamSmem s_w[TRACE_WARPS];
-    __shared__ unsigned long long s_hsig[INSTR ? TRACE_WARPS * HITQ : 1];
-    __shared__ unsigned s_hist[TRACE_WARPS][16];
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    if (lane < 16) s_hist[warp][lane] = 0;
-    __syncwarp();
-    BeamSmem &W = s_w[warp];
-    unsigned long long *hsig = s_hsig + (INSTR ? warp * HITQ : 0);
-    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    BeamCounters bc = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
-    const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
-    const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
-    Pool pool;
-    pool.cap = (uint32_t)a.pool_cap; pool.mask = pool.cap - 1u; pool.head = pool.tail = 0u;
-    pool.base = a.pool + (size_t)(blockIdx.x * TRACE_WARPS + warp) * (size_t)(INSTR ? POOL_FIELDS_INSTR : POOL_FIELDS) * pool.cap;
-
-    // Appends this lane's ray (if `push`) to the pool; warp-wide call.
-    auto pool_push = [&](bool push, const float3 &o, const float3 &d, uint32_t i, uint32_t p, uint32_t sd,
-                         unsigned long long sig) {
-        const unsigned m = __ballot_sync(FULL, push);
-        if (push) {
-            const uint32_t pos = pool.tail + (uint32_t)__popc(m & lt_mask);
-            pool_st(pool, 0, pos, __float_as_uint(o.x)); pool_st(pool, 1, pos, __float_as_uint(o.y));
-            pool_st(pool, 2, pos, __float_as_uint(o.z)); pool_st(pool, 3, pos, __float_as_uint(d.x));
-            pool_st(pool, 4, pos, __float_as_uint(d.y)); pool_st(pool, 5, pos, __float_as_uint(d.z));
-            pool_st(pool, 6, pos, i); pool_st(pool, 7, pos, p); pool_st(pool, 8, pos, sd);
-            if (INSTR) { pool_st(pool, 9, pos, (uint32_t)sig); pool_st(pool, 10, pos, (uint32_t)(sig >> 32)); }
-        }
-        pool.tail += (uint32_t)__popc(m);
-        SRP_CHECK(pool.tail - pool.head <= pool.cap, "ray pool");
-    };
-
-    // ---- S5-S7 for <= 32 queued hits, converged; survivors go back to the pool ----
-    int nhit = 0;                                                  // warp-uniform
-    auto shade_batch = [&]() {
-        const int take = nhit < 32 ? nhit : 32;
-        int fate = -1, src = -1, depth = 0;
-        float3 o = f3(0, 0, 0), d = f3(0, 0, 1);
-        uint32_t i = 0, p = 0;
-        unsigned long long sig = 0;
-        if (lane < take) {
-            const int e = nhit - take + lane;
-            o = f3(__uint_as_float(W.u.s.hq[0][e]), __uint_as_float(W.u.s.hq[1][e]), __uint_as_float(W.u.s.hq[2][e]));
-            d = f3(__uint_as_float(W.u.s.hq[3][e]), __uint_as_float(W.u.s.hq[4][e]), __uint_as_float(W.u.s.hq[5][e]));
-            i = W.u.s.hq[6][e]; p = W.u.s.hq[7][e];
-            depth = (int)(W.u.s.hq[8][e] >> 27);
-            const int best = (int)W.u.s.hq[9][e];
-            const float t = __uint_as_float(W.u.s.hq[10][e]);
-            int k, j;
-            pair_of32(a, p, k, j);
-            const long long tb = a.dz.tri_off[k];
-            const float4 *lt = a.dz.tri + 3 * tb;
-            RayGen g;
-            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque<TORQUE>(g, a, k);
-            g.inv_nx = inv_nx; g.inv_ny = inv_ny;
-            atomicAdd(&s_hist[warp][depth], 1u);
-            if (INSTR) sig = hsig[e] * 1000003ULL + (unsigned long long)(a.dz.perm[tb + best] + 1);
-            float3 dep = f3(0, 0, 0), dep_t = f3(0, 0, 0);
-            fate = shade<TORQUE>(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
-                         a.deposit, o, d, src, depth, dep, dep_t);
-            if (fate == SHADE_ABSORBED) cn.absorbed++;
-            if (fate == SHADE_CAPPED) cn.capped++;
-            unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * (long long)p);
-            if (dep.x != 0.0f) atomicAdd(dst + 0, (unsigned long long)__double2ll_rn((double)dep.x * SRP_ACC_SCALE));
-            if (dep.y != 0.0f) atomicAdd(dst + 1, (unsigned long long)__double2ll_rn((double)dep.y * SRP_ACC_SCALE));
-            if (dep.z != 0.0f) atomicAdd(dst + 2, (unsigned long long)__double2ll_rn((double)dep.z * SRP_ACC_SCALE));
-            if (TORQUE) {
-                if (dep_t.x != 0.0f) atomicAdd(dst + 3, (unsigned long long)__double2ll_rn((double)dep_t.x * SRP_ACC_SCALE));
-                if (dep_t.y != 0.0f) atomicAdd(dst + 4, (unsigned long long)__double2ll_rn((double)dep_t.y * SRP_ACC_SCALE));
-                if (dep_t.z != 0.0f) atomicAdd(dst + 5, (unsigned long long)__double2ll_rn((double)dep_t.z * SRP_ACC_SCALE));
-            }
-            if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[(long long)p * a.N + i] = sig;
-        }
-        nhit -= take;
-        __syncwarp();
-        pool_push(fate == SHADE_CONTINUE, o, d, i, p, ((uint32_t)depth << 27) | (uint32_t)src, sig);
-    };
-
-    // ---- per-ray traversal of everything in the pool (S4 for incoherent rays, S6) ----
-    auto drain = [&]() {
-        constexpr int STRIDE = 32, NSMEM = BEAM_STACK;
-        int *s_stack = W.u.s.stack + lane;
-        int ovf[STACK_OVF];
-        bool has = false;
-        int cur = CUR_DONE, sp = 0, best = -1, src = -1;
-        float tbest = FLT_MAX;
-        float3 o = f3(0, 0, 0), d = f3(0, 0, 1);
-        float idx = 0.f, idy = 0.f, idz = 0.f, oxi = 0.f, oyi = 0.f, ozi = 0.f;
-        uint32_t ri = 0, rp = 0, rsd = 0;
-        unsigned long long rsig = 0;
-        const float4 *ln = a.dz.nodes, *lt = a.dz.tri;
-        unsigned nt = 0;
-        for (;;) {
-            // lanes without a ray take the next rays of the pool
-            const unsigned idle = __ballot_sync(FULL, !has);
-            uint32_t navail = pool.tail - pool.head;
-            if (idle != 0u && navail != 0u) {
-                const uint32_t rank = (uint32_t)__popc(idle & lt_mask);
-                if (!has && rank < navail) {
-                    const uint32_t pos = pool.head + rank;
-                    o = f3(__uint_as_float(pool_ld(pool, 0, pos)), __uint_as_float(pool_ld(pool, 1, pos)),
-                           __uint_as_float(pool_ld(pool, 2, pos)));
-                    d = f3(__uint_as_float(pool_ld(pool, 3, pos)), __uint_as_float(pool_ld(pool, 4, pos)),
-                           __uint_as_float(pool_ld(pool, 5, pos)));
-                    ri = pool_ld(pool, 6, pos); rp = pool_ld(pool, 7, pos); rsd = pool_ld(pool, 8, pos);
-                    if (INSTR) rsig = (unsigned long long)pool_ld(pool, 9, pos) | ((unsigned long long)pool_ld(pool, 10, pos) << 32);
-                    int k, j;
-                    pair_of32(a, rp, k, j);
-                    const long long tb = a.dz.tri_off[k];
-                    ln = a.dz.nodes + 4 * tb; lt = a.dz.tri + 3 * tb;
-                    const uint32_t s27 = rsd & SRC_NONE;
-                    src = s27 == SRC_NONE ? -1 : (int)s27;
-                    idx = safe_rcp(d.x); idy = safe_rcp(d.y); idz = safe_rcp(d.z);
-                    oxi = o.x * idx; oyi = o.y * idy; ozi = o.z * idz;
-                    has = true; cur = 0; sp = 0; tbest = FLT_MAX; best = -1;
-                    if ((rsd >> 27) != 0u) cn.segments++;            // primaries were counted when generated
-                }
-                const uint32_t want = (uint32_t)__popc(idle);
-                pool.head += want < navail ? want : navail;
-                navail = pool.tail - pool.head;
-            }
-            if (!__any_sync(FULL, has)) {
-                if (nhit > 0) { shade_batch(); continue; }          // shading may put rays back
-                break;
-            }
-            // traverse until every lane is done, or enough lanes are free and rays are waiting
-            for (;;) {
-#pragma unroll 1
-                for (int steps = 0; steps < NODE_RUN_CAP && (unsigned)cur < (unsigned)CUR_DONE; ++steps) {
-                    if (INSTR) cn.n_box += 2;
-                    cur = bvh_node_step<STRIDE, NSMEM>(ln, cur, sp, s_stack, ovf, idx, idy, idz, oxi, oyi, ozi, tbest);
-                }
-                if (cur < 0) cur = bvh_leaf_step<STRIDE, NSMEM>(lt, cur, sp, s_stack, ovf, o, d, src, tbest, best, nt);
-                const unsigned act = __ballot_sync(FULL, cur != CUR_DONE);
-                if (act == 0u || (navail != 0u && __popc(act) < DRAIN_ACTIVE_MIN)) break;
-            }
-            // retire the rays that ended
-            const bool fin = has && cur == CUR_DONE;
-            const bool hit = fin && best >= 0;
-            if (fin && !hit) {
-                if ((rsd >> 27) == 0u) cn.pmiss++; else cn.escaped++;
-                if (INSTR && a.sig_out) a.sig_out[(long long)rp * a.N + ri] = rsig;
-            }
-            const unsigned mh = __ballot_sync(FULL, hit);
-            SRP_CHECK(nhit + __popc(mh) <= HITQ, "hit queue");
-            if (hit) {
-                const int e = nhit + __popc(mh & lt_mask);
-                W.u.s.hq[0][e] = __float_as_uint(o.x); W.u.s.hq[1][e] = __float_as_uint(o.y); W.u.s.hq[2][e] = __float_as_uint(o.z);
-                W.u.s.hq[3][e] = __float_as_uint(d.x); W.u.s.hq[4][e] = __float_as_uint(d.y); W.u.s.hq[5][e] = __float_as_uint(d.z);
-                W.u.s.hq[6][e] = ri; W.u.s.hq[7][e] = rp; W.u.s.hq[8][e] = rsd;
-                W.u.s.hq[9][e] = (uint32_t)best; W.u.s.hq[10][e] = __float_as_uint(tbest);
-                if (INSTR) hsig[e] = rsig;
-            }
-            nhit += __popc(mh);
-            if (fin) has = false;
-            __syncwarp();
-            if (nhit >= 32) shade_batch();
-        }
-        if (INSTR) cn.n_tri += nt;
-    };
-
-    // ---- S2-S5 for the primaries of one tile, as beams ----
-    auto process_tile = [&](unsigned long long tile) {
-        const long long p = (long long)(tile / a.tiles_per_pair);
-        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
-        int k, j;
-        pair_of(a, p, k, j);
-        const float4 blo = a.dz.box[2 * k], bhi = a.dz.box[2 * k + 1];
-        const Emitter em = make_emitter(a.sun_dirs, j, blo, bhi);
-        if (!(em.Ae > 0.0f)) return;                              // edge-on flat design: F = 0, nothing launched
-        const long long tbase = a.dz.tri_off[k];
-        const float4 *gtri = a.dz.tri + 3 * tbase;
-        const float4 *gnodes = a.dz.nodes + 4 * tbase;
-        RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque<TORQUE>(g, a, k);
-        g.inv_nx = inv_nx; g.inv_ny = inv_ny;
-        BeamFrame bf;
-        bf.uh = f3(0.5f * em.u.x, 0.5f * em.u.y, 0.5f * em.u.z);
-        bf.vh = f3(0.5f * em.v.x, 0.5f * em.v.y, 0.5f * em.v.z);
-        bf.auh = f3(fabsf(bf.uh.x), fabsf(bf.uh.y), fabsf(bf.uh.z));
-        bf.avh = f3(fabsf(bf.vh.x), fabsf(bf.vh.y), fabsf(bf.vh.z));
-        bf.csu = em.du * inv_nx; bf.csv = em.dv * inv_ny;
-        {   // fp32 projections of points of this design are off by < 1e-6 of this scale; 10x that
-            const float L = fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
-                            fmaxf(fabsf(blo.z), fabsf(bhi.z));
-            bf.margin = 1.0e-5f * L;
-        }
-        const uint32_t start = (uint32_t)(q * a.tile_rays);
-        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
-        const uint32_t nt = end - start;                          // a power of two
-        const int tbits = 31 - __clz((int)nt);
-        float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
-
-        // tile level: frontier descent to an entry list
-        const uint32_t tcx0 = compact_even_bits(start), tcy0 = compact_even_bits(start >> 1);
-        const float t_offu = fmaf((float)tcx0 * inv_nx, em.du, em.u0), t_offv = fmaf((float)tcy0 * inv_ny, em.dv, em.v0);
-        const float t_wu = (float)(1u << ((tbits + 1) >> 1)) * bf.csu, t_wv = (float)(1u << (tbits >> 1)) * bf.csv;
-        int n_en = 1, n_el = 0;
-        if (lane == 0) W.u.b.enode[0] = 0;
-        __syncwarp();
-        for (int lvl = 0; lvl < 24 && n_en > 0 && n_en <= 32 && n_el <= 32; ++lvl) {
-            const int node = lane < n_en ? W.u.b.enode[lane] : -1;
-            __syncwarp();
-            bool h0, h1; int l0, l1;
-            beam_node<INSTR>(gnodes, node, bf, t_offu, t_offv, t_wu, t_wv, h0, h1, l0, l1, bc.beam_box);
-            const bool p0 = h0 && l0 >= 0, p1 = h1 && l1 >= 0, f0 = h0 && l0 < 0, f1 = h1 && l1 < 0;
-            const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
-            const unsigned mf0 = __ballot_sync(FULL, f0), mf1 = __ballot_sync(FULL, f1);
-            const int np0 = __popc(mp0), nf0 = __popc(mf0), nf1 = __popc(mf1);
-            SRP_CHECK(np0 + __popc(mp1) <= BEAM_EN, "entry nodes"); SRP_CHECK(n_el + nf0 + nf1 <= BEAM_EL, "entry leaves");
-            if (p0) W.u.b.enode[__popc(mp0 & lt_mask)] = l0;
-            if (p1) W.u.b.enode[np0 + __popc(mp1 & lt_mask)] = l1;
-            if (f0) W.u.b.eleaf[n_el + __popc(mf0 & lt_mask)] = l0;
-            if (f1) W.u.b.eleaf[n_el + nf0 + __popc(mf1 & lt_mask)] = l1;
-            n_en = np0 + __popc(mp1); n_el += nf0 + nf1;
-            __syncwarp();
-        }
-        if (n_en == 0 && n_el == 0) {                             // the tile's beam meets nothing: nt primary misses
-            const unsigned c = nt >= 32u ? nt >> 5 : (unsigned)(lane < (int)nt);
-            cn.launched += c; cn.pmiss += c; cn.segments += c; bc.tile_miss += c;
-            return;
-        }
-
-        // Sub-blocks are adaptive: a block whose lists overflow is halved (down to one group of 32 rays, whose
-        // rays then go to the pool for per-ray traversal); the size grows back at the next aligned position.
-        const uint32_t nb_max = nt < (uint32_t)BEAM_SB ? nt : (uint32_t)BEAM_SB;
-        uint32_t nb = nb_max;                                     // rays in the current sub-block
-        for (uint32_t sb = start; sb < end;) {
-            const int sbits = 31 - __clz((int)nb);
-            const uint32_t s_wx = 1u << ((sbits + 1) >> 1), s_wy = 1u << (sbits >> 1);
-            const uint32_t g_wx = nb >= 32u ? 8u : s_wx, g_wy = nb >= 32u ? 4u : s_wy;
-            const float s_wu = (float)s_wx * bf.csu, s_wv = (float)s_wy * bf.csv;
-            const uint32_t scx0 = compact_even_bits(sb), scy0 = compact_even_bits(sb >> 1);
-            const float s_offu = fmaf((float)scx0 * inv_nx, em.du, em.u0), s_offv = fmaf((float)scy0 * inv_ny, em.dv, em.v0);
-            bool ovf = false;
-            int ncand = 0;
-            {
-                // sub-block level: descent from the entry list to candidate triangles
-                for (int x = lane; x < n_en; x += 32) W.u.b.nq[x] = W.u.b.enode[x];
-                int qn = n_en;
-                for (int base = 0; base < n_el && !ovf; base += 32) {
-                    const int x = base + lane;
-                    int first = 0, cnt = 0;
-                    if (x < n_el) { const unsigned u = (unsigned)~W.u.b.eleaf[x]; first = (int)(u >> 3); cnt = (int)(u & 7u) + 1; }
-                    if (!beam_push_tris(W.u.b.cid, ncand, first, cnt, 0, 0, lane)) ovf = true;
-                }
-                __syncwarp();
-                while (qn > 0 && !ovf) {
-                    const int take = qn < 32 ? qn : 32;
-                    const int node = lane < take ? W.u.b.nq[qn - take + lane] : -1;
-                    qn -= take;
-                    __syncwarp();
-                    bool h0, h1; int l0, l1;
-                    beam_node<INSTR>(gnodes, node, bf, s_offu, s_offv, s_wu, s_wv, h0, h1, l0, l1, bc.beam_box);
-                    const bool p0 = h0 && l0 >= 0, p1 = h1 && l1 >= 0, f0 = h0 && l0 < 0, f1 = h1 && l1 < 0;
-                    const unsigned mp0 = __ballot_sync(FULL, p0), mp1 = __ballot_sync(FULL, p1);
-                    const int np0 = __popc(mp0), np1 = __popc(mp1);
-                    if (qn + np0 + np1 > BEAM_QN) { ovf = true; break; }
-                    if (p0) W.u.b.nq[qn + __popc(mp0 & lt_mask)] = l0;
-                    if (p1) W.u.b.nq[qn + np0 + __popc(mp1 & lt_mask)] = l1;
-                    qn += np0 + np1;
-                    if (__any_sync(FULL, f0 || f1)) {
-                        const unsigned u0 = (unsigned)~l0, u1 = (unsigned)~l1;
-                        if (!beam_push_tris(W.u.b.cid, ncand, (int)(u0 >> 3), f0 ? (int)(u0 & 7u) + 1 : 0, (int)(u1 >> 3),
-                                            f1 ? (int)(u1 & 7u) + 1 : 0, lane))
-                            ovf = true;
-                    }
-                    __syncwarp();
-                }
-                if (!ovf && ncand == 0) {                        // empty sub-block
-                    const unsigned c = nb >= 32u ? nb >> 5 : (unsigned)(lane < (int)nb);
-                    cn.launched += c; cn.pmiss += c; cn.segments += c; bc.block_miss += c;
-                    sb += nb;
-                    if (nb < nb_max && (sb & (2u * nb - 1u)) == 0u) nb <<= 1;
-                    continue;
-                }
-                if (ovf && nb > 32u) { nb >>= 1; continue; }     // retry this position with half the rays
-                if (!ovf) {
-                    __syncwarp();
-                    for (int c = lane; c < ncand; c += 32) {
-                        const int f = W.u.b.cid[c];
-                        if (INSTR) bc.setups++;
-                        beam_setup(__ldg(gtri + 3 * f), __ldg(gtri + 3 * f + 1), __ldg(gtri + 3 * f + 2), em, s_offu, s_offv,
-                                   W.u.b.eq + 3 * c);
-                    }
-                    __syncwarp();
-                }
-            }
-
-            // groups of 32 rays
-            for (uint32_t gs = sb; gs < sb + nb; gs += 32) {
-                const uint32_t gcx = compact_even_bits(gs) - scx0, gcy = compact_even_bits(gs >> 1) - scy0;
-                int ng = 0;
-                if (!ovf) {
-                    const float gu0 = (float)gcx * bf.csu, gu1 = (float)(gcx + g_wx) * bf.csu;
-                    const float gv0 = (float)gcy * bf.csv, gv1 = (float)(gcy + g_wy) * bf.csv;
-                    for (int base = 0; base < ncand; base += 32) {
-                        const int c = base + lane;
-                        bool keep = false;
-                        if (c < ncand) {
-                            if (INSTR) bc.rect++;
-                            const float4 E0 = W.u.b.eq[3 * c], E1 = W.u.b.eq[3 * c + 1], E2 = W.u.b.eq[3 * c + 2];
-                            // largest value of each edge function over the rectangle (monotone in fp32 too)
-                            const float m0 = fmaf(E0.x, E0.x >= 0.f ? gu1 : gu0, fmaf(E0.y, E0.y >= 0.f ? gv1 : gv0, E0.z));
-                            const float m1 = fmaf(E1.x, E1.x >= 0.f ? gu1 : gu0, fmaf(E1.y, E1.y >= 0.f ? gv1 : gv0, E1.z));
-                            const float m2 = fmaf(E2.x, E2.x >= 0.f ? gu1 : gu0, fmaf(E2.y, E2.y >= 0.f ? gv1 : gv0, E2.z));
-                            keep = fminf(m0, fminf(m1, m2)) >= 0.0f;
-                        }
-                        const unsigned m = __ballot_sync(FULL, keep);
-                        SRP_CHECK(ng + __popc(m) <= BEAM_CMAX, "group list");
-                        if (keep) W.u.b.glist[ng + __popc(m & lt_mask)] = (unsigned char)c;
-                        ng += __popc(m);
-                    }
-                    __syncwarp();
-                    if (ng == 0) {                               // 32 primary misses, no ray generated
-                        const unsigned c = (unsigned)(lane < (int)nb);
-                        cn.launched += c; cn.pmiss += c; cn.segments += c; bc.group_miss += c;
-                        continue;
-                    }
-                }
-                // O-step 3 for this lane's ray
-                const bool on = lane < (int)nb;
-                const uint32_t i = gs + (uint32_t)lane;
-                float3 o = f3(0, 0, 0), d = em.s;
-                float lu = 0.f, lv = 0.f;
-                if (on) {
-                    uint32_t r0, r1, r2, r3;
-                    philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
-                    const float xi0 = uniform23(r0), xi1 = uniform23(r1);
-                    const uint32_t cx = nb >= 32u ? scx0 + gcx + ldx : compact_even_bits(i);
-                    const uint32_t cy = nb >= 32u ? scy0 + gcy + ldy : compact_even_bits(i >> 1);
-                    const float fu = ((float)cx + xi0) * inv_nx, fv = ((float)cy + xi1) * inv_ny;
-                    const float pu = fmaf(fu, em.du, em.u0), pv = fmaf(fv, em.dv, em.v0);
-                    o = f3(fmaf(pu, em.u.x, fmaf(pv, em.v.x, em.worg * em.s.x)),
-                           fmaf(pu, em.u.y, fmaf(pv, em.v.y, em.worg * em.s.y)),
-                           fmaf(pu, em.u.z, fmaf(pv, em.v.z, em.worg * em.s.z)));
-                    lu = ((float)(cx - scx0) + xi0) * bf.csu;
-                    lv = ((float)(cy - scy0) + xi1) * bf.csv;
-                    cn.launched++; cn.segments++;
-                }
-                if (ovf) {                                       // too much geometry behind this group: per-ray traversal
-                    if (on) bc.fallback++;
-                    pool_push(on, o, d, i, (uint32_t)p, SRC_NONE, 0ULL);
-                    continue;
-                }
-                // O-step 4 against the shared list: all lanes converged, operands broadcast
-                float tbest = FLT_MAX;
-                int best = -1;
-                for (int e = 0; e < ng; ++e) {
-                    const int c = W.u.b.glist[e];
-                    const float4 E0 = W.u.b.eq[3 * c], E1 = W.u.b.eq[3 * c + 1], E2 = W.u.b.eq[3 * c + 2];
-                    const float e0 = fmaf(E0.x, lu, fmaf(E0.y, lv, E0.z));
-                    const float e1 = fmaf(E1.x, lu, fmaf(E1.y, lv, E1.z));
-                    const float e2 = fmaf(E2.x, lu, fmaf(E2.y, lv, E2.z));
-                    const float t = fmaf(E0.w, lu, fmaf(E1.w, lv, E2.w));
-                    if (fminf(e0, fminf(e1, e2)) >= 0.0f && t < tbest) { tbest = t; best = c; }
-                }
-                if (INSTR && on) bc.tri2d += (unsigned)ng;
-                if (best >= 0) best = W.u.b.cid[best];
-                if (!on) best = -1;
-                int fate = -1, src = -1, depth = 0;
-                unsigned long long sig = 0;
-                if (on) {
-                    if (best < 0) cn.pmiss++;
-                    else {
-                        atomicAdd(&s_hist[warp][0], 1u);
-                        if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                        fate = shade<TORQUE>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                     best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
-                        if (fate == SHADE_ABSORBED) cn.absorbed++;
-                        if (fate == SHADE_CAPPED) cn.capped++;
-                    }
-                    if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
-                }
-                pool_push(fate == SHADE_CONTINUE, o, d, i, (uint32_t)p, ((uint32_t)depth << 27) | (uint32_t)src, sig);
-            }
-            sb += nb;
-            if (nb < nb_max && (sb & (2u * nb - 1u)) == 0u) nb <<= 1;
-        }
-
-        // S7 for the tile's primaries: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
-    };
-
-    // ---- persistent loop: tiles until the pool is worth draining ----
-    bool more = true;
-    for (;;) {
-        if (more) {
-            unsigned long long tile = 0;
-            if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
-            tile = __shfl_sync(FULL, tile, 0);
-            if (tile >= total_tiles) more = false;
-            else process_tile(tile);
-        }
-        __syncwarp();
-        const uint32_t cnt = pool.tail - pool.head;
-        if (cnt >= (uint32_t)POOL_HIGH || (!more && cnt != 0u)) { drain(); __syncwarp(); }
-        if (!more && pool.tail == pool.head) break;
-    }
-    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
-    flush_beam_counters(a, bc, lane);
-}
-
-// ---- designs without a hierarchy (T <= SRP_BRUTE_MAX_TRIS), stratified sampler ----
-// "Test all triangles" with the same two ideas as the beam kernel.  The primaries of
-// a tile are parallel, so every triangle is set up ONCE per tile as three 2-D edge functions and a
-// depth plane in the emitter frame (16 instructions per ray-triangle test instead of the ~45 of
-// Moller-Trumbore), and a block of rays whose rectangle no edge function admits is a block of
-// misses: no Philox call, no test.  Levels: tile -> 256 rays -> 32 rays (one per lane).  Bounce rays
-// collect in the warp's shared-memory queue and are traced 32 at a time against all triangles
-// (Moller-Trumbore from shared memory; every ray costs the same, so passes stay converged).
-struct SmallSmem {                  // per warp
-    float4 tri[3 * SRP_BRUTE_MAX_TRIS];     // the design's packed triangles (S4 for bounce rays, S5)
-    float4 eq[3 * SRP_BRUTE_MAX_TRIS];      // per tile: edge functions + depth plane of every triangle
-    unsigned char tl[SRP_BRUTE_MAX_TRIS], sl[SRP_BRUTE_MAX_TRIS], gl[SRP_BRUTE_MAX_TRIS];   // tile / sub-block / group lists
-    unsigned long long vis[2][SRP_BRUTE_MAX_TRIS];   // per design: triangles with a vertex in front of / behind each facet
-    WarpQueue q;
-};
-
-// Candidates of `in` (n_in of them; nullptr = all triangles 0..n_in-1) whose edge functions admit the
-// rectangle [u0,u1] x [v0,v1] -> out; returns how many.  Warp-wide call.
-template <bool INSTR>
-__device__ __forceinline__ int small_filter(const float4 *eq, const unsigned char *in, int n_in, float u0, float u1,
-                                            float v0, float v1, unsigned char *out, int lane, unsigned lt_mask,
-                                            unsigned &n_rect)
-{
-    int n = 0;
-    for (int base = 0; base < n_in; base += 32) {
-        const int x = base + lane;
-        bool keep = false;
-        int c = 0;
-        if (x < n_in) {
-            if (INSTR) ++n_rect;
-            c = in ? (int)in[x] : x;
-            const float4 E0 = eq[3 * c], E1 = eq[3 * c + 1], E2 = eq[3 * c + 2];
-            const float m0 = fmaf(E0.x, E0.x >= 0.f ? u1 : u0, fmaf(E0.y, E0.y >= 0.f ? v1 : v0, E0.z));
-            const float m1 = fmaf(E1.x, E1.x >= 0.f ? u1 : u0, fmaf(E1.y, E1.y >= 0.f ? v1 : v0, E1.z));
-            const float m2 = fmaf(E2.x, E2.x >= 0.f ? u1 : u0, fmaf(E2.y, E2.y >= 0.f ? v1 : v0, E2.z));
-            keep = fminf(m0, fminf(m1, m2)) >= 0.0f;
-        }
-        const unsigned m = __ballot_sync(FULL, keep);
-        SRP_CHECK(n + __popc(m) <= SRP_BRUTE_MAX_TRIS, "small-design list");
-        if (keep) out[n + __popc(m & lt_mask)] = (unsigned char)c;
-        n += __popc(m);
-    }
-    __syncwarp();
-    return n;
-}
-
-template <bool INSTR, bool TORQUE>
-__global__ void __launch_bounds__(TRACE_THREADS, 6)
-small_beam_kernel(const TraceArgs a)
-{
-    __shared__ SmallSmem s_w[TRACE_WARPS];
-    __shared__ unsigned long long s_qsig[INSTR ? TRACE_WARPS * QCAP : 1];
-    __shared__ unsigned s_hist[TRACE_WARPS][16];
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    if (lane < 16) s_hist[warp][lane] = 0;
-    __syncwarp();
-    SmallSmem &W = s_w[warp];
-    WarpQueue &Q = W.q;
-    unsigned long long *qsig = s_qsig + (INSTR ? warp * QCAP : 0);
-    LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    BeamCounters bc = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
-    const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
-    const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
-    int loaded_k = -1;
-
-    for (;;) {
-        unsigned long long tile = 0;
-        if (lane == 0) tile = atomicAdd(a.work_counter, 1ULL);
-        tile = __shfl_sync(FULL, tile, 0);
-        if (tile >= total_tiles) break;
-        const long long p = (long long)(tile / a.tiles_per_pair);
-        const long long q = (long long)(tile - (unsigned long long)p * a.tiles_per_pair);
-        int k, j;
-        pair_of(a, p, k, j);
-        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
-        if (!(em.Ae > 0.0f)) continue;                      // edge-on flat design: F = 0, nothing launched
-        const long long tbase = a.dz.tri_off[k];
-        const int T = (int)(a.dz.tri_off[k + 1] - tbase);
-        if (loaded_k != k) {
-            const float4 *gtri = a.dz.tri + 3 * tbase;
-            __syncwarp();
-            for (int x = lane; x < 3 * T; x += 32) W.tri[x] = gtri[x];
-            loaded_k = k;
-            __syncwarp();
-            // A ray that leaves facet f on the side of +n (or -n) can only hit triangles with a vertex on that
-            // side of f's plane: two 64-bit masks per facet, built once per design.  The margin (1e-5 of the
-            // design's extent) keeps only coplanar neighbours out, which exact arithmetic never hits.
-            const float4 blo = a.dz.box[2 * k], bhi = a.dz.box[2 * k + 1];
-            const float eps = 1.0e-5f * (fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
-                                         fmaxf(fabsf(blo.z), fabsf(bhi.z)));
-            for (int f = lane; f < T; f += 32) {
-                const float4 q0 = W.tri[3 * f], q1 = W.tri[3 * f + 1], q2 = W.tri[3 * f + 2];
-                float3 n = cross3(f3(q1.x, q1.y, q1.z), f3(q2.x, q2.y, q2.z));
-                const float il = rsqrtf(dot3(n, n));
-                n = f3(n.x * il, n.y * il, n.z * il);
-                unsigned long long front = 0, back = 0;
-                for (int t = 0; t < T; ++t) {
-                    if (t == f) continue;
-                    const float4 p0 = W.tri[3 * t], p1 = W.tri[3 * t + 1], p2 = W.tri[3 * t + 2];
-                    const float3 r = f3(p0.x - q0.x, p0.y - q0.y, p0.z - q0.z);
-                    const float d0 = dot3(n, r), d1 = d0 + dot3(n, f3(p1.x, p1.y, p1.z)), d2 = d0 + dot3(n, f3(p2.x, p2.y, p2.z));
-                    if (fmaxf(d0, fmaxf(d1, d2)) > eps) front |= 1ULL << t;
-                    if (fminf(d0, fminf(d1, d2)) < -eps) back |= 1ULL << t;
-                }
-                W.vis[0][f] = front; W.vis[1][f] = back;
-            }
-        }
-        __syncwarp();
-        RayGen g;
-        g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = 0; set_torque<TORQUE>(g, a, k);
-        g.inv_nx = inv_nx; g.inv_ny = inv_ny;
-        const float csu = em.du * inv_nx, csv = em.dv * inv_ny;
-        const uint32_t start = (uint32_t)(q * a.tile_rays);
-        const uint32_t end = (uint32_t)min((long long)a.N, (q + 1) * (long long)a.tile_rays);
-        const uint32_t nt = end - start;                          // a power of two
-        const int tbits = 31 - __clz((int)nt);
-        int qcount = 0;                                           // warp-uniform
-        float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
-
-        // a pass of <= 32 queued bounce rays against all triangles (S4, S6)
-        auto secondary_pass = [&]() {
-            const int take = qcount < 32 ? qcount : 32;
-            bool alive = false;
-            uint32_t i = 0;
-            float3 o = f3(0, 0, 0), d = em.s;
-            int src = -1, depth = 0;
-            unsigned long long sig = 0;
-            if (lane < take) {
-                const int e = qcount - take + lane;
-                o = f3(Q.ox[e], Q.oy[e], Q.oz[e]); d = f3(Q.dx[e], Q.dy[e], Q.dz[e]);
-                i = Q.i[e]; src = Q.src_depth[e] & 0x07ffffff; depth = (int)((unsigned)Q.src_depth[e] >> 27);
-                if (INSTR) sig = qsig[e];
-                alive = true;
-            }
-            qcount -= take;
-            __syncwarp();
-            int fate = -1;
-            if (alive) {
-                float tbest = FLT_MAX; int best = -1;
-                cn.segments++;
-                {   // only the triangles on the side of the source facet the ray leaves on, in index order
-                    const float3 ns = cross3(f3(W.tri[3 * src + 1].x, W.tri[3 * src + 1].y, W.tri[3 * src + 1].z),
-                                             f3(W.tri[3 * src + 2].x, W.tri[3 * src + 2].y, W.tri[3 * src + 2].z));
-                    unsigned long long m = W.vis[dot3(ns, d) > 0.0f ? 0 : 1][src];
-                    if (INSTR) cn.n_tri += (unsigned)__popcll(m);
-                    while (m) {
-                        const int f = __ffsll((long long)m) - 1;
-                        m &= m - 1;
-                        tri_test(W.tri[3 * f], W.tri[3 * f + 1], W.tri[3 * f + 2], o, d, f, tbest, best);
-                    }
-                }
-                if (best < 0) cn.escaped++;
-                else {
-                    atomicAdd(&s_hist[warp][depth], 1u);
-                    if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    fate = shade<TORQUE>(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
-                                 a.deposit, o, d, src, depth, acc, acc_t);
-                    if (fate == SHADE_ABSORBED) cn.absorbed++;
-                    if (fate == SHADE_CAPPED) cn.capped++;
-                }
-                if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
-            }
-            const unsigned cont = __ballot_sync(FULL, fate == SHADE_CONTINUE);
-            if (fate == SHADE_CONTINUE) {
-                const int e = qcount + __popc(cont & lt_mask);
-                Q.ox[e] = o.x; Q.oy[e] = o.y; Q.oz[e] = o.z; Q.dx[e] = d.x; Q.dy[e] = d.y; Q.dz[e] = d.z;
-                Q.i[e] = i; Q.src_depth[e] = (depth << 27) | src;
-                if (INSTR) qsig[e] = sig;
-            }
-            qcount += __popc(cont);
-            __syncwarp();
-        };
-
-        // tile level: set every triangle up in the tile's local emitter frame; which ones touch the tile?
-        const uint32_t tcx0 = compact_even_bits(start), tcy0 = compact_even_bits(start >> 1);
-        const float offu = fmaf((float)tcx0 * inv_nx, em.du, em.u0), offv = fmaf((float)tcy0 * inv_ny, em.dv, em.v0);
-        for (int c = lane; c < T; c += 32) {
-            if (INSTR) bc.setups++;
-            beam_setup(W.tri[3 * c], W.tri[3 * c + 1], W.tri[3 * c + 2], em, offu, offv, W.eq + 3 * c);
-        }
-        __syncwarp();
-        const float t_wu = (float)(1u << ((tbits + 1) >> 1)) * csu, t_wv = (float)(1u << (tbits >> 1)) * csv;
-        const int n_tl = small_filter<INSTR>(W.eq, nullptr, T, 0.0f, t_wu, 0.0f, t_wv, W.tl, lane, lt_mask, bc.rect);
-        if (n_tl == 0) {
-            const unsigned c = nt >= 32u ? nt >> 5 : (unsigned)(lane < (int)nt);
-            cn.launched += c; cn.pmiss += c; cn.segments += c; bc.tile_miss += c;
-            continue;
-        }
-        const uint32_t nb = nt < 256u ? nt : 256u;               // rays per sub-block
-        const int sbits = 31 - __clz((int)nb);
-        const uint32_t s_wx = 1u << ((sbits + 1) >> 1), s_wy = 1u << (sbits >> 1);
-        const uint32_t g_wx = nb >= 32u ? 8u : s_wx, g_wy = nb >= 32u ? 4u : s_wy;
-        for (uint32_t sb = start; sb < end; sb += nb) {
-            const uint32_t scx = compact_even_bits(sb) - tcx0, scy = compact_even_bits(sb >> 1) - tcy0;   // cells from the tile corner
-            const int n_sl = small_filter<INSTR>(W.eq, W.tl, n_tl, (float)scx * csu, (float)(scx + s_wx) * csu, (float)scy * csv,
-                                          (float)(scy + s_wy) * csv, W.sl, lane, lt_mask, bc.rect);
-            if (n_sl == 0) {
-                const unsigned c = nb >= 32u ? nb >> 5 : (unsigned)(lane < (int)nb);
-                cn.launched += c; cn.pmiss += c; cn.segments += c; bc.block_miss += c;
-                continue;
-            }
-            for (uint32_t gs = sb; gs < sb + nb; gs += 32) {
-                const uint32_t gcx = compact_even_bits(gs) - tcx0, gcy = compact_even_bits(gs >> 1) - tcy0;
-                const int ng = small_filter<INSTR>(W.eq, W.sl, n_sl, (float)gcx * csu, (float)(gcx + g_wx) * csu, (float)gcy * csv,
-                                            (float)(gcy + g_wy) * csv, W.gl, lane, lt_mask, bc.rect);
-                if (ng == 0) {
-                    const unsigned c = (unsigned)(lane < (int)nb);
-                    cn.launched += c; cn.pmiss += c; cn.segments += c; bc.group_miss += c;
-                    continue;
-                }
-                // O-step 3 for this lane's ray
-                const bool on = lane < (int)nb;
-                const uint32_t i = gs + (uint32_t)lane;
-                float3 o = f3(0, 0, 0), d = em.s;
-                float lu = 0.f, lv = 0.f;
-                if (on) {
-                    uint32_t r0, r1, r2, r3;
-                    philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
-                    const float xi0 = uniform23(r0), xi1 = uniform23(r1);
-                    const uint32_t cx = nb >= 32u ? tcx0 + gcx + ldx : compact_even_bits(i);
-                    const uint32_t cy = nb >= 32u ? tcy0 + gcy + ldy : compact_even_bits(i >> 1);
-                    const float fu = ((float)cx + xi0) * inv_nx, fv = ((float)cy + xi1) * inv_ny;
-                    const float pu = fmaf(fu, em.du, em.u0), pv = fmaf(fv, em.dv, em.v0);
-                    o = f3(fmaf(pu, em.u.x, fmaf(pv, em.v.x, em.worg * em.s.x)),
-                           fmaf(pu, em.u.y, fmaf(pv, em.v.y, em.worg * em.s.y)),
-                           fmaf(pu, em.u.z, fmaf(pv, em.v.z, em.worg * em.s.z)));
-                    lu = ((float)(cx - tcx0) + xi0) * csu;
-                    lv = ((float)(cy - tcy0) + xi1) * csv;
-                    cn.launched++; cn.segments++;
-                }
-                // O-step 4 against the group's list: all lanes converged, operands broadcast
-                float tbest = FLT_MAX;
-                int best = -1;
-                for (int e = 0; e < ng; ++e) {
-                    const int c = W.gl[e];
-                    const float4 E0 = W.eq[3 * c], E1 = W.eq[3 * c + 1], E2 = W.eq[3 * c + 2];
-                    const float e0 = fmaf(E0.x, lu, fmaf(E0.y, lv, E0.z));
-                    const float e1 = fmaf(E1.x, lu, fmaf(E1.y, lv, E1.z));
-                    const float e2 = fmaf(E2.x, lu, fmaf(E2.y, lv, E2.z));
-                    const float t = fmaf(E0.w, lu, fmaf(E1.w, lv, E2.w));
-                    // ties -> smallest index, as O-step 4 (the list is in index order)
-                    if (fminf(e0, fminf(e1, e2)) >= 0.0f && t < tbest) { tbest = t; best = c; }
-                }
-                if (INSTR && on) bc.tri2d += (unsigned)ng;
-                if (!on) best = -1;
-                int fate = -1, src = -1, depth = 0;
-                unsigned long long sig = 0;
-                if (on) {
-                    if (best < 0) cn.pmiss++;
-                    else {
-                        atomicAdd(&s_hist[warp][0], 1u);
-                        if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                        fate = shade<TORQUE>(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
-                                     a.deposit, o, d, src, depth, acc, acc_t);
-                        if (fate == SHADE_ABSORBED) cn.absorbed++;
-                        if (fate == SHADE_CAPPED) cn.capped++;
-                    }
-                    if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
-                }
-                const unsigned cont = __ballot_sync(FULL, fate == SHADE_CONTINUE);
-                if (fate == SHADE_CONTINUE) {
-                    const int e = qcount + __popc(cont & lt_mask);
-                    Q.ox[e] = o.x; Q.oy[e] = o.y; Q.oz[e] = o.z; Q.dx[e] = d.x; Q.dy[e] = d.y; Q.dz[e] = d.z;
-                    Q.i[e] = i; Q.src_depth[e] = (depth << 27) | src;
-                    if (INSTR) qsig[e] = sig;
-                }
-                qcount += __popc(cont);
-                __syncwarp();
-                while (qcount >= 32) secondary_pass();
-            }
-        }
-        while (qcount > 0) secondary_pass();
-
-        // S7: warp reduction in fp64, then one fixed-point atomic per component
-        flush_tile_acc<TORQUE>(a, p, acc, acc_t, lane);
-    }
-    flush_counters<INSTR>(a, cn, s_hist[warp], lane);
-    flush_beam_counters(a, bc, lane);
-}
-
-// F[p] = accum[p] * 2^-32 * P * A_e / N
-__global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float *out, float *out_torque)
-{
-    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= a.n_pairs) return;
-    int k, j;
-    pair_of(a, p, k, j);
-    const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
-    const double w = em.Ae > 0.0f ? a.P * (double)em.Ae / (double)a.N / SRP_ACC_SCALE : 0.0;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) out[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + c] * w);
-    if (a.torque && out_torque)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) out_torque[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + 3 + c] * w);
-}
-
-// debug: primary-hit triangle (original index) of every ray of the listed pairs
-template <int MODE>
-__global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArgs a, int *out_prim)
-{
-    __shared__ int s_stack[MODE == MODE_BVH ? STACK_SMEM * TRACE_THREADS : 1];
-    const long long total = a.n_pairs * a.N;
-    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < total;
-         r += (long long)gridDim.x * blockDim.x) {
-        const long long p = r / a.N;
-        const uint32_t i = (uint32_t)(r - p * a.N);
-        int k, j;
-        pair_of(a, p, k, j);
-        const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
-        int best = -1;
-        if (em.Ae > 0.0f) {
-            const long long tbase = a.dz.tri_off[k];
-            const int T = (int)(a.dz.tri_off[k + 1] - tbase);
-            RayGen g;
-            g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; g.xc = f3(0.f, 0.f, 0.f);
-            g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
-            g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
-            float3 o;
-            make_ray(em, g, i, o);
-            float tbest = FLT_MAX;
-            unsigned nb = 0, nt = 0;
-            if (MODE == MODE_BVH)
-                closest_bvh<false>(a.dz.nodes + 4 * tbase, a.dz.tri + 3 * tbase, o, em.s, -1, tbest, best,
-                                   s_stack + threadIdx.x, nb, nt);
-            else
-                closest_brute<false>(a.dz.tri + 3 * tbase, T, o, em.s, -1, tbest, best, nt);
-            if (best >= 0) best = a.dz.perm[tbase + best];
-        }
-        out_prim[r] = best;
-    }
-}
-
-} // namespace
 
 // ---- roofline probes ----
 namespace {
@@ -1596,86 +95,4 @@ cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops
     cudaFree(out); cudaFree(buf);
     *fp32_tflops = best_f; *l2_gbs = best_l;
     return e;
-}
-
-// ---- launchers ----
-template <typename K>
-static cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStream_t stream)
-{
-    int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, 0);
-    if (e != cudaSuccess) return e;
-    if (per_sm < 1) per_sm = 1;
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
-    unsigned long long blocks = (unsigned long long)num_sms * per_sm;       // persistent: fill the machine once
-    const unsigned long long needed = (total_tiles + TRACE_WARPS - 1) / TRACE_WARPS;
-    if (blocks > needed) blocks = needed;
-    if (blocks < 1) blocks = 1;
-    kernel<<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a);
-    return cudaGetLastError();
-}
-
-int srp_trace_blocks_per_sm(bool brute, bool beam)
-{
-    int per_sm = 0;
-    if (brute && beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_beam_kernel<false, false>, TRACE_THREADS, 0);
-    else if (brute) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODE_BRUTE_SMEM, false, false>, TRACE_THREADS, 0);
-    else if (beam) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false, false>, TRACE_THREADS, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bvh_trace_kernel<false, false>, TRACE_THREADS, 0);
-    return per_sm * TRACE_WARPS;
-}
-
-// Words of global memory the beam kernel's per-warp ray pools need, and the ring capacity per warp.
-size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *cap_out)
-{
-    int per_sm = 0, per_sm_t = 0;
-    if (instrumented) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<true, false>, TRACE_THREADS, 0);
-    else {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, beam_trace_kernel<false, false>, TRACE_THREADS, 0);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_t, beam_trace_kernel<false, true>, TRACE_THREADS, 0);
-        if (per_sm_t > per_sm) per_sm = per_sm_t;
-    }
-    if (per_sm < 1) per_sm = 1;
-    int cap = 64;
-    while (cap < POOL_HIGH + tile_rays + 64) cap <<= 1;
-    *cap_out = cap;
-    return (size_t)num_sms * per_sm * TRACE_WARPS * (instrumented ? POOL_FIELDS_INSTR : POOL_FIELDS) * (size_t)cap;
-}
-
-// Three builds of each trace kernel: plain, instrumented (test counters, path signatures), and with torque
-// accumulation.  Instrumented torque runs are refused by the caller (srp_api.cu).
-#define SRP_LAUNCH3(K_, ...)                                                                              \
-    (instrumented ? launch_persistent(K_<__VA_ARGS__ true, false>, a, num_sms, stream)                       \
-                  : a.torque ? launch_persistent(K_<__VA_ARGS__ false, true>, a, num_sms, stream)            \
-                             : launch_persistent(K_<__VA_ARGS__ false, false>, a, num_sms, stream))
-
-cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms, cudaStream_t stream)
-{
-    if (brute) {
-        if (a.dz.has_bvh)       // forced brute force over a design that also has a hierarchy (test use)
-            return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_GLOBAL,);
-        if (a.sampler == 0 && a.primary_mode != 1) return SRP_LAUNCH3(small_beam_kernel);
-        return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_SMEM,);
-    }
-    if (a.sampler == 0 && a.pool != nullptr)          // beams chosen by the caller (srp_api.cu, want_beams)
-        return SRP_LAUNCH3(beam_trace_kernel);
-    return SRP_LAUNCH3(bvh_trace_kernel);
-}
-
-cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream)
-{
-    finalize_kernel<<<(unsigned)((a.n_pairs + 255) / 256), 256, 0, stream>>>(a, out_forces, out_torques);
-    return cudaGetLastError();
-}
-
-cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream)
-{
-    const long long total = a.n_pairs * a.N;
-    long long blocks = (total + TRACE_THREADS - 1) / TRACE_THREADS;
-    if (blocks > 148 * 64) blocks = 148 * 64;
-    if (method == 0 && a.dz.has_bvh)
-        first_hit_kernel<MODE_BVH><<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a, out_prim);
-    else
-        first_hit_kernel<MODE_BRUTE_GLOBAL><<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a, out_prim);
-    return cudaGetLastError();
 }
