@@ -61,7 +61,7 @@ srp_status ensure_workspace(srp_context *ctx, size_t accum_items)
     return SRP_OK;
 }
 
-// Beam tracing of the primaries (trace.cu, beam_trace_kernel) pays when many rays share a triangle: a
+// Beam tracing of the primaries (trace_beam.cu, beam_trace_kernel) pays when many rays share a triangle: a
 // beam's candidate list is then short and serves many rays.  With about one ray per triangle (the
 // 1M-triangle sail at N = 2^20) every beam overflows its lists, so primaries walk the BVH one by one.
 bool want_beams(const srp_context *ctx, bool brute, long long max_tris, long long N, long long n_pairs)
