@@ -24,27 +24,28 @@ srp_status cuda_fail(srp_context *ctx, const char *what, cudaError_t e)
 
 #define TRY_CUDA(ctx, call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, what, e_); } while (0)
 
-void free_designs_mem(srp_designs *d)
+// design arrays come from the device's stream-ordered pool (no device-wide synchronisation per build)
+void free_designs_mem(srp_context *ctx, srp_designs *d)
 {
-    cudaFree(d->verts_orig); cudaFree(d->mats_orig); cudaFree(d->tri); cudaFree(d->nodes);
-    cudaFree(d->tri_off_dev); cudaFree(d->box); cudaFree(d->perm);
+    void *ptrs[7] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm };
+    for (void *q : ptrs)
+        if (q) cudaFreeAsync(q, ctx->stream);
 }
 
 // allocates everything that depends on tri_off / sumT
 srp_status alloc_designs(srp_context *ctx, srp_designs *d)
 {
     const long long sumT = d->sumT;
-    TRY_CUDA(ctx, cudaMalloc(&d->verts_orig, sizeof(float) * 9 * sumT), "alloc verts");
-    TRY_CUDA(ctx, cudaMalloc(&d->mats_orig, sizeof(float) * 3 * sumT), "alloc mats");
-    TRY_CUDA(ctx, cudaMalloc(&d->tri, sizeof(float4) * 3 * sumT), "alloc packed triangles");
-    if (d->has_bvh) TRY_CUDA(ctx, cudaMalloc(&d->nodes, sizeof(float4) * 4 * sumT), "alloc nodes");
-    TRY_CUDA(ctx, cudaMalloc(&d->tri_off_dev, sizeof(long long) * (d->D + 1)), "alloc offsets");
-    TRY_CUDA(ctx, cudaMalloc(&d->box, sizeof(float4) * 2 * d->D), "alloc boxes");
-    TRY_CUDA(ctx, cudaMalloc(&d->perm, sizeof(int) * sumT), "alloc perm");
+    TRY_CUDA(ctx, cudaMallocAsync(&d->verts_orig, sizeof(float) * 9 * sumT, ctx->stream), "alloc verts");
+    TRY_CUDA(ctx, cudaMallocAsync(&d->mats_orig, sizeof(float) * 3 * sumT, ctx->stream), "alloc mats");
+    TRY_CUDA(ctx, cudaMallocAsync(&d->tri, sizeof(float4) * 3 * sumT, ctx->stream), "alloc packed triangles");
+    if (d->has_bvh) TRY_CUDA(ctx, cudaMallocAsync(&d->nodes, sizeof(float4) * 4 * sumT, ctx->stream), "alloc nodes");
+    TRY_CUDA(ctx, cudaMallocAsync(&d->tri_off_dev, sizeof(long long) * (d->D + 1), ctx->stream), "alloc offsets");
+    TRY_CUDA(ctx, cudaMallocAsync(&d->box, sizeof(float4) * 2 * d->D, ctx->stream), "alloc boxes");
+    TRY_CUDA(ctx, cudaMallocAsync(&d->perm, sizeof(int) * sumT, ctx->stream), "alloc perm");
     TRY_CUDA(ctx, cudaMemcpyAsync(d->tri_off_dev, d->tri_off.data(), sizeof(long long) * (d->D + 1),
                                   cudaMemcpyHostToDevice, ctx->stream), "copy offsets");
-    // the pageable host vector must outlive the async copy
-    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync offsets");
+    // d->tri_off (the pageable source) lives as long as the handle
     return SRP_OK;
 }
 
@@ -177,6 +178,13 @@ srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
     ctx->opt.force_brute = 0; ctx->opt.instrumented = 0; ctx->opt.primary_mode = 0;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
+    {   // keep freed blocks in the stream-ordered pool: builds reuse them instead of going back to the driver
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, cuda_device) == cudaSuccess) {
+            unsigned long long keep = ~0ULL;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
     *out = ctx;
     return SRP_OK;
 }
@@ -188,6 +196,8 @@ srp_status srp_destroy(srp_context *ctx)
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->pool);
     cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);
+    cudaMemPool_t pool;                                       // hand the pooled design memory back
+    if (cudaDeviceGetDefaultMemPool(&pool, ctx->device) == cudaSuccess) cudaMemPoolTrimTo(pool, 0);
     delete ctx;
     return SRP_OK;
 }
@@ -242,11 +252,11 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
     for (int k = 0; k <= D; ++k) d->tri_off[k] = (long long)k * T;
     d->has_bvh = T > SRP_BRUTE_MAX_TRIS;
     srp_status st = alloc_designs(ctx, d);
-    if (st != SRP_OK) { free_designs_mem(d); delete d; return st; }
+    if (st != SRP_OK) { free_designs_mem(ctx, d); delete d; return st; }
     cudaError_t e = srp_launch_mesh_gen((int)family, theta, D, n_params, mesh_seed, T, d->verts_orig,
                                         d->mats_orig, ctx->stream);
     if (e == cudaSuccess) e = srp_launch_build(d, ctx->stream);
-    if (e != cudaSuccess) { free_designs_mem(d); delete d; return cuda_fail(ctx, "design build", e); }
+    if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     *out = d;
     return SRP_OK;
 }
@@ -275,12 +285,12 @@ srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, c
     d->tri_off.assign(tri_offsets, tri_offsets + D + 1);
     d->has_bvh = maxT > SRP_BRUTE_MAX_TRIS;
     srp_status st = alloc_designs(ctx, d);
-    if (st != SRP_OK) { free_designs_mem(d); delete d; return st; }
+    if (st != SRP_OK) { free_designs_mem(ctx, d); delete d; return st; }
     cudaError_t e = cudaMemcpyAsync(d->verts_orig, verts, sizeof(float) * 9 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(d->mats_orig, mats, sizeof(float) * 3 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e == cudaSuccess) e = srp_launch_build(d, ctx->stream);
-    if (e != cudaSuccess) { free_designs_mem(d); delete d; return cuda_fail(ctx, "design build", e); }
+    if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     *out = d;
     return SRP_OK;
 }
@@ -328,7 +338,7 @@ srp_status srp_free_designs(srp_context *ctx, srp_designs *dz)
     if (!dz) return SRP_OK;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    free_designs_mem(dz);
+    free_designs_mem(ctx, dz);
     delete dz;
     return SRP_OK;
 }
