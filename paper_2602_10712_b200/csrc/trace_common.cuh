@@ -210,9 +210,6 @@ __device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, i
         SRP_CHECK(sp < NSMEM + STACK_OVF, "traversal stack");
         if (sp < NSMEM) s_stack[sp * STRIDE] = l1; else ovf[sp - NSMEM] = l1;
         ++sp;
-#ifdef SRP_PREFETCH_PUSH
-        if (l1 >= 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(nodes + 4 * l1));
-#endif
         return l0;
     }
     if (h0) return l0;

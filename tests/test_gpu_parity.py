@@ -368,6 +368,14 @@ def test_edge_cases(ctx, oracle):
         ctx.srp_build_designs(W.FAMILY_BOXWING, th)                      # wrong n_params
     with pytest.raises(SrpError):
         ctx.srp_build_designs(7, th)
+    with pytest.raises(SrpError):
+        ctx.srp_set_options(primary_mode=3)
+    ctx.srp_set_options(instrumented=1)
+    try:
+        with pytest.raises(SrpError):                                    # torques come from the plain kernels only
+            ctx.srp_forces_torques(dz, om, 1 << 10, 1, 0)
+    finally:
+        ctx.srp_set_options()
     ctx.srp_set_options(sampler=1)
     try:
         Fi = ctx.srp_forces(dz, om, 1000, 1, 0).cpu().numpy()[0]         # ragged N in i.i.d. mode
