@@ -116,6 +116,41 @@ def test_lbvh_mixed_sizes_and_duplicates(ctx):
     dz.free()
 
 
+@pytest.mark.parametrize("primary_mode", [1, 2])
+def test_forces_on_mixed_batch_match_oracle(ctx, oracle, primary_mode):
+    """One batch with a hierarchy holding designs of 1, 3, 70 (identical copies) and 500 random triangles: forces of
+    every design against the oracle, per-ray and as beams (one-triangle root, empty child slot, equal Morton keys)."""
+    rng = np.random.default_rng(0)
+    one = quad([0, 0, 0], [1, 0, 0], [0, 1, 0])[:1]
+    three = rng.normal(size=(3, 3, 3)).astype(np.float32)
+    dup = np.repeat(one, 70, axis=0)
+    big = (rng.normal(size=(500, 1, 3)) + 0.1 * rng.normal(size=(500, 3, 3))).astype(np.float32)
+    verts = np.concatenate([one, three, dup, big])
+    mats = W.dirichlet_materials(len(verts), 1)
+    off = np.cumsum([0, 1, 3, 70, 500])
+    dz = ctx.srp_build_designs_from_meshes(verts, mats, off)
+    sun = W.fibonacci_sphere(6)
+    N, B = 1 << 12, 3
+    ctx.srp_set_options(primary_mode=primary_mode)
+    try:
+        F = ctx.srp_forces(dz, cuda(sun), N, B, 4).cpu().numpy()
+        st = ctx.srp_get_stats()
+    finally:
+        ctx.srp_set_options()
+    assert st["launched"] == st["primary_miss"] + st["absorbed"] + st["escaped"] + st["capped"]
+    for k in range(4):
+        if k == 2:
+            continue          # 70 coincident triangles: every hit is a 70-way tie in t, the winner is not unique (R11)
+        r = oracle.forces(verts[off[k]:off[k + 1]], mats[off[k]:off[k + 1]], sun, N, B, seed=4, k=k)
+        assert_parity(F[k], r["F"], r["sigma"], tol_agg=5e-3)
+    # the coincident copies: whichever copy wins, the hit geometry is the plate's; materials differ per copy, so only
+    # the direction-independent bound |F| <= 2 P A cos(theta) is checked
+    for j in range(len(sun)):
+        cos = abs(sun[j][2]) / np.linalg.norm(sun[j])
+        assert np.linalg.norm(F[2, j]) <= 2.0 * P0 * 0.5 * cos * (1 + 1e-3) + 1e-12
+    dz.free()
+
+
 # ---------------------------------------------------------------- S3/S4: rays and closest hit
 @pytest.mark.parametrize("family,N", [(W.FAMILY_BOXWING, 1 << 12), (W.FAMILY_DETAILED, 1 << 12),
                                       (W.FAMILY_SAIL, 1 << 10)])
