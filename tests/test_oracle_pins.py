@@ -247,3 +247,23 @@ def test_invalid_arguments(oracle):
     oracle.forces(verts, mats, om, 1000, 1, sampler=1)
     with pytest.raises(ValueError):
         oracle.forces(verts, mats, om, 1024, 16)
+
+
+def test_p12_self_shadowing_direct_light_by_surface_integration(oracle):
+    """B = 0 on box-wings (bus and panels shadow each other) against an independent SURFACE quadrature with shadow
+    rays (helpers.direct_force_by_surface_quadrature): same integral, other measure and other visibility query."""
+    from helpers import direct_force_by_surface_quadrature
+    th = W.draw_params(W.FAMILY_BOXWING, 3)
+    sun = np.array([[0.2, 0.9, 0.3], [-0.6, 0.5, 0.6], [0.1, -0.95, -0.2], [0.7, 0.1, -0.7]], np.float32)
+    matters = 0
+    for k in range(3):
+        verts, mats = oracle.build_mesh(W.FAMILY_BOXWING, th[k], k=k)
+        r = oracle.forces(verts, mats, sun, 1 << 18, 0, seed=1, k=k)
+        for j in range(len(sun)):
+            Fq = direct_force_by_surface_quadrature(verts, mats, sun[j])
+            assert np.linalg.norm(r["F"][j] - Fq) <= 4.0 * r["sigma"][j] + 6e-3 * np.linalg.norm(Fq), (k, j)
+            F_lit = direct_force_by_surface_quadrature(verts, mats, sun[j], shadows=False)
+            if np.linalg.norm(F_lit - Fq) > 0.05 * np.linalg.norm(Fq):
+                matters += 1
+                assert np.linalg.norm(r["F"][j] - F_lit) > 4.0 * r["sigma"][j] + 6e-3 * np.linalg.norm(Fq)
+    assert matters >= 3          # along the panel axis the bus and the panels do shadow each other
