@@ -75,6 +75,10 @@ def lib():
             ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats), ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_forces_torques.restype = ctypes.c_int
         L.srp_oracle_forces_torques.argtypes = L.srp_oracle_forces.argtypes + [ctypes.c_void_p] * 3
+        L.srp_oracle_thermal.restype = ctypes.c_int
+        L.srp_oracle_thermal.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p,
+                                         ctypes.c_longlong, ctypes.c_int, ctypes.c_ulonglong, ctypes.POINTER(Options),
+                                         ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats)]
         L.srp_oracle_philox.restype = None
         L.srp_oracle_philox.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_uniform.restype = ctypes.c_double
@@ -158,3 +162,24 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
         out["T"] = Tq
         out["sigma_T"] = np.sqrt(np.maximum(TQ - Tq * Tq / float(N), 0.0).sum(axis=1))
     return out
+
+
+def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0):
+    """Recoil force of ONE design's thermal (Lambertian) facet emitters: facet_power float32[T]
+    in watts, signed (sign = emitting side), N photons per emitting facet.  Returns dict(F f64[3] newtons,
+    sigma f64 (i.i.d. standard error of |F| over all emitted photons), stats)."""
+    verts = np.ascontiguousarray(verts, dtype=np.float32).reshape(-1, 3, 3)
+    mats = np.ascontiguousarray(mats, dtype=np.float32).reshape(-1, 3)
+    pw = np.ascontiguousarray(facet_power, dtype=np.float32).reshape(-1)
+    T = verts.shape[0]
+    assert mats.shape[0] == T and pw.shape[0] == T
+    F = np.zeros(3); Q = np.zeros(3)
+    st = Stats()
+    opt = Options(float(SOLAR_PRESSURE), 0, int(deposit))
+    rc = lib().srp_oracle_thermal(verts.ctypes.data, mats.ctypes.data, T, int(k), pw.ctypes.data, int(N), int(B),
+                                  int(seed), ctypes.byref(opt), F.ctypes.data, Q.ctypes.data, ctypes.byref(st))
+    if rc != 0:
+        raise ValueError("srp_oracle_thermal: invalid arguments")
+    n = max(int(st.launched), 1)
+    sigma = float(np.sqrt(np.maximum(Q - F * F / n, 0.0).sum()))
+    return {"F": F, "sigma": sigma, "stats": st.as_dict()}

@@ -76,6 +76,79 @@ static void orc_deposit(const double dd[3], orc_v3 x, orc_v3 xc, double dp[3], d
     dq[2] += r.x * dd[1] - r.y * dd[0];
 }
 
+typedef struct { const double *v0, *e1, *e2, *nrm; long T; } orc_geom;
+
+/* O-steps 4-7 for ONE photon that starts at o along d (src = the triangle it leaves, -1 for none) with momentum
+ * weight wph: closest hit, deposit (force total dp, torque total dq about xc), lobe selection, continuation,
+ * until it is absorbed, escapes or has been reflected B times.  The lobe draw of the hit at `depth` uses the
+ * Philox counter (i, j, k, (depth + 1) | cflag). */
+static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 d, long src, double wph,
+                         uint32_t i, uint32_t j, uint32_t k, uint32_t cflag, const uint32_t key[2],
+                         const orc_options *opt, int B, orc_v3 xc, orc_stats *st, double dp[3], double dq[3],
+                         int *first_hit, unsigned long long *sig)
+{
+    int depth = 0;
+    for (;;) {
+        /* O-step 4 */
+        double t;
+        st->segments++;
+        long f = closest_hit(G->v0, G->e1, G->e2, G->T, o, d, src, &t);
+        if (depth == 0 && first_hit) *first_hit = (int)f;
+        if (f < 0) {
+            if (depth == 0) st->primary_miss++; else st->escaped++;
+            break;
+        }
+        st->hits_at_depth[depth]++;
+        *sig = *sig * 1000003ULL + (unsigned long long)(f + 1);
+        /* O-step 5: facing normal, mirror direction, deposit. */
+        orc_v3 n = orc_mk(G->nrm[3 * f], G->nrm[3 * f + 1], G->nrm[3 * f + 2]);
+        orc_v3 nf = (orc_dot(n, d) > 0.0) ? orc_scale(n, -1.0) : n;
+        double cost = -orc_dot(d, nf);
+        orc_v3 refl = orc_add(d, orc_scale(nf, 2.0 * cost));
+        orc_v3 x = orc_add(o, orc_scale(d, t));
+        const double al = mats[3 * f], rs = mats[3 * f + 1], rd = mats[3 * f + 2];
+        /* dd = this hit's momentum deposit, made at x; Eq. 4: torque += (x - x_COM) x dd */
+        double dd[3] = { 0, 0, 0 };
+        if (opt->deposit == 0) {
+            double a = al + rs + rd;
+            dd[0] = wph * (a * d.x - rs * refl.x - (2.0 / 3.0) * rd * nf.x);
+            dd[1] = wph * (a * d.y - rs * refl.y - (2.0 / 3.0) * rd * nf.y);
+            dd[2] = wph * (a * d.z - rs * refl.z - (2.0 / 3.0) * rd * nf.z);
+        }
+        /* O-step 6: lobe selection (thresholds in fp32, R17). */
+        uint32_t c2[4] = { i, j, k, (uint32_t)(depth + 1) | cflag }, y[4];
+        orc_philox4x32_10(c2, key, y);
+        const double z0 = orc_uniform(y[0]), z1 = orc_uniform(y[1]), z2 = orc_uniform(y[2]);
+        const float th1 = mats[3 * f];
+        const float th2 = mats[3 * f] + mats[3 * f + 1];
+        orc_v3 dnew;
+        if (z0 < (double)th1) {
+            if (opt->deposit == 1) { dd[0] = wph * d.x; dd[1] = wph * d.y; dd[2] = wph * d.z; }
+            orc_deposit(dd, x, xc, dp, dq);
+            st->absorbed++;
+            break;
+        } else if (z0 < (double)th2) {
+            dnew = refl;
+        } else {
+            double phi = 6.283185307179586476925286766559 * z1, rho = sqrt(z2);
+            double lx = rho * cos(phi), ly = rho * sin(phi), lz = sqrt(1.0 - z2);
+            /* tangent frame (R18): first edge of the facet and nf x edge -- defined by the
+             * mesh itself, so it has no discontinuity that rounding noise in nf could trip
+             * (the step-1 rule flips across nf.z = 0, where axis-aligned facets sit) */
+            orc_v3 tu = orc_normalize(orc_mk(G->e1[3 * f], G->e1[3 * f + 1], G->e1[3 * f + 2]));
+            orc_v3 tv = orc_cross(nf, tu);
+            dnew = orc_add(orc_add(orc_scale(tu, lx), orc_scale(tv, ly)), orc_scale(nf, lz));
+        }
+        if (opt->deposit == 1) {
+            dd[0] = wph * (d.x - dnew.x); dd[1] = wph * (d.y - dnew.y); dd[2] = wph * (d.z - dnew.z);
+        }
+        orc_deposit(dd, x, xc, dp, dq);
+        /* O-step 7: depth cap. */
+        if (depth == B) { st->capped++; break; }
+        o = x; d = dnew; src = f; depth += 1;
+    }
+}
+
 static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
 {
     uint32_t x = 0, y = 0;
@@ -138,6 +211,7 @@ int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int
         nrm[3 * f] = n.x / len; nrm[3 * f + 1] = n.y / len; nrm[3 * f + 2] = n.z / len;
     }
     orc_stats st; memset(&st, 0, sizeof st);
+    const orc_geom G = { v0, e1, e2, nrm, T };
 
     for (int jj = 0; jj < S; ++jj) {
         const uint32_t j = (uint32_t)(j0 + jj);
@@ -175,70 +249,11 @@ int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int
             }
             orc_v3 o = orc_add(orc_add(orc_scale(bu, pu), orc_scale(bv, pv)), orc_scale(s, w0 - 1.0));
             orc_v3 d = s;
-            long src = -1;
-            int depth = 0;
             double dp[3] = { 0, 0, 0 }, dq[3] = { 0, 0, 0 };
             unsigned long long sig = 0;
             st.launched++;
-            for (;;) {
-                /* O-step 4 */
-                double t;
-                st.segments++;
-                long f = closest_hit(v0, e1, e2, T, o, d, src, &t);
-                if (depth == 0 && first_hit) first_hit[(long long)jj * N + i] = (int)f;
-                if (f < 0) {
-                    if (depth == 0) st.primary_miss++; else st.escaped++;
-                    break;
-                }
-                st.hits_at_depth[depth]++;
-                sig = sig * 1000003ULL + (unsigned long long)(f + 1);
-                /* O-step 5: facing normal, mirror direction, deposit. */
-                orc_v3 n = orc_mk(nrm[3 * f], nrm[3 * f + 1], nrm[3 * f + 2]);
-                orc_v3 nf = (orc_dot(n, d) > 0.0) ? orc_scale(n, -1.0) : n;
-                double cost = -orc_dot(d, nf);
-                orc_v3 refl = orc_add(d, orc_scale(nf, 2.0 * cost));
-                orc_v3 x = orc_add(o, orc_scale(d, t));
-                const double al = mats[3 * f], rs = mats[3 * f + 1], rd = mats[3 * f + 2];
-                /* dd = this hit's momentum deposit, made at x; Eq. 4: torque += (x - x_COM) x dd */
-                double dd[3] = { 0, 0, 0 };
-                if (opt->deposit == 0) {
-                    double a = al + rs + rd;
-                    dd[0] = wph * (a * d.x - rs * refl.x - (2.0 / 3.0) * rd * nf.x);
-                    dd[1] = wph * (a * d.y - rs * refl.y - (2.0 / 3.0) * rd * nf.y);
-                    dd[2] = wph * (a * d.z - rs * refl.z - (2.0 / 3.0) * rd * nf.z);
-                }
-                /* O-step 6: lobe selection (thresholds in fp32, R17). */
-                uint32_t c2[4] = { (uint32_t)i, j, (uint32_t)k, (uint32_t)(depth + 1) }, y[4];
-                orc_philox4x32_10(c2, key, y);
-                const double z0 = orc_uniform(y[0]), z1 = orc_uniform(y[1]), z2 = orc_uniform(y[2]);
-                const float th1 = mats[3 * f];
-                const float th2 = mats[3 * f] + mats[3 * f + 1];
-                orc_v3 dnew;
-                if (z0 < (double)th1) {
-                    if (opt->deposit == 1) { dd[0] = wph * d.x; dd[1] = wph * d.y; dd[2] = wph * d.z; }
-                    orc_deposit(dd, x, xc, dp, dq);
-                    st.absorbed++;
-                    break;
-                } else if (z0 < (double)th2) {
-                    dnew = refl;
-                } else {
-                    double phi = 6.283185307179586476925286766559 * z1, rho = sqrt(z2);
-                    double lx = rho * cos(phi), ly = rho * sin(phi), lz = sqrt(1.0 - z2);
-                    /* tangent frame (R18): first edge of the facet and nf x edge -- defined by the
-                     * mesh itself, so it has no discontinuity that rounding noise in nf could trip
-                     * (the step-1 rule flips across nf.z = 0, where axis-aligned facets sit) */
-                    orc_v3 tu = orc_normalize(orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]));
-                    orc_v3 tv = orc_cross(nf, tu);
-                    dnew = orc_add(orc_add(orc_scale(tu, lx), orc_scale(tv, ly)), orc_scale(nf, lz));
-                }
-                if (opt->deposit == 1) {
-                    dd[0] = wph * (d.x - dnew.x); dd[1] = wph * (d.y - dnew.y); dd[2] = wph * (d.z - dnew.z);
-                }
-                orc_deposit(dd, x, xc, dp, dq);
-                /* O-step 7: depth cap. */
-                if (depth == B) { st.capped++; break; }
-                o = x; d = dnew; src = f; depth += 1;
-            }
+            trace_photon(&G, mats, o, d, -1, wph, (uint32_t)i, j, (uint32_t)k, 0u, key, opt, B, xc, &st, dp, dq,
+                         first_hit ? &first_hit[(long long)jj * N + i] : NULL, &sig);
             for (int c = 0; c < 3; ++c) {
                 Fj[c] += dp[c]; Qj[c] += dp[c] * dp[c];
                 Tj[c] += dq[c]; TQj[c] += dq[c] * dq[c];
@@ -270,6 +285,77 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
 {
     return srp_oracle_forces_torques(verts, mats, T, k, sun_dirs, S, j0, N, B, seed, opt, F, sumsq, stats,
                                      first_hit, path_sig, NULL, NULL, NULL);
+}
+
+/*
+ * Thermal (local Lambertian) emitters, PAPER.md:606-612 (Sec. 5.9): "our simulation easily handles local sources
+ * in the same way it does handle distant sun light ... we model thermal emission as Lambertian"; a Lambertian
+ * emitter's momentum flux is 2/3 of a collimated beam's.  DESIGN.md reading R22.
+ * Facet f of design k radiates |W_f| watts from the side of its normal n = normalize(e1 x e2) (W_f > 0) or of -n
+ * (W_f < 0).  It launches N photons of momentum weight w = |W_f| / (c N) [newtons]: ray i draws
+ * Philox(key = seed; ctr = (i, f, k, 0x80000000)) -> xi0..xi3; origin = uniform point of the triangle
+ * x = v0 + sqrt(xi0) (1 - xi1) e1 + sqrt(xi0) xi1 e2; direction cosine-weighted about the emitting normal n_e in the
+ * frame (t_u = e1/|e1|, t_v = n_e x t_u): phi = 2 pi xi2, rho = sqrt(xi3).  Recoil at emission: expected-value
+ * deposit -(2/3) w n_e, analog deposit -w d, made at x.  The photon is then followed like any other (O-steps 4-7,
+ * source triangle f excluded, lobe draws with counters (i, f, k, 0x80000000 | depth + 1)).
+ * F double[3] (N), sumsq double[3] (per-photon totals squared, may be NULL), stats may be NULL.
+ */
+int srp_oracle_thermal(const float *verts, const float *mats, long T, int k, const float *facet_power,
+                       long long N, int B, unsigned long long seed, const orc_options *opt,
+                       double *F, double *sumsq, orc_stats *stats)
+{
+    if (!verts || !mats || !facet_power || !F || !opt || T <= 0 || N <= 0 || B < 0 || B > 15) return -1;
+    const double C_LIGHT = 299792458.0;
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    double *v0 = malloc(sizeof(double) * 3 * T), *e1 = malloc(sizeof(double) * 3 * T),
+           *e2 = malloc(sizeof(double) * 3 * T), *nrm = malloc(sizeof(double) * 3 * T);
+    for (long f = 0; f < T; ++f) {
+        for (int c = 0; c < 3; ++c) {
+            double a = verts[9 * f + c], b = verts[9 * f + 3 + c], cc = verts[9 * f + 6 + c];
+            v0[3 * f + c] = a; e1[3 * f + c] = b - a; e2[3 * f + c] = cc - a;
+        }
+        orc_v3 n = orc_cross(orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]),
+                             orc_mk(e2[3 * f], e2[3 * f + 1], e2[3 * f + 2]));
+        double len = sqrt(orc_dot(n, n));
+        nrm[3 * f] = n.x / len; nrm[3 * f + 1] = n.y / len; nrm[3 * f + 2] = n.z / len;
+    }
+    const orc_geom G = { v0, e1, e2, nrm, T };
+    orc_stats st; memset(&st, 0, sizeof st);
+    double Ft[3] = { 0, 0, 0 }, Qt[3] = { 0, 0, 0 };
+    const orc_v3 xc = orc_mk(0.0, 0.0, 0.0);
+    for (long f = 0; f < T; ++f) {
+        const double W = facet_power[f];
+        if (W == 0.0) continue;
+        const double w = fabs(W) / (C_LIGHT * (double)N);
+        const orc_v3 E1 = orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]), E2 = orc_mk(e2[3 * f], e2[3 * f + 1], e2[3 * f + 2]);
+        const orc_v3 n = orc_mk(nrm[3 * f], nrm[3 * f + 1], nrm[3 * f + 2]);
+        const orc_v3 ne = W > 0.0 ? n : orc_scale(n, -1.0);
+        const orc_v3 tu = orc_normalize(E1), tv = orc_cross(ne, tu);
+        for (long long i = 0; i < N; ++i) {
+            uint32_t ctr[4] = { (uint32_t)i, (uint32_t)f, (uint32_t)k, 0x80000000u }, r[4];
+            orc_philox4x32_10(ctr, key, r);
+            const double x0 = orc_uniform(r[0]), x1 = orc_uniform(r[1]), x2 = orc_uniform(r[2]), x3 = orc_uniform(r[3]);
+            const double su = sqrt(x0);
+            const orc_v3 x = orc_add(orc_mk(v0[3 * f], v0[3 * f + 1], v0[3 * f + 2]),
+                                     orc_add(orc_scale(E1, su * (1.0 - x1)), orc_scale(E2, su * x1)));
+            const double phi = 6.283185307179586476925286766559 * x2, rho = sqrt(x3);
+            const double lx = rho * cos(phi), ly = rho * sin(phi), lz = sqrt(1.0 - x3);
+            const orc_v3 d = orc_add(orc_add(orc_scale(tu, lx), orc_scale(tv, ly)), orc_scale(ne, lz));
+            double dp[3] = { 0, 0, 0 }, dq[3] = { 0, 0, 0 }, dd[3];
+            if (opt->deposit == 0) { dd[0] = -(2.0 / 3.0) * w * ne.x; dd[1] = -(2.0 / 3.0) * w * ne.y; dd[2] = -(2.0 / 3.0) * w * ne.z; }
+            else { dd[0] = -w * d.x; dd[1] = -w * d.y; dd[2] = -w * d.z; }
+            orc_deposit(dd, x, xc, dp, dq);
+            unsigned long long sig = 0;
+            st.launched++;
+            trace_photon(&G, mats, x, d, f, w, (uint32_t)i, (uint32_t)f, (uint32_t)k, 0x80000000u, key, opt, B, xc, &st,
+                         dp, dq, NULL, &sig);
+            for (int c = 0; c < 3; ++c) { Ft[c] += dp[c]; Qt[c] += dp[c] * dp[c]; }
+        }
+    }
+    for (int c = 0; c < 3; ++c) { F[c] = Ft[c]; if (sumsq) sumsq[c] = Qt[c]; }
+    if (stats) *stats = st;
+    free(v0); free(e1); free(e2); free(nrm);
+    return 0;
 }
 
 /* Philox and the uniform map exposed for the known-answer tests. */
