@@ -156,6 +156,19 @@ srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *designs
                                     unsigned long long seed, const float *x_com, float *out_forces,
                                     float *out_torques);
 
+/* Thermal (local Lambertian) emitters, PAPER.md:606-612 (Sec. 5.9: "local sources [are handled] in the same way
+ * ... thermal emission as Lambertian", recoil 2/3 of a collimated beam); R22.
+ * facet_power DEVICE float[sumT] in watts, ORIGINAL triangle order of all designs back to back (tri_offsets of
+ * srp_designs_info); sign = emitting side (+: the side of normalize((v1-v0) x (v2-v0)), -: the other side); zero =
+ * no emission.  Every emitting facet launches rays_per_facet photons (uniform origin on the triangle,
+ * cosine-weighted direction, Philox counter (ray, facet, design, 0x80000000 | depth)) which are followed for up to
+ * max_bounces reflections like sun photons.  out_forces DEVICE float[D,3]: net recoil force per design in newtons
+ * (emission recoil plus what the emitted photons deposit on the design itself).  srp_options.deposit applies;
+ * srp_get_stats counts the emitted photons.  Enqueues only. */
+srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *designs, const float *facet_power,
+                              long long rays_per_facet, int max_bounces, unsigned long long seed,
+                              float *out_forces);
+
 /* Host-buffer convenience (the end-to-end call): theta-independent; sun_dirs_host HOST float[S,3],
  * out_forces_host HOST float[D,S,3].  Copies in, runs srp_forces, copies out, syncs. */
 srp_status srp_forces_host(srp_context *ctx, const srp_designs *designs, const float *sun_dirs_host,

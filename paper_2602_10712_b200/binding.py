@@ -51,7 +51,7 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_family_n_params", "srp_family_tri_count", "srp_build_designs",
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
-           "srp_forces_torques", "srp_forces_torques_pairs",
+           "srp_forces_torques", "srp_forces_torques_pairs", "srp_thermal_forces",
            "srp_first_hits", "srp_path_signatures", "srp_get_stats", "srp_probe_peaks"]
 
 _lib = None
@@ -87,6 +87,7 @@ def load_library():
     L.srp_forces_host.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
     L.srp_forces_torques.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp, vp]
     L.srp_forces_torques_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp, vp]
+    L.srp_thermal_forces.argtypes = [vp, vp, vp, ll, ci, ull, vp]
     L.srp_first_hits.argtypes = [vp, vp, vp, ci, vp, ll, ll, ull, ci, vp]
     L.srp_path_signatures.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_get_stats.argtypes = [vp, ctypes.POINTER(srp_stats)]
@@ -248,6 +249,18 @@ class Context:
                                                       T.data_ptr()))
         self.stream.synchronize()
         return F, T
+
+    def srp_thermal_forces(self, designs, facet_power, rays_per_facet, max_bounces, seed=0):
+        """facet_power: float32 [sumT] watts in original triangle order (signed: emitting side); returns CUDA
+        float32 [D,3] recoil forces in newtons."""
+        pw = torch.as_tensor(facet_power).to(device=self.device, dtype=torch.float32).contiguous()
+        if pw.numel() != int(designs.tri_offsets[-1]):
+            raise ValueError("facet_power must have one entry per triangle of the batch")
+        out = torch.empty((designs.D, 3), dtype=torch.float32, device=self.device)
+        self._check(self.lib.srp_thermal_forces(self.handle, designs.handle, pw.data_ptr(), rays_per_facet, max_bounces,
+                                                seed, out.data_ptr()))
+        self.stream.synchronize()
+        return out
 
     def force_maps(self, designs, n_lat, n_lon, rays_per_dir, max_bounces, seed=0):
         """The paper's force-map figures (Fig. 5): forces over a latitude-longitude image of sun

@@ -30,6 +30,7 @@ SOURCES = {
     "trace_perray.cu": [],
     "trace_beam.cu": [],
     "trace_small.cu": [],
+    "trace_thermal.cu": [],
 }
 
 

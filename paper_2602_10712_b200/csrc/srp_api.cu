@@ -375,6 +375,40 @@ srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *dz, con
     return run_forces(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed, out_forces, x_com, out_torques);
 }
 
+srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *dz, const float *facet_power, long long N, int B,
+                              unsigned long long seed, float *out_forces)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!dz || !facet_power || !out_forces) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    if (N <= 0 || N > (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "rays_per_facet must be in [1, 2^31]");
+    if (B < 0 || B > 15) return fail(ctx, SRP_ERR_INVALID, "max_bounces must be in [0, 15]");
+    if (dz->sumT >= (1LL << 31)) return fail(ctx, SRP_ERR_UNSUPPORTED, "too many triangles for the emitter list");
+    cudaSetDevice(ctx->device);
+    srp_status st = ensure_workspace(ctx, (size_t)dz->D * 3);
+    if (st != SRP_OK) return st;
+    TraceArgs a;
+    memset(&a, 0, sizeof a);
+    a.dz = dz->dev();
+    a.n_pairs = dz->D; a.S = 1; a.N = N; a.B = B;
+    a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
+    a.sampler = 0; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
+    a.accum = ctx->accum; a.acc_stride = 3; a.stats = ctx->stats; a.work_counter = ctx->work_counter;
+    a.tile_rays = (int)(N < 8192 ? N : 8192);
+    a.tiles_per_pair = (N + a.tile_rays - 1) / a.tile_rays;
+    int *emit_list = nullptr, *n_emit = nullptr;
+    float *design_power = nullptr;
+    TRY_CUDA(ctx, cudaMallocAsync(&emit_list, sizeof(int) * dz->sumT, ctx->stream), "alloc emitter list");
+    TRY_CUDA(ctx, cudaMallocAsync(&n_emit, sizeof(int), ctx->stream), "alloc emitter count");
+    TRY_CUDA(ctx, cudaMallocAsync(&design_power, sizeof(float) * dz->D, ctx->stream), "alloc design power");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * dz->D, ctx->stream), "zero accumulators");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
+    TRY_CUDA(ctx, srp_launch_thermal(a, facet_power, dz->sumT, emit_list, n_emit, design_power, out_forces, ctx->num_sms,
+                                     ctx->stream), "thermal launch");
+    cudaFreeAsync(emit_list, ctx->stream); cudaFreeAsync(n_emit, ctx->stream); cudaFreeAsync(design_power, ctx->stream);
+    return SRP_OK;
+}
+
 srp_status srp_forces_pairs(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
                             long long n_pairs, long long N, int B, unsigned long long seed, float *out)
 {

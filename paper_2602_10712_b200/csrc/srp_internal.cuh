@@ -109,6 +109,8 @@ cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, 
                              cudaStream_t stream);
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream);
 cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream);
+cudaError_t srp_launch_thermal(const TraceArgs &a, const float *facet_power, long long sumT, int *emit_list, int *n_emit,
+                               float *design_power, float *out_forces, int num_sms, cudaStream_t stream);
 cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
 
 long long srp_family_tris_host(int family);

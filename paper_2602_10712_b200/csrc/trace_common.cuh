@@ -272,7 +272,9 @@ struct BeamCounters {       // rays resolved per beam level (lane-distributed co
 // O-steps 5-7 at a hit: deposit, lobe selection, continuation.
 // Returns SHADE_CONTINUE if the photon goes on (o, d, src, depth updated), else how it ended.
 enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2 };
-template <bool TORQUE>
+// CFLAG is OR-ed into the Philox counter word that holds the depth: 0 for sun photons, 0x80000000 for photons of
+// thermal emitters (R22), so the two families draw from disjoint streams.
+template <bool TORQUE, uint32_t CFLAG = 0u>
 __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
                                       const int deposit, float3 &o, float3 &d, int &src, int &depth,
@@ -301,7 +303,7 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
         put(f3(a * d.x - rs * refl.x - c * nf.x, a * d.y - rs * refl.y - c * nf.y, a * d.z - rs * refl.z - c * nf.z));
     }
     uint32_t y0, y1, y2, y3;
-    philox4(i, g.j, g.k, (uint32_t)(depth + 1), g.key0, g.key1, y0, y1, y2, y3);
+    philox4(i, g.j, g.k, (uint32_t)(depth + 1) | CFLAG, g.key0, g.key1, y0, y1, y2, y3);
     const float z0 = uniform23(y0);
     float3 dn;
     if (z0 < al) {                                                // absorbed

@@ -591,6 +591,73 @@ def test_torque_closed_forms_on_gpu(ctx):
     dz.free()
 
 
+# ---------------------------------------------------------------- thermal emitters (R22)
+@pytest.mark.parametrize("family,D,N,B,deposit", [(W.FAMILY_BOXWING, 3, 1 << 12, 4, 0), (W.FAMILY_BOXWING6, 2, 1 << 12, 4, 1),
+                                                  (W.FAMILY_DETAILED, 1, 1 << 9, 8, 0)])
+def test_thermal_forces_match_oracle(ctx, oracle, family, D, N, B, deposit):
+    """srp_thermal_forces against the oracle's emitters on the same Philox streams: a few facets per design radiate
+    (both signs), brute-force and BVH designs, expected-value and analog deposits; counters agree."""
+    th = W.draw_params(family, D)
+    T = W.TRI_COUNT[family]
+    rng = np.random.default_rng(3)
+    power = np.zeros((D, T), np.float32)
+    for k in range(D):
+        idx = rng.choice(T, size=min(6, T), replace=False)
+        power[k, idx] = rng.uniform(100.0, 700.0, len(idx)) * rng.choice([-1.0, 1.0], len(idx))
+    dz = ctx.srp_build_designs(family, th)
+    ctx.srp_set_options(deposit=deposit)
+    try:
+        F = ctx.srp_thermal_forces(dz, power.reshape(-1), N, B, seed=6).cpu().numpy()
+        st = ctx.srp_get_stats()
+    finally:
+        ctx.srp_set_options()
+    tot = None
+    for k in range(D):
+        v, m = oracle.build_mesh(family, th[k], k=k)
+        r = oracle.thermal(v, m, power[k], N, B, seed=6, k=k, deposit=deposit)
+        err = np.linalg.norm(F[k] - r["F"])
+        assert err <= 1e-4 * np.linalg.norm(r["F"]) or err <= 4 * r["sigma"], (k, err, r["sigma"])
+        assert err <= 3e-3 * np.linalg.norm(r["F"])
+        tot = r["stats"] if tot is None else {a: ([x + y for x, y in zip(tot[a], b)] if isinstance(b, list) else tot[a] + b)
+                                               for a, b in r["stats"].items()}
+    assert st["launched"] == tot["launched"] == N * int((power != 0).sum())
+    for key in ("primary_miss", "absorbed", "escaped", "capped", "segments"):
+        assert abs(st[key] - tot[key]) <= 8, (key, st[key], tot[key])
+    assert st["launched"] == st["primary_miss"] + st["absorbed"] + st["escaped"] + st["capped"]
+    dz.free()
+
+
+def test_thermal_closed_forms_on_gpu(ctx):
+    """Isolated emitter: F = -(2/3) (W/c) n; emitter in a closed black cavity: no net force."""
+    c = 299792458.0
+    verts = quad([0, 0, 0], [1, 0, 0], [0, 0.5, 0.5])
+    n = unit(np.cross([1, 0, 0], [0, 0.5, 0.5]))
+    dz = ctx.srp_build_designs_from_meshes(verts, const_mats(2, 0.2, 0.5, 0.3), [0, 2])
+    F = ctx.srp_thermal_forces(dz, [35000.0, 35000.0], 1 << 14, 3).cpu().numpy()[0]
+    np.testing.assert_allclose(F, -(2.0 / 3.0) * 70000.0 / c * n, rtol=2e-6)
+    F = ctx.srp_thermal_forces(dz, [0.0, -35000.0], 1 << 14, 3).cpu().numpy()[0]
+    np.testing.assert_allclose(F, +(2.0 / 3.0) * 35000.0 / c * n, rtol=2e-6)
+    assert ctx.srp_get_stats()["launched"] == 1 << 14
+    F = ctx.srp_thermal_forces(dz, [0.0, 0.0], 1 << 10, 3).cpu().numpy()[0]
+    assert np.all(F == 0) and ctx.srp_get_stats()["launched"] == 0
+    dz.free()
+    from test_oracle_thermal import box
+    room = box([-1, -1, -1], [1, 1, 1], inward=True)
+    emitter = quad([-0.2, -0.2, -0.3], [0.4, 0, 0], [0, 0.4, 0.1])
+    verts = np.concatenate([room, emitter])
+    power = np.zeros(len(verts), np.float32); power[-2:] = 500.0
+    dz = ctx.srp_build_designs_from_meshes(verts, const_mats(len(verts), 1.0, 0.0, 0.0), [0, len(verts)])
+    ctx.srp_set_options(deposit=1)
+    try:
+        F = ctx.srp_thermal_forces(dz, power, 1 << 14, 4).cpu().numpy()[0]
+        st = ctx.srp_get_stats()
+    finally:
+        ctx.srp_set_options()
+    assert st["absorbed"] == st["launched"] == 2 << 14
+    assert np.linalg.norm(F) < 1e-5 * 1000.0 / c            # per-lane fp32 sums of +-d cancel to rounding
+    dz.free()
+
+
 # ---------------------------------------------------------------- full sizes, in bench.py's launch configuration
 def test_cfg2_full_size_sampled_against_oracle(ctx, oracle):
     """The whole 256 x 1024 x 2^18 job in one srp_forces call (as bench.py launches it); 24 sampled
