@@ -65,6 +65,13 @@ typedef struct {
                                0 = auto: as beams (blocks of rays share one BVH descent) when
                                    rays_per_dir >= 8 x the largest design's triangle count, else one by one,
                                1 = every primary walks the BVH on its own, 2 = beams always; test use   */
+    int escape_masks;       /* per-triangle masks of the directions in which a ray leaving the triangle could hit
+                               anything (designs with a BVH); bounce rays outside them are counted as escaped
+                               without a traversal (results unchanged).  Built inside the first srp_forces* /
+                               srp_thermal_forces call that wants them and kept with the designs handle (which
+                               is therefore not to be used from two contexts at once).
+                               0 = never, 1 (default) = when the call traces >= 32768 photons per triangle of
+                               the batch (the build is repaid), 2 = always; test use                          */
 } srp_options;
 
 /* Photon bookkeeping of the last srp_forces call (DESIGN.md "Pins" P8).
@@ -82,6 +89,8 @@ typedef struct {
        rectangle-vs-triangle culling tests.  box_tests / tri_tests count per-ray slab tests and
        Moller-Trumbore tests only. */
     unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
+    unsigned long long mask_escapes;   /* bounce rays resolved as "escaped" by the escape masks (also counted in
+                                          escaped and segments) */
 } srp_stats;
 
 /* Creates a context on CUDA device `cuda_device`; `cuda_stream` is a cudaStream_t (may be NULL =

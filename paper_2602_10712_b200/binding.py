@@ -27,7 +27,7 @@ class SrpError(RuntimeError):
 
 class srp_options(ctypes.Structure):
     _fields_ = [("solar_pressure", ctypes.c_double), ("sampler", ctypes.c_int), ("deposit", ctypes.c_int),
-                ("force_brute", ctypes.c_int), ("instrumented", ctypes.c_int), ("primary_mode", ctypes.c_int)]
+                ("force_brute", ctypes.c_int), ("instrumented", ctypes.c_int), ("primary_mode", ctypes.c_int), ("escape_masks", ctypes.c_int)]
 
 
 class srp_stats(ctypes.Structure):
@@ -36,13 +36,13 @@ class srp_stats(ctypes.Structure):
                [("hits_at_depth", ctypes.c_ulonglong * 16), ("box_tests", ctypes.c_ulonglong),
                 ("tri_tests", ctypes.c_ulonglong)] + \
                [(n, ctypes.c_ulonglong) for n in ("beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback",
-                                                  "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests")]
+                                                  "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests", "mask_escapes")]
 
     def as_dict(self):
         d = {n: int(getattr(self, n)) for n in
              ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "box_tests", "tri_tests",
               "beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback",
-              "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests")}
+              "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests", "mask_escapes")}
         d["hits_at_depth"] = [int(x) for x in self.hits_at_depth]
         return d
 
@@ -172,8 +172,8 @@ class Context:
             self.handle = None
 
     def srp_set_options(self, solar_pressure=W.SOLAR_PRESSURE, sampler=0, deposit=0, force_brute=0, instrumented=0,
-                        primary_mode=0):
-        o = srp_options(solar_pressure, sampler, deposit, force_brute, instrumented, primary_mode)
+                        primary_mode=0, escape_masks=1):
+        o = srp_options(solar_pressure, sampler, deposit, force_brute, instrumented, primary_mode, escape_masks)
         self._check(self.lib.srp_set_options(self.handle, ctypes.byref(o)))
 
     def srp_build_designs(self, family, theta, mesh_seed=W.MESH_SEED):

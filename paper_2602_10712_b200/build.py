@@ -26,6 +26,7 @@ SOURCES = {
     "srp_api.cu": [],
     "mesh_gen.cu": ["--fmad=false"],
     "lbvh.cu": [],
+    "escape_mask.cu": [],
     "trace.cu": [],
     "trace_perray.cu": [],
     "trace_beam.cu": [],
@@ -57,7 +58,7 @@ def build_library(force=False, verbose=False, bounds_check=False):
         LIB_PATH = os.path.join(HERE, "libsrp_b200_chk.so")
         extra_all = ["-DSRP_BOUNDS_CHECK"]
     os.makedirs(OBJ_DIR, exist_ok=True)
-    headers = [os.path.join(CSRC, "srp_internal.cuh"), os.path.join(CSRC, "trace_common.cuh"), os.path.join(INCLUDE, "srp.h"), os.path.abspath(__file__)]
+    headers = [os.path.join(CSRC, "srp_internal.cuh"), os.path.join(CSRC, "trace_common.cuh"), os.path.join(CSRC, "escape_bins.cuh"), os.path.join(INCLUDE, "srp.h"), os.path.abspath(__file__)]
     nvcc = _nvcc()
     objs, procs = [], []
     for src, extra in SOURCES.items():

@@ -238,7 +238,50 @@ emit_kernel(const unsigned long long *keys_all, const long long *off, long long 
     nodes[4 * g + 0] = make_float4(lo[0].x, lo[0].y, lo[0].z, hi[0].x);
     nodes[4 * g + 1] = make_float4(hi[0].y, hi[0].z, lo[1].x, lo[1].y);
     nodes[4 * g + 2] = make_float4(lo[1].z, hi[1].x, hi[1].y, hi[1].z);
-    nodes[4 * g + 3] = make_float4(__int_as_float(link[0]), __int_as_float(link[1]), 0.f, 0.f);
+    // spare words: the node's own sorted triangle range (first, count) -- read by node_plane_kernel
+    nodes[4 * g + 3] = make_float4(__int_as_float(link[0]), __int_as_float(link[1]),
+                                   __int_as_float(n == 1 ? 0 : range_first[g]), __int_as_float(n == 1 ? 1 : range_count[g]));
+}
+
+// ---- per-node plane slab (for the escape masks): the tightest slab dmin <= n . x <= dmax that holds all vertices
+// of the node's triangles, along n = the normalised sum of their area normals.  A flat patch gives dmax - dmin ~ 1e-6;
+// escape_mask.cu uses it to tell "this whole subtree lies in my plane" where the axis-aligned box of a tilted patch
+// cannot.  One thread per internal node, two passes over its (contiguous, sorted) triangle range.
+__global__ void __launch_bounds__(256)
+node_plane_kernel(const DesignsDev dz, long long sumT, float4 *nplane)
+{
+    long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= sumT) return;
+    const int k = find_design(dz.tri_off, dz.D, g);
+    const long long base = dz.tri_off[k];
+    const int n = (int)(dz.tri_off[k + 1] - base);
+    const int i = (int)(g - base);
+    if (i >= n - 1 && !(n == 1 && i == 0)) return;
+    const float4 rec = dz.nodes[4 * g + 3];
+    const int first = __float_as_int(rec.z), cnt = __float_as_int(rec.w);
+    const float4 *tri = dz.tri;
+    const float4 *t = tri + 3 * (base + first);
+    float sx = 0.f, sy = 0.f, sz = 0.f;
+    for (int f = 0; f < cnt; ++f) {
+        const float4 e1 = t[3 * f + 1], e2 = t[3 * f + 2];
+        sx += e1.y * e2.z - e1.z * e2.y; sy += e1.z * e2.x - e1.x * e2.z; sz += e1.x * e2.y - e1.y * e2.x;
+    }
+    const float len = sqrtf(sx * sx + sy * sy + sz * sz);
+    if (!(len > 0.f)) {                                   // normals cancel: no usable plane
+        nplane[2 * g] = make_float4(0.f, 0.f, 0.f, -FLT_MAX); nplane[2 * g + 1] = make_float4(FLT_MAX, 0.f, 0.f, 0.f);
+        return;
+    }
+    sx /= len; sy /= len; sz /= len;
+    float dmin = FLT_MAX, dmax = -FLT_MAX;
+    for (int f = 0; f < cnt; ++f) {
+        const float4 a = t[3 * f], e1 = t[3 * f + 1], e2 = t[3 * f + 2];
+        const float d0 = sx * a.x + sy * a.y + sz * a.z;
+        const float d1 = sx * (a.x + e1.x) + sy * (a.y + e1.y) + sz * (a.z + e1.z);
+        const float d2 = sx * (a.x + e2.x) + sy * (a.y + e2.y) + sz * (a.z + e2.z);
+        dmin = fminf(dmin, fminf(d0, fminf(d1, d2))); dmax = fmaxf(dmax, fmaxf(d0, fmaxf(d1, d2)));
+    }
+    nplane[2 * g] = make_float4(sx, sy, sz, dmin);
+    nplane[2 * g + 1] = make_float4(dmax, 0.f, 0.f, 0.f);
 }
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return e_; } while (0)
@@ -296,4 +339,11 @@ cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream)
     cudaFreeAsync(vals_out, stream); cudaFreeAsync(ibuf, stream); cudaFreeAsync(lbox, stream);
     cudaFreeAsync(nbox, stream); cudaFreeAsync(tmp, stream);
     return e;
+}
+
+// Per-node plane slabs for the escape masks (built lazily with them, srp_api.cu).
+cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream)
+{
+    node_plane_kernel<<<(unsigned)((sumT + 255) / 256), 256, 0, stream>>>(dz, sumT, nplane);
+    return cudaGetLastError();
 }

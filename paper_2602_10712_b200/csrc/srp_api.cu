@@ -27,7 +27,7 @@ srp_status cuda_fail(srp_context *ctx, const char *what, cudaError_t e)
 // design arrays come from the device's stream-ordered pool (no device-wide synchronisation per build)
 void free_designs_mem(srp_context *ctx, srp_designs *d)
 {
-    void *ptrs[7] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm };
+    void *ptrs[9] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm, d->esc, d->nplane };
     for (void *q : ptrs)
         if (q) cudaFreeAsync(q, ctx->stream);
 }
@@ -94,6 +94,32 @@ srp_status ensure_pool(srp_context *ctx, TraceArgs &a, bool brute, bool instrume
     return SRP_OK;
 }
 
+// Escape masks (escape_mask.cu) are built the first time a call can repay them: the build costs about 0.1 us per
+// triangle, a masked bounce ray saves about 10 ps per segment of the call, so `rays` (all photons of the call) must
+// exceed the triangle count by a few 10^4.  They stay with the handle afterwards.  escape_masks: 0 never, 1 this
+// rule, 2 always.
+srp_status ensure_masks(srp_context *ctx, const srp_designs *dz, double rays)
+{
+    srp_designs *d = const_cast<srp_designs *>(dz);           // a cache inside the handle, not a change of its meaning
+    if (d->esc || d->esc_failed || !d->has_bvh || ctx->opt.escape_masks == 0 || d->D > 65535) return SRP_OK;
+    if (ctx->opt.escape_masks == 1 && rays < 32768.0 * (double)d->sumT) return SRP_OK;
+    unsigned *esc = nullptr;
+    float4 *nplane = nullptr;
+    if (cudaMallocAsync(&esc, sizeof(unsigned) * 14 * d->sumT, ctx->stream) != cudaSuccess ||
+        cudaMallocAsync(&nplane, sizeof(float4) * 2 * d->sumT, ctx->stream) != cudaSuccess) {
+        cudaGetLastError();                                   // no room: trace without masks
+        if (esc) cudaFreeAsync(esc, ctx->stream);
+        d->esc_failed = true;
+        return SRP_OK;
+    }
+    d->nplane = nplane;
+    cudaError_t e = srp_launch_node_planes(d->dev(), d->sumT, nplane, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_escape_masks(d->dev(), d->maxT, esc, ctx->stream);
+    if (e != cudaSuccess) { cudaFreeAsync(esc, ctx->stream); return cuda_fail(ctx, "escape mask build", e); }
+    d->esc = esc;
+    return SRP_OK;
+}
+
 srp_status check_trace_args(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S,
                             long long N, int B, const void *out)
 {
@@ -146,8 +172,13 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
         return fail(ctx, SRP_ERR_UNSUPPORTED, "torques are not available from the instrumented kernels");
     srp_status st = ensure_workspace(ctx, (size_t)n_pairs * stride);
     if (st != SRP_OK) return st;
+    if (B > 0 && !(ctx->opt.force_brute != 0)) {
+        st = ensure_masks(ctx, dz, (double)n_pairs * (double)N);
+        if (st != SRP_OK) return st;
+    }
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
     a.accum = ctx->accum; a.acc_stride = stride; a.torque = out_torques ? 1 : 0; a.xcom = x_com;
+    if (ctx->opt.escape_masks == 0) a.dz.esc = nullptr;        // masks an earlier call built stay unused
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * stride * n_pairs, ctx->stream), "zero accumulators");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
@@ -176,7 +207,7 @@ srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
     ctx->device = cuda_device;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt.solar_pressure = 4.56e-6; ctx->opt.sampler = 0; ctx->opt.deposit = 0;
-    ctx->opt.force_brute = 0; ctx->opt.instrumented = 0; ctx->opt.primary_mode = 0;
+    ctx->opt.force_brute = 0; ctx->opt.instrumented = 0; ctx->opt.primary_mode = 0; ctx->opt.escape_masks = 1;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
     {   // keep freed blocks in the stream-ordered pool: builds reuse them instead of going back to the driver
@@ -208,7 +239,7 @@ srp_status srp_set_options(srp_context *ctx, const srp_options *opt)
     if (!ctx) return SRP_ERR_INVALID;
     if (!opt) return fail(ctx, SRP_ERR_INVALID, "null options");
     if (!(opt->solar_pressure > 0.0) || opt->sampler < 0 || opt->sampler > 1 || opt->deposit < 0 || opt->deposit > 1 ||
-        opt->primary_mode < 0 || opt->primary_mode > 2)
+        opt->primary_mode < 0 || opt->primary_mode > 2 || opt->escape_masks < 0 || opt->escape_masks > 2)
         return fail(ctx, SRP_ERR_INVALID, "option out of range");
     ctx->opt = *opt;
     return SRP_OK;
@@ -386,10 +417,13 @@ srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *dz, const flo
     cudaSetDevice(ctx->device);
     srp_status st = ensure_workspace(ctx, (size_t)dz->D * 3);
     if (st != SRP_OK) return st;
+    st = ensure_masks(ctx, dz, (double)N * (double)dz->sumT);
+    if (st != SRP_OK) return st;
     TraceArgs a;
     memset(&a, 0, sizeof a);
     a.dz = dz->dev();
     a.n_pairs = dz->D; a.S = 1; a.N = N; a.B = B;
+    if (ctx->opt.escape_masks == 0) a.dz.esc = nullptr;
     a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
     a.sampler = 0; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
     a.accum = ctx->accum; a.acc_stride = 3; a.stats = ctx->stats; a.work_counter = ctx->work_counter;
@@ -468,9 +502,14 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const fl
     cudaSetDevice(ctx->device);
     st = ensure_workspace(ctx, (size_t)n_pairs * 3);
     if (st != SRP_OK) return st;
+    if (B > 0 && ctx->opt.force_brute == 0) {
+        st = ensure_masks(ctx, dz, (double)n_pairs * (double)N);
+        if (st != SRP_OK) return st;
+    }
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
     a.accum = ctx->accum;
     a.sig_out = out_sig;
+    if (ctx->opt.escape_masks == 0) a.dz.esc = nullptr;
     TRY_CUDA(ctx, cudaMemsetAsync(out_sig, 0, sizeof(unsigned long long) * n_pairs * N, ctx->stream), "zero signatures");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * n_pairs, ctx->stream), "zero accumulators");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");

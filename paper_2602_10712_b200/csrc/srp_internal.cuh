@@ -25,6 +25,8 @@ struct DesignsDev {
     const long long *tri_off; // [D + 1]
     const float4 *box;        // [D * 2]: (lo, -), (hi, -)
     const int *perm;          // [sumT]: sorted position -> original index within the design
+    const unsigned *esc;      // [sumT * 14]: escape masks (escape_mask.cu), or nullptr
+    const float4 *nplane;     // [sumT * 2]: per-node plane slab (n, dmin), (dmax) -- lbvh.cu; with esc
     int D;
     int has_bvh;
 };
@@ -41,10 +43,13 @@ struct srp_designs {
     long long *tri_off_dev = nullptr;
     float4 *box = nullptr;
     int *perm = nullptr;
+    unsigned *esc = nullptr;
+    float4 *nplane = nullptr;
+    bool esc_failed = false;  // the mask allocation failed once: do not try again
     bool has_bvh = false;
     DesignsDev dev() const {
         DesignsDev d;
-        d.tri = tri; d.nodes = nodes; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.D = D;
+        d.tri = tri; d.nodes = nodes; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.esc = esc; d.nplane = nplane; d.D = D;
         d.has_bvh = has_bvh ? 1 : 0;
         return d;
     }
@@ -56,6 +61,7 @@ struct DevStats {           // device mirror of srp_stats
     unsigned long long box_tests, tri_tests;
     unsigned long long beam_tile_miss, beam_block_miss, beam_group_miss, beam_fallback;
     unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
+    unsigned long long mask_escapes;
 };
 
 struct srp_context {
@@ -105,6 +111,8 @@ cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_par
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
                                 cudaStream_t stream);
 cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream);
+cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream);
+cudaError_t srp_launch_escape_masks(const DesignsDev &dz, long long maxT, unsigned *esc, cudaStream_t stream);
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms,
                              cudaStream_t stream);
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream);

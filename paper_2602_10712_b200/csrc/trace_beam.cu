@@ -216,7 +216,8 @@ beam_trace_kernel(const TraceArgs a)
             if (INSTR) sig = hsig[e] * 1000003ULL + (unsigned long long)(a.dz.perm[tb + best] + 1);
             float3 dep = f3(0, 0, 0), dep_t = f3(0, 0, 0);
             fate = shade<TORQUE>(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
-                         a.deposit, o, d, src, depth, dep, dep_t);
+                         a.deposit, o, d, src, depth, dep, dep_t, a.dz.esc, tb + best);
+            if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
             if (fate == SHADE_ABSORBED) cn.absorbed++;
             if (fate == SHADE_CAPPED) cn.capped++;
             unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * (long long)p);
@@ -525,7 +526,8 @@ beam_trace_kernel(const TraceArgs a)
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
                         fate = shade<TORQUE>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                     best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
+                                     best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best);
+                        if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
                         if (fate == SHADE_CAPPED) cn.capped++;
                     }

@@ -11,6 +11,7 @@
 #pragma once
 #include <cfloat>
 #include "srp_internal.cuh"
+#include "escape_bins.cuh"
 
 // Debug build (nvcc -DSRP_BOUNDS_CHECK): every write into a fixed-capacity shared-memory list, stack or ray pool
 // checks its index and traps with a message.  compute-sanitizer is not available on the target pool.
@@ -263,6 +264,7 @@ __device__ __forceinline__ void closest_bvh(const float4 *__restrict__ nodes, co
 
 struct LaneCounters {
     unsigned launched, pmiss, absorbed, escaped, capped, segments, n_box, n_tri;
+    unsigned mesc;          // bounce rays resolved by the escape masks (also in escaped and segments)
 };
 struct BeamCounters {       // rays resolved per beam level (lane-distributed counts); instrumented: beam work
     unsigned tile_miss, block_miss, group_miss, fallback;
@@ -271,14 +273,15 @@ struct BeamCounters {       // rays resolved per beam level (lane-distributed co
 
 // O-steps 5-7 at a hit: deposit, lobe selection, continuation.
 // Returns SHADE_CONTINUE if the photon goes on (o, d, src, depth updated), else how it ended.
-enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2 };
+enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2, SHADE_ESCAPES = 3 };   // ESCAPES: goes on, but the
+// escape mask of the facet (escape_mask.cu) shows that its next segment cannot hit anything
 // CFLAG is OR-ed into the Philox counter word that holds the depth: 0 for sun photons, 0x80000000 for photons of
 // thermal emitters (R22), so the two families draw from disjoint streams.
 template <bool TORQUE, uint32_t CFLAG = 0u>
 __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
                                       const int deposit, float3 &o, float3 &d, int &src, int &depth,
-                                      float3 &acc, float3 &acc_t)
+                                      float3 &acc, float3 &acc_t, const unsigned *esc = nullptr, long long gidx = 0)
 {
     (void)q0;
     // every deposit of this hit is made at the hit point x; Eq. 4: torque += (x - x_COM) x deposit
@@ -326,6 +329,8 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     }
     if (deposit == 1) put(f3(d.x - dn.x, d.y - dn.y, d.z - dn.z));
     if (depth == B) return SHADE_CAPPED;                         // R5: B reflections followed
+    // the photon leaves on the side it came from (nf): side 0 = the side of e1 x e2
+    if (esc && esc_escapes(esc, gidx, nd > 0.0f ? 1 : 0, dn.x, dn.y, dn.z)) return SHADE_ESCAPES;
     // Hit point in fp32 is off the facet's plane by a few ulp of |x| + t (micrometres here).  An origin
     // that ends up BELOW the plane lets the outgoing ray hit a coplanar or convex neighbour from
     // behind -- a path the exact arithmetic of the definition never takes.  Lift the origin along the
@@ -386,6 +391,12 @@ __device__ __forceinline__ void flush_counters(const TraceArgs &a, const LaneCou
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
         if (lane == 0 && v) atomicAdd(st + (c < 6 ? c : 22 + (c - 6)), v);
+    }
+    {
+        unsigned long long v = cn.mesc;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+        if (lane == 0 && v) atomicAdd(st + 32, v);
     }
     __syncwarp();
     if (lane < 16 && hist[lane]) atomicAdd(st + 6 + lane, (unsigned long long)hist[lane]);

@@ -183,7 +183,8 @@ bvh_trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
                     fate = shade<TORQUE>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
+                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best);
+                    if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                 }

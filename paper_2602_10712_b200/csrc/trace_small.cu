@@ -92,10 +92,10 @@ small_beam_kernel(const TraceArgs a)
             loaded_k = k;
             __syncwarp();
             // A ray that leaves facet f on the side of +n (or -n) can only hit triangles with a vertex on that
-            // side of f's plane: two 64-bit masks per facet, built once per design.  The margin (1e-5 of the
+            // side of f's plane: two 64-bit masks per facet, built once per design.  The margin (1e-6 of the
             // design's extent) keeps only coplanar neighbours out, which exact arithmetic never hits.
             const float4 blo = a.dz.box[2 * k], bhi = a.dz.box[2 * k + 1];
-            const float eps = 1.0e-5f * (fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
+            const float eps = 1.0e-6f * (fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
                                          fmaxf(fabsf(blo.z), fabsf(bhi.z)));
             for (int f = lane; f < T; f += 32) {
                 const float4 q0 = W.tri[3 * f], q1 = W.tri[3 * f + 1], q2 = W.tri[3 * f + 2];

@@ -140,6 +140,9 @@ thermal_trace_kernel(const TraceArgs a, const ThermalArgs h)
                     const float lift = 1.0e-6f * (fabsf(x.x) + fabsf(x.y) + fabsf(x.z));
                     o = f3(fmaf(lift, ne.x, x.x), fmaf(lift, ne.y, x.y), fmaf(lift, ne.z, x.z));
                     alive = true; cn.launched++;
+                    if (a.dz.esc && esc_escapes(a.dz.esc, gpos, W > 0.0f ? 0 : 1, d.x, d.y, d.z)) {
+                        alive = false; cn.segments++; cn.pmiss++; cn.mesc++;      // nothing in that direction
+                    }
                 }
                 next = (end - next) < 32u ? end : next + 32u;
             } else break;
@@ -155,7 +158,8 @@ thermal_trace_kernel(const TraceArgs a, const ThermalArgs h)
                 } else {
                     atomicAdd(&s_hist[warp][depth], 1u);
                     fate = shade<false, THERMAL_FLAG>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2),
-                                                      tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t);
+                                                      tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best);
+                    if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                 }

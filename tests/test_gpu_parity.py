@@ -221,20 +221,21 @@ def test_small_design_configs_full_N(ctx, oracle, name, n_pairs):
     dz.free()
 
 
-@pytest.mark.parametrize("primary_mode", [1, 2])          # primaries one by one / as beams (auto picks by N / T)
-def test_cfg3_detailed_reduced_N(ctx, oracle, primary_mode):
+@pytest.mark.parametrize("primary_mode,masks", [(1, 0), (2, 0), (1, 2), (2, 2)])   # primaries one by one / as beams
+def test_cfg3_detailed_reduced_N(ctx, oracle, primary_mode, masks):                  # (auto picks by N / T); escape masks off / forced
     cfg = W.CONFIGS["cfg3_detailed"]
     th, sun = cfg.params(), cfg.sun_dirs()
     dz = ctx.srp_build_designs(cfg.family, th)
     N = 1 << 12
     rng = np.random.default_rng(6)
     pairs = np.stack([np.arange(cfg.D), rng.integers(0, cfg.S, cfg.D)], 1).astype(np.int32)   # one per design
-    ctx.srp_set_options(primary_mode=primary_mode)
+    ctx.srp_set_options(primary_mode=primary_mode, escape_masks=masks)
     try:
         F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
         psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
     finally:
         ctx.srp_set_options()
+    assert (st["mask_escapes"] > 0.3 * st["escaped"]) if masks else st["mask_escapes"] == 0
     if primary_mode == 2:
         assert st["beam_tile_miss"] + st["beam_block_miss"] + st["beam_group_miss"] > 0.5 * st["launched"]
     else:
@@ -256,8 +257,8 @@ def test_cfg3_detailed_reduced_N(ctx, oracle, primary_mode):
     dz.free()
 
 
-@pytest.mark.parametrize("primary_mode", [1, 2])
-def test_cfg5_sail_reduced_N(ctx, oracle, primary_mode):
+@pytest.mark.parametrize("primary_mode,masks", [(1, 0), (2, 0), (1, 2)])
+def test_cfg5_sail_reduced_N(ctx, oracle, primary_mode, masks):
     cfg = W.CONFIGS["cfg5_sail"]
     th = cfg.params()
     dz = ctx.srp_build_designs(cfg.family, th)
@@ -266,7 +267,7 @@ def test_cfg5_sail_reduced_N(ctx, oracle, primary_mode):
     sun = np.array([[1, 0.2, 0.02], [0.3, -1, -0.03], [0.5, 0.4, 0.7], [-0.2, 0.6, -0.6],
                     [0.05, 0.02, 1], [0.01, -0.03, -1]], np.float32)
     pairs = np.stack([np.zeros(len(sun)), np.arange(len(sun))], 1).astype(np.int32)
-    ctx.srp_set_options(primary_mode=primary_mode)       # 2: ~1000 triangles per ray, every beam list overflows
+    ctx.srp_set_options(primary_mode=primary_mode, escape_masks=masks)   # 2: ~1000 triangles per ray, every beam list overflows
     try:
         F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
         psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
@@ -760,4 +761,109 @@ def test_force_maps_direct_and_indirect(ctx):
     assert tuple(total.shape) == (2, 4, 8, 3)
     assert float(indirect.abs().max()) > 1e-3 * float(total.abs().max())
     assert float(indirect.abs().max()) < float(direct.abs().max())
+    dz.free()
+
+
+# ---------------------------------------------------------------- escape masks (escape_mask.cu)
+def _mask_meshes():
+    """Meshes that stress the mask build: a sphere (convex: every outward direction escapes), an open-topped room
+    with a box in it, entered through the opening (inside, almost nothing escapes), two facing finely tessellated
+    plates (coplanar neighbours by the thousand, everything opposite within a narrow cone), a random triangle soup
+    (no structure at all)."""
+    from test_oracle_thermal import box
+    rng = np.random.default_rng(11)
+
+    def tess(o, u, v, n):                                   # n x n quads, normal u x v
+        o, u, v = (np.asarray(x, float) for x in (o, u, v))
+        return np.concatenate([quad(o + u * i / n + v * j / n, u / n, v / n) for i in range(n) for j in range(n)])
+
+    sphere = W.icosphere(3, 1.0)
+    walls = [tess([-2, -2, -2], [0, 4, 0], [0, 0, 4], 6), tess([2, -2, -2], [0, 0, 4], [0, 4, 0], 6),     # normals inward
+             tess([-2, -2, -2], [0, 0, 4], [4, 0, 0], 6), tess([-2, 2, -2], [4, 0, 0], [0, 0, 4], 6),
+             tess([-2, -2, -2], [4, 0, 0], [0, 4, 0], 6)]
+    room = np.concatenate(walls + [box([-0.5, -0.4, -1.3], [0.4, 0.5, 0.6])])
+    plates = np.concatenate([tess([-1, -1, 0], [2, 0, 0], [0, 2, 0], 24), tess([-1, -1, 0.7], [0, 2, 0], [2, 0, 0], 24)])
+    c = rng.uniform(-1, 1, (1500, 1, 3))
+    soup = (c + rng.normal(0, 0.15, (1500, 3, 3))).astype(np.float32)
+    return {"sphere": sphere, "room": room.astype(np.float32), "plates": plates.astype(np.float32), "soup": soup}
+
+
+@pytest.mark.parametrize("name", ["sphere", "room", "plates", "soup", "detailed", "sail"])
+def test_escape_masks_change_no_photon(ctx, name):
+    """The masks only say "no triangle lies this way": with them forced on, every photon follows the same path
+    (identical signatures) and all photon counters agree; the forces agree to fp32 rounding (a lane that skips a
+    traversal takes its next ray earlier, so the per-lane fp32 partial sums group the same deposits differently);
+    only the share of escaped rays that never walked the BVH (mask_escapes) differs."""
+    rng = np.random.default_rng(3)
+    if name == "detailed":
+        dz = ctx.srp_build_designs(W.FAMILY_DETAILED, W.draw_params(W.FAMILY_DETAILED, 3))
+        D = 3
+    elif name == "sail":
+        dz = ctx.srp_build_designs(W.FAMILY_SAIL, np.array([[0.8]], np.float32))
+        D = 1
+    else:
+        verts = _mask_meshes()[name]
+        mats = np.tile(np.array([[0.2, 0.5, 0.3]], np.float32), (len(verts), 1))
+        dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
+        D = 1
+    sun = W.fibonacci_sphere(7)
+    pairs = np.array([[k, j] for k in range(D) for j in range(7)], np.int32)
+    N, B = 1 << 13, 6
+    res = {}
+    for mode in (1, 2):
+        for masks in (0, 2):
+            ctx.srp_set_options(primary_mode=mode, escape_masks=masks)
+            try:
+                F, st = run_pairs(ctx, dz, sun, pairs, N, B, seed=9)
+                sg = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, B, 9).cpu().numpy()
+            finally:
+                ctx.srp_set_options()
+            res[mode, masks] = (F, st, sg)
+        (F0, s0, g0), (F2, s2, g2) = res[mode, 0], res[mode, 2]
+        assert np.array_equal(g0, g2), (name, mode, int((g0 != g2).sum()))
+        assert np.abs(F2 - F0).max() <= 2e-6 * np.abs(F0).max(), (name, mode)
+        for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "hits_at_depth"):
+            assert s0[key] == s2[key], (name, mode, key)
+        assert s0["mask_escapes"] == 0
+        print(name, "mode", mode, "escaped", s2["escaped"], "by mask", s2["mask_escapes"])
+        if name == "sphere":
+            assert s2["mask_escapes"] == s2["escaped"] > 0          # convex: no bounce ray needs a traversal
+        if name == "room":                                          # sun 0 looks into the opening: photons bounce inside
+            assert s2["capped"] + s2["absorbed"] > 0 and sum(s2["hits_at_depth"][2:]) > 0
+        if name in ("detailed", "plates"):
+            assert s2["mask_escapes"] > 0.3 * s2["escaped"]
+    dz.free()
+
+
+def test_escape_masks_thermal_and_auto_rule(ctx):
+    """Thermal emitters use the same masks (emitted rays and their bounces); the default option builds them only
+    when the call traces >= 32768 photons per triangle."""
+    th = W.draw_params(W.FAMILY_DETAILED, 1)
+    rng = np.random.default_rng(4)
+    power = np.zeros(W.TRI_COUNT[W.FAMILY_DETAILED], np.float32)
+    power[rng.choice(len(power), 64, replace=False)] = 50.0
+    out = {}
+    for masks in (0, 2):
+        dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+        ctx.srp_set_options(escape_masks=masks)
+        try:
+            F = ctx.srp_thermal_forces(dz, power, 1 << 12, 4, seed=2).cpu().numpy()
+            out[masks] = (F, ctx.srp_get_stats())
+        finally:
+            ctx.srp_set_options()
+        dz.free()
+    assert rel_l2(out[2][0], out[0][0]).max() < 2e-6
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments"):
+        assert out[0][1][key] == out[2][1][key], key
+    assert out[0][1]["mask_escapes"] == 0 < out[2][1]["mask_escapes"]
+    # auto: 2 pairs x 2^12 rays on 49 840 triangles is far below the rule, 2^20 rays x 2048 pairs is above it
+    sun = W.fibonacci_sphere(2048)
+    dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    ctx.srp_forces(dz, cuda(sun[:2]), 1 << 12, 4, 0)
+    assert ctx.srp_get_stats()["mask_escapes"] == 0
+    pairs = np.stack([np.zeros(2048), np.arange(2048)], 1).astype(np.int32)
+    ctx.srp_forces_pairs(dz, cuda(sun), pairs, 1 << 20, 1, 0)
+    assert ctx.srp_get_stats()["mask_escapes"] > 0
+    ctx.srp_forces(dz, cuda(sun[:2]), 1 << 12, 4, 0)               # once built they stay with the handle
+    assert ctx.srp_get_stats()["mask_escapes"] > 0
     dz.free()
