@@ -38,9 +38,9 @@ FLOP_BOX, FLOP_TRI, FLOP_TRI2D, FLOP_HIT = 12.0, 44.0, 20.0, 80.0
 FLOP_BEAM_BOX, FLOP_RECT, FLOP_SETUP = 32.0, 14.0, 110.0
 BYTES_NODE, BYTES_TRI = 64.0, 48.0
 # DRAM bytes per segment of the dominant kernel from the committed `ncu --set full` captures
-# (dram__bytes_read.sum + dram__bytes_write.sum over the segments of the captured launch; profiles/r1c_final_round1.md,
-# profiles/r1b_beam_trace_cfg3.md)
-NCU_DRAM_BYTES_PER_SEGMENT = {"cfg3_detailed": 33.9e9 / 4.72e9, "cfg2_boxwing": 0.7e6 / 5.26e9}
+# (dram__bytes_read.sum + dram__bytes_write.sum over the segments of the captured launch; cfg3: the half-size launch of
+# profiles/r1d_escape_masks.md, 59.3 + 60.3 GB over 3.78e10 segments; cfg2: profiles/r1b_beam_trace_cfg3.md)
+NCU_DRAM_BYTES_PER_SEGMENT = {"cfg3_detailed": 119.6e9 / 3.778e10, "cfg2_boxwing": 0.7e6 / 5.26e9}
 
 
 def parse():
@@ -218,6 +218,7 @@ def run_ours(args, rank, world, local_rank):
 
     # dominant kernel alone (trace_kernel): CUDA events around srp_forces only, designs resident
     dz = ctx.srp_build_designs(cfg.family, theta, W.MESH_SEED)
+    ctx.srp_forces(dz, sun, cfg.N, cfg.B, 0, out=out)                   # builds the escape masks if this workload repays them
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     flush.zero_()
@@ -250,11 +251,12 @@ def run_ours(args, rank, world, local_rank):
                 "unit": "TFLOP/s", "frac": ach_tflops / FP32_PEAK_TFLOPS,
                 "traffic": (NCU_DRAM_BYTES_PER_SEGMENT[args.workload] * st_k["segments"]
                             if args.workload in NCU_DRAM_BYTES_PER_SEGMENT else None),
-                "traffic_source": "ncu capture of a 1/16 slice (profiles/r1c_final_round1.md), bytes per segment x this launch's segments",
+                "traffic_source": "ncu --set full capture of a slice of this workload (profiles/r1d_escape_masks.md), bytes per segment x this launch's segments",
                 "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz; probed FMA chain %.1f TFLOP/s" % peaks["fp32_tflops"],
                 "flop_per_segment": flop_ps, "tests_per_segment": per, "hits_per_segment": hit_ps,
                 "beam_resolved": {k: st_k[k] / max(st_k["launched"], 1) for k in
                                   ("beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback")},
+                "escapes_resolved_by_mask": st_k["mask_escapes"] / max(st_k["escaped"], 1),
                 "l2": {"achieved_gbs": bytes_ps * st_k["segments"] / t_kernel / 1e9, "probed_peak_gbs": peaks["l2_read_gbs"],
                        "bytes_per_segment": bytes_ps},
                 "kernel_ms": 1e3 * t_kernel, "kernel_segments": st_k["segments"]}
@@ -303,7 +305,7 @@ def run_ours(args, rank, world, local_rank):
                 "forces_per_s": pairs_all * args.steps / t_max,
                 "primary_hit_fraction": 1.0 - pmiss / max(launched, 1), "hits_per_photon": hits / max(launched, 1),
                 "segments_per_photon": segs / max(launched, 1),
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": (10 if W.TRI_COUNT[cfg.family] > 64 else 6) * args.steps,
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": ((10 + (2 if st["mask_escapes"] > 0 else 0)) if W.TRI_COUNT[cfg.family] > 64 else 6) * args.steps,
                 "clocks": clocks}
         print(json.dumps(line), flush=True)
     ctx.close()

@@ -213,20 +213,31 @@ escape_mask_kernel(const DesignsDev dz, unsigned *esc)
             // signed distance range of the box from THIS lane's plane
             const float dc = n.x * cx + n.y * cy + n.z * cz - pd;
             const float dr = fabsf(n.x) * hx + fabsf(n.y) * hy + fabsf(n.z) * hz;
-            // slab half-width: the plane's offset error plus the error of its fp32 normal (from 5 cm edges of
-            // vertices rounded to 1e-6 m: ~2e-5 rad) over the distance to the farthest point of the box
-            const float reach = fabsf(cx - ct.x) + fabsf(cy - ct.y) + fabsf(cz - ct.z) + hx + hy + hz;
-            const float slab = eps + ESC_ANGLE_EPS * reach;
+            // slab half-width: geometry this close to the plane counts as coplanar with the triangle (R20).  eps covers
+            // the fp32 rounding of the vertices; the angular term covers the error of the fp32 normal (from 5 cm
+            // edges of vertices rounded to 1e-6 m: ~2e-5 rad) and grows with the CLEARANCE between the triangle and
+            // the box, not with the box's size: a facet hovering just above the triangle keeps a slab of eps
+            const float mx = fmaxf(fabsf(cx - ct.x) - hx, 0.0f), my = fmaxf(fabsf(cy - ct.y) - hy, 0.0f),
+                        mz = fmaxf(fabsf(cz - ct.z) - hz, 0.0f);
+            const float clear = fmaxf(sqrtf(mx * mx + my * my + mz * mz) - rt, 0.0f);
+            const float slab = eps + ESC_ANGLE_EPS * clear;
             bool plus = dc + dr > slab, minus = dc - dr < -slab;
             if (link[c] >= 0 && (plus || minus)) {
-                // the box of a tilted flat patch is fat; the subtree's own plane slab (lbvh.cu) is not: if it is
-                // parallel to this lane's plane within the angular margin, its offsets decide
+                // the box of a tilted flat patch is fat; the subtree's own plane slab (lbvh.cu) is not.  If the
+                // patch is parallel to this lane's plane within the angular margin, measure with the patch's normal
+                // (an area-weighted mean, far more accurate than one small triangle's).  "Parallel" is judged to the
+                // accuracy of this triangle's own fp32 normal, ang = min(ESC_ANGLE_EPS, 4 eps / rt) -- a large
+                // triangle has an accurate normal -- so its own vertices deviate by at most ang * rt <= 4 eps from
+                // its centroid's offset
                 const float4 pn = __ldg(dz.nplane + 2 * (tbase + link[c])), pm = __ldg(dz.nplane + 2 * (tbase + link[c]) + 1);
                 const float kx = n.y * pn.z - n.z * pn.y, ky = n.z * pn.x - n.x * pn.z, kz = n.x * pn.y - n.y * pn.x;
-                if (kx * kx + ky * ky + kz * kz <= ESC_ANGLE_EPS * ESC_ANGLE_EPS) {
+                const float ang = fminf(ESC_ANGLE_EPS, 4.0f * eps / rt);
+                if (kx * kx + ky * ky + kz * kz <= ang * ang) {
                     const bool same = n.x * pn.x + n.y * pn.y + n.z * pn.z > 0.0f;
-                    const float lo_d = (same ? pn.w : -pm.x) - pd, hi_d = (same ? pm.x : -pn.w) - pd;
-                    plus = hi_d > slab; minus = lo_d < -slab;
+                    const float pc = pn.x * ct.x + pn.y * ct.y + pn.z * ct.z;
+                    const float lo_d = same ? pn.w - pc : pc - pm.x, hi_d = same ? pm.x - pc : pc - pn.w;
+                    const float slab_n = 2.0f * eps + ang * rt + ESC_ANGLE_EPS * clear;
+                    plus = hi_d > slab_n; minus = lo_d < -slab_n;
                 }
             }
             plus = plus && !fullp; minus = minus && !fullm;
@@ -253,8 +264,11 @@ escape_mask_kernel(const DesignsDev dz, unsigned *esc)
                                  v2 = make_float3(p0.x + p2.x, p0.y + p2.y, p0.z + p2.z);
                     const float d0 = n.x * v0.x + n.y * v0.y + n.z * v0.z - pd, d1 = n.x * v1.x + n.y * v1.y + n.z * v1.z - pd,
                                 d2 = n.x * v2.x + n.y * v2.y + n.z * v2.z - pd;
-                    const float slab_f = eps + ESC_ANGLE_EPS * (fabsf(v0.x - ct.x) + fabsf(v0.y - ct.y) + fabsf(v0.z - ct.z) +
-                                                                fabsf(p1.x) + fabsf(p1.y) + fabsf(p1.z) + fabsf(p2.x) + fabsf(p2.y) + fabsf(p2.z));
+                    // clearance between the two triangles' bounding spheres (v0's distance less f's longest edge
+                    // bounds f's nearest point from below)
+                    const float e1l = sqrtf(p1.x * p1.x + p1.y * p1.y + p1.z * p1.z), e2l = sqrtf(p2.x * p2.x + p2.y * p2.y + p2.z * p2.z);
+                    const float v0d = sqrtf((v0.x - ct.x) * (v0.x - ct.x) + (v0.y - ct.y) * (v0.y - ct.y) + (v0.z - ct.z) * (v0.z - ct.z));
+                    const float slab_f = eps + ESC_ANGLE_EPS * fmaxf(v0d - fmaxf(e1l, e2l) - rt, 0.0f);
                     const bool fp = f != t && !fullp && fmaxf(d0, fmaxf(d1, d2)) > slab_f,
                                fm = f != t && !fullm && fminf(d0, fminf(d1, d2)) < -slab_f;
                     if (!__any_sync(FULLW, fp || fm)) continue;

@@ -250,7 +250,9 @@ emit_kernel(const unsigned long long *keys_all, const long long *off, long long 
 __global__ void __launch_bounds__(256)
 node_plane_kernel(const DesignsDev dz, long long sumT, float4 *nplane)
 {
-    long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // one warp per node: the top nodes span the whole design, so the lanes share a node's triangle range
+    const long long g = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (g >= sumT) return;
     const int k = find_design(dz.tri_off, dz.D, g);
     const long long base = dz.tri_off[k];
@@ -259,29 +261,39 @@ node_plane_kernel(const DesignsDev dz, long long sumT, float4 *nplane)
     if (i >= n - 1 && !(n == 1 && i == 0)) return;
     const float4 rec = dz.nodes[4 * g + 3];
     const int first = __float_as_int(rec.z), cnt = __float_as_int(rec.w);
-    const float4 *tri = dz.tri;
-    const float4 *t = tri + 3 * (base + first);
+    const float4 *t = dz.tri + 3 * (base + first);
     float sx = 0.f, sy = 0.f, sz = 0.f;
-    for (int f = 0; f < cnt; ++f) {
+    for (int f = lane; f < cnt; f += 32) {
         const float4 e1 = t[3 * f + 1], e2 = t[3 * f + 2];
         sx += e1.y * e2.z - e1.z * e2.y; sy += e1.z * e2.x - e1.x * e2.z; sz += e1.x * e2.y - e1.y * e2.x;
     }
+    for (int off = 16; off > 0; off >>= 1) {               // xor tree: every lane ends with the same sums
+        sx += __shfl_xor_sync(0xffffffffu, sx, off); sy += __shfl_xor_sync(0xffffffffu, sy, off);
+        sz += __shfl_xor_sync(0xffffffffu, sz, off);
+    }
     const float len = sqrtf(sx * sx + sy * sy + sz * sz);
     if (!(len > 0.f)) {                                   // normals cancel: no usable plane
-        nplane[2 * g] = make_float4(0.f, 0.f, 0.f, -FLT_MAX); nplane[2 * g + 1] = make_float4(FLT_MAX, 0.f, 0.f, 0.f);
+        if (lane == 0) {
+            nplane[2 * g] = make_float4(0.f, 0.f, 0.f, -FLT_MAX); nplane[2 * g + 1] = make_float4(FLT_MAX, 0.f, 0.f, 0.f);
+        }
         return;
     }
     sx /= len; sy /= len; sz /= len;
     float dmin = FLT_MAX, dmax = -FLT_MAX;
-    for (int f = 0; f < cnt; ++f) {
+    for (int f = lane; f < cnt; f += 32) {
         const float4 a = t[3 * f], e1 = t[3 * f + 1], e2 = t[3 * f + 2];
         const float d0 = sx * a.x + sy * a.y + sz * a.z;
         const float d1 = sx * (a.x + e1.x) + sy * (a.y + e1.y) + sz * (a.z + e1.z);
         const float d2 = sx * (a.x + e2.x) + sy * (a.y + e2.y) + sz * (a.z + e2.z);
         dmin = fminf(dmin, fminf(d0, fminf(d1, d2))); dmax = fmaxf(dmax, fmaxf(d0, fmaxf(d1, d2)));
     }
-    nplane[2 * g] = make_float4(sx, sy, sz, dmin);
-    nplane[2 * g + 1] = make_float4(dmax, 0.f, 0.f, 0.f);
+    for (int off = 16; off > 0; off >>= 1) {
+        dmin = fminf(dmin, __shfl_xor_sync(0xffffffffu, dmin, off)); dmax = fmaxf(dmax, __shfl_xor_sync(0xffffffffu, dmax, off));
+    }
+    if (lane == 0) {
+        nplane[2 * g] = make_float4(sx, sy, sz, dmin);
+        nplane[2 * g + 1] = make_float4(dmax, 0.f, 0.f, 0.f);
+    }
 }
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return e_; } while (0)
@@ -344,6 +356,6 @@ cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream)
 // Per-node plane slabs for the escape masks (built lazily with them, srp_api.cu).
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream)
 {
-    node_plane_kernel<<<(unsigned)((sumT + 255) / 256), 256, 0, stream>>>(dz, sumT, nplane);
+    node_plane_kernel<<<(unsigned)((sumT + 7) / 8), 256, 0, stream>>>(dz, sumT, nplane);
     return cudaGetLastError();
 }

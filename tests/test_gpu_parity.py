@@ -867,3 +867,34 @@ def test_escape_masks_thermal_and_auto_rule(ctx):
     ctx.srp_forces(dz, cuda(sun[:2]), 1 << 12, 4, 0)               # once built they stay with the handle
     assert ctx.srp_get_stats()["mask_escapes"] > 0
     dz.free()
+
+
+@pytest.mark.parametrize("gap", [2e-5, 1e-3])
+def test_escape_masks_see_a_plate_hovering_above_the_emitter(ctx, gap):
+    """Coplanar pruning must not swallow real geometry: a 2 m plate hovering 20 um (and 1 mm) above another, both
+    finely tessellated.  The lower plate radiates upwards; all but the photons leaving through the rim gap
+    (<= gap / size of them) are absorbed by the plate above -- with the masks as without."""
+    def tess(o, u, v, n):
+        o, u, v = (np.asarray(x, float) for x in (o, u, v))
+        return np.concatenate([quad(o + u * i / n + v * j / n, u / n, v / n) for i in range(n) for j in range(n)])
+    lower = tess([-1, -1, 0], [2, 0, 0], [0, 2, 0], 8)            # normal +z
+    upper = tess([-1, -1, gap], [0, 2, 0], [2, 0, 0], 5)          # normal -z
+    verts = np.concatenate([lower, upper]).astype(np.float32)
+    mats = const_mats(len(verts), 1.0, 0.0, 0.0)
+    power = np.zeros(len(verts), np.float32); power[:len(lower)] = 10.0
+    res = {}
+    for masks in (0, 2):
+        dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
+        ctx.srp_set_options(escape_masks=masks)
+        try:
+            F = ctx.srp_thermal_forces(dz, power, 1 << 10, 2, seed=1).cpu().numpy()
+            res[masks] = (F, ctx.srp_get_stats())
+        finally:
+            ctx.srp_set_options()
+        dz.free()
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments"):
+        assert res[0][1][key] == res[2][1][key], key
+    st = res[2][1]
+    assert st["launched"] == len(lower) << 10
+    assert st["absorbed"] >= (1.0 - 4 * gap) * st["launched"]
+    assert np.abs(res[2][0] - res[0][0]).max() <= 2e-6 * np.abs(res[0][0]).max() + 1e-30
