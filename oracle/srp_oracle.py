@@ -75,10 +75,16 @@ def lib():
             ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats), ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_forces_torques.restype = ctypes.c_int
         L.srp_oracle_forces_torques.argtypes = L.srp_oracle_forces.argtypes + [ctypes.c_void_p] * 3
+        L.srp_oracle_forces_torques_glossy.restype = ctypes.c_int
+        a = L.srp_oracle_forces_torques.argtypes
+        L.srp_oracle_forces_torques_glossy.argtypes = a[:2] + [ctypes.c_void_p] + a[2:]
         L.srp_oracle_thermal.restype = ctypes.c_int
         L.srp_oracle_thermal.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p,
                                          ctypes.c_longlong, ctypes.c_int, ctypes.c_ulonglong, ctypes.POINTER(Options),
                                          ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(Stats)]
+        L.srp_oracle_thermal_glossy.restype = ctypes.c_int
+        a = L.srp_oracle_thermal.argtypes
+        L.srp_oracle_thermal_glossy.argtypes = a[:2] + [ctypes.c_void_p] + a[2:]
         L.srp_oracle_philox.restype = None
         L.srp_oracle_philox.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_uniform.restype = ctypes.c_double
@@ -123,13 +129,14 @@ def build_mesh(family, theta, k=0, mesh_seed=2):
 
 
 def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sampler=0,
-           deposit=0, want_first_hit=False, want_path_sig=False, x_com=None):
+           deposit=0, want_first_hit=False, want_path_sig=False, x_com=None, shininess=None):
     """Forces of ONE design for the given sun directions.
 
     Returns dict(F f64[S,3], sumsq f64[S,3], sigma f64[S] (i.i.d. standard error of |F|,
     conservative for the stratified sampler), stats dict, first_hit int32[S,N] or None).
     With x_com (3 floats, the centre of mass of PAPER.md:136 Eq. 4) also T f64[S,3] (torque, N m)
-    and sigma_T f64[S].
+    and sigma_T f64[S].  shininess float32[T]: Phong exponent of each facet's specular lobe, < 0 = ideal mirror
+    (R23); None = ideal mirrors throughout.
     """
     verts = np.ascontiguousarray(verts, dtype=np.float32).reshape(-1, 3, 3)
     mats = np.ascontiguousarray(mats, dtype=np.float32).reshape(-1, 3)
@@ -147,7 +154,17 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
             fh.ctypes.data if fh is not None else None,
             ps.ctypes.data if ps is not None else None)
     Tq = TQ = None
-    if x_com is None:
+    if shininess is not None:
+        sh = np.ascontiguousarray(shininess, dtype=np.float32).reshape(-1)
+        assert sh.shape[0] == T
+        xc = None if x_com is None else np.ascontiguousarray(x_com, dtype=np.float64).reshape(3)
+        if xc is not None:
+            Tq = np.zeros((S, 3)); TQ = np.zeros((S, 3))
+        rc = lib().srp_oracle_forces_torques_glossy(*args[:2], sh.ctypes.data, *args[2:],
+                                                    xc.ctypes.data if xc is not None else None,
+                                                    Tq.ctypes.data if xc is not None else None,
+                                                    TQ.ctypes.data if xc is not None else None)
+    elif x_com is None:
         rc = lib().srp_oracle_forces(*args)
     else:
         xc = np.ascontiguousarray(x_com, dtype=np.float64).reshape(3)
@@ -164,7 +181,7 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
     return out
 
 
-def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0):
+def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0, shininess=None):
     """Recoil force of ONE design's thermal (Lambertian) facet emitters: facet_power float32[T]
     in watts, signed (sign = emitting side), N photons per emitting facet.  Returns dict(F f64[3] newtons,
     sigma f64 (i.i.d. standard error of |F| over all emitted photons), stats)."""
@@ -176,8 +193,11 @@ def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0):
     F = np.zeros(3); Q = np.zeros(3)
     st = Stats()
     opt = Options(float(SOLAR_PRESSURE), 0, int(deposit))
-    rc = lib().srp_oracle_thermal(verts.ctypes.data, mats.ctypes.data, T, int(k), pw.ctypes.data, int(N), int(B),
-                                  int(seed), ctypes.byref(opt), F.ctypes.data, Q.ctypes.data, ctypes.byref(st))
+    sh = None if shininess is None else np.ascontiguousarray(shininess, dtype=np.float32).reshape(-1)
+    assert sh is None or sh.shape[0] == T
+    rc = lib().srp_oracle_thermal_glossy(verts.ctypes.data, mats.ctypes.data, sh.ctypes.data if sh is not None else None,
+                                         T, int(k), pw.ctypes.data, int(N), int(B),
+                                         int(seed), ctypes.byref(opt), F.ctypes.data, Q.ctypes.data, ctypes.byref(st))
     if rc != 0:
         raise ValueError("srp_oracle_thermal: invalid arguments")
     n = max(int(st.launched), 1)

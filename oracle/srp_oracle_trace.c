@@ -17,10 +17,15 @@
  * Torque (Eq. 4): tau = int_M (x - x_COM) x f(x) dx -- every
  * momentum deposit, made at hit point x, also contributes (x - x_COM) x deposit.
  *
+ * Glossy specular lobe ("per-face Phong material parameters"; DESIGN.md
+ * reading R23): a facet with shininess n >= 0 scatters its specular part into the Phong lobe cos^n about the
+ * mirror direction, importance-sampled, directions below the facet's horizon rejected and redrawn.
+ *
  * Pins (tests/test_oracle_*.py): Philox KAT, flat plate, convex polyhedron,
  * cannonball limit, occlusion, V-groove, perpendicular-plate form factor,
  * conservation, symmetries, N^-1/2 decay, estimator agreement; torque: off-centre
- * plate, two-plate windmill, centre-of-mass shift identity, centred sphere.
+ * plate, two-plate windmill, centre-of-mass shift identity, centred sphere; glossy lobe (test_oracle_glossy.py):
+ * mean cosine (n+1)/(n+2), mirror limit, lobe axis at oblique incidence, horizon rejection, bookkeeping.
  */
 #include <stdlib.h>
 #include <string.h>
@@ -76,7 +81,7 @@ static void orc_deposit(const double dd[3], orc_v3 x, orc_v3 xc, double dp[3], d
     dq[2] += r.x * dd[1] - r.y * dd[0];
 }
 
-typedef struct { const double *v0, *e1, *e2, *nrm; long T; } orc_geom;
+typedef struct { const double *v0, *e1, *e2, *nrm; long T; const float *shin; } orc_geom;
 
 /* O-steps 4-7 for ONE photon that starts at o along d (src = the triangle it leaves, -1 for none) with momentum
  * weight wph: closest hit, deposit (force total dp, torque total dq about xc), lobe selection, continuation,
@@ -109,11 +114,21 @@ static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 
         const double al = mats[3 * f], rs = mats[3 * f + 1], rd = mats[3 * f + 2];
         /* dd = this hit's momentum deposit, made at x; Eq. 4: torque += (x - x_COM) x dd */
         double dd[3] = { 0, 0, 0 };
-        if (opt->deposit == 0) {
+        /* R23: shininess < 0 (or none given) = the ideal mirror of R5; >= 0 = Phong lobe cos^n about refl */
+        const int glossy = G->shin != NULL && G->shin[f] >= 0.0f;
+        if (opt->deposit == 0 && !glossy) {
             double a = al + rs + rd;
             dd[0] = wph * (a * d.x - rs * refl.x - (2.0 / 3.0) * rd * nf.x);
             dd[1] = wph * (a * d.y - rs * refl.y - (2.0 / 3.0) * rd * nf.y);
             dd[2] = wph * (a * d.z - rs * refl.z - (2.0 / 3.0) * rd * nf.z);
+        }
+        if (opt->deposit == 0 && glossy) {
+            /* absorbed and diffuse parts in expectation at every hit; the specular part has no closed-form mean
+             * once the horizon truncates the lobe: it is deposited as d - d' when that lobe is drawn (below) */
+            double a = al + rd;
+            dd[0] = wph * (a * d.x - (2.0 / 3.0) * rd * nf.x);
+            dd[1] = wph * (a * d.y - (2.0 / 3.0) * rd * nf.y);
+            dd[2] = wph * (a * d.z - (2.0 / 3.0) * rd * nf.z);
         }
         /* O-step 6: lobe selection (thresholds in fp32, R17). */
         uint32_t c2[4] = { i, j, k, (uint32_t)(depth + 1) | cflag }, y[4];
@@ -127,8 +142,37 @@ static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 
             orc_deposit(dd, x, xc, dp, dq);
             st->absorbed++;
             break;
-        } else if (z0 < (double)th2) {
+        } else if (z0 < (double)th2 && !glossy) {
             dnew = refl;
+        } else if (z0 < (double)th2) {
+            /* Phong lobe: cos(theta) = xi^(1/(n+1)) about refl, phi uniform; attempt a = 0 uses (z1, z2) of the
+             * lobe draw, attempt a >= 1 words 1 and 2 of Philox(i, j, k, (depth + 1) | cflag | a << 8).  The local
+             * sample is laid out in the facet's frame (t_u, t_v, nf) of R18 and carried to refl by the rotation
+             * that takes nf to refl about nf x refl (1 + nf . refl >= 1: no singular direction).  A direction
+             * with d' . nf <= 0 is rejected; after 8 rejections the photon takes refl itself. */
+            const double ns = (double)G->shin[f];
+            orc_v3 tu = orc_normalize(orc_mk(G->e1[3 * f], G->e1[3 * f + 1], G->e1[3 * f + 2]));
+            orc_v3 tv = orc_cross(nf, tu);
+            orc_v3 kx = orc_cross(nf, refl);
+            const double cc = orc_dot(nf, refl);
+            double u1 = z1, u2 = z2;
+            dnew = refl;
+            for (int a = 0; a < 8; ++a) {
+                if (a > 0) {
+                    uint32_t c3[4] = { i, j, k, (uint32_t)(depth + 1) | cflag | ((uint32_t)a << 8) }, w[4];
+                    orc_philox4x32_10(c3, key, w);
+                    u1 = orc_uniform(w[1]); u2 = orc_uniform(w[2]);
+                }
+                const double ct = pow(u2, 1.0 / (ns + 1.0)), sn = sqrt(fmax(0.0, 1.0 - ct * ct));
+                const double phi = 6.283185307179586476925286766559 * u1;
+                orc_v3 L = orc_add(orc_add(orc_scale(tu, sn * cos(phi)), orc_scale(tv, sn * sin(phi))), orc_scale(nf, ct));
+                orc_v3 kL = orc_cross(kx, L);
+                orc_v3 cand = orc_add(orc_add(L, kL), orc_scale(orc_cross(kx, kL), 1.0 / (1.0 + cc)));
+                if (orc_dot(cand, nf) > 0.0) { dnew = cand; break; }
+            }
+            if (opt->deposit == 0) {
+                dd[0] += wph * (d.x - dnew.x); dd[1] += wph * (d.y - dnew.y); dd[2] += wph * (d.z - dnew.z);
+            }
         } else {
             double phi = 6.283185307179586476925286766559 * z1, rho = sqrt(z2);
             double lx = rho * cos(phi), ly = rho * sin(phi), lz = sqrt(1.0 - z2);
@@ -174,9 +218,10 @@ static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
  *       sig = sig*1000003 + (triangle index + 1) at every hit (mod 2^64)
  *   x_com double[3] centre of mass (Eq. 4), Tq double[S][3] torque in N m, tq_sumsq double[S][3]
  *       sum of squared per-photon torque totals: all three may be NULL (no torque)
+ *   shininess float[T] or NULL: Phong exponent of each facet's specular lobe, < 0 = ideal mirror (R23)
  * Returns 0, or -1 on invalid arguments.
  */
-int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int k,
+int srp_oracle_forces_torques_glossy(const float *verts, const float *mats, const float *shininess, long T, int k,
                               const float *sun_dirs, int S, int j0, long long N, int B,
                               unsigned long long seed, const orc_options *opt,
                               double *F, double *sumsq, orc_stats *stats, int *first_hit,
@@ -211,7 +256,7 @@ int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int
         nrm[3 * f] = n.x / len; nrm[3 * f + 1] = n.y / len; nrm[3 * f + 2] = n.z / len;
     }
     orc_stats st; memset(&st, 0, sizeof st);
-    const orc_geom G = { v0, e1, e2, nrm, T };
+    const orc_geom G = { v0, e1, e2, nrm, T, shininess };
 
     for (int jj = 0; jj < S; ++jj) {
         const uint32_t j = (uint32_t)(j0 + jj);
@@ -276,6 +321,18 @@ int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int
     return 0;
 }
 
+/* Ideal-mirror specular lobes on every facet (R5): the call of the hot path. */
+int srp_oracle_forces_torques(const float *verts, const float *mats, long T, int k,
+                              const float *sun_dirs, int S, int j0, long long N, int B,
+                              unsigned long long seed, const orc_options *opt,
+                              double *F, double *sumsq, orc_stats *stats, int *first_hit,
+                              unsigned long long *path_sig, const double *x_com, double *Tq,
+                              double *tq_sumsq)
+{
+    return srp_oracle_forces_torques_glossy(verts, mats, NULL, T, k, sun_dirs, S, j0, N, B, seed, opt, F, sumsq,
+                                            stats, first_hit, path_sig, x_com, Tq, tq_sumsq);
+}
+
 /* Forces only (the call the force tests and timings use). */
 int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
                       const float *sun_dirs, int S, int j0, long long N, int B,
@@ -300,9 +357,9 @@ int srp_oracle_forces(const float *verts, const float *mats, long T, int k,
  * source triangle f excluded, lobe draws with counters (i, f, k, 0x80000000 | depth + 1)).
  * F double[3] (N), sumsq double[3] (per-photon totals squared, may be NULL), stats may be NULL.
  */
-int srp_oracle_thermal(const float *verts, const float *mats, long T, int k, const float *facet_power,
-                       long long N, int B, unsigned long long seed, const orc_options *opt,
-                       double *F, double *sumsq, orc_stats *stats)
+int srp_oracle_thermal_glossy(const float *verts, const float *mats, const float *shininess, long T, int k,
+                              const float *facet_power, long long N, int B, unsigned long long seed,
+                              const orc_options *opt, double *F, double *sumsq, orc_stats *stats)
 {
     if (!verts || !mats || !facet_power || !F || !opt || T <= 0 || N <= 0 || B < 0 || B > 15) return -1;
     const double C_LIGHT = 299792458.0;
@@ -319,7 +376,7 @@ int srp_oracle_thermal(const float *verts, const float *mats, long T, int k, con
         double len = sqrt(orc_dot(n, n));
         nrm[3 * f] = n.x / len; nrm[3 * f + 1] = n.y / len; nrm[3 * f + 2] = n.z / len;
     }
-    const orc_geom G = { v0, e1, e2, nrm, T };
+    const orc_geom G = { v0, e1, e2, nrm, T, shininess };
     orc_stats st; memset(&st, 0, sizeof st);
     double Ft[3] = { 0, 0, 0 }, Qt[3] = { 0, 0, 0 };
     const orc_v3 xc = orc_mk(0.0, 0.0, 0.0);
@@ -364,3 +421,10 @@ void srp_oracle_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
     orc_philox4x32_10(ctr, key, out);
 }
 double srp_oracle_uniform(uint32_t x) { return orc_uniform(x); }
+
+int srp_oracle_thermal(const float *verts, const float *mats, long T, int k, const float *facet_power,
+                       long long N, int B, unsigned long long seed, const orc_options *opt,
+                       double *F, double *sumsq, orc_stats *stats)
+{
+    return srp_oracle_thermal_glossy(verts, mats, NULL, T, k, facet_power, N, B, seed, opt, F, sumsq, stats);
+}

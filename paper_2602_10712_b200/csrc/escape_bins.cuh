@@ -3,9 +3,13 @@
 #pragma once
 #include <cuda_runtime.h>
 
-constexpr int ESC_GRID = 6;
+#ifndef ESC_GRID_DEF
+#define ESC_GRID_DEF 6
+#endif
+constexpr int ESC_GRID = ESC_GRID_DEF;                  // <= 8: a face's cells fit one 64-bit word while building
 constexpr int ESC_BINS = 6 * ESC_GRID * ESC_GRID;      // 216
 constexpr int ESC_WORDS = (ESC_BINS + 31) / 32;         // 7 words per side; 2 sides per triangle
+constexpr unsigned long long ESC_CELLS = ESC_GRID == 8 ? ~0ULL : (1ULL << ((ESC_GRID * ESC_GRID) & 63)) - 1ULL;
 
 // bin of direction d (any length > 0): face = 2 * major axis + (negative ? 1 : 0), cell from the other two
 // coordinates over |major| in axis order.

@@ -95,7 +95,7 @@ __device__ __forceinline__ void mark_cone(const BinTable &B, float3 a, float sin
             // angle(a, centre_b) <= alpha + beta_b  <=>  dot >= cos(alpha + beta_b)   (alpha <= pi/2, beta < pi/4)
             h0 = a.x * B.cx[b] + a.y * B.cy[b] + a.z * B.cz[b] >= cosa * B.cosb[b] - sina * B.sinb[b];
         }
-        if (lane < ESC_GRID * ESC_GRID - 32) {
+        if (lane < ESC_GRID * ESC_GRID - 32) {   // (compile-time grid: at most 32 more cells)
             const int b = face * ESC_GRID * ESC_GRID + 32 + lane; // cells 32..35
             h1 = a.x * B.cx[b] + a.y * B.cy[b] + a.z * B.cz[b] >= cosa * B.cosb[b] - sina * B.sinb[b];
         }
@@ -193,7 +193,7 @@ escape_mask_kernel(const DesignsDev dz, unsigned *esc)
         __syncwarp();
         if (++visits > ESC_MAX_VISITS) { giveup = true; break; }
         if ((visits & 31) == 0) {                                   // a side whose mask is full has nothing to gain
-            const unsigned long long cells = (1ULL << (ESC_GRID * ESC_GRID)) - 1ULL;
+            const unsigned long long cells = ESC_CELLS;
             bool fp_ = true, fm_ = true;
 #pragma unroll
             for (int w = 0; w < 6; ++w) { fp_ = fp_ && (M.p[w] & cells) == cells; fm_ = fm_ && (M.m[w] & cells) == cells; }
@@ -298,7 +298,7 @@ escape_mask_kernel(const DesignsDev dz, unsigned *esc)
                     const float sina = (rf + rt) * 1.0002f / dist;
                     if (!(fp || fm)) continue;
                     {   // nothing to add if this lane's masks of the sides that see f are full already
-                        const unsigned long long cells = (1ULL << (ESC_GRID * ESC_GRID)) - 1ULL;
+                        const unsigned long long cells = ESC_CELLS;
                         bool fullp = true, fullm = true;
 #pragma unroll
                         for (int w = 0; w < 6; ++w) { fullp = fullp && (M.p[w] & cells) == cells; fullm = fullm && (M.m[w] & cells) == cells; }
@@ -320,16 +320,17 @@ escape_mask_kernel(const DesignsDev dz, unsigned *esc)
     if (!live) return;
     // pack: bit (face * 36 + cell) of the 216-bit mask of each side
     unsigned *out = esc + (size_t)(tbase + t) * (2 * ESC_WORDS);
-    unsigned wp[ESC_WORDS + 1], wm[ESC_WORDS + 1];
+    unsigned wp[ESC_WORDS + 2], wm[ESC_WORDS + 2];
 #pragma unroll
-    for (int w = 0; w <= ESC_WORDS; ++w) wp[w] = wm[w] = 0u;
+    for (int w = 0; w < ESC_WORDS + 2; ++w) wp[w] = wm[w] = 0u;
 #pragma unroll
     for (int face = 0; face < 6; ++face) {
         const int pos = face * ESC_GRID * ESC_GRID, w0 = pos >> 5, sh = pos & 31;
-        const unsigned long long cells = (1ULL << (ESC_GRID * ESC_GRID)) - 1ULL;
-        const unsigned long long a = (M.p[face] & cells) << sh, b = (M.m[face] & cells) << sh;   // 36 + sh <= 56 bits
-        wp[w0] |= (unsigned)a; wp[w0 + 1] |= (unsigned)(a >> 32);
-        wm[w0] |= (unsigned)b; wm[w0 + 1] |= (unsigned)(b >> 32);
+        const unsigned long long cells = ESC_CELLS;
+        const unsigned long long a = M.p[face] & cells, b = M.m[face] & cells;
+        wp[w0] |= (unsigned)(a << sh); wm[w0] |= (unsigned)(b << sh);
+        if (w0 + 1 <= ESC_WORDS) { wp[w0 + 1] |= (unsigned)(a >> (32 - sh)); wm[w0 + 1] |= (unsigned)(b >> (32 - sh)); }
+        if (sh != 0 && w0 + 2 <= ESC_WORDS) { wp[w0 + 2] |= (unsigned)(a >> (64 - sh)); wm[w0 + 2] |= (unsigned)(b >> (64 - sh)); }
     }
 #pragma unroll
     for (int w = 0; w < ESC_WORDS; ++w) { out[w] = all ? 0xffffffffu : wp[w]; out[ESC_WORDS + w] = all ? 0xffffffffu : wm[w]; }

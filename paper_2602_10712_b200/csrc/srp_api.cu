@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include "srp_internal.cuh"
+#include "escape_bins.cuh"
 
 namespace {
 
@@ -105,7 +106,7 @@ srp_status ensure_masks(srp_context *ctx, const srp_designs *dz, double rays)
     if (ctx->opt.escape_masks == 1 && rays < 32768.0 * (double)d->sumT) return SRP_OK;
     unsigned *esc = nullptr;
     float4 *nplane = nullptr;
-    if (cudaMallocAsync(&esc, sizeof(unsigned) * 14 * d->sumT, ctx->stream) != cudaSuccess ||
+    if (cudaMallocAsync(&esc, sizeof(unsigned) * 2 * ESC_WORDS * d->sumT, ctx->stream) != cudaSuccess ||
         cudaMallocAsync(&nplane, sizeof(float4) * 2 * d->sumT, ctx->stream) != cudaSuccess) {
         cudaGetLastError();                                   // no room: trace without masks
         if (esc) cudaFreeAsync(esc, ctx->stream);
