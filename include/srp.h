@@ -165,6 +165,18 @@ srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *designs
                                     unsigned long long seed, const float *x_com, float *out_forces,
                                     float *out_torques);
 
+/* Glossy specular lobes, PAPER.md:148 (meshes carry "per-face Phong material parameters"); R23.
+ * shininess DEVICE float[sumT], ORIGINAL triangle order of all designs back to back (tri_offsets of
+ * srp_designs_info): the Phong exponent n of each facet's specular part.  n >= 0: a photon that draws the specular
+ * lobe leaves in a direction distributed as cos^n about the mirror direction (importance-sampled; directions below
+ * the facet's horizon are redrawn, at most 8 times); n < 0: the ideal mirror, which is also what every facet is
+ * while no shininess is set.  NULL removes the array.  The values are copied (reordered) on the context's stream;
+ * they apply to every later srp_forces* / srp_thermal_forces / srp_path_signatures call on this handle.  With the
+ * expected-value deposit a glossy facet's specular momentum is deposited per drawn direction (its mean has no
+ * closed form under the horizon cut), the absorbed and diffuse parts in expectation as before.
+ * SRP_ERR_INVALID on a null handle.  Enqueues only. */
+srp_status srp_designs_set_shininess(srp_context *ctx, srp_designs *designs, const float *shininess);
+
 /* Thermal (local Lambertian) emitters, PAPER.md:606-612 (Sec. 5.9: "local sources [are handled] in the same way
  * ... thermal emission as Lambertian", recoil 2/3 of a collimated beam); R22.
  * facet_power DEVICE float[sumT] in watts, ORIGINAL triangle order of all designs back to back (tri_offsets of

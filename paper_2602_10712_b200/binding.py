@@ -51,7 +51,7 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_family_n_params", "srp_family_tri_count", "srp_build_designs",
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
-           "srp_forces_torques", "srp_forces_torques_pairs", "srp_thermal_forces",
+           "srp_forces_torques", "srp_forces_torques_pairs", "srp_thermal_forces", "srp_designs_set_shininess",
            "srp_first_hits", "srp_path_signatures", "srp_get_stats", "srp_probe_peaks"]
 
 _lib = None
@@ -88,6 +88,7 @@ def load_library():
     L.srp_forces_torques.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp, vp]
     L.srp_forces_torques_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp, vp]
     L.srp_thermal_forces.argtypes = [vp, vp, vp, ll, ci, ull, vp]
+    L.srp_designs_set_shininess.argtypes = [vp, vp, vp]
     L.srp_first_hits.argtypes = [vp, vp, vp, ci, vp, ll, ll, ull, ci, vp]
     L.srp_path_signatures.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_get_stats.argtypes = [vp, ctypes.POINTER(srp_stats)]
@@ -249,6 +250,18 @@ class Context:
                                                       T.data_ptr()))
         self.stream.synchronize()
         return F, T
+
+    def srp_designs_set_shininess(self, designs, shininess):
+        """shininess: float32 [sumT] Phong exponents in original triangle order (< 0 = ideal mirror), or None to
+        remove them (R23)."""
+        if shininess is None:
+            self._check(self.lib.srp_designs_set_shininess(self.handle, designs.handle, None))
+            return
+        sh = torch.as_tensor(shininess).to(device=self.device, dtype=torch.float32).contiguous()
+        if sh.numel() != int(designs.tri_offsets[-1]):
+            raise ValueError("shininess must have one entry per triangle of the batch")
+        self._check(self.lib.srp_designs_set_shininess(self.handle, designs.handle, sh.data_ptr()))
+        self.stream.synchronize()          # sh may be a temporary
 
     def srp_thermal_forces(self, designs, facet_power, rays_per_facet, max_bounces, seed=0):
         """facet_power: float32 [sumT] watts in original triangle order (signed: emitting side); returns CUDA

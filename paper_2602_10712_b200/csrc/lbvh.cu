@@ -353,6 +353,23 @@ cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream)
     return e;
 }
 
+// Shininess (R23) comes in the caller's triangle order; the trace kernels index triangles by sorted position.
+__global__ void __launch_bounds__(256)
+gather_shininess_kernel(const DesignsDev dz, long long sumT, const float *__restrict__ shin_orig, float *__restrict__ shin_sorted)
+{
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= sumT) return;
+    const int k = find_design(dz.tri_off, dz.D, g);
+    shin_sorted[g] = shin_orig[dz.tri_off[k] + dz.perm[g]];
+}
+
+cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted,
+                                        cudaStream_t stream)
+{
+    gather_shininess_kernel<<<(unsigned)((sumT + 255) / 256), 256, 0, stream>>>(dz, sumT, shin_orig, shin_sorted);
+    return cudaGetLastError();
+}
+
 // Per-node plane slabs for the escape masks (built lazily with them, srp_api.cu).
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream)
 {

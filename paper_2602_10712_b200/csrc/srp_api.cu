@@ -28,7 +28,7 @@ srp_status cuda_fail(srp_context *ctx, const char *what, cudaError_t e)
 // design arrays come from the device's stream-ordered pool (no device-wide synchronisation per build)
 void free_designs_mem(srp_context *ctx, srp_designs *d)
 {
-    void *ptrs[9] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm, d->esc, d->nplane };
+    void *ptrs[10] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm, d->esc, d->nplane, d->shin };
     for (void *q : ptrs)
         if (q) cudaFreeAsync(q, ctx->stream);
 }
@@ -362,6 +362,21 @@ srp_status srp_designs_read_bvh(srp_context *ctx, const srp_designs *dz, int des
     if (nodes_host && nn > 0)
         TRY_CUDA(ctx, cudaMemcpy(nodes_host, dz->nodes + 4 * b, sizeof(float4) * 4 * nn, cudaMemcpyDeviceToHost), "read nodes");
     if (perm_host) TRY_CUDA(ctx, cudaMemcpy(perm_host, dz->perm + b, sizeof(int) * T, cudaMemcpyDeviceToHost), "read perm");
+    return SRP_OK;
+}
+
+srp_status srp_designs_set_shininess(srp_context *ctx, srp_designs *dz, const float *shininess)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!dz) return fail(ctx, SRP_ERR_INVALID, "null designs handle");
+    cudaSetDevice(ctx->device);
+    if (!shininess) {                                  // back to ideal mirrors
+        if (dz->shin) cudaFreeAsync(dz->shin, ctx->stream);
+        dz->shin = nullptr;
+        return SRP_OK;
+    }
+    if (!dz->shin) TRY_CUDA(ctx, cudaMallocAsync(&dz->shin, sizeof(float) * dz->sumT, ctx->stream), "alloc shininess");
+    TRY_CUDA(ctx, srp_launch_gather_shininess(dz->dev(), dz->sumT, shininess, dz->shin, ctx->stream), "shininess gather");
     return SRP_OK;
 }
 

@@ -26,6 +26,7 @@ struct DesignsDev {
     const float4 *box;        // [D * 2]: (lo, -), (hi, -)
     const int *perm;          // [sumT]: sorted position -> original index within the design
     const unsigned *esc;      // [sumT * 14]: escape masks (escape_mask.cu), or nullptr
+    const float *shin;        // [sumT] sorted order: Phong exponent of the specular lobe (R23), or nullptr = ideal mirrors
     const float4 *nplane;     // [sumT * 2]: per-node plane slab (n, dmin), (dmax) -- lbvh.cu; with esc
     int D;
     int has_bvh;
@@ -45,11 +46,12 @@ struct srp_designs {
     int *perm = nullptr;
     unsigned *esc = nullptr;
     float4 *nplane = nullptr;
+    float *shin = nullptr;
     bool esc_failed = false;  // the mask allocation failed once: do not try again
     bool has_bvh = false;
     DesignsDev dev() const {
         DesignsDev d;
-        d.tri = tri; d.nodes = nodes; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.esc = esc; d.nplane = nplane; d.D = D;
+        d.tri = tri; d.nodes = nodes; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.esc = esc; d.nplane = nplane; d.shin = shin; d.D = D;
         d.has_bvh = has_bvh ? 1 : 0;
         return d;
     }
@@ -111,6 +113,7 @@ cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_par
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
                                 cudaStream_t stream);
 cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream);
+cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted, cudaStream_t stream);
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream);
 cudaError_t srp_launch_escape_masks(const DesignsDev &dz, long long maxT, unsigned *esc, cudaStream_t stream);
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms,

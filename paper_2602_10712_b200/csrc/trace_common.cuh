@@ -273,15 +273,44 @@ struct BeamCounters {       // rays resolved per beam level (lane-distributed co
 
 // O-steps 5-7 at a hit: deposit, lobe selection, continuation.
 // Returns SHADE_CONTINUE if the photon goes on (o, d, src, depth updated), else how it ended.
+// R23: one direction of the Phong lobe cos^ns about refl, for a facet with facing normal nf and first-edge tangent
+// tu; directions below the facet's horizon are redrawn (attempt a >= 1: words 1, 2 of Philox(i, j, k, cword | a << 8)),
+// after 8 rejections the photon takes refl.  Not inlined: facets without shininess never come here.
+__device__ __noinline__ float3 phong_direction(const float ns, const float3 nf, const float3 refl, const float3 tu,
+                                               float z1, float z2, const uint32_t i, const uint32_t j, const uint32_t k,
+                                               const uint32_t cword, const uint32_t key0, const uint32_t key1)
+{
+    const float3 tv = cross3(nf, tu), kx = cross3(nf, refl);
+    const float icc = 1.0f / (1.0f + dot3(nf, refl));
+    for (int a = 0; a < 8; ++a) {
+        if (a > 0) {
+            uint32_t w0, w1, w2, w3;
+            philox4(i, j, k, cword | ((uint32_t)a << 8), key0, key1, w0, w1, w2, w3);
+            z1 = uniform23(w1); z2 = uniform23(w2);
+        }
+        const float ct = powf(z2, 1.0f / (ns + 1.0f)), st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
+        float sn, cs;
+        sincospif(2.0f * z1, &sn, &cs);
+        const float lx = st * cs, ly = st * sn;
+        const float3 L = f3(fmaf(lx, tu.x, fmaf(ly, tv.x, ct * nf.x)), fmaf(lx, tu.y, fmaf(ly, tv.y, ct * nf.y)),
+                            fmaf(lx, tu.z, fmaf(ly, tv.z, ct * nf.z)));
+        const float3 kL = cross3(kx, L), kkL = cross3(kx, kL);
+        const float3 c = f3(L.x + kL.x + kkL.x * icc, L.y + kL.y + kkL.y * icc, L.z + kL.z + kkL.z * icc);
+        if (dot3(c, nf) > 0.0f) return c;
+    }
+    return refl;
+}
+
 enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2, SHADE_ESCAPES = 3 };   // ESCAPES: goes on, but the
 // escape mask of the facet (escape_mask.cu) shows that its next segment cannot hit anything
 // CFLAG is OR-ed into the Philox counter word that holds the depth: 0 for sun photons, 0x80000000 for photons of
 // thermal emitters (R22), so the two families draw from disjoint streams.
-template <bool TORQUE, uint32_t CFLAG = 0u>
+template <bool TORQUE, uint32_t CFLAG = 0u, bool GLOSSY = false>
 __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
                                       const int deposit, float3 &o, float3 &d, int &src, int &depth,
-                                      float3 &acc, float3 &acc_t, const unsigned *esc = nullptr, long long gidx = 0)
+                                      float3 &acc, float3 &acc_t, const unsigned *esc = nullptr, long long gidx = 0,
+                                      const float *shin = nullptr)
 {
     (void)q0;
     // every deposit of this hit is made at the hit point x; Eq. 4: torque += (x - x_COM) x deposit
@@ -301,9 +330,14 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     const float3 nf = nd > 0.0f ? f3(-n.x, -n.y, -n.z) : n;      // facets are two-sided (R6)
     const float cost = fabsf(nd);
     const float3 refl = f3(fmaf(2.0f * cost, nf.x, d.x), fmaf(2.0f * cost, nf.y, d.y), fmaf(2.0f * cost, nf.z, d.z));
+    // R23: shininess >= 0 = Phong lobe about refl; none, or < 0 = ideal mirror
+    // (GLOSSY is a build of its own, so that the ideal-mirror kernels carry none of this)
+    const float ns = (GLOSSY && shin) ? __ldg(shin + gidx) : -1.0f;
+    const bool glossy = GLOSSY && ns >= 0.0f;
     if (deposit == 0) {                                           // expected-value deposit
-        const float a = al + rs + rd, c = (2.0f / 3.0f) * rd;
-        put(f3(a * d.x - rs * refl.x - c * nf.x, a * d.y - rs * refl.y - c * nf.y, a * d.z - rs * refl.z - c * nf.z));
+        const float rsm = glossy ? 0.0f : rs;                     // a glossy specular part is deposited when drawn
+        const float a = al + rsm + rd, c = (2.0f / 3.0f) * rd;
+        put(f3(a * d.x - rsm * refl.x - c * nf.x, a * d.y - rsm * refl.y - c * nf.y, a * d.z - rsm * refl.z - c * nf.z));
     }
     uint32_t y0, y1, y2, y3;
     philox4(i, g.j, g.k, (uint32_t)(depth + 1) | CFLAG, g.key0, g.key1, y0, y1, y2, y3);
@@ -312,8 +346,14 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     if (z0 < al) {                                                // absorbed
         if (deposit == 1) put(d);
         return SHADE_ABSORBED;
-    } else if (z0 < al + rs) {                                    // ideal mirror (R3)
+    } else if (z0 < al + rs) {                                    // ideal mirror (R3), or the Phong lobe about it
         dn = refl;
+        if (glossy) {
+            const float ie = rsqrtf(q1.x * q1.x + q1.y * q1.y + q1.z * q1.z);
+            dn = phong_direction(ns, nf, refl, f3(q1.x * ie, q1.y * ie, q1.z * ie), uniform23(y1), uniform23(y2), i, g.j, g.k,
+                                 (uint32_t)(depth + 1) | CFLAG, g.key0, g.key1);
+            if (deposit == 0) put(f3(d.x - dn.x, d.y - dn.y, d.z - dn.z));
+        }
     } else {                                                      // Lambertian: cosine-weighted about nf
         const float z1 = uniform23(y1), z2 = uniform23(y2);
         float sn, cs;
@@ -482,11 +522,15 @@ int blocks_per_sm(K kernel)
     return per_sm;
 }
 
-// Three builds of each trace kernel: plain, instrumented (test counters, path signatures), and with torque
-// accumulation.  Instrumented torque runs are refused by the caller (srp_api.cu).
+// Builds of each trace kernel: plain, instrumented (test counters, path signatures), and with torque
+// accumulation -- each also with glossy specular lobes (R23), used when the designs carry
+// shininess.  Instrumented torque runs are refused by the caller (srp_api.cu).
+#define SRP_LAUNCH_G(K_, I_, T_, ...)                                                                     \
+    (a.dz.shin ? launch_persistent(K_<__VA_ARGS__ I_, T_, true>, a, num_sms, stream)                      \
+               : launch_persistent(K_<__VA_ARGS__ I_, T_, false>, a, num_sms, stream))
 #define SRP_LAUNCH3(K_, ...)                                                                              \
-    (instrumented ? launch_persistent(K_<__VA_ARGS__ true, false>, a, num_sms, stream)                       \
-                  : a.torque ? launch_persistent(K_<__VA_ARGS__ false, true>, a, num_sms, stream)            \
-                             : launch_persistent(K_<__VA_ARGS__ false, false>, a, num_sms, stream))
+    (instrumented ? SRP_LAUNCH_G(K_, true, false, __VA_ARGS__)                                            \
+                  : a.torque ? SRP_LAUNCH_G(K_, false, true, __VA_ARGS__)                                 \
+                             : SRP_LAUNCH_G(K_, false, false, __VA_ARGS__))
 
 } // namespace

@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(256) thermal_list_kernel(const float *power, c
     if (power[base + dz.perm[g]] != 0.0f) emit_list[atomicAdd(n_emit, 1)] = (int)g;
 }
 
-template <bool BVH>
+template <bool BVH, bool GLOSSY>
 __global__ void __launch_bounds__(TRACE_THREADS, 8)
 thermal_trace_kernel(const TraceArgs a, const ThermalArgs h)
 {
@@ -157,8 +157,8 @@ thermal_trace_kernel(const TraceArgs a, const ThermalArgs h)
                     if (depth == 0) cn.pmiss++; else cn.escaped++;
                 } else {
                     atomicAdd(&s_hist[warp][depth], 1u);
-                    fate = shade<false, THERMAL_FLAG>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2),
-                                                      tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best);
+                    fate = shade<false, THERMAL_FLAG, GLOSSY>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2),
+                                                      tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best, a.dz.shin);
                     if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
@@ -203,11 +203,18 @@ cudaError_t srp_launch_thermal(const TraceArgs &a, const float *facet_power, lon
     thermal_list_kernel<<<(unsigned)((sumT + 255) / 256), 256, 0, stream>>>(facet_power, a.dz, sumT, emit_list, n_emit);
     ThermalArgs h;
     h.power = facet_power; h.emit_list = emit_list; h.n_emit = n_emit; h.design_power = design_power;
-    int per_sm = a.dz.has_bvh ? blocks_per_sm(thermal_trace_kernel<true>) : blocks_per_sm(thermal_trace_kernel<false>);
+    const bool gl = a.dz.shin != nullptr;
+    int per_sm = a.dz.has_bvh ? (gl ? blocks_per_sm(thermal_trace_kernel<true, true>) : blocks_per_sm(thermal_trace_kernel<true, false>))
+                              : (gl ? blocks_per_sm(thermal_trace_kernel<false, true>) : blocks_per_sm(thermal_trace_kernel<false, false>));
     if (per_sm < 1) per_sm = 1;
     const unsigned blocks = (unsigned)(num_sms * per_sm);             // persistent; the item count lives on the device
-    if (a.dz.has_bvh) thermal_trace_kernel<true><<<blocks, TRACE_THREADS, 0, stream>>>(a, h);
-    else thermal_trace_kernel<false><<<blocks, TRACE_THREADS, 0, stream>>>(a, h);
+    if (a.dz.has_bvh) {
+        if (gl) thermal_trace_kernel<true, true><<<blocks, TRACE_THREADS, 0, stream>>>(a, h);
+        else thermal_trace_kernel<true, false><<<blocks, TRACE_THREADS, 0, stream>>>(a, h);
+    } else {
+        if (gl) thermal_trace_kernel<false, true><<<blocks, TRACE_THREADS, 0, stream>>>(a, h);
+        else thermal_trace_kernel<false, false><<<blocks, TRACE_THREADS, 0, stream>>>(a, h);
+    }
     thermal_finalize_kernel<<<(a.dz.D + 255) / 256, 256, 0, stream>>>(a, design_power, out_forces);
     return cudaGetLastError();
 }

@@ -898,3 +898,110 @@ def test_escape_masks_see_a_plate_hovering_above_the_emitter(ctx, gap):
     assert st["launched"] == len(lower) << 10
     assert st["absorbed"] >= (1.0 - 4 * gap) * st["launched"]
     assert np.abs(res[2][0] - res[0][0]).max() <= 2e-6 * np.abs(res[0][0]).max() + 1e-30
+
+
+# ---------------------------------------------------------------- glossy specular lobes (R23)
+def _glossy_cases():
+    """(name, verts, mats, offsets, shininess): small designs (no hierarchy), a sphere and the open room (hierarchy,
+    many bounces), every facet with its own exponent from {mirror, 0, 3, 40, 800}."""
+    rng = np.random.default_rng(21)
+    out = {}
+    th = W.draw_params(W.FAMILY_BOXWING, 3)
+    out["boxwing"] = (W.FAMILY_BOXWING, th)
+    room = _mask_meshes()["room"]
+    out["room"] = (room, np.tile(np.array([[0.15, 0.7, 0.15]], np.float32), (len(room), 1)))
+    sph = W.icosphere(3, 1.0)
+    out["sphere"] = (sph, W.dirichlet_materials(len(sph), 2))
+    return out, rng
+
+
+@pytest.mark.parametrize("deposit", [0, 1])
+@pytest.mark.parametrize("name,mode", [("boxwing", 0), ("boxwing", 1), ("room", 1), ("room", 2), ("sphere", 2)])
+def test_glossy_forces_match_oracle(ctx, oracle, name, mode, deposit):
+    cases, rng = _glossy_cases()
+    if name == "boxwing":
+        family, th = cases[name]
+        dz = ctx.srp_build_designs(family, th)
+        meshes = {k: oracle.build_mesh(family, th[k], k=k) for k in range(len(th))}
+    else:
+        verts, mats = cases[name]
+        dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
+        meshes = {0: (verts, mats)}
+    sumT = int(dz.tri_offsets[-1])
+    sh = rng.choice([-1.0, 0.0, 3.0, 40.0, 800.0], sumT).astype(np.float32)
+    ctx.srp_designs_set_shininess(dz, sh)
+    sun = W.fibonacci_sphere(5)
+    pairs = np.array([[k, j] for k in range(dz.D) for j in range(5)], np.int32)
+    N, B = 1 << 12, 5
+    ctx.srp_set_options(primary_mode=mode, deposit=deposit, escape_masks=2)
+    try:
+        F, st = run_pairs(ctx, dz, sun, pairs, N, B, seed=8)
+        psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, B, 8).cpu().numpy().astype(np.uint64)
+    finally:
+        ctx.srp_set_options()
+    Fo = np.zeros((len(pairs), 3)); sig = np.zeros(len(pairs)); n_div = np.zeros(len(pairs), int)
+    ost = None
+    for q, (k, j) in enumerate(pairs):
+        v, m = meshes[int(k)]
+        off = int(dz.tri_offsets[k])
+        r = oracle.forces(v, m, sun[j:j + 1], N, B, seed=8, k=int(k), j0=int(j), deposit=deposit, want_path_sig=True,
+                          shininess=sh[off:off + len(v)])
+        Fo[q], sig[q] = r["F"][0], r["sigma"][0]
+        n_div[q] = int((psig[q] != r["path_sig"][0]).sum())
+        ost = r["stats"] if ost is None else {kk: (vv + r["stats"][kk] if not isinstance(vv, list) else
+                                                   [a + b for a, b in zip(vv, r["stats"][kk])]) for kk, vv in ost.items()}
+    print(name, "mode", mode, "deposit", deposit, "divergent rays", int(n_div.sum()), "of", N * len(pairs))
+    assert n_div.sum() <= 3e-4 * N * len(pairs) + 2
+    assert_parity(F, Fo, sig, diverged=n_div > 0, tol_agg=1e-3 if n_div.sum() == 0 else 5e-3)
+    counters_close(st, ost, tol=4 * int(n_div.sum()) + 2)
+    # removing the shininess restores the mirrors
+    ctx.srp_designs_set_shininess(dz, None)
+    ctx.srp_set_options(primary_mode=mode, deposit=deposit)
+    try:
+        F0, _ = run_pairs(ctx, dz, sun, pairs[:3], N, B, seed=8)
+    finally:
+        ctx.srp_set_options()
+    for q, (k, j) in enumerate(pairs[:3]):
+        v, m = meshes[int(k)]
+        r = oracle.forces(v, m, sun[j:j + 1], N, B, seed=8, k=int(k), j0=int(j), deposit=deposit)
+        assert rel_l2(F0[q], r["F"][0]).max() < 1e-3
+    dz.free()
+
+
+def test_glossy_closed_forms_on_gpu(ctx):
+    """G1 / G3 through the CUDA path: mean cosine (n+1)/(n+2) at normal incidence, lobe axis at 50 degrees."""
+    verts = quad([-0.5, -0.5, 0], [1, 0, 0], [0, 1, 0])
+    dz = ctx.srp_build_designs_from_meshes(verts, const_mats(2, 0.0, 1.0, 0.0), [0, 2])
+    for ns in (0.0, 10.0):
+        ctx.srp_designs_set_shininess(dz, [ns, ns])
+        F = ctx.srp_forces(dz, cuda(np.array([[0, 0, 1]], np.float32)), 1 << 18, 1, 0).cpu().numpy()[0, 0]
+        Fc = np.array([0, 0, -P0 * (1.0 + (ns + 1.0) / (ns + 2.0))])
+        assert np.linalg.norm(F - Fc) < 4e-3 * P0, (ns, F, Fc)
+    th = np.radians(50.0)
+    om = np.array([np.sin(th) * np.cos(0.7), np.sin(th) * np.sin(0.7), np.cos(th)])
+    refl = -om + 2 * np.cos(th) * np.array([0, 0, 1.0])
+    ctx.srp_designs_set_shininess(dz, [400.0, 400.0])
+    F = ctx.srp_forces(dz, cuda(om[None].astype(np.float32)), 1 << 18, 1, 0).cpu().numpy()[0, 0]
+    Fc = P0 * np.cos(th) * (-om - (401.0 / 402.0) * refl)
+    assert np.linalg.norm(F - Fc) < 2e-3 * np.linalg.norm(Fc)
+    dz.free()
+
+
+def test_glossy_thermal_matches_oracle(ctx, oracle):
+    th = W.draw_params(W.FAMILY_BOXWING6, 2)
+    dz = ctx.srp_build_designs(W.FAMILY_BOXWING6, th)
+    rng = np.random.default_rng(2)
+    sh = rng.choice([-1.0, 1.0, 25.0], 32).astype(np.float32)
+    power = np.zeros((2, 16), np.float32); power[:, :12] = 40.0
+    ctx.srp_designs_set_shininess(dz, sh)
+    N, B = 1 << 12, 4
+    F = ctx.srp_thermal_forces(dz, power.reshape(-1), N, B, seed=3).cpu().numpy()
+    st = ctx.srp_get_stats()
+    tot = 0
+    for k in range(2):
+        v, m = oracle.build_mesh(W.FAMILY_BOXWING6, th[k], k=k)
+        r = oracle.thermal(v, m, power[k], N, B, seed=3, k=k, shininess=sh[16 * k:16 * k + 16])
+        assert np.linalg.norm(F[k] - r["F"]) <= 4 * r["sigma"] + 1e-4 * np.linalg.norm(r["F"])
+        assert np.linalg.norm(F[k] - r["F"]) <= 2e-3 * np.linalg.norm(r["F"])
+        tot += r["stats"]["segments"]
+    assert abs(st["segments"] - tot) <= 1e-3 * tot
