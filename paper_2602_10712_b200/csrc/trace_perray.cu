@@ -110,7 +110,9 @@ trace_kernel(const TraceArgs a)
 // Mixing the two kinds in one pass left the short secondaries waiting for the long primaries
 // (14 of 32 lanes active, profiles/ round 1); this is S6's "compaction between bounces".
 
-template <bool INSTR, bool TORQUE, bool GLOSSY>
+// MASKS: the designs carry escape masks (a build of its own: the lookup's branch costs the sail 2.8 % when it is
+// only a run-time null test -- 603.9 against 620.9 ms, profiles/r1d_escape_masks.md).
+template <bool MASKS, bool INSTR, bool TORQUE, bool GLOSSY>
 __global__ void __launch_bounds__(TRACE_THREADS, 8)
 bvh_trace_kernel(const TraceArgs a)
 {
@@ -184,7 +186,7 @@ bvh_trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
                     fate = shade<TORQUE, 0u, GLOSSY>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
-                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best, a.dz.shin);
+                                 best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, MASKS ? a.dz.esc : nullptr, tbase + best, a.dz.shin);
                     if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
@@ -265,7 +267,7 @@ __global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArg
 
 int srp_perray_blocks_per_sm(bool brute)
 {
-    return brute ? blocks_per_sm(trace_kernel<MODE_BRUTE_SMEM, false, false, false>) : blocks_per_sm(bvh_trace_kernel<false, false, false>);
+    return brute ? blocks_per_sm(trace_kernel<MODE_BRUTE_SMEM, false, false, false>) : blocks_per_sm(bvh_trace_kernel<false, false, false, false>);
 }
 
 // mode: MODE_BVH (0 is BRUTE_SMEM, 1 BVH, 2 BRUTE_GLOBAL -- the enum of trace_common.cuh)
@@ -273,7 +275,7 @@ cudaError_t srp_launch_perray(const TraceArgs &a, int mode, bool instrumented, i
 {
     if (mode == MODE_BRUTE_GLOBAL) return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_GLOBAL,);
     if (mode == MODE_BRUTE_SMEM) return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_SMEM,);
-    return SRP_LAUNCH3(bvh_trace_kernel);
+    return a.dz.esc ? SRP_LAUNCH3(bvh_trace_kernel, true,) : SRP_LAUNCH3(bvh_trace_kernel, false,);
 }
 
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream)
