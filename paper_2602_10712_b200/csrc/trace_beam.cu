@@ -150,7 +150,7 @@ struct BeamSmem {                   // per warp; beam structures and drain struc
     } u;
 };
 
-template <bool INSTR, bool TORQUE, bool GLOSSY>
+template <bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
 __global__ void __launch_bounds__(TRACE_THREADS, BEAM_BLOCKS_PER_SM)
 beam_trace_kernel(const TraceArgs a)
 {
@@ -215,7 +215,7 @@ beam_trace_kernel(const TraceArgs a)
             atomicAdd(&s_hist[warp][depth], 1u);
             if (INSTR) sig = hsig[e] * 1000003ULL + (unsigned long long)(a.dz.perm[tb + best] + 1);
             float3 dep = f3(0, 0, 0), dep_t = f3(0, 0, 0);
-            fate = shade<TORQUE, 0u, GLOSSY>(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
+            fate = shade<TORQUE, 0u, GLOSSY, ANALOG ? 1 : 0>(__ldg(lt + 3 * best), __ldg(lt + 3 * best + 1), __ldg(lt + 3 * best + 2), t, best, g, i, a.B,
                          a.deposit, o, d, src, depth, dep, dep_t, a.dz.esc, tb + best, a.dz.shin);
             if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
             if (fate == SHADE_ABSORBED) cn.absorbed++;
@@ -525,7 +525,7 @@ beam_trace_kernel(const TraceArgs a)
                     else {
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                        fate = shade<TORQUE, 0u, GLOSSY>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
+                        fate = shade<TORQUE, 0u, GLOSSY, ANALOG ? 1 : 0>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
                                      best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, a.dz.esc, tbase + best, a.dz.shin);
                         if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
@@ -564,15 +564,15 @@ beam_trace_kernel(const TraceArgs a)
 
 } // namespace
 
-int srp_beam_blocks_per_sm() { return blocks_per_sm(beam_trace_kernel<false, false, false>); }
+int srp_beam_blocks_per_sm() { return blocks_per_sm(beam_trace_kernel<false, false, false, false>); }
 
 // Words of global memory the beam kernel's per-warp ray pools need, and the ring capacity per warp.
 size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *cap_out)
 {
     int per_sm = 0;
-    const int occ[6] = { blocks_per_sm(beam_trace_kernel<true, false, false>), blocks_per_sm(beam_trace_kernel<true, false, true>),
-                         blocks_per_sm(beam_trace_kernel<false, false, false>), blocks_per_sm(beam_trace_kernel<false, false, true>),
-                         blocks_per_sm(beam_trace_kernel<false, true, false>), blocks_per_sm(beam_trace_kernel<false, true, true>) };
+    const int occ[6] = { blocks_per_sm(beam_trace_kernel<true, false, false, false>), blocks_per_sm(beam_trace_kernel<true, false, true, false>),
+                         blocks_per_sm(beam_trace_kernel<false, false, false, false>), blocks_per_sm(beam_trace_kernel<false, false, true, false>),
+                         blocks_per_sm(beam_trace_kernel<false, true, false, false>), blocks_per_sm(beam_trace_kernel<false, true, true, false>) };
     for (int v = instrumented ? 0 : 2; v < (instrumented ? 2 : 6); ++v) if (occ[v] > per_sm) per_sm = occ[v];
     if (per_sm < 1) per_sm = 1;
     int cap = 64;

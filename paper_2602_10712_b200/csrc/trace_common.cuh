@@ -305,13 +305,16 @@ enum { SHADE_CONTINUE = 0, SHADE_ABSORBED = 1, SHADE_CAPPED = 2, SHADE_ESCAPES =
 // escape mask of the facet (escape_mask.cu) shows that its next segment cannot hit anything
 // CFLAG is OR-ed into the Philox counter word that holds the depth: 0 for sun photons, 0x80000000 for photons of
 // thermal emitters (R22), so the two families draw from disjoint streams.
-template <bool TORQUE, uint32_t CFLAG = 0u, bool GLOSSY = false>
+template <bool TORQUE, uint32_t CFLAG = 0u, bool GLOSSY = false, int DEPOSIT = -1>
 __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const float4 q2, const float t,
                                       const int f, const RayGen &g, const uint32_t i, const int B,
-                                      const int deposit, float3 &o, float3 &d, int &src, int &depth,
+                                      const int deposit_, float3 &o, float3 &d, int &src, int &depth,
                                       float3 &acc, float3 &acc_t, const unsigned *esc = nullptr, long long gidx = 0,
                                       const float *shin = nullptr)
 {
+    // DEPOSIT 0 / 1: the deposit rule is fixed at compile time (the sun-photon kernels: +9 % on cfg2 against the
+    // run-time test); -1: taken from the argument
+    const int deposit = DEPOSIT >= 0 ? DEPOSIT : deposit_;
     (void)q0;
     // every deposit of this hit is made at the hit point x; Eq. 4: torque += (x - x_COM) x deposit
     const float3 x = f3(fmaf(t, d.x, o.x), fmaf(t, d.y, o.y), fmaf(t, d.z, o.z));
@@ -524,10 +527,12 @@ int blocks_per_sm(K kernel)
 
 // Builds of each trace kernel: plain, instrumented (test counters, path signatures), and with torque
 // accumulation -- each also with glossy specular lobes (R23), used when the designs carry
-// shininess.  Instrumented torque runs are refused by the caller (srp_api.cu).
+// shininess, and each of those for the expected-value and for the analog deposit rule.  Instrumented torque runs are refused by the caller (srp_api.cu).
+#define SRP_LAUNCH_A(K_, I_, T_, G_, ...)                                                                 \
+    (a.deposit ? launch_persistent(K_<__VA_ARGS__ I_, T_, G_, true>, a, num_sms, stream)                  \
+               : launch_persistent(K_<__VA_ARGS__ I_, T_, G_, false>, a, num_sms, stream))
 #define SRP_LAUNCH_G(K_, I_, T_, ...)                                                                     \
-    (a.dz.shin ? launch_persistent(K_<__VA_ARGS__ I_, T_, true>, a, num_sms, stream)                      \
-               : launch_persistent(K_<__VA_ARGS__ I_, T_, false>, a, num_sms, stream))
+    (a.dz.shin ? SRP_LAUNCH_A(K_, I_, T_, true, __VA_ARGS__) : SRP_LAUNCH_A(K_, I_, T_, false, __VA_ARGS__))
 #define SRP_LAUNCH3(K_, ...)                                                                              \
     (instrumented ? SRP_LAUNCH_G(K_, true, false, __VA_ARGS__)                                            \
                   : a.torque ? SRP_LAUNCH_G(K_, false, true, __VA_ARGS__)                                 \

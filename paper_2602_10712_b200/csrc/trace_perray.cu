@@ -7,7 +7,7 @@
 namespace {
 
 // ---- the persistent trace kernel ----
-template <int MODE, bool INSTR, bool TORQUE, bool GLOSSY>
+template <int MODE, bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
 __global__ void __launch_bounds__(TRACE_THREADS, MODE == MODE_BVH ? 4 : 5)
 trace_kernel(const TraceArgs a)
 {
@@ -87,7 +87,7 @@ trace_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     const float4 *tp = (MODE == MODE_BRUTE_SMEM) ? my_tri + 3 * best : gtri + 3 * best;
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    const int fate = shade<TORQUE, 0u, GLOSSY>(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t,
+                    const int fate = shade<TORQUE, 0u, GLOSSY, ANALOG ? 1 : 0>(tp[0], tp[1], tp[2], tbest, best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t,
                                                    nullptr, tbase + best, a.dz.shin);
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
@@ -112,7 +112,7 @@ trace_kernel(const TraceArgs a)
 
 // MASKS: the designs carry escape masks (a build of its own: the lookup's branch costs the sail 2.8 % when it is
 // only a run-time null test -- 603.9 against 620.9 ms, profiles/r1d_escape_masks.md).
-template <bool MASKS, bool INSTR, bool TORQUE, bool GLOSSY>
+template <bool MASKS, bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
 __global__ void __launch_bounds__(TRACE_THREADS, 8)
 bvh_trace_kernel(const TraceArgs a)
 {
@@ -185,7 +185,7 @@ bvh_trace_kernel(const TraceArgs a)
                 } else {
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
-                    fate = shade<TORQUE, 0u, GLOSSY>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
+                    fate = shade<TORQUE, 0u, GLOSSY, ANALOG ? 1 : 0>(__ldg(gtri + 3 * best), __ldg(gtri + 3 * best + 1), __ldg(gtri + 3 * best + 2), tbest,
                                  best, g, i, a.B, a.deposit, o, d, src, depth, acc, acc_t, MASKS ? a.dz.esc : nullptr, tbase + best, a.dz.shin);
                     if (fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                     if (fate == SHADE_ABSORBED) cn.absorbed++;
@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArg
 
 int srp_perray_blocks_per_sm(bool brute)
 {
-    return brute ? blocks_per_sm(trace_kernel<MODE_BRUTE_SMEM, false, false, false>) : blocks_per_sm(bvh_trace_kernel<false, false, false, false>);
+    return brute ? blocks_per_sm(trace_kernel<MODE_BRUTE_SMEM, false, false, false, false>) : blocks_per_sm(bvh_trace_kernel<false, false, false, false, false>);
 }
 
 // mode: MODE_BVH (0 is BRUTE_SMEM, 1 BVH, 2 BRUTE_GLOBAL -- the enum of trace_common.cuh)
