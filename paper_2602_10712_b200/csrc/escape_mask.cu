@@ -336,6 +336,98 @@ escape_mask_kernel(const DesignsDev dz, unsigned *esc)
     for (int w = 0; w < ESC_WORDS; ++w) { out[w] = all ? 0xffffffffu : wp[w]; out[ESC_WORDS + w] = all ? 0xffffffffu : wm[w]; }
 }
 
+// design of global triangle position g: tri_off[k] <= g < tri_off[k + 1]
+__device__ inline int find_design_of(const long long *off, int D, long long g)
+{
+    int lo = 0, hi = D;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (off[mid] <= g) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// ---- designs without a hierarchy (T <= 64): one warp per triangle t, every other triangle f tested exactly enough.
+// The directions from a point of t to a point of f are the cone over the Minkowski difference f - t, the convex hull
+// of the 9 vertex differences.  A bin of the cube map is the pyramid {d_m >= 0, s0 d_m <= d_s <= s1 d_m,
+// t0 d_m <= d_t <= t1 d_m}; if all 9 differences lie outside one of its 5 planes, so does the whole cone, and the bin
+// stays clear.  Otherwise it is marked (conservative: only the bin's own planes are tried as separators).  Which
+// side of t sees f is decided as in small_beam_kernel's facet-side masks (R20).  Lane l owns bins l, l + 32, ...
+__global__ void __launch_bounds__(128)
+escape_mask_small_kernel(const DesignsDev dz, long long sumT, unsigned *esc)
+{
+    const long long g = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;     // global triangle position
+    const int lane = threadIdx.x & 31;
+    if (g >= sumT) return;
+    const int k = find_design_of(dz.tri_off, dz.D, g);
+    const long long tbase = dz.tri_off[k];
+    const int T = (int)(dz.tri_off[k + 1] - tbase), t = (int)(g - tbase);
+    const float4 *tri = dz.tri + 3 * tbase;
+    const float4 q0 = __ldg(tri + 3 * t), q1 = __ldg(tri + 3 * t + 1), q2 = __ldg(tri + 3 * t + 2);
+    const float3 a[3] = { make_float3(q0.x, q0.y, q0.z), make_float3(q0.x + q1.x, q0.y + q1.y, q0.z + q1.z),
+                          make_float3(q0.x + q2.x, q0.y + q2.y, q0.z + q2.z) };
+    float3 n = make_float3(q1.y * q2.z - q1.z * q2.y, q1.z * q2.x - q1.x * q2.z, q1.x * q2.y - q1.y * q2.x);
+    const float il = rsqrtf(n.x * n.x + n.y * n.y + n.z * n.z);
+    n = make_float3(n.x * il, n.y * il, n.z * il);
+    const float4 blo = dz.box[2 * k], bhi = dz.box[2 * k + 1];
+    const float eps = 1.0e-6f * (fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
+                                 fmaxf(fabsf(blo.z), fabsf(bhi.z)));
+    constexpr int ROUNDS = (ESC_BINS + 31) / 32;
+    unsigned mp[ROUNDS], mm[ROUNDS];                                 // bit r of lane l = bin 32 r + l, front / back side
+#pragma unroll
+    for (int r = 0; r < ROUNDS; ++r) mp[r] = mm[r] = 0u;
+    for (int f = 0; f < T; ++f) {
+        if (f == t) continue;
+        const float4 p0 = __ldg(tri + 3 * f), p1 = __ldg(tri + 3 * f + 1), p2 = __ldg(tri + 3 * f + 2);
+        const float3 b[3] = { make_float3(p0.x, p0.y, p0.z), make_float3(p0.x + p1.x, p0.y + p1.y, p0.z + p1.z),
+                              make_float3(p0.x + p2.x, p0.y + p2.y, p0.z + p2.z) };
+        const float r0 = n.x * (p0.x - q0.x) + n.y * (p0.y - q0.y) + n.z * (p0.z - q0.z);
+        const float d0 = r0, d1 = r0 + n.x * p1.x + n.y * p1.y + n.z * p1.z, d2 = r0 + n.x * p2.x + n.y * p2.y + n.z * p2.z;
+        const bool fp = fmaxf(d0, fmaxf(d1, d2)) > eps, fm = fminf(d0, fminf(d1, d2)) < -eps;
+        if (!fp && !fm) continue;                                    // coplanar with t: never hit from t
+        float3 v[9];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) v[3 * i + j] = make_float3(b[i].x - a[j].x, b[i].y - a[j].y, b[i].z - a[j].z);
+#pragma unroll
+        for (int r = 0; r < ROUNDS; ++r) {
+            const int bin = 32 * r + lane;
+            if (bin >= ESC_BINS) break;
+            const int face = bin / (ESC_GRID * ESC_GRID), cell = bin % (ESC_GRID * ESC_GRID);
+            const int is = cell % ESC_GRID, it = cell / ESC_GRID;
+            const float s0 = -1.0f + 2.0f * is / ESC_GRID, s1 = -1.0f + 2.0f * (is + 1) / ESC_GRID;
+            const float t0 = -1.0f + 2.0f * it / ESC_GRID, t1 = -1.0f + 2.0f * (it + 1) / ESC_GRID;
+            const float sg = (face & 1) ? -1.0f : 1.0f;
+            bool out_m = true, out_s0 = true, out_s1 = true, out_t0 = true, out_t1 = true;
+#pragma unroll
+            for (int c = 0; c < 9; ++c) {
+                // (m, s, t) components in the face's axis order (escape_bins.cuh)
+                const float dm = sg * (face < 2 ? v[c].x : face < 4 ? v[c].y : v[c].z);
+                const float ds = face < 2 ? v[c].y : v[c].x;
+                const float dt = face < 4 ? v[c].z : v[c].y;
+                const float tol = 1.0e-5f * (fabsf(dm) + fabsf(ds) + fabsf(dt));   // bin edges and esc_bin's rounding
+                out_m = out_m && dm <= tol;
+                out_s0 = out_s0 && ds - s0 * dm <= tol;
+                out_s1 = out_s1 && s1 * dm - ds <= tol;
+                out_t0 = out_t0 && dt - t0 * dm <= tol;
+                out_t1 = out_t1 && t1 * dm - dt <= tol;
+            }
+            if (!(out_m || out_s0 || out_s1 || out_t0 || out_t1)) {
+                if (fp) mp[r] |= 1u;
+                if (fm) mm[r] |= 1u;
+            }
+        }
+    }
+    // word w of a side = bins 32 w .. 32 w + 31 = bit of round w from every lane
+    unsigned *out = esc + (size_t)g * (2 * ESC_WORDS);
+#pragma unroll
+    for (int r = 0; r < ROUNDS; ++r) {
+        const unsigned wp = __ballot_sync(FULLW, mp[r] != 0u), wm = __ballot_sync(FULLW, mm[r] != 0u);
+        if (lane == 0 && r < ESC_WORDS) { out[r] = wp; out[ESC_WORDS + r] = wm; }
+    }
+}
+
 } // namespace
 
 cudaError_t srp_launch_escape_masks(const DesignsDev &dz, long long maxT, unsigned *esc, cudaStream_t stream)
@@ -343,5 +435,11 @@ cudaError_t srp_launch_escape_masks(const DesignsDev &dz, long long maxT, unsign
     if (dz.D > 65535) return cudaErrorInvalidValue;                 // grid.y; the caller builds no masks then
     const dim3 grid((unsigned)((maxT + 127) / 128), (unsigned)dz.D);
     escape_mask_kernel<<<grid, 128, 0, stream>>>(dz, esc);
+    return cudaGetLastError();
+}
+
+cudaError_t srp_launch_escape_masks_small(const DesignsDev &dz, long long sumT, unsigned *esc, cudaStream_t stream)
+{
+    escape_mask_small_kernel<<<(unsigned)((sumT + 3) / 4), 128, 0, stream>>>(dz, sumT, esc);
     return cudaGetLastError();
 }

@@ -102,20 +102,25 @@ srp_status ensure_pool(srp_context *ctx, TraceArgs &a, bool brute, bool instrume
 srp_status ensure_masks(srp_context *ctx, const srp_designs *dz, double rays)
 {
     srp_designs *d = const_cast<srp_designs *>(dz);           // a cache inside the handle, not a change of its meaning
-    if (d->esc || d->esc_failed || !d->has_bvh || ctx->opt.escape_masks == 0 || d->D > 65535) return SRP_OK;
+    if (d->esc || d->esc_failed || ctx->opt.escape_masks == 0 || (d->has_bvh && d->D > 65535)) return SRP_OK;
     if (ctx->opt.escape_masks == 1 && rays < 32768.0 * (double)d->sumT) return SRP_OK;
     unsigned *esc = nullptr;
     float4 *nplane = nullptr;
     if (cudaMallocAsync(&esc, sizeof(unsigned) * 2 * ESC_WORDS * d->sumT, ctx->stream) != cudaSuccess ||
-        cudaMallocAsync(&nplane, sizeof(float4) * 2 * d->sumT, ctx->stream) != cudaSuccess) {
+        (d->has_bvh && cudaMallocAsync(&nplane, sizeof(float4) * 2 * d->sumT, ctx->stream) != cudaSuccess)) {
         cudaGetLastError();                                   // no room: trace without masks
         if (esc) cudaFreeAsync(esc, ctx->stream);
         d->esc_failed = true;
         return SRP_OK;
     }
-    d->nplane = nplane;
-    cudaError_t e = srp_launch_node_planes(d->dev(), d->sumT, nplane, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_escape_masks(d->dev(), d->maxT, esc, ctx->stream);
+    cudaError_t e;
+    if (d->has_bvh) {
+        d->nplane = nplane;
+        e = srp_launch_node_planes(d->dev(), d->sumT, nplane, ctx->stream);
+        if (e == cudaSuccess) e = srp_launch_escape_masks(d->dev(), d->maxT, esc, ctx->stream);
+    } else {
+        e = srp_launch_escape_masks_small(d->dev(), d->sumT, esc, ctx->stream);   // T <= 64: every pair of triangles
+    }
     if (e != cudaSuccess) { cudaFreeAsync(esc, ctx->stream); return cuda_fail(ctx, "escape mask build", e); }
     d->esc = esc;
     return SRP_OK;

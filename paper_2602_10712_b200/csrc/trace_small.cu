@@ -50,7 +50,7 @@ __device__ __forceinline__ int small_filter(const float4 *eq, const unsigned cha
     return n;
 }
 
-template <bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
+template <bool MASKS, bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
 __global__ void __launch_bounds__(TRACE_THREADS, 6)
 small_beam_kernel(const TraceArgs a)
 {
@@ -163,8 +163,9 @@ small_beam_kernel(const TraceArgs a)
                     atomicAdd(&s_hist[warp][depth], 1u);
                     if (INSTR) sig = sig * 1000003ULL + (unsigned long long)(a.dz.perm[tbase + best] + 1);
                     fate = shade<TORQUE, 0u, GLOSSY, ANALOG ? 1 : 0>(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
-                                 a.deposit, o, d, src, depth, acc, acc_t, nullptr, tbase + best, a.dz.shin);
-                    if (fate == SHADE_ABSORBED) cn.absorbed++;
+                                 a.deposit, o, d, src, depth, acc, acc_t, MASKS ? a.dz.esc : nullptr, tbase + best, a.dz.shin);
+                    if (MASKS && fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
+                        if (fate == SHADE_ABSORBED) cn.absorbed++;
                     if (fate == SHADE_CAPPED) cn.capped++;
                 }
                 if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[p * a.N + i] = sig;
@@ -260,7 +261,8 @@ small_beam_kernel(const TraceArgs a)
                         atomicAdd(&s_hist[warp][0], 1u);
                         if (INSTR) sig = (unsigned long long)(a.dz.perm[tbase + best] + 1);
                         fate = shade<TORQUE, 0u, GLOSSY, ANALOG ? 1 : 0>(W.tri[3 * best], W.tri[3 * best + 1], W.tri[3 * best + 2], tbest, best, g, i, a.B,
-                                     a.deposit, o, d, src, depth, acc, acc_t, nullptr, tbase + best, a.dz.shin);
+                                     a.deposit, o, d, src, depth, acc, acc_t, MASKS ? a.dz.esc : nullptr, tbase + best, a.dz.shin);
+                        if (MASKS && fate == SHADE_ESCAPES) { cn.segments++; cn.escaped++; cn.mesc++; }
                         if (fate == SHADE_ABSORBED) cn.absorbed++;
                         if (fate == SHADE_CAPPED) cn.capped++;
                     }
@@ -289,9 +291,9 @@ small_beam_kernel(const TraceArgs a)
 
 } // namespace
 
-int srp_small_blocks_per_sm() { return blocks_per_sm(small_beam_kernel<false, false, false, false>); }
+int srp_small_blocks_per_sm() { return blocks_per_sm(small_beam_kernel<false, false, false, false, false>); }
 
 cudaError_t srp_launch_small(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream)
 {
-    return SRP_LAUNCH3(small_beam_kernel);
+    return a.dz.esc ? SRP_LAUNCH3(small_beam_kernel, true,) : SRP_LAUNCH3(small_beam_kernel, false,);
 }

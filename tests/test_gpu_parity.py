@@ -788,7 +788,7 @@ def _mask_meshes():
     return {"sphere": sphere, "room": room.astype(np.float32), "plates": plates.astype(np.float32), "soup": soup}
 
 
-@pytest.mark.parametrize("name", ["sphere", "room", "plates", "soup", "detailed", "sail"])
+@pytest.mark.parametrize("name", ["sphere", "room", "plates", "soup", "detailed", "sail", "boxwing", "boxwing6", "plate"])
 def test_escape_masks_change_no_photon(ctx, name):
     """The masks only say "no triangle lies this way": with them forced on, every photon follows the same path
     (identical signatures) and all photon counters agree; the forces agree to fp32 rounding (a lane that skips a
@@ -801,6 +801,10 @@ def test_escape_masks_change_no_photon(ctx, name):
     elif name == "sail":
         dz = ctx.srp_build_designs(W.FAMILY_SAIL, np.array([[0.8]], np.float32))
         D = 1
+    elif name in ("boxwing", "boxwing6", "plate"):              # no hierarchy: masks from all pairs of triangles
+        fam = {"boxwing": W.FAMILY_BOXWING, "boxwing6": W.FAMILY_BOXWING6, "plate": W.FAMILY_PLATE}[name]
+        D = 1 if name == "plate" else 5
+        dz = ctx.srp_build_designs(fam, W.draw_params(fam, D))
     else:
         verts = _mask_meshes()[name]
         mats = np.tile(np.array([[0.2, 0.5, 0.3]], np.float32), (len(verts), 1))
@@ -832,6 +836,10 @@ def test_escape_masks_change_no_photon(ctx, name):
             assert s2["capped"] + s2["absorbed"] > 0 and sum(s2["hits_at_depth"][2:]) > 0
         if name in ("detailed", "plates"):
             assert s2["mask_escapes"] > 0.3 * s2["escaped"]
+        if name in ("boxwing", "boxwing6") and mode == 2:            # mode 1 is the brute-force kernel: no masks
+            assert s2["mask_escapes"] > 0.5 * s2["escaped"]
+        if name == "plate":
+            assert s2["mask_escapes"] == s2["escaped"] or mode == 1
     dz.free()
 
 
