@@ -1,17 +1,18 @@
 // escape_mask.cu -- per-triangle "escape masks" (part of S1, the per-design build).
 //
-// Most bounce rays leave the spacecraft for good (92 % on the detailed config), yet each one walks the whole
+// Most bounce rays leave the spacecraft for good (91 % on the detailed config), yet each one walks the whole
 // chain of BVH nodes that contain its origin before that is known.  For every triangle t and each of its two
-// sides this kernel marks the direction bins (a 6 x 6 x 6 cube map of the sphere, 216 bins) in which SOME ray
-// that starts on t could hit another triangle; a bounce ray whose direction falls in an unmarked bin escapes,
-// and the tracer counts it as such without a traversal.  The masks are conservative, so no result changes
-// (R20): a triangle f is left out for side s of t only if all its vertices lie behind t's plane or
-// within 1e-6 x the design's extent of it (the fp32 evaluation error of the plane: coplanar neighbours, which exact
-// arithmetic never hits); otherwise
-// every bin that meets the cone of directions from t's bounding sphere to the bounding sphere of f -- or of a
-// whole BVH subtree, once that cone is narrow -- is marked.
+// sides these kernels mark the direction bins (a cube map of the sphere, 6 x 6 cells per face, 216 bins) in which
+// SOME ray that starts on t could hit another triangle; a bounce ray whose direction falls in an unmarked bin
+// escapes, and the tracer counts it as such without a traversal.  The masks are conservative, so no result changes
+// (R20): a triangle f is left out for side s of t only if all its vertices lie behind t's plane or are
+// coplanar with it (within 1e-6 x the design's extent, the fp32 rounding of the vertices, plus 1e-4 rad x the
+// clearance between the two: coplanar neighbours, which exact arithmetic never hits); otherwise every bin that
+// meets the cone of directions from t's bounding sphere to the bounding sphere of f -- or of a whole BVH subtree,
+// once that cone is narrow -- is marked.
 //
-// One warp per cluster of 32 neighbouring triangles, depth-first over the design's BVH2 (see the kernel).
+// Designs with a BVH: one warp per cluster of 32 neighbouring triangles, depth-first over the design's BVH2
+// (escape_mask_kernel).  Designs without (T <= 64): all pairs of triangles (escape_mask_small_kernel).
 #include <cfloat>
 #include "srp_internal.cuh"
 #include "escape_bins.cuh"
@@ -26,12 +27,12 @@ constexpr int ESC_MAX_VISITS = ESC_MAX_VISITS_DEF;      // beyond this the trian
 #ifndef ESC_SIN_DESCEND_DEF
 #define ESC_SIN_DESCEND_DEF 0.25f
 #endif
-constexpr float ESC_SIN_DESCEND = ESC_SIN_DESCEND_DEF;
+constexpr float ESC_SIN_DESCEND = ESC_SIN_DESCEND_DEF;  // subtrees seen under a wider cone than this are opened
 #ifndef ESC_SIN_SHARED_DEF
 #define ESC_SIN_SHARED_DEF 0.8f
 #endif
 constexpr float ESC_SIN_SHARED = ESC_SIN_SHARED_DEF;   // leaf triangles seen from the cluster under a narrower cone share one cone
-constexpr float ESC_ANGLE_EPS = 1.0e-4f;  // a triangle within this angle of the plane (seen from t) counts as coplanar  // subtrees seen under a wider cone than this are opened
+constexpr float ESC_ANGLE_EPS = 1.0e-4f;  // a triangle within this angle of the plane (seen from t) counts as coplanar
 
 struct BinTable {                          // per block, in shared memory
     float cx[ESC_BINS], cy[ESC_BINS], cz[ESC_BINS];   // bin centre directions

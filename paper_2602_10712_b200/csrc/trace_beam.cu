@@ -117,7 +117,10 @@ constexpr int POOL_FIELDS_INSTR = 11;
 #endif
 constexpr int POOL_HIGH = POOL_HIGH_DEF;          // drain when the pool holds at least this many rays
 constexpr int HITQ = 64;                 // queued hits per warp
-constexpr int DRAIN_ACTIVE_MIN = 24;     // leave the traversal loop to refill when fewer lanes are busy
+#ifndef DRAIN_ACTIVE_MIN_DEF
+#define DRAIN_ACTIVE_MIN_DEF 24
+#endif
+constexpr int DRAIN_ACTIVE_MIN = DRAIN_ACTIVE_MIN_DEF;     // leave the traversal loop to refill when fewer lanes are busy
 constexpr uint32_t SRC_NONE = 0x07ffffffu;
 
 struct Pool {

@@ -176,7 +176,10 @@ __device__ __forceinline__ float safe_rcp(float x)
 constexpr int CUR_DONE = 0x7fffffff;
 // "while-while" traversal lets a lane walk nodes until it reaches a leaf while the lanes that already hold one
 // wait.  Capping a node run (and not unrolling it) bounds that wait: cfg3 bounce rays +9 %, per-ray primaries +13 %.
-constexpr int NODE_RUN_CAP = 8;
+#ifndef NODE_RUN_CAP_DEF
+#define NODE_RUN_CAP_DEF 8
+#endif
+constexpr int NODE_RUN_CAP = NODE_RUN_CAP_DEF;
 
 #define SRP_POP(cur_)                                                                     \
     do {                                                                                  \
