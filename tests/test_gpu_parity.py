@@ -696,6 +696,18 @@ def test_cfg3_full_N_consistent_with_reduced_N_oracle(ctx, oracle):
     Fo, sig, _ = oracle_pairs(oracle, meshes, pairs, sun, 1 << 12, cfg.B, seed=cfg.seed, sampler=1)
     err = np.linalg.norm(F[pairs[:, 0], pairs[:, 1]] - Fo, axis=1)
     assert np.all(err <= 4 * sig)
+    # the full job also runs with the escape masks (its photons-per-triangle count is above the rule; this slice is
+    # below it, so they are forced here): same photons, same counters, forces equal to fp32 rounding
+    ctx.srp_set_options(escape_masks=2)
+    try:
+        Fm = ctx.srp_forces(dz, cuda(sun), cfg.N, cfg.B, cfg.seed).cpu().numpy()
+        sm = ctx.srp_get_stats()
+    finally:
+        ctx.srp_set_options()
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "hits_at_depth"):
+        assert sm[key] == st[key], key
+    assert sm["mask_escapes"] > 0.5 * sm["escaped"] and st["mask_escapes"] == 0
+    assert np.abs(Fm - F).max() <= 2e-6 * np.abs(F).max()
     dz.free()
 
 
