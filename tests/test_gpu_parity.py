@@ -218,6 +218,19 @@ def test_small_design_configs_full_N(ctx, oracle, name, n_pairs):
     assert n_div <= n_pairs // 20
     counters_close(st, ost, tol=n_pairs)            # <= ~1 divergent ray per pair at these sizes
     assert sum(st["hits_at_depth"][1:]) > 0         # bounces do happen (panel <-> bus)
+    # the full job runs with the escape masks (above the photons-per-triangle rule; these sampled pairs are below
+    # it, so the masks are forced): same photons and counters, same parity with the oracle
+    assert st["mask_escapes"] == 0
+    ctx.srp_set_options(escape_masks=2)
+    try:
+        Fm, sm = run_pairs(ctx, dz, sun, pairs, cfg.N, cfg.B, cfg.seed)
+    finally:
+        ctx.srp_set_options()
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "hits_at_depth"):
+        assert sm[key] == st[key], key
+    assert sm["mask_escapes"] > 0.4 * sm["escaped"]
+    assert np.abs(Fm - F).max() <= 2e-6 * np.abs(F).max()
+    assert_parity(Fm, Fo, sig)
     dz.free()
 
 
