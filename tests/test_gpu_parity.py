@@ -116,8 +116,8 @@ def test_lbvh_mixed_sizes_and_duplicates(ctx):
     dz.free()
 
 
-@pytest.mark.parametrize("primary_mode", [1, 2])
-def test_forces_on_mixed_batch_match_oracle(ctx, oracle, primary_mode):
+@pytest.mark.parametrize("primary_mode,masks", [(1, 0), (2, 0), (1, 2), (2, 2)])
+def test_forces_on_mixed_batch_match_oracle(ctx, oracle, primary_mode, masks):
     """One batch with a hierarchy holding designs of 1, 3, 70 (identical copies) and 500 random triangles: forces of
     every design against the oracle, per-ray and as beams (one-triangle root, empty child slot, equal Morton keys)."""
     rng = np.random.default_rng(0)
@@ -131,7 +131,7 @@ def test_forces_on_mixed_batch_match_oracle(ctx, oracle, primary_mode):
     dz = ctx.srp_build_designs_from_meshes(verts, mats, off)
     sun = W.fibonacci_sphere(6)
     N, B = 1 << 12, 3
-    ctx.srp_set_options(primary_mode=primary_mode)
+    ctx.srp_set_options(primary_mode=primary_mode, escape_masks=masks)
     try:
         F = ctx.srp_forces(dz, cuda(sun), N, B, 4).cpu().numpy()
         st = ctx.srp_get_stats()
