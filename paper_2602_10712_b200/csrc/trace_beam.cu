@@ -25,7 +25,7 @@ namespace {
 // overflows (a beam along an edge-on panel, a bundle of thin facets) sends its 32 primaries to the
 // pool as well, so any input is handled.
 #ifndef BEAM_BLOCKS_PER_SM
-#define BEAM_BLOCKS_PER_SM 4
+#define BEAM_BLOCKS_PER_SM 5
 #endif
 #ifndef BEAM_SB_DEF
 #define BEAM_SB_DEF 256

@@ -112,8 +112,11 @@ trace_kernel(const TraceArgs a)
 
 // MASKS: the designs carry escape masks (a build of its own: the lookup's branch costs the sail 2.8 % when it is
 // only a run-time null test -- 603.9 against 620.9 ms, profiles/r1d_escape_masks.md).
+#ifndef PERRAY_BLOCKS_PER_SM
+#define PERRAY_BLOCKS_PER_SM 10
+#endif
 template <bool MASKS, bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
-__global__ void __launch_bounds__(TRACE_THREADS, 8)
+__global__ void __launch_bounds__(TRACE_THREADS, PERRAY_BLOCKS_PER_SM)
 bvh_trace_kernel(const TraceArgs a)
 {
     __shared__ int s_stack[STACK_SMEM * TRACE_THREADS];
