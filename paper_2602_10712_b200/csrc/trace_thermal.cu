@@ -56,8 +56,11 @@ __global__ void __launch_bounds__(256) thermal_list_kernel(const float *power, c
     if (power[base + dz.perm[g]] != 0.0f) emit_list[atomicAdd(n_emit, 1)] = (int)g;
 }
 
+#ifndef THERMAL_BLOCKS_PER_SM
+#define THERMAL_BLOCKS_PER_SM 8
+#endif
 template <bool BVH, bool GLOSSY>
-__global__ void __launch_bounds__(TRACE_THREADS, 8)
+__global__ void __launch_bounds__(TRACE_THREADS, THERMAL_BLOCKS_PER_SM)
 thermal_trace_kernel(const TraceArgs a, const ThermalArgs h)
 {
     __shared__ int s_stack[BVH ? STACK_SMEM * TRACE_THREADS : 1];
