@@ -26,7 +26,10 @@ namespace {
 
 constexpr int TRACE_THREADS = 128;
 constexpr int TRACE_WARPS = TRACE_THREADS / 32;
-constexpr int STACK_SMEM = 20;       // traversal stack entries per thread kept in shared memory
+#ifndef STACK_SMEM_DEF
+#define STACK_SMEM_DEF 20
+#endif
+constexpr int STACK_SMEM = STACK_SMEM_DEF;   // traversal stack entries per thread kept in shared memory
 constexpr int STACK_OVF = 80;        // deeper entries spill to local memory (degenerate trees only)
 constexpr unsigned FULL = 0xffffffffu;
 
