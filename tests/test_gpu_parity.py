@@ -1074,3 +1074,66 @@ def test_glossy_torque_matches_oracle(ctx, oracle, name, mode, deposit):
         assert_parity(F[k], r["F"], r["sigma"], tol_agg=3e-3)
         assert_parity(T[k], r["T"], r["sigma_T"], tol_agg=3e-3)
     dz.free()
+
+
+def _random_mask_mesh(seed):
+    """Random meshes for the mask stress test: a sparse soup of small triangles, scattered boxes (outward and inward
+    normals, touching and nested), a paraboloid bowl (either winding) with objects inside and across it, stacks of
+    tessellated near-coplanar plates with gaps from 1e-5 to 0.3."""
+    from test_oracle_thermal import box
+    rng = np.random.default_rng(100 + seed)
+    kind = seed % 4
+    if kind == 0:
+        n = int(rng.integers(100, 3000)); sz = rng.uniform(0.01, 0.2)
+        verts = (rng.uniform(-1, 1, (n, 1, 3)) + rng.normal(0, sz, (n, 3, 3))).astype(np.float32)
+    elif kind == 1:
+        bs = []
+        for _ in range(int(rng.integers(6, 40))):
+            lo = rng.uniform(-1, 1, 3)
+            bs.append(box(lo, lo + rng.uniform(0.05, 0.6, 3), inward=bool(rng.integers(0, 2))))
+        verts = np.concatenate(bs)
+    elif kind == 2:
+        n, depth, flip = int(rng.integers(8, 40)), rng.uniform(0.1, 1.5), bool(rng.integers(0, 2))
+        P = lambda a, b: np.array([-1 + 2 * a / n, -1 + 2 * b / n, depth * ((-1 + 2 * a / n) ** 2 + (-1 + 2 * b / n) ** 2)])
+        tris = []
+        for i in range(n):
+            for j in range(n):
+                p00, p10, p11, p01 = P(i, j), P(i + 1, j), P(i + 1, j + 1), P(i, j + 1)
+                tris += [[p00, p11, p10], [p00, p01, p11]] if flip else [[p00, p10, p11], [p00, p11, p01]]
+        verts = np.concatenate([np.array(tris, np.float32), box([-0.1, -0.1, 0.5], [0.1, 0.1, 0.7]),
+                                quad([-0.02, -1.2, 0.0], [0, 2.4, 0.9], [0.04, 0, 0])])
+    else:
+        ps, z = [], 0.0
+        for _ in range(int(rng.integers(2, 6))):
+            n, s, off = int(rng.integers(3, 14)), rng.uniform(0.3, 1.0), rng.uniform(-0.3, 0.3, 2)
+            ps += [quad([off[0] - s + 2 * s * i / n, off[1] - s + 2 * s * j / n, z], [2 * s / n, 0, 0], [0, 2 * s / n, 0])
+                   for i in range(n) for j in range(n)]
+            z += 10 ** rng.uniform(-5, -0.5)
+        verts = np.concatenate(ps).astype(np.float32)
+    return verts.astype(np.float32)
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_escape_masks_random_meshes(ctx, seed):
+    """Conservativeness of the mask build on geometry it was not tuned on: with the masks forced on, every photon
+    path signature and every counter equals the run without masks."""
+    verts = _random_mask_mesh(seed)
+    mats = np.tile(np.array([[0.1, 0.6, 0.3]], np.float32), (len(verts), 1))
+    dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
+    sun = W.fibonacci_sphere(6) if seed % 3 else np.array([[0, 0, 1], [0, 0, -1], [1, 0, 0.01], [0.3, 0.3, 0.9], [0, 1, 0],
+                                                            [-1, -1, -1]], np.float32)
+    pairs = np.array([[0, j] for j in range(6)], np.int32)
+    res = {}
+    for masks in (0, 2):
+        ctx.srp_set_options(primary_mode=1 + seed % 2, escape_masks=masks)
+        try:
+            F, st = run_pairs(ctx, dz, sun, pairs, 1 << 12, 6, seed=seed)
+            sg = ctx.srp_path_signatures(dz, cuda(sun), pairs, 1 << 12, 6, seed).cpu().numpy()
+        finally:
+            ctx.srp_set_options()
+        res[masks] = (F, st, sg)
+    assert np.array_equal(res[0][2], res[2][2])
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "hits_at_depth"):
+        assert res[0][1][key] == res[2][1][key], key
+    assert np.abs(res[2][0] - res[0][0]).max() <= 2e-6 * np.abs(res[0][0]).max() + 1e-30
+    dz.free()
