@@ -305,7 +305,8 @@ def run_ours(args, rank, world, local_rank):
                 "forces_per_s": pairs_all * args.steps / t_max,
                 "primary_hit_fraction": 1.0 - pmiss / max(launched, 1), "hits_per_photon": hits / max(launched, 1),
                 "segments_per_photon": segs / max(launched, 1),
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": ((10 + (2 if st["mask_escapes"] > 0 else 0)) if W.TRI_COUNT[cfg.family] > 64 else 6) * args.steps,
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": ((10 + (2 if st["mask_escapes"] > 0 else 0)) if W.TRI_COUNT[cfg.family] > 64
+                                 else (6 + (1 if st["mask_escapes"] > 0 else 0))) * args.steps,
                 "clocks": clocks}
         print(json.dumps(line), flush=True)
     ctx.close()
