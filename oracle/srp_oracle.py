@@ -85,6 +85,8 @@ def lib():
         L.srp_oracle_thermal_glossy.restype = ctypes.c_int
         a = L.srp_oracle_thermal.argtypes
         L.srp_oracle_thermal_glossy.argtypes = a[:2] + [ctypes.c_void_p] + a[2:]
+        L.srp_oracle_sail_height.restype = ctypes.c_double
+        L.srp_oracle_sail_height.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_uint64]
         L.srp_oracle_philox.restype = None
         L.srp_oracle_philox.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_uniform.restype = ctypes.c_double
@@ -103,6 +105,11 @@ def philox(ctr, key):
 
 def uniform(x):
     return lib().srp_oracle_uniform(int(x) & 0xFFFFFFFF)
+
+
+def sail_height(x, y, amp=0.05, mesh_seed=2):
+    """Height of the SAIL family's noise surface above (x, y)."""
+    return lib().srp_oracle_sail_height(float(x), float(y), float(amp), int(mesh_seed))
 
 
 def n_params(family):

@@ -23,8 +23,10 @@
  *   TUBE  (ns,nl,r,len): q(i,j) = (r cos phi_i, r sin phi_i, len*j/nl);
  *                   cell c = j*ns+i -> (q(i,j), q(i+1,j), q(i+1,j+1)),
  *                   (q(i,j), q(i+1,j+1), q(i,j+1)).
- * "Parity unpinned" item: the sail's gradient-noise values are defined by
- * DESIGN.md, not by the paper; only structural properties are pinned.
+ * The sail's gradient noise is defined by DESIGN.md, not by the paper; it is pinned
+ * through srp_oracle_sail_height (tests/test_oracle_mesh.py: exact zeros on the
+ * coarsest lattice, hand-expanded values at half- and quarter-cell points, the
+ * lattice gradient, C2 continuity of the quintic fade).
  */
 #include <stdlib.h>
 #include <string.h>
@@ -227,6 +229,12 @@ static double sail_height(double x, double y, double amp, uint64_t seed)
         w *= 0.5; s *= 2.0;
     }
     return amp * f / (1.875 * sqrt(0.5));
+}
+
+/* Height of the sail's surface above (x, y), exported so that the noise can be pinned on its own. */
+double srp_oracle_sail_height(double x, double y, double amp, uint64_t mesh_seed)
+{
+    return sail_height(x, y, amp, mesh_seed);
 }
 
 /* ---- vertex of a patch ---- */
