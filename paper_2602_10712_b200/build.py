@@ -30,6 +30,7 @@ SOURCES = {
     "trace.cu": [],
     "trace_perray.cu": [],
     "trace_beam.cu": [],
+    "trace_bounce.cu": [],
     "trace_small.cu": [],
     "trace_thermal.cu": [],
 }

@@ -74,24 +74,57 @@ bool want_beams(const srp_context *ctx, bool brute, long long max_tris, long lon
     return N >= 8 * max_tris;
 }
 
-// The beam kernel's per-warp ray pools; grown on demand.
-srp_status ensure_pool(srp_context *ctx, TraceArgs &a, bool brute, bool instrumented)
+// The ray queue between the beam kernel and the bounce kernel.  The beam warps stop taking
+// tiles once rq_high rays are queued; every resident warp may still add the rays of the tile it is working on, hence
+// the reserve.  The memory is the caller's (srp_set_workspace) or, failing that, allocated here once.
+#define SRP_RQ_DEFAULT_RAYS (1u << 25)
+srp_status ensure_queue(srp_context *ctx, TraceArgs &a, bool brute, bool instrumented)
 {
-    a.pool = nullptr; a.pool_cap = 0;
+    a.rq = nullptr; a.rq_cap = 0; a.rq_high = 0; a.rq_ctr = nullptr;
     if (!want_beams(ctx, brute, a.max_tris, a.N, a.n_pairs)) return SRP_OK;
-    int cap = 0;
-    const size_t words = srp_beam_pool_words(ctx->num_sms, instrumented, a.tile_rays, &cap);
-    if (ctx->pool_words < words) {
-        TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before pool growth");
-        cudaFree(ctx->pool); ctx->pool = nullptr; ctx->pool_words = 0;
-        if (cudaMalloc(&ctx->pool, sizeof(unsigned) * words) != cudaSuccess) {
-            cudaGetLastError();                 // no room for the pools: trace every ray on its own instead
-            ctx->pool = nullptr;
-            return SRP_OK;
-        }
-        ctx->pool_words = words;
+    const size_t fields = instrumented ? SRP_RQ_FIELDS_INSTR : SRP_RQ_FIELDS;
+    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * (size_t)a.tile_rays;
+    const size_t min_rays = reserve + (1u << 20);
+    if (!ctx->rq_ctr) {
+        TRY_CUDA(ctx, cudaMalloc(&ctx->rq_ctr, 4 * sizeof(unsigned)), "alloc queue counters");
+        TRY_CUDA(ctx, cudaMemsetAsync(ctx->rq_ctr, 0, 4 * sizeof(unsigned), ctx->stream), "zero queue counters");
     }
-    a.pool = ctx->pool; a.pool_cap = cap;
+    if (ctx->rq_words < min_rays * fields) {
+        if (ctx->rq && !ctx->rq_owned)
+            return fail(ctx, SRP_ERR_OOM, "the workspace given to srp_set_workspace is too small for this call's ray queue");
+        TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before queue growth");
+        cudaFree(ctx->rq); ctx->rq = nullptr; ctx->rq_words = 0; ctx->rq_owned = false;
+        size_t rays = SRP_RQ_DEFAULT_RAYS > 2 * min_rays ? SRP_RQ_DEFAULT_RAYS : 2 * min_rays;
+        cudaError_t e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * SRP_RQ_FIELDS_INSTR);
+        if (e != cudaSuccess) {                                 // less room than we would like: the smallest queue that works
+            cudaGetLastError();
+            rays = min_rays;
+            e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * SRP_RQ_FIELDS_INSTR);
+        }
+        if (e != cudaSuccess) return cuda_fail(ctx, "alloc ray queue", e);
+        ctx->rq_words = rays * SRP_RQ_FIELDS_INSTR; ctx->rq_owned = true;
+    }
+    const size_t rays = ctx->rq_words / fields;
+    a.rq = ctx->rq; a.rq_ctr = ctx->rq_ctr;
+    a.rq_cap = (unsigned)(rays < 0xfffffff0u ? rays : 0xfffffff0u);
+    a.rq_high = (unsigned)(a.rq_cap - reserve);
+    return SRP_OK;
+}
+
+// Enqueues S2-S7.  With beams: the beam kernel (primaries) and the bounce kernel (everything queued) alternate until
+// the tiles run out; a launch that finds nothing to do returns at once.
+srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bool instrumented)
+{
+    if (!a.rq) {
+        TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "trace launch");
+        return SRP_OK;
+    }
+    const double primaries = (double)a.n_pairs * (double)a.N;
+    const long long iters = (long long)(primaries / (double)a.rq_high) + 1;
+    for (long long it = 0; it < iters; ++it) {
+        TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "beam launch");
+        TRY_CUDA(ctx, srp_launch_bounce(a, instrumented, ctx->num_sms, ctx->stream), "bounce launch");
+    }
     return SRP_OK;
 }
 
@@ -189,9 +222,10 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
-    st = ensure_pool(ctx, a, brute, ctx->opt.instrumented != 0);
+    st = ensure_queue(ctx, a, brute, ctx->opt.instrumented != 0);
     if (st != SRP_OK) return st;
-    TRY_CUDA(ctx, srp_launch_trace(a, brute, ctx->opt.instrumented != 0, ctx->num_sms, ctx->stream), "trace launch");
+    st = launch_trace_all(ctx, a, brute, ctx->opt.instrumented != 0);
+    if (st != SRP_OK) return st;
     TRY_CUDA(ctx, srp_launch_finalize(a, out, out_torques, ctx->stream), "finalize launch");
     return SRP_OK;
 }
@@ -232,7 +266,8 @@ srp_status srp_destroy(srp_context *ctx)
     if (!ctx) return SRP_ERR_INVALID;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->pool);
+    cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->rq_ctr);
+    if (ctx->rq_owned) cudaFree(ctx->rq);
     cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);
     cudaMemPool_t pool;                                       // hand the pooled design memory back
     if (cudaDeviceGetDefaultMemPool(&pool, ctx->device) == cudaSuccess) cudaMemPoolTrimTo(pool, 0);
@@ -536,10 +571,9 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const fl
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
-    st = ensure_pool(ctx, a, brute, true);
+    st = ensure_queue(ctx, a, brute, true);
     if (st != SRP_OK) return st;
-    TRY_CUDA(ctx, srp_launch_trace(a, brute, true, ctx->num_sms, ctx->stream), "trace launch");
-    return SRP_OK;
+    return launch_trace_all(ctx, a, brute, true);
 }
 
 srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out)

@@ -76,7 +76,9 @@ struct srp_context {
     long long *accum = nullptr;   size_t accum_items = 0;     // int64 fixed-point [pairs*3]
     DevStats *stats = nullptr;
     unsigned long long *work_counter = nullptr;
-    unsigned *pool = nullptr;     size_t pool_words = 0;      // beam kernel's ray pools
+    unsigned *rq = nullptr;       size_t rq_words = 0;        // ray queue between the beam and the bounce kernel
+    unsigned *rq_ctr = nullptr;                               // its counters: [0] tail, [1] head, [2] warps done
+    bool rq_owned = false;                                    // allocated by the library (else srp_set_workspace)
     float *stage_dirs = nullptr;  size_t stage_dirs_items = 0; // srp_forces_host staging
     float *stage_out = nullptr;   size_t stage_out_items = 0;
 };
@@ -102,8 +104,11 @@ struct TraceArgs {
     long long tiles_per_pair;
     int tile_rays;
     unsigned long long *sig_out;   // debug (instrumented kernels): [n_pairs, N] path signatures, or nullptr
-    unsigned *pool;                // beam kernel: per-warp ray pools (srp_beam_pool_words), or nullptr
-    int pool_cap;                  // rays per pool (a power of two)
+    // ray queue (trace_beam.cu -> trace_bounce.cu): continuing photons the beam kernel hands to the bounce kernel
+    unsigned *rq;                  // field-major: field f of ray r at rq[f * rq_cap + r]; nullptr = no beams
+    unsigned rq_cap;               // rays the queue holds
+    unsigned rq_high;              // beam warps stop taking tiles once this many rays are queued
+    unsigned *rq_ctr;              // [0] tail (rays queued), [1] head (rays claimed), [2] bounce warps done
     long long max_tris;            // largest design of the batch
     int primary_mode;              // srp_options.primary_mode
 };
@@ -119,6 +124,7 @@ cudaError_t srp_launch_escape_masks_small(const DesignsDev &dz, long long sumT, 
 cudaError_t srp_launch_escape_masks(const DesignsDev &dz, long long maxT, unsigned *esc, cudaStream_t stream);
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms,
                              cudaStream_t stream);
+cudaError_t srp_launch_bounce(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream);
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream);
 cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream);
 cudaError_t srp_launch_thermal(const TraceArgs &a, const float *facet_power, long long sumT, int *emit_list, int *n_emit,
@@ -127,4 +133,6 @@ cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops
 
 long long srp_family_tris_host(int family);
 int srp_trace_blocks_per_sm(bool brute, bool beam);
-size_t srp_beam_pool_words(int num_sms, bool instrumented, int tile_rays, int *cap_out);
+int srp_beam_warps(int num_sms);                       // resident warps of the beam kernel (queue sizing)
+#define SRP_RQ_FIELDS 9                                // origin, direction, ray index, pair index, src | depth << 27
+#define SRP_RQ_FIELDS_INSTR 11                         // + 64-bit path signature

@@ -28,7 +28,7 @@ cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, 
         if (a.sampler == 0 && a.primary_mode != 1) return srp_launch_small(a, instrumented, num_sms, stream);
         return srp_launch_perray(a, 0, instrumented, num_sms, stream);
     }
-    if (a.sampler == 0 && a.pool != nullptr)          // beams chosen by the caller (srp_api.cu, want_beams)
+    if (a.sampler == 0 && a.rq != nullptr)          // beams chosen by the caller (srp_api.cu, want_beams)
         return srp_launch_beam(a, instrumented, num_sms, stream);
     return srp_launch_perray(a, 1, instrumented, num_sms, stream);
 }

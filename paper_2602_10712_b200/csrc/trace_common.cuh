@@ -452,6 +452,36 @@ __device__ __forceinline__ void flush_counters(const TraceArgs &a, const LaneCou
 }
 
 
+// ---- ray queue (beam kernel -> bounce kernel), DESIGN.md "Data layout" ----
+// A ray is 9 words: origin, direction, ray index i, pair index p, src | depth << 27 (src = SRC_NONE for a primary),
+// plus the 64-bit path signature in the instrumented build; field-major, so that the appends of a warp and the
+// fetches of the bounce kernel coalesce.  Written with st.cg / read with ld.cg: the data crosses kernels through L2.
+constexpr uint32_t SRC_NONE = 0x07ffffffu;
+
+template <bool INSTR>
+__device__ __forceinline__ void rq_store(const TraceArgs &a, uint32_t pos, const float3 &o, const float3 &d, uint32_t i,
+                                         uint32_t p, uint32_t sd, unsigned long long sig)
+{
+    unsigned *q = a.rq + pos;
+    const size_t c = a.rq_cap;
+    __stcg(q, __float_as_uint(o.x)); __stcg(q + c, __float_as_uint(o.y)); __stcg(q + 2 * c, __float_as_uint(o.z));
+    __stcg(q + 3 * c, __float_as_uint(d.x)); __stcg(q + 4 * c, __float_as_uint(d.y)); __stcg(q + 5 * c, __float_as_uint(d.z));
+    __stcg(q + 6 * c, i); __stcg(q + 7 * c, p); __stcg(q + 8 * c, sd);
+    if (INSTR) { __stcg(q + 9 * c, (uint32_t)sig); __stcg(q + 10 * c, (uint32_t)(sig >> 32)); }
+}
+
+template <bool INSTR>
+__device__ __forceinline__ void rq_load(const TraceArgs &a, uint32_t pos, float3 &o, float3 &d, uint32_t &i, uint32_t &p,
+                                        uint32_t &sd, unsigned long long &sig)
+{
+    const unsigned *q = a.rq + pos;
+    const size_t c = a.rq_cap;
+    o = f3(__uint_as_float(__ldcg(q)), __uint_as_float(__ldcg(q + c)), __uint_as_float(__ldcg(q + 2 * c)));
+    d = f3(__uint_as_float(__ldcg(q + 3 * c)), __uint_as_float(__ldcg(q + 4 * c)), __uint_as_float(__ldcg(q + 5 * c)));
+    i = __ldcg(q + 6 * c); p = __ldcg(q + 7 * c); sd = __ldcg(q + 8 * c);
+    if (INSTR) sig = (unsigned long long)__ldcg(q + 9 * c) | ((unsigned long long)__ldcg(q + 10 * c) << 32);
+}
+
 // Per-warp shared-memory queue of bounce rays (bvh_trace_kernel, small_beam_kernel).
 constexpr int QCAP = 64;
 struct WarpQueue {
