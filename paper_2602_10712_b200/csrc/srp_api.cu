@@ -111,20 +111,64 @@ srp_status ensure_queue(srp_context *ctx, TraceArgs &a, bool brute, bool instrum
     return SRP_OK;
 }
 
+// Destroys the loop graphs of earlier calls that have finished (all of them when `all`, after a sync by the caller).
+void reap_graphs(srp_context *ctx, bool all)
+{
+    size_t keep = 0;
+    for (size_t x = 0; x < ctx->graphs.size(); ++x) {
+        srp_context::PendingGraph &g = ctx->graphs[x];
+        if (all || cudaEventQuery(g.done) == cudaSuccess) {
+            cudaGraphExecDestroy(g.exec); cudaGraphDestroy(g.graph); cudaEventDestroy(g.done);
+        } else ctx->graphs[keep++] = g;
+    }
+    cudaGetLastError();                                        // cudaErrorNotReady of the query is not an error
+    ctx->graphs.resize(keep);
+}
+
 // Enqueues S2-S7.  With beams: the beam kernel (primaries) and the bounce kernel (everything queued) alternate until
-// the tiles run out; a launch that finds nothing to do returns at once.
+// the tiles run out.  How often is known only on the device (it depends on how many photons go on), so the loop is
+// a conditional WHILE node of a CUDA graph: body = beam kernel, bounce kernel, and a one-thread kernel that sets the
+// condition from the tile counter.  Nothing is synchronised and no launch is wasted.
 srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bool instrumented)
 {
     if (!a.rq) {
         TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "trace launch");
         return SRP_OK;
     }
-    const double primaries = (double)a.n_pairs * (double)a.N;
-    const long long iters = (long long)(primaries / (double)a.rq_high) + 1;
-    for (long long it = 0; it < iters; ++it) {
-        TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "beam launch");
-        TRY_CUDA(ctx, srp_launch_bounce(a, instrumented, ctx->num_sms, ctx->stream), "bounce launch");
+    reap_graphs(ctx, false);
+    if (!ctx->capture_stream)
+        TRY_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "create capture stream");
+    srp_context::PendingGraph g = { nullptr, nullptr, nullptr };
+    cudaError_t e = cudaGraphCreate(&g.graph, 0);
+    cudaGraphConditionalHandle handle;
+    if (e == cudaSuccess) e = cudaGraphConditionalHandleCreate(&handle, g.graph, 1, cudaGraphCondAssignDefault);
+    cudaGraphNodeParams cp = { cudaGraphNodeTypeConditional };
+    cp.conditional.handle = handle; cp.conditional.type = cudaGraphCondTypeWhile; cp.conditional.size = 1;
+    cudaGraphNode_t cnode;
+    if (e == cudaSuccess) e = cudaGraphAddNode(&cnode, g.graph, nullptr, 0, &cp);
+    if (e == cudaSuccess) {
+        cudaGraph_t body = cp.conditional.phGraph_out[0];
+        e = cudaStreamBeginCaptureToGraph(ctx->capture_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+        if (e == cudaSuccess) {
+            cudaError_t e1 = srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->capture_stream);
+            if (e1 == cudaSuccess) e1 = srp_launch_bounce(a, instrumented, ctx->num_sms, ctx->capture_stream);
+            if (e1 == cudaSuccess) e1 = srp_launch_loop_cond(handle, a, ctx->capture_stream);
+            cudaGraph_t same = nullptr;
+            e = cudaStreamEndCapture(ctx->capture_stream, &same);
+            if (e1 != cudaSuccess) e = e1;
+        }
     }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&g.exec, g.graph, 0);
+    if (e == cudaSuccess) e = cudaGraphLaunch(g.exec, ctx->stream);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g.done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventRecord(g.done, ctx->stream);
+    if (e != cudaSuccess) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        if (g.graph) cudaGraphDestroy(g.graph);
+        if (g.done) cudaEventDestroy(g.done);
+        return cuda_fail(ctx, "beam / bounce loop graph", e);
+    }
+    ctx->graphs.push_back(g);
     return SRP_OK;
 }
 
@@ -266,6 +310,8 @@ srp_status srp_destroy(srp_context *ctx)
     if (!ctx) return SRP_ERR_INVALID;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    reap_graphs(ctx, true);
+    if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
     cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->rq_ctr);
     if (ctx->rq_owned) cudaFree(ctx->rq);
     cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);

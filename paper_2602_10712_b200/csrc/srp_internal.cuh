@@ -79,6 +79,9 @@ struct srp_context {
     unsigned *rq = nullptr;       size_t rq_words = 0;        // ray queue between the beam and the bounce kernel
     unsigned *rq_ctr = nullptr;                               // its counters: [0] tail, [1] head, [2] warps done
     bool rq_owned = false;                                    // allocated by the library (else srp_set_workspace)
+    cudaStream_t capture_stream = nullptr;                    // the beam / bounce loop is captured here into a graph
+    struct PendingGraph { cudaGraphExec_t exec; cudaGraph_t graph; cudaEvent_t done; };
+    std::vector<PendingGraph> graphs;                         // launched loops; destroyed once they have run
     float *stage_dirs = nullptr;  size_t stage_dirs_items = 0; // srp_forces_host staging
     float *stage_out = nullptr;   size_t stage_out_items = 0;
 };
@@ -125,6 +128,7 @@ cudaError_t srp_launch_escape_masks(const DesignsDev &dz, long long maxT, unsign
 cudaError_t srp_launch_trace(const TraceArgs &a, bool brute, bool instrumented, int num_sms,
                              cudaStream_t stream);
 cudaError_t srp_launch_bounce(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream);
+cudaError_t srp_launch_loop_cond(cudaGraphConditionalHandle handle, const TraceArgs &a, cudaStream_t stream);
 cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *out_torques, cudaStream_t stream);
 cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream);
 cudaError_t srp_launch_thermal(const TraceArgs &a, const float *facet_power, long long sumT, int *emit_list, int *n_emit,

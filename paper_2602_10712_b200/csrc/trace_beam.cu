@@ -71,8 +71,13 @@ __device__ __forceinline__ void beam_node(const float4 *__restrict__ nodes, int 
 {
     h0 = h1 = false; l0 = l1 = 0;
     if (node < 0) return;
+#ifdef SRP_NO_LD256
     const float4 n0 = __ldg(nodes + 4 * node), n1 = __ldg(nodes + 4 * node + 1), n2 = __ldg(nodes + 4 * node + 2),
                  n3 = __ldg(nodes + 4 * node + 3);
+#else
+    const F8 lo_ = ldg256(nodes + 4 * node), hi_ = ldg256(nodes + 4 * node + 2);
+    const float4 n0 = lo_.a, n1 = lo_.b, n2 = hi_.a, n3 = hi_.b;
+#endif
     h0 = beam_box(f, offu, offv, wu, wv, n0.x, n0.y, n0.z, n0.w, n1.x, n1.y);
     h1 = beam_box(f, offu, offv, wu, wv, n1.z, n1.w, n2.x, n2.y, n2.z, n2.w);
     l0 = __float_as_int(n3.x); l1 = __float_as_int(n3.y);

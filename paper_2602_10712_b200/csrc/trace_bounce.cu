@@ -226,6 +226,14 @@ bounce_trace_kernel(const TraceArgs a)
     }
 }
 
+// Loop condition of the beam / bounce loop (a conditional WHILE node of a CUDA graph): go round again while tiles
+// are left.  Runs after the bounce kernel, which has emptied the queue.
+__global__ void loop_cond_kernel(cudaGraphConditionalHandle handle, const unsigned long long *work_counter,
+                                 unsigned long long total_tiles)
+{
+    cudaGraphSetConditional(handle, *work_counter < total_tiles ? 1u : 0u);
+}
+
 template <typename K>
 cudaError_t launch_bounce(K kernel, const TraceArgs &a, int num_sms, cudaStream_t stream)
 {
@@ -242,6 +250,12 @@ cudaError_t launch_bounce(K kernel, const TraceArgs &a, int num_sms, cudaStream_
 #define SRP_BOUNCE_G(I_, T_) (a.dz.shin ? SRP_BOUNCE_A(I_, T_, true) : SRP_BOUNCE_A(I_, T_, false))
 
 } // namespace
+
+cudaError_t srp_launch_loop_cond(cudaGraphConditionalHandle handle, const TraceArgs &a, cudaStream_t stream)
+{
+    loop_cond_kernel<<<1, 1, 0, stream>>>(handle, a.work_counter, (unsigned long long)a.n_pairs * a.tiles_per_pair);
+    return cudaGetLastError();
+}
 
 cudaError_t srp_launch_bounce(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream)
 {

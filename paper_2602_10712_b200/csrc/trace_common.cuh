@@ -131,6 +131,17 @@ __device__ __forceinline__ void make_ray(const Emitter &e, const RayGen &g, uint
            fmaf(pu, e.u.z, fmaf(pv, e.v.z, e.worg * e.s.z)));
 }
 
+// 32-byte load (sm_100: LDG.E.256): a 64-byte BVH2 node is two of them instead of four 16-byte loads -- half the
+// load instructions and half the L1 tag look-ups of a divergent node fetch.
+struct __align__(32) F8 { float4 a, b; };
+__device__ __forceinline__ F8 ldg256(const float4 *p)
+{
+    F8 r;
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(r.a.x), "=f"(r.a.y), "=f"(r.a.z), "=f"(r.a.w), "=f"(r.b.x), "=f"(r.b.y), "=f"(r.b.z), "=f"(r.b.w) : "l"(p));
+    return r;
+}
+
 // O-step 4, one triangle: Moller-Trumbore on (v0, e1, e2) in the division-free sign-normalised
 // form: accept det != 0, u >= 0, v >= 0, u+v <= 1, t > 0; t = T/|det| only for accepted hits.
 __device__ __forceinline__ void tri_test(const float4 q0, const float4 q1, const float4 q2, const float3 o,
@@ -198,8 +209,13 @@ template <int STRIDE, int NSMEM>
 __device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, int cur, int &sp, int *s_stack, int *ovf,
                                              float idx, float idy, float idz, float oxi, float oyi, float ozi, float tbest)
 {
+#ifdef SRP_NO_LD256
     const float4 n0 = __ldg(nodes + 4 * cur), n1 = __ldg(nodes + 4 * cur + 1),
                  n2 = __ldg(nodes + 4 * cur + 2), n3 = __ldg(nodes + 4 * cur + 3);
+#else
+    const F8 lo_ = ldg256(nodes + 4 * cur), hi_ = ldg256(nodes + 4 * cur + 2);
+    const float4 n0 = lo_.a, n1 = lo_.b, n2 = hi_.a, n3 = hi_.b;
+#endif
     float a0 = fmaf(n0.x, idx, -oxi), a1 = fmaf(n0.w, idx, -oxi);
     float b0 = fmaf(n0.y, idy, -oyi), b1 = fmaf(n1.x, idy, -oyi);
     float c0 = fmaf(n0.z, idz, -ozi), c1 = fmaf(n1.y, idz, -ozi);
