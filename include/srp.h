@@ -72,6 +72,13 @@ typedef struct {
                                is therefore not to be used from two contexts at once).
                                0 = never, 1 (default) = when the call traces >= 32768 photons per triangle of
                                the batch (the build is repaid), 2 = always; test use                          */
+    int plain_launches;     /* designs with a BVH traced as beams run a loop of two kernels (beam kernel, bounce kernel)
+                               whose trip count is known only on the device.  0 (default) = the loop is a
+                               conditional WHILE node of a CUDA graph; 1 = the same kernels as plain launches, a fixed
+                               sufficient number of rounds (surplus rounds find nothing to do) -- for profilers that do
+                               not list kernels inside conditional graph nodes.  Results are identical.            */
+    int leaf_max;           /* LBVH: subtrees with at most this many triangles become one leaf, 1..8; 0 = default (2).
+                               Read by srp_build_designs*; test and tuning use                                       */
 } srp_options;
 
 /* Photon bookkeeping of the last srp_forces call (DESIGN.md "Pins" P8).

@@ -9,7 +9,6 @@
 // hierarchy: the tracer tests all their triangles (the paper's own method).
 #include <cub/device/device_radix_sort.cuh>
 #include <cfloat>
-#include <cstdlib>
 #include "srp_internal.cuh"
 
 namespace {
@@ -302,7 +301,7 @@ node_plane_kernel(const DesignsDev dz, long long sumT, float4 *nplane)
 
 // Builds box / tri / perm (and nodes when the batch has a design above the brute-force limit) from
 // verts_orig / mats_orig.  All device arrays of `dz` are already allocated.
-cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream)
+cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaStream_t stream)
 {
     const long long sumT = dz->sumT;
     const int D = dz->D;
@@ -342,8 +341,7 @@ cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream)
                                                  pleaf, rfirst, rcount);
     refit_kernel<<<blocks, 256, 0, stream>>>(dz->tri, dz->tri_off_dev, D, sumT, left, right, pnode, pleaf,
                                              flags, lbox, nbox);
-    int leaf_max = SRP_LEAF_MAX;
-    if (const char *e = getenv("SRP_LEAF_MAX")) { int v = atoi(e); if (v >= 1 && v <= 8) leaf_max = v; }   // tuning aid
+    if (leaf_max < 1 || leaf_max > 8) leaf_max = SRP_LEAF_MAX;       // srp_options.leaf_max; 0 = default
     emit_kernel<<<blocks, 256, 0, stream>>>(keys_out, dz->tri_off_dev, sumT, left, right, rfirst, rcount,
                                             lbox, nbox, dz->nodes, leaf_max);
     cudaError_t e = cudaGetLastError();

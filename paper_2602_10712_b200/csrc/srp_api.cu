@@ -135,6 +135,14 @@ srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bo
         TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "trace launch");
         return SRP_OK;
     }
+    if (ctx->opt.plain_launches) {                          // a sufficient number of rounds; surplus ones find nothing to do
+        const long long rounds = (long long)((double)a.n_pairs * (double)a.N / (double)a.rq_high) + 1;
+        for (long long r = 0; r < rounds; ++r) {
+            TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "beam launch");
+            TRY_CUDA(ctx, srp_launch_bounce(a, instrumented, ctx->num_sms, ctx->stream), "bounce launch");
+        }
+        return SRP_OK;
+    }
     reap_graphs(ctx, false);
     if (!ctx->capture_stream)
         TRY_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "create capture stream");
@@ -292,6 +300,7 @@ srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt.solar_pressure = 4.56e-6; ctx->opt.sampler = 0; ctx->opt.deposit = 0;
     ctx->opt.force_brute = 0; ctx->opt.instrumented = 0; ctx->opt.primary_mode = 0; ctx->opt.escape_masks = 1;
+    ctx->opt.plain_launches = 0; ctx->opt.leaf_max = 0;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
     {   // keep freed blocks in the stream-ordered pool: builds reuse them instead of going back to the driver
@@ -326,7 +335,8 @@ srp_status srp_set_options(srp_context *ctx, const srp_options *opt)
     if (!ctx) return SRP_ERR_INVALID;
     if (!opt) return fail(ctx, SRP_ERR_INVALID, "null options");
     if (!(opt->solar_pressure > 0.0) || opt->sampler < 0 || opt->sampler > 1 || opt->deposit < 0 || opt->deposit > 1 ||
-        opt->primary_mode < 0 || opt->primary_mode > 2 || opt->escape_masks < 0 || opt->escape_masks > 2)
+        opt->primary_mode < 0 || opt->primary_mode > 2 || opt->escape_masks < 0 || opt->escape_masks > 2 ||
+        opt->plain_launches < 0 || opt->plain_launches > 1 || opt->leaf_max < 0 || opt->leaf_max > 8)
         return fail(ctx, SRP_ERR_INVALID, "option out of range");
     ctx->opt = *opt;
     return SRP_OK;
@@ -374,7 +384,7 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
     if (st != SRP_OK) { free_designs_mem(ctx, d); delete d; return st; }
     cudaError_t e = srp_launch_mesh_gen((int)family, theta, D, n_params, mesh_seed, T, d->verts_orig,
                                         d->mats_orig, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_build(d, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->stream);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     *out = d;
     return SRP_OK;
@@ -408,7 +418,7 @@ srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, c
     cudaError_t e = cudaMemcpyAsync(d->verts_orig, verts, sizeof(float) * 9 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(d->mats_orig, mats, sizeof(float) * 3 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_build(d, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->stream);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     *out = d;
     return SRP_OK;

@@ -9,7 +9,7 @@
 #include "srp.h"
 
 #define SRP_BRUTE_MAX_TRIS 64      // designs with T <= this are traced without a hierarchy (one leaf)
-#define SRP_LEAF_MAX 3             // LBVH subtrees with <= this many triangles become one leaf
+#define SRP_LEAF_MAX 2             // LBVH subtrees with <= this many triangles become one leaf (cfg3 -7 %, cfg5 -3 % against 3)
 #define SRP_ACC_SCALE 4294967296.0 // fixed-point scale (2^32) of the dimensionless force accumulators
 
 // Packed, BVH-sorted triangle: 3 x float4 = 48 B, fetched as three 16-byte loads.
@@ -120,7 +120,7 @@ struct TraceArgs {
 cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_params,
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
                                 cudaStream_t stream);
-cudaError_t srp_launch_build(srp_designs *dz, cudaStream_t stream);
+cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaStream_t stream);
 cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted, cudaStream_t stream);
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream);
 cudaError_t srp_launch_escape_masks_small(const DesignsDev &dz, long long sumT, unsigned *esc, cudaStream_t stream);

@@ -499,13 +499,15 @@ def test_small_design_beams_equal_brute_force(ctx, family, D, S, N, B):
 
 
 @pytest.mark.parametrize("leaf_max", [1, 8])
-def test_beams_with_other_leaf_sizes(ctx, leaf_max, monkeypatch):
+def test_beams_with_other_leaf_sizes(ctx, leaf_max):
     """Single-triangle leaves fill the beam's leaf lists (a tile-level frontier of 32 nodes can add 64 leaves at
     once -- the list once held 64 and overflowed), 8-triangle leaves its candidate list: same photons either way."""
-    monkeypatch.setenv("SRP_LEAF_MAX", str(leaf_max))            # read by srp_build_designs (tuning aid)
     th = W.draw_params(W.FAMILY_DETAILED, 1)
-    dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
-    monkeypatch.delenv("SRP_LEAF_MAX")
+    ctx.srp_set_options(leaf_max=leaf_max)                        # read by srp_build_designs
+    try:
+        dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    finally:
+        ctx.srp_set_options()
     sun = W.fibonacci_sphere(4)
     pairs = np.array([[0, j] for j in range(4)], np.int32)
     res = {}
