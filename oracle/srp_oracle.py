@@ -78,6 +78,11 @@ def lib():
         L.srp_oracle_forces_torques_glossy.restype = ctypes.c_int
         a = L.srp_oracle_forces_torques.argtypes
         L.srp_oracle_forces_torques_glossy.argtypes = a[:2] + [ctypes.c_void_p] + a[2:]
+        L.srp_oracle_forces_split.restype = ctypes.c_int
+        L.srp_oracle_forces_split.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int,
+                                              ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int,
+                                              ctypes.c_ulonglong, ctypes.POINTER(Options), ctypes.c_void_p, ctypes.c_void_p,
+                                              ctypes.POINTER(Stats)]
         L.srp_oracle_thermal.restype = ctypes.c_int
         L.srp_oracle_thermal.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p,
                                          ctypes.c_longlong, ctypes.c_int, ctypes.c_ulonglong, ctypes.POINTER(Options),
@@ -186,6 +191,25 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
         out["T"] = Tq
         out["sigma_T"] = np.sqrt(np.maximum(TQ - Tq * Tq / float(N), 0.0).sum(axis=1))
     return out
+
+
+def forces_split(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sampler=0, deposit=0, shininess=None):
+    """Total force and its direct part (momentum deposited where sun light first meets the surface)
+    Fig. 5: dict(F f64[S,3], F_direct f64[S,3], F_indirect = F - F_direct, stats)."""
+    verts = np.ascontiguousarray(verts, dtype=np.float32).reshape(-1, 3, 3)
+    mats = np.ascontiguousarray(mats, dtype=np.float32).reshape(-1, 3)
+    sun = np.ascontiguousarray(sun_dirs, dtype=np.float32).reshape(-1, 3)
+    T, S = verts.shape[0], sun.shape[0]
+    sh = None if shininess is None else np.ascontiguousarray(shininess, dtype=np.float32).reshape(-1)
+    F = np.zeros((S, 3)); Fd = np.zeros((S, 3))
+    st = Stats()
+    opt = Options(float(P), int(sampler), int(deposit))
+    rc = lib().srp_oracle_forces_split(verts.ctypes.data, mats.ctypes.data, sh.ctypes.data if sh is not None else None, T,
+                                       int(k), sun.ctypes.data, S, int(j0), int(N), int(B), int(seed), ctypes.byref(opt),
+                                       F.ctypes.data, Fd.ctypes.data, ctypes.byref(st))
+    if rc != 0:
+        raise ValueError("srp_oracle_forces_split: invalid arguments")
+    return {"F": F, "F_direct": Fd, "F_indirect": F - Fd, "stats": st.as_dict()}
 
 
 def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0, shininess=None):

@@ -26,6 +26,12 @@
  * conservation, symmetries, N^-1/2 decay, estimator agreement; torque: off-centre
  * plate, two-plate windmill, centre-of-mass shift identity, centred sphere; glossy lobe (test_oracle_glossy.py):
  * mean cosine (n+1)/(n+2), mirror limit, lobe axis at oblique incidence, horizon rejection, bookkeeping.
+ *
+ * Direct / indirect split (Fig. 5 rows 3-4; "OursGridNB" = no bounces): F_direct = the
+ * momentum deposited where sun light first meets the surface (depth 0), F_indirect = F - F_direct = everything
+ * deposited by light that has been reflected at least once.  Pins (tests/test_oracle_split.py): convex body =>
+ * indirect = 0; direct = the B = 0 force, photon by photon; direct = the shadow-ray surface quadrature of P12;
+ * V-groove: direct and indirect each P A_p.
  */
 #include <stdlib.h>
 #include <string.h>
@@ -90,7 +96,7 @@ typedef struct { const double *v0, *e1, *e2, *nrm; long T; const float *shin; } 
 static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 d, long src, double wph,
                          uint32_t i, uint32_t j, uint32_t k, uint32_t cflag, const uint32_t key[2],
                          const orc_options *opt, int B, orc_v3 xc, orc_stats *st, double dp[3], double dq[3],
-                         int *first_hit, unsigned long long *sig)
+                         int *first_hit, unsigned long long *sig, double *dp0 /* deposits at depth 0, or NULL */)
 {
     int depth = 0;
     for (;;) {
@@ -140,6 +146,7 @@ static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 
         if (z0 < (double)th1) {
             if (opt->deposit == 1) { dd[0] = wph * d.x; dd[1] = wph * d.y; dd[2] = wph * d.z; }
             orc_deposit(dd, x, xc, dp, dq);
+            if (depth == 0 && dp0) { dp0[0] += dd[0]; dp0[1] += dd[1]; dp0[2] += dd[2]; }
             st->absorbed++;
             break;
         } else if (z0 < (double)th2 && !glossy) {
@@ -187,6 +194,7 @@ static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 
             dd[0] = wph * (d.x - dnew.x); dd[1] = wph * (d.y - dnew.y); dd[2] = wph * (d.z - dnew.z);
         }
         orc_deposit(dd, x, xc, dp, dq);
+        if (depth == 0 && dp0) { dp0[0] += dd[0]; dp0[1] += dd[1]; dp0[2] += dd[2]; }
         /* O-step 7: depth cap. */
         if (depth == B) { st->capped++; break; }
         o = x; d = dnew; src = f; depth += 1;
@@ -221,12 +229,12 @@ static void deinterleave(uint64_t i, uint32_t *cx, uint32_t *cy)
  *   shininess float[T] or NULL: Phong exponent of each facet's specular lobe, < 0 = ideal mirror (R23)
  * Returns 0, or -1 on invalid arguments.
  */
-int srp_oracle_forces_torques_glossy(const float *verts, const float *mats, const float *shininess, long T, int k,
-                              const float *sun_dirs, int S, int j0, long long N, int B,
-                              unsigned long long seed, const orc_options *opt,
-                              double *F, double *sumsq, orc_stats *stats, int *first_hit,
-                              unsigned long long *path_sig, const double *x_com, double *Tq,
-                              double *tq_sumsq)
+static int forces_core(const float *verts, const float *mats, const float *shininess, long T, int k,
+                       const float *sun_dirs, int S, int j0, long long N, int B,
+                       unsigned long long seed, const orc_options *opt,
+                       double *F, double *sumsq, orc_stats *stats, int *first_hit,
+                       unsigned long long *path_sig, const double *x_com, double *Tq,
+                       double *tq_sumsq, double *F_direct /* double[S][3] or NULL */)
 {
     if (!verts || !mats || !sun_dirs || !F || !opt || T <= 0 || S <= 0 || N <= 0 || B < 0 || B > 15)
         return -1;
@@ -275,7 +283,7 @@ int srp_oracle_forces_torques_glossy(const float *verts, const float *mats, cons
         }
         const double Ae = (u1 - u0) * (vv1 - vv0);
         const double wph = P * Ae / (double)N;
-        double Fj[3] = { 0, 0, 0 }, Qj[3] = { 0, 0, 0 }, Tj[3] = { 0, 0, 0 }, TQj[3] = { 0, 0, 0 };
+        double Fj[3] = { 0, 0, 0 }, Qj[3] = { 0, 0, 0 }, Tj[3] = { 0, 0, 0 }, TQj[3] = { 0, 0, 0 }, Dj[3] = { 0, 0, 0 };
         const orc_v3 xc = x_com ? orc_mk(x_com[0], x_com[1], x_com[2]) : orc_mk(0.0, 0.0, 0.0);
 
         for (long long i = 0; i < N && Ae > 0.0; ++i) {
@@ -298,7 +306,7 @@ int srp_oracle_forces_torques_glossy(const float *verts, const float *mats, cons
             unsigned long long sig = 0;
             st.launched++;
             trace_photon(&G, mats, o, d, -1, wph, (uint32_t)i, j, (uint32_t)k, 0u, key, opt, B, xc, &st, dp, dq,
-                         first_hit ? &first_hit[(long long)jj * N + i] : NULL, &sig);
+                         first_hit ? &first_hit[(long long)jj * N + i] : NULL, &sig, F_direct ? Dj : NULL);
             for (int c = 0; c < 3; ++c) {
                 Fj[c] += dp[c]; Qj[c] += dp[c] * dp[c];
                 Tj[c] += dq[c]; TQj[c] += dq[c] * dq[c];
@@ -314,11 +322,33 @@ int srp_oracle_forces_torques_glossy(const float *verts, const float *mats, cons
             if (sumsq) sumsq[3 * jj + c] = Qj[c];
             if (Tq) Tq[3 * jj + c] = Tj[c];
             if (tq_sumsq) tq_sumsq[3 * jj + c] = TQj[c];
+            if (F_direct) F_direct[3 * jj + c] = Dj[c];
         }
     }
     if (stats) *stats = st;
     free(v0); free(e1); free(e2); free(nrm);
     return 0;
+}
+
+int srp_oracle_forces_torques_glossy(const float *verts, const float *mats, const float *shininess, long T, int k,
+                              const float *sun_dirs, int S, int j0, long long N, int B,
+                              unsigned long long seed, const orc_options *opt,
+                              double *F, double *sumsq, orc_stats *stats, int *first_hit,
+                              unsigned long long *path_sig, const double *x_com, double *Tq,
+                              double *tq_sumsq)
+{
+    return forces_core(verts, mats, shininess, T, k, sun_dirs, S, j0, N, B, seed, opt, F, sumsq, stats, first_hit,
+                       path_sig, x_com, Tq, tq_sumsq, NULL);
+}
+
+/* Total force and its direct part (depth-0 deposits); F_indirect = F - F_direct. */
+int srp_oracle_forces_split(const float *verts, const float *mats, const float *shininess, long T, int k,
+                            const float *sun_dirs, int S, int j0, long long N, int B, unsigned long long seed,
+                            const orc_options *opt, double *F, double *F_direct, orc_stats *stats)
+{
+    if (!F_direct) return -1;
+    return forces_core(verts, mats, shininess, T, k, sun_dirs, S, j0, N, B, seed, opt, F, NULL, stats, NULL, NULL,
+                       NULL, NULL, NULL, F_direct);
 }
 
 /* Ideal-mirror specular lobes on every facet (R5): the call of the hot path. */
@@ -405,7 +435,7 @@ int srp_oracle_thermal_glossy(const float *verts, const float *mats, const float
             unsigned long long sig = 0;
             st.launched++;
             trace_photon(&G, mats, x, d, f, w, (uint32_t)i, (uint32_t)f, (uint32_t)k, 0x80000000u, key, opt, B, xc, &st,
-                         dp, dq, NULL, &sig);
+                         dp, dq, NULL, &sig, NULL);
             for (int c = 0; c < 3; ++c) { Ft[c] += dp[c]; Qt[c] += dp[c] * dp[c]; }
         }
     }
