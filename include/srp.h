@@ -16,7 +16,10 @@
  *    the boundary.  srp_last_error(ctx) gives the text of the last failure of that context.
  *  - Pointers marked DEVICE are CUDA device pointers on the context's device (e.g. a torch tensor's
  *    data_ptr()); pointers marked HOST are ordinary host memory.  The caller owns every buffer it
- *    passes; the library owns the opaque handles and an internal workspace (cudaMalloc'ed lazily).
+ *    passes; the library owns the opaque handles, small counters and accumulators, and -- unless the caller provides
+ *    it with srp_set_workspace -- the ray queue of the beam / bounce loop (cudaMalloc'ed on first use; a failed
+ *    allocation is SRP_ERR_OOM, never a silent change of method).  Design arrays come from a stream-ordered memory
+ *    pool of the context's own.
  *  - srp_build_designs* and srp_forces only ENQUEUE work on the context's stream; the caller
  *    synchronises that stream.  Functions documented "syncs" wait for the stream.
  *  - Same inputs + same seed => bit-identical output (integer fixed-point accumulation).
@@ -98,6 +101,11 @@ typedef struct {
     unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
     unsigned long long mask_escapes;   /* bounce rays resolved as "escaped" by the escape masks (also counted in
                                           escaped and segments) */
+    unsigned long long queued_rays;    /* rays the beam kernel handed to the bounce kernel through the ray queue */
+    unsigned long long loop_rounds;    /* rounds of the beam / bounce loop that had rays queued (counted on the device) */
+    unsigned long long kernel_launches;/* kernels of this library the last srp_forces* / srp_thermal_forces call ran:
+                                          those enqueued by the host plus, for the beam / bounce loop, the rounds the
+                                          device counted (CUB's sort kernels of a build are not included) */
 } srp_stats;
 
 /* Creates a context on CUDA device `cuda_device`; `cuda_stream` is a cudaStream_t (may be NULL =
@@ -119,7 +127,9 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
                              int n_params, unsigned long long mesh_seed, srp_designs **out);
 
 /* User-supplied meshes (the paper's general design->mesh map):
- * verts DEVICE float[sumT,3,3] (v0,v1,v2), mats DEVICE float[sumT,3] = (alpha, rho_s, rho_d),
+ * verts DEVICE float[sumT,3,3] (v0,v1,v2), mats DEVICE float[sumT,3] = (alpha, rho_s, rho_d), each >= 0 and
+ * summing to 1 (they are used as given: the lobe draw reads alpha and alpha + rho_s as thresholds and takes the rest
+ * as diffuse, the expected-value deposit uses all three; the Python binding checks host arrays),
  * tri_offsets HOST long long[D+1], tri_offsets[0] = 0, strictly increasing.  Enqueues only. */
 srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, const float *mats,
                                          const long long *tri_offsets, int D, srp_designs **out);
@@ -145,7 +155,7 @@ srp_status srp_designs_read_bvh(srp_context *ctx, const srp_designs *designs, in
 srp_status srp_free_designs(srp_context *ctx, srp_designs *designs);   /* syncs */
 
 /* S2-S7: sun_dirs DEVICE float[S,3], body->sun (the paper's omega), any non-zero
- * length; rays_per_dir N > 0 (a power of two when sampler = 0); 0 <= max_bounces <= 15 reflections
+ * length (a zero or non-finite direction gives F = 0 for its pairs); rays_per_dir N > 0 (a power of two when sampler = 0); 0 <= max_bounces <= 15 reflections
  * followed (R5); seed keys Philox4x32-10 with counter (ray, direction, design, depth).
  * out_forces DEVICE float[D,S,3], newtons, body frame.  Enqueues only. */
 srp_status srp_forces(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
@@ -153,7 +163,8 @@ srp_status srp_forces(srp_context *ctx, const srp_designs *designs, const float 
                       float *out_forces);
 
 /* Same, restricted to an explicit list of pairs: pairs DEVICE int[n_pairs,2] = (design k,
- * direction j); out_forces DEVICE float[n_pairs,3].  The Philox counters use (k, j), so the result
+ * direction j), 0 <= k < D, 0 <= j < S (entries out of range are clamped into it on the device: memory-safe,
+ * meaningless); out_forces DEVICE float[n_pairs,3].  The Philox counters use (k, j), so the result
  * of a pair equals the corresponding entry of the full srp_forces call bit for bit. */
 srp_status srp_forces_pairs(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
                             const int *pairs, long long n_pairs, long long rays_per_dir,
@@ -171,6 +182,18 @@ srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *designs
                                     const int *pairs, long long n_pairs, long long rays_per_dir, int max_bounces,
                                     unsigned long long seed, const float *x_com, float *out_forces,
                                     float *out_torques);
+
+/* Forces and their DIRECT part (Fig. 5 rows 3-4: direct and indirect force maps; the
+ * no-bounce variant): out_direct DEVICE float[D,S,3] (or [n_pairs,3]) = the momentum deposited where sun light first
+ * meets the surface -- what srp_forces returns with max_bounces = 0 (same photons; bit for bit from the beam kernels,
+ * to the rounding of per-lane fp32 partial sums otherwise) -- from the same trace that gives out_forces; the indirect part (everything deposited by light reflected at least once) is out_forces - out_direct.
+ * Enqueues only. */
+srp_status srp_forces_split(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                            long long rays_per_dir, int max_bounces, unsigned long long seed, float *out_forces,
+                            float *out_direct);
+srp_status srp_forces_split_pairs(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                                  const int *pairs, long long n_pairs, long long rays_per_dir, int max_bounces,
+                                  unsigned long long seed, float *out_forces, float *out_direct);
 
 /* Glossy specular lobes, PAPER.md:148 (meshes carry "per-face Phong material parameters"); R23.
  * shininess DEVICE float[sumT], ORIGINAL triangle order of all designs back to back (tri_offsets of
@@ -219,6 +242,18 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *designs, con
 
 /* Counters of the last srp_forces* call on this context.  Syncs. */
 srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out);
+
+/* Kernels of this library that this context has run since srp_create (builds, mask builds, trace kernels, loop
+ * rounds as counted on the device, finalisation; not CUB's sort kernels, not the probes).  Syncs. */
+srp_status srp_launch_count(srp_context *ctx, unsigned long long *n_kernels);
+
+/* Workspace from the caller (PyTorch stays the only allocator): `bytes` of DEVICE memory at `ptr` (256-byte aligned)
+ * that the library uses for the ray queue between the beam kernel and the bounce kernel instead of allocating one
+ * itself (36 bytes per queued ray, 44 in the instrumented build).  The memory must stay valid until the next srp_set_workspace or srp_destroy;
+ * (NULL, 0) hands the choice back to the library.  A workspace smaller than srp_workspace_bytes_min(ctx) is refused
+ * with SRP_ERR_INVALID; a larger one means fewer rounds of the beam / bounce loop.  Syncs. */
+srp_status srp_set_workspace(srp_context *ctx, void *ptr, unsigned long long bytes);
+unsigned long long srp_workspace_bytes_min(const srp_context *ctx);
 
 /* Micro-benchmarks for the roofline denominators: register-resident FP32
  * FMA chains, and an L2-resident 16-byte-load sweep.  Syncs; results in TFLOP/s and GB/s. */

@@ -37,13 +37,15 @@ class srp_stats(ctypes.Structure):
                [("hits_at_depth", ctypes.c_ulonglong * 16), ("box_tests", ctypes.c_ulonglong),
                 ("tri_tests", ctypes.c_ulonglong)] + \
                [(n, ctypes.c_ulonglong) for n in ("beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback",
-                                                  "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests", "mask_escapes")]
+                                                  "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests", "mask_escapes",
+                                                  "queued_rays", "loop_rounds", "kernel_launches")]
 
     def as_dict(self):
         d = {n: int(getattr(self, n)) for n in
              ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "box_tests", "tri_tests",
               "beam_tile_miss", "beam_block_miss", "beam_group_miss", "beam_fallback",
-              "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests", "mask_escapes")}
+              "beam_box_tests", "tri2d_tests", "tri_setups", "rect_tests", "mask_escapes", "queued_rays", "loop_rounds",
+              "kernel_launches")}
         d["hits_at_depth"] = [int(x) for x in self.hits_at_depth]
         return d
 
@@ -52,8 +54,9 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_family_n_params", "srp_family_tri_count", "srp_build_designs",
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
-           "srp_forces_torques", "srp_forces_torques_pairs", "srp_thermal_forces", "srp_designs_set_shininess",
-           "srp_first_hits", "srp_path_signatures", "srp_get_stats", "srp_probe_peaks"]
+           "srp_forces_torques", "srp_forces_torques_pairs", "srp_forces_split", "srp_forces_split_pairs",
+           "srp_thermal_forces", "srp_designs_set_shininess", "srp_first_hits", "srp_path_signatures", "srp_get_stats",
+           "srp_launch_count", "srp_set_workspace", "srp_workspace_bytes_min", "srp_probe_peaks"]
 
 _lib = None
 
@@ -88,6 +91,12 @@ def load_library():
     L.srp_forces_host.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
     L.srp_forces_torques.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp, vp]
     L.srp_forces_torques_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp, vp]
+    L.srp_forces_split.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp]
+    L.srp_forces_split_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp]
+    L.srp_launch_count.argtypes = [vp, ctypes.POINTER(ull)]
+    L.srp_set_workspace.argtypes = [vp, vp, ull]
+    L.srp_workspace_bytes_min.argtypes = [vp]
+    L.srp_workspace_bytes_min.restype = ull
     L.srp_thermal_forces.argtypes = [vp, vp, vp, ll, ci, ull, vp]
     L.srp_designs_set_shininess.argtypes = [vp, vp, vp]
     L.srp_first_hits.argtypes = [vp, vp, vp, ci, vp, ll, ll, ull, ci, vp]
@@ -95,7 +104,7 @@ def load_library():
     L.srp_get_stats.argtypes = [vp, ctypes.POINTER(srp_stats)]
     L.srp_probe_peaks.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     for name in EXPORTS:
-        if name not in ("srp_last_error", "srp_family_tri_count"):
+        if name not in ("srp_last_error", "srp_family_tri_count", "srp_workspace_bytes_min"):
             getattr(L, name).restype = ci
     _lib = L
     return L
@@ -104,6 +113,15 @@ def load_library():
 def _f32_cuda(t, device):
     t = torch.as_tensor(t)
     return t.to(device=device, dtype=torch.float32).contiguous()
+
+
+def _check_cuda_f32(t, name, device, shape_tail=None):
+    """A contiguous float32 CUDA tensor on `device` (its data_ptr() is handed to the library as a DEVICE pointer)."""
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.device == device and t.dtype == torch.float32 and t.is_contiguous()):
+        raise ValueError("%s must be a contiguous float32 CUDA tensor on %s" % (name, device))
+    if shape_tail is not None and tuple(t.shape[-len(shape_tail):]) != tuple(shape_tail):
+        raise ValueError("%s must have shape [..., %s]" % (name, ", ".join(map(str, shape_tail))))
+    return t
 
 
 class Designs:
@@ -190,8 +208,14 @@ class Context:
         return Designs(self, h)
 
     def srp_build_designs_from_meshes(self, verts, mats, tri_offsets):
+        if isinstance(mats, np.ndarray):           # host data: check what the header asks of the materials
+            m = np.asarray(mats, np.float64).reshape(-1, 3)
+            if not (np.all(m >= 0.0) and np.all(np.abs(m.sum(1) - 1.0) <= 1e-5)):
+                raise ValueError("materials must be >= 0 and sum to 1 per facet")
         verts, mats = _f32_cuda(verts, self.device), _f32_cuda(mats, self.device)
         off = np.ascontiguousarray(tri_offsets, dtype=np.int64)
+        if verts.numel() != 9 * int(off[-1]) or mats.numel() != 3 * int(off[-1]):
+            raise ValueError("verts / mats do not match tri_offsets")
         h = ctypes.c_void_p()
         self._check(self.lib.srp_build_designs_from_meshes(self.handle, verts.data_ptr(), mats.data_ptr(),
                                                            off.ctypes.data, len(off) - 1, ctypes.byref(h)))
@@ -200,17 +224,28 @@ class Context:
 
     def srp_forces(self, designs, sun_dirs, rays_per_dir, max_bounces, seed=0, out=None):
         """sun_dirs: CUDA float32 [S,3]; returns CUDA float32 [D,S,3] (asynchronous on the stream)."""
-        if not (sun_dirs.is_cuda and sun_dirs.dtype == torch.float32 and sun_dirs.is_contiguous()):
-            raise ValueError("sun_dirs must be a contiguous CUDA float32 tensor")
+        _check_cuda_f32(sun_dirs, "sun_dirs", self.device, (3,))
         S = sun_dirs.shape[0]
         if out is None:
             out = torch.empty((designs.D, S, 3), dtype=torch.float32, device=self.device)
+        elif _check_cuda_f32(out, "out", self.device).numel() != designs.D * S * 3:
+            raise ValueError("out must hold [D, S, 3] floats")
         self._check(self.lib.srp_forces(self.handle, designs.handle, sun_dirs.data_ptr(), S, rays_per_dir,
                                         max_bounces, seed, out.data_ptr()))
         return out
 
-    def srp_forces_pairs(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0):
+    def _pairs(self, designs, sun_dirs, pairs):
+        _check_cuda_f32(sun_dirs, "sun_dirs", self.device, (3,))
         pairs = torch.as_tensor(pairs).to(device=self.device, dtype=torch.int32).contiguous()
+        if pairs.dim() != 2 or pairs.shape[1] != 2 or pairs.shape[0] == 0:
+            raise ValueError("pairs must be [n, 2]")
+        lo, hi = pairs.min(0).values.tolist(), pairs.max(0).values.tolist()
+        if lo[0] < 0 or lo[1] < 0 or hi[0] >= designs.D or hi[1] >= sun_dirs.shape[0]:
+            raise ValueError("pairs out of range")
+        return pairs
+
+    def srp_forces_pairs(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0):
+        pairs = self._pairs(designs, sun_dirs, pairs)
         out = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
         self._check(self.lib.srp_forces_pairs(self.handle, designs.handle, sun_dirs.data_ptr(), sun_dirs.shape[0],
                                               pairs.data_ptr(), pairs.shape[0], rays_per_dir, max_bounces, seed,
@@ -228,8 +263,7 @@ class Context:
 
     def srp_forces_torques(self, designs, sun_dirs, rays_per_dir, max_bounces, seed=0, x_com=None):
         """Forces and torques about x_com ([D,3], None = origin): two CUDA float32 [D,S,3] tensors."""
-        if not (sun_dirs.is_cuda and sun_dirs.dtype == torch.float32 and sun_dirs.is_contiguous()):
-            raise ValueError("sun_dirs must be a contiguous CUDA float32 tensor")
+        _check_cuda_f32(sun_dirs, "sun_dirs", self.device, (3,))
         S = sun_dirs.shape[0]
         x = self._xcom(designs, x_com)
         F = torch.empty((designs.D, S, 3), dtype=torch.float32, device=self.device)
@@ -241,7 +275,7 @@ class Context:
         return F, T
 
     def srp_forces_torques_pairs(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0, x_com=None):
-        pairs = torch.as_tensor(pairs).to(device=self.device, dtype=torch.int32).contiguous()
+        pairs = self._pairs(designs, sun_dirs, pairs)
         x = self._xcom(designs, x_com)
         F = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
         T = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
@@ -277,16 +311,54 @@ class Context:
         self.stream.synchronize()
         return out
 
+    def srp_forces_split(self, designs, sun_dirs, rays_per_dir, max_bounces, seed=0):
+        """Forces and their direct part (momentum deposited where sun light first meets the surface)
+        from one trace: two CUDA float32 [D,S,3] tensors (asynchronous on the stream)."""
+        _check_cuda_f32(sun_dirs, "sun_dirs", self.device, (3,))
+        S = sun_dirs.shape[0]
+        F = torch.empty((designs.D, S, 3), dtype=torch.float32, device=self.device)
+        Fd = torch.empty((designs.D, S, 3), dtype=torch.float32, device=self.device)
+        self._check(self.lib.srp_forces_split(self.handle, designs.handle, sun_dirs.data_ptr(), S, rays_per_dir,
+                                              max_bounces, seed, F.data_ptr(), Fd.data_ptr()))
+        return F, Fd
+
+    def srp_forces_split_pairs(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0):
+        pairs = self._pairs(designs, sun_dirs, pairs)
+        F = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
+        Fd = torch.empty((pairs.shape[0], 3), dtype=torch.float32, device=self.device)
+        self._check(self.lib.srp_forces_split_pairs(self.handle, designs.handle, sun_dirs.data_ptr(), sun_dirs.shape[0],
+                                                    pairs.data_ptr(), pairs.shape[0], rays_per_dir, max_bounces, seed,
+                                                    F.data_ptr(), Fd.data_ptr()))
+        self.stream.synchronize()
+        return F, Fd
+
     def force_maps(self, designs, n_lat, n_lon, rays_per_dir, max_bounces, seed=0):
         """The paper's force-map figures (Fig. 5): forces over a latitude-longitude image of sun
-        directions, and their split into direct light (no bounce, the paper's "NB" variant) and
-        indirect light (the rest).  Two srp_forces calls; returns CUDA float32 [D, n_lat, n_lon, 3] tensors
-        (total, direct, indirect)."""
+        directions (workloads.latlong_directions) with their direct part, from one srp_forces_split call, reshaped:
+        two CUDA float32 [D, n_lat, n_lon, 3] tensors (total, direct); the indirect map is their difference."""
         sun = torch.from_numpy(W.latlong_directions(n_lat, n_lon)).to(self.device)
-        total = self.srp_forces(designs, sun, rays_per_dir, max_bounces, seed)
-        direct = self.srp_forces(designs, sun, rays_per_dir, 0, seed)
+        total, direct = self.srp_forces_split(designs, sun, rays_per_dir, max_bounces, seed)
         shape = (designs.D, n_lat, n_lon, 3)
-        return total.reshape(shape), direct.reshape(shape), (total - direct).reshape(shape)
+        return total.reshape(shape), direct.reshape(shape)
+
+    def srp_set_workspace(self, tensor):
+        """Hands the library a CUDA tensor (any dtype, contiguous) as the ray queue of its beam / bounce loop, or
+        None to let it allocate its own.  The tensor is kept alive by this object."""
+        if tensor is None:
+            self._check(self.lib.srp_set_workspace(self.handle, None, 0))
+        else:
+            if not (tensor.is_cuda and tensor.device == self.device and tensor.is_contiguous()):
+                raise ValueError("workspace must be a contiguous CUDA tensor on %s" % self.device)
+            self._check(self.lib.srp_set_workspace(self.handle, tensor.data_ptr(), tensor.numel() * tensor.element_size()))
+        self._workspace = tensor
+
+    def srp_workspace_bytes_min(self):
+        return int(self.lib.srp_workspace_bytes_min(self.handle))
+
+    def srp_launch_count(self):
+        n = ctypes.c_ulonglong()
+        self._check(self.lib.srp_launch_count(self.handle, ctypes.byref(n)))
+        return n.value
 
     def srp_forces_host(self, designs, sun_dirs_host, rays_per_dir, max_bounces, seed=0, out_host=None):
         """Host buffers in and out (numpy float32 or pinned CPU tensors); synchronous."""
@@ -300,7 +372,7 @@ class Context:
         return out_host
 
     def srp_first_hits(self, designs, sun_dirs, pairs, rays_per_dir, seed=0, method=0):
-        pairs = torch.as_tensor(pairs).to(device=self.device, dtype=torch.int32).contiguous()
+        pairs = self._pairs(designs, sun_dirs, pairs)
         out = torch.empty((pairs.shape[0], rays_per_dir), dtype=torch.int32, device=self.device)
         self._check(self.lib.srp_first_hits(self.handle, designs.handle, sun_dirs.data_ptr(), sun_dirs.shape[0],
                                             pairs.data_ptr(), pairs.shape[0], rays_per_dir, seed, method,
@@ -309,7 +381,7 @@ class Context:
         return out
 
     def srp_path_signatures(self, designs, sun_dirs, pairs, rays_per_dir, max_bounces, seed=0):
-        pairs = torch.as_tensor(pairs).to(device=self.device, dtype=torch.int32).contiguous()
+        pairs = self._pairs(designs, sun_dirs, pairs)
         out = torch.empty((pairs.shape[0], rays_per_dir), dtype=torch.int64, device=self.device)
         self._check(self.lib.srp_path_signatures(self.handle, designs.handle, sun_dirs.data_ptr(), sun_dirs.shape[0],
                                                  pairs.data_ptr(), pairs.shape[0], rays_per_dir, max_bounces, seed,

@@ -301,7 +301,7 @@ node_plane_kernel(const DesignsDev dz, long long sumT, float4 *nplane)
 
 // Builds box / tri / perm (and nodes when the batch has a design above the brute-force limit) from
 // verts_orig / mats_orig.  All device arrays of `dz` are already allocated.
-cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaStream_t stream)
+cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, cudaStream_t stream)
 {
     const long long sumT = dz->sumT;
     const int D = dz->D;
@@ -312,42 +312,46 @@ cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaStream_t stream)
                                                 nullptr, dz->tri, dz->perm);
         return cudaGetLastError();
     }
+    // scratch of the build, from the context's pool; freed (stream-ordered) whether or not the build succeeds
     u64 *keys = nullptr, *keys_out = nullptr;
     unsigned *vals = nullptr, *vals_out = nullptr;
     int *ibuf = nullptr;          // left, right, parent_node, parent_leaf, range_first, range_count, flags
     float4 *lbox = nullptr, *nbox = nullptr;
     void *tmp = nullptr; size_t tmp_bytes = 0;
-    CK(cudaMallocAsync(&keys, sizeof(u64) * sumT, stream));
-    CK(cudaMallocAsync(&keys_out, sizeof(u64) * sumT, stream));
-    CK(cudaMallocAsync(&vals, sizeof(unsigned) * sumT, stream));
-    CK(cudaMallocAsync(&vals_out, sizeof(unsigned) * sumT, stream));
-    CK(cudaMallocAsync(&ibuf, sizeof(int) * 7 * sumT, stream));
-    CK(cudaMallocAsync(&lbox, sizeof(float4) * 2 * sumT, stream));
-    CK(cudaMallocAsync(&nbox, sizeof(float4) * 2 * sumT, stream));
-    int end_bit = 48;
-    while ((1LL << (end_bit - 48)) < D) ++end_bit;
-    CK(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys_out, vals, vals_out, (int)sumT, 0,
-                                       end_bit, stream));
-    CK(cudaMallocAsync(&tmp, tmp_bytes, stream));
-    morton_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->tri_off_dev, D, sumT, dz->box, keys, vals);
-    CK(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys_out, vals, vals_out, (int)sumT, 0,
-                                       end_bit, stream));
-    pack_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->mats_orig, dz->tri_off_dev, D, sumT,
-                                            vals_out, dz->tri, dz->perm);
-    int *left = ibuf, *right = ibuf + sumT, *pnode = ibuf + 2 * sumT, *pleaf = ibuf + 3 * sumT,
-        *rfirst = ibuf + 4 * sumT, *rcount = ibuf + 5 * sumT, *flags = ibuf + 6 * sumT;
-    CK(cudaMemsetAsync(flags, 0, sizeof(int) * sumT, stream));
-    hierarchy_kernel<<<blocks, 256, 0, stream>>>(keys_out, dz->tri_off_dev, D, sumT, left, right, pnode,
-                                                 pleaf, rfirst, rcount);
-    refit_kernel<<<blocks, 256, 0, stream>>>(dz->tri, dz->tri_off_dev, D, sumT, left, right, pnode, pleaf,
-                                             flags, lbox, nbox);
     if (leaf_max < 1 || leaf_max > 8) leaf_max = SRP_LEAF_MAX;       // srp_options.leaf_max; 0 = default
-    emit_kernel<<<blocks, 256, 0, stream>>>(keys_out, dz->tri_off_dev, sumT, left, right, rfirst, rcount,
-                                            lbox, nbox, dz->nodes, leaf_max);
-    cudaError_t e = cudaGetLastError();
-    cudaFreeAsync(keys, stream); cudaFreeAsync(keys_out, stream); cudaFreeAsync(vals, stream);
-    cudaFreeAsync(vals_out, stream); cudaFreeAsync(ibuf, stream); cudaFreeAsync(lbox, stream);
-    cudaFreeAsync(nbox, stream); cudaFreeAsync(tmp, stream);
+    auto build = [&]() -> cudaError_t {
+        CK(cudaMallocFromPoolAsync((void **)&keys, sizeof(u64) * sumT, pool, stream));
+        CK(cudaMallocFromPoolAsync((void **)&keys_out, sizeof(u64) * sumT, pool, stream));
+        CK(cudaMallocFromPoolAsync((void **)&vals, sizeof(unsigned) * sumT, pool, stream));
+        CK(cudaMallocFromPoolAsync((void **)&vals_out, sizeof(unsigned) * sumT, pool, stream));
+        CK(cudaMallocFromPoolAsync((void **)&ibuf, sizeof(int) * 7 * sumT, pool, stream));
+        CK(cudaMallocFromPoolAsync((void **)&lbox, sizeof(float4) * 2 * sumT, pool, stream));
+        CK(cudaMallocFromPoolAsync((void **)&nbox, sizeof(float4) * 2 * sumT, pool, stream));
+        int end_bit = 48;
+        while ((1LL << (end_bit - 48)) < D) ++end_bit;
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys_out, vals, vals_out, (int)sumT, 0,
+                                           end_bit, stream));
+        CK(cudaMallocFromPoolAsync(&tmp, tmp_bytes, pool, stream));
+        morton_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->tri_off_dev, D, sumT, dz->box, keys, vals);
+        CK(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys_out, vals, vals_out, (int)sumT, 0,
+                                           end_bit, stream));
+        pack_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->mats_orig, dz->tri_off_dev, D, sumT,
+                                                vals_out, dz->tri, dz->perm);
+        int *left = ibuf, *right = ibuf + sumT, *pnode = ibuf + 2 * sumT, *pleaf = ibuf + 3 * sumT,
+            *rfirst = ibuf + 4 * sumT, *rcount = ibuf + 5 * sumT, *flags = ibuf + 6 * sumT;
+        CK(cudaMemsetAsync(flags, 0, sizeof(int) * sumT, stream));
+        hierarchy_kernel<<<blocks, 256, 0, stream>>>(keys_out, dz->tri_off_dev, D, sumT, left, right, pnode,
+                                                     pleaf, rfirst, rcount);
+        refit_kernel<<<blocks, 256, 0, stream>>>(dz->tri, dz->tri_off_dev, D, sumT, left, right, pnode, pleaf,
+                                                 flags, lbox, nbox);
+        emit_kernel<<<blocks, 256, 0, stream>>>(keys_out, dz->tri_off_dev, sumT, left, right, rfirst, rcount,
+                                                lbox, nbox, dz->nodes, leaf_max);
+        return cudaGetLastError();
+    };
+    const cudaError_t e = build();
+    void *scratch[8] = { keys, keys_out, vals, vals_out, ibuf, lbox, nbox, tmp };
+    for (void *q : scratch)
+        if (q) cudaFreeAsync(q, stream);
     return e;
 }
 

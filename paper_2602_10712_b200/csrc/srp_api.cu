@@ -2,6 +2,7 @@
 // handle ownership, workspace, and the enqueue order of the kernels in mesh_gen.cu / lbvh.cu /
 // trace.cu.  No arithmetic of the method lives here.
 #include <cstdio>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include "srp_internal.cuh"
@@ -23,9 +24,28 @@ srp_status cuda_fail(srp_context *ctx, const char *what, cudaError_t e)
     return fail(ctx, e == cudaErrorMemoryAllocation ? SRP_ERR_OOM : SRP_ERR_CUDA, what, e);
 }
 
+void count_launches(srp_context *ctx, unsigned n) { ctx->launches_total += n; ctx->launches_call += n; }
+
 #define TRY_CUDA(ctx, call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, what, e_); } while (0)
 
-// design arrays come from the device's stream-ordered pool (no device-wide synchronisation per build)
+// design arrays come from the context's own stream-ordered pool (no device-wide synchronisation per build; the
+// device's default pool is left alone)
+cudaError_t pool_alloc(srp_context *ctx, void **p, size_t bytes)
+{
+    return cudaMallocFromPoolAsync(p, bytes, ctx->mempool, ctx->stream);
+}
+template <typename T> cudaError_t pool_alloc(srp_context *ctx, T **p, size_t bytes) { return pool_alloc(ctx, (void **)p, bytes); }
+
+// Fixed-point scale of the accumulators: the largest power of two <= 2^32 with which N photons of at most B + 1 hits
+// (each deposit at most 2 photon weights; torque arms are summed in units of the design's extent) stay below 2^62.
+double acc_scale_for(double photons, int B)
+{
+    const double bound = photons * 2.0 * (double)(B + 2);
+    int bits = SRP_ACC_BITS_MAX;
+    while (bits > 0 && bound * ldexp(1.0, bits) >= ldexp(1.0, 62)) --bits;
+    return ldexp(1.0, bits);
+}
+
 void free_designs_mem(srp_context *ctx, srp_designs *d)
 {
     void *ptrs[10] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm, d->esc, d->nplane, d->shin };
@@ -37,13 +57,13 @@ void free_designs_mem(srp_context *ctx, srp_designs *d)
 srp_status alloc_designs(srp_context *ctx, srp_designs *d)
 {
     const long long sumT = d->sumT;
-    TRY_CUDA(ctx, cudaMallocAsync(&d->verts_orig, sizeof(float) * 9 * sumT, ctx->stream), "alloc verts");
-    TRY_CUDA(ctx, cudaMallocAsync(&d->mats_orig, sizeof(float) * 3 * sumT, ctx->stream), "alloc mats");
-    TRY_CUDA(ctx, cudaMallocAsync(&d->tri, sizeof(float4) * 3 * sumT, ctx->stream), "alloc packed triangles");
-    if (d->has_bvh) TRY_CUDA(ctx, cudaMallocAsync(&d->nodes, sizeof(float4) * 4 * sumT, ctx->stream), "alloc nodes");
-    TRY_CUDA(ctx, cudaMallocAsync(&d->tri_off_dev, sizeof(long long) * (d->D + 1), ctx->stream), "alloc offsets");
-    TRY_CUDA(ctx, cudaMallocAsync(&d->box, sizeof(float4) * 2 * d->D, ctx->stream), "alloc boxes");
-    TRY_CUDA(ctx, cudaMallocAsync(&d->perm, sizeof(int) * sumT, ctx->stream), "alloc perm");
+    TRY_CUDA(ctx, pool_alloc(ctx, &d->verts_orig, sizeof(float) * 9 * sumT), "alloc verts");
+    TRY_CUDA(ctx, pool_alloc(ctx, &d->mats_orig, sizeof(float) * 3 * sumT), "alloc mats");
+    TRY_CUDA(ctx, pool_alloc(ctx, &d->tri, sizeof(float4) * 3 * sumT), "alloc packed triangles");
+    if (d->has_bvh) TRY_CUDA(ctx, pool_alloc(ctx, &d->nodes, sizeof(float4) * 4 * sumT), "alloc nodes");
+    TRY_CUDA(ctx, pool_alloc(ctx, &d->tri_off_dev, sizeof(long long) * (d->D + 1)), "alloc offsets");
+    TRY_CUDA(ctx, pool_alloc(ctx, &d->box, sizeof(float4) * 2 * d->D), "alloc boxes");
+    TRY_CUDA(ctx, pool_alloc(ctx, &d->perm, sizeof(int) * sumT), "alloc perm");
     TRY_CUDA(ctx, cudaMemcpyAsync(d->tri_off_dev, d->tri_off.data(), sizeof(long long) * (d->D + 1),
                                   cudaMemcpyHostToDevice, ctx->stream), "copy offsets");
     // d->tri_off (the pageable source) lives as long as the handle
@@ -53,6 +73,10 @@ srp_status alloc_designs(srp_context *ctx, srp_designs *d)
 srp_status ensure_workspace(srp_context *ctx, size_t accum_items)
 {
     if (!ctx->stats) TRY_CUDA(ctx, cudaMalloc(&ctx->stats, sizeof(DevStats)), "alloc stats");
+    if (!ctx->rounds_total) {
+        TRY_CUDA(ctx, cudaMalloc(&ctx->rounds_total, sizeof(unsigned long long)), "alloc round counter");
+        TRY_CUDA(ctx, cudaMemsetAsync(ctx->rounds_total, 0, sizeof(unsigned long long), ctx->stream), "zero round counter");
+    }
     if (!ctx->work_counter) TRY_CUDA(ctx, cudaMalloc(&ctx->work_counter, sizeof(unsigned long long)), "alloc counter");
     if (ctx->accum_items < accum_items) {
         TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before workspace growth");
@@ -133,9 +157,11 @@ srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bo
 {
     if (!a.rq) {
         TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "trace launch");
+        count_launches(ctx, 1);
         return SRP_OK;
     }
     if (ctx->opt.plain_launches) {                          // a sufficient number of rounds; surplus ones find nothing to do
+        count_launches(ctx, 1);
         const long long rounds = (long long)((double)a.n_pairs * (double)a.N / (double)a.rq_high) + 1;
         for (long long r = 0; r < rounds; ++r) {
             TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "beam launch");
@@ -143,6 +169,7 @@ srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bo
         }
         return SRP_OK;
     }
+    count_launches(ctx, 1);                                 // at least one beam launch; the rounds are counted on the device
     reap_graphs(ctx, false);
     if (!ctx->capture_stream)
         TRY_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "create capture stream");
@@ -191,8 +218,8 @@ srp_status ensure_masks(srp_context *ctx, const srp_designs *dz, double rays)
     if (ctx->opt.escape_masks == 1 && rays < 32768.0 * (double)d->sumT) return SRP_OK;
     unsigned *esc = nullptr;
     float4 *nplane = nullptr;
-    if (cudaMallocAsync(&esc, sizeof(unsigned) * 2 * ESC_WORDS * d->sumT, ctx->stream) != cudaSuccess ||
-        (d->has_bvh && cudaMallocAsync(&nplane, sizeof(float4) * 2 * d->sumT, ctx->stream) != cudaSuccess)) {
+    if (pool_alloc(ctx, &esc, sizeof(unsigned) * 2 * ESC_WORDS * d->sumT) != cudaSuccess ||
+        (d->has_bvh && pool_alloc(ctx, &nplane, sizeof(float4) * 2 * d->sumT) != cudaSuccess)) {
         cudaGetLastError();                                   // no room: trace without masks
         if (esc) cudaFreeAsync(esc, ctx->stream);
         d->esc_failed = true;
@@ -207,6 +234,7 @@ srp_status ensure_masks(srp_context *ctx, const srp_designs *dz, double rays)
         e = srp_launch_escape_masks_small(d->dev(), d->sumT, esc, ctx->stream);   // T <= 64: every pair of triangles
     }
     if (e != cudaSuccess) { cudaFreeAsync(esc, ctx->stream); return cuda_fail(ctx, "escape mask build", e); }
+    count_launches(ctx, d->has_bvh ? 2 : 1);
     d->esc = esc;
     return SRP_OK;
 }
@@ -236,7 +264,8 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
     a.sampler = ctx->opt.sampler; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
     a.accum = ctx->accum; a.acc_stride = 3; a.torque = 0; a.xcom = nullptr;
-    a.stats = ctx->stats; a.work_counter = ctx->work_counter;
+    a.stats = ctx->stats; a.work_counter = ctx->work_counter; a.rounds_total = ctx->rounds_total;
+    a.acc_scale = acc_scale_for((double)N, B);
     // tile size: large tiles amortise the per-item set-up and the drain at the end of a tile; shrink
     // them only when there would be too few items to occupy every resident warp several times
     const bool brute = !dz->has_bvh;
@@ -253,14 +282,17 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     return a;
 }
 
-// out_torques != nullptr: also the torque about x_com (DEVICE float[D,3], or nullptr = the origin), Eq. 4.
+// out_second != nullptr: a second output from the same trace -- second = 1: the torque about x_com (DEVICE float[D,3],
+// or nullptr = the origin), Eq. 4; second = 2: the direct part of the force.
 srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
                       long long n_pairs, long long N, int B, unsigned long long seed, float *out,
-                      const float *x_com = nullptr, float *out_torques = nullptr)
+                      const float *x_com = nullptr, float *out_second = nullptr, int second = 1)
 {
+    float *out_torques = out_second;
     const int stride = out_torques ? 6 : 3;
+    ctx->launches_call = 0;
     if (out_torques && ctx->opt.instrumented)
-        return fail(ctx, SRP_ERR_UNSUPPORTED, "torques are not available from the instrumented kernels");
+        return fail(ctx, SRP_ERR_UNSUPPORTED, "a second output is not available from the instrumented kernels");
     srp_status st = ensure_workspace(ctx, (size_t)n_pairs * stride);
     if (st != SRP_OK) return st;
     if (B > 0 && !(ctx->opt.force_brute != 0)) {
@@ -268,7 +300,7 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
         if (st != SRP_OK) return st;
     }
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
-    a.accum = ctx->accum; a.acc_stride = stride; a.torque = out_torques ? 1 : 0; a.xcom = x_com;
+    a.accum = ctx->accum; a.acc_stride = stride; a.torque = out_torques ? second : 0; a.xcom = x_com;
     if (ctx->opt.escape_masks == 0) a.dz.esc = nullptr;        // masks an earlier call built stay unused
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * stride * n_pairs, ctx->stream), "zero accumulators");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
@@ -279,6 +311,7 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
     st = launch_trace_all(ctx, a, brute, ctx->opt.instrumented != 0);
     if (st != SRP_OK) return st;
     TRY_CUDA(ctx, srp_launch_finalize(a, out, out_torques, ctx->stream), "finalize launch");
+    count_launches(ctx, 1);
     return SRP_OK;
 }
 
@@ -303,12 +336,14 @@ srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
     ctx->opt.plain_launches = 0; ctx->opt.leaf_max = 0;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
-    {   // keep freed blocks in the stream-ordered pool: builds reuse them instead of going back to the driver
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, cuda_device) == cudaSuccess) {
-            unsigned long long keep = ~0ULL;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
+    {   // a pool of the context's own that keeps freed blocks: builds reuse them instead of going back to the driver
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned; props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice; props.location.id = cuda_device;
+        if (cudaMemPoolCreate(&ctx->mempool, &props) != cudaSuccess) { delete ctx; return SRP_ERR_CUDA; }
+        unsigned long long keep = ~0ULL;
+        cudaMemPoolSetAttribute(ctx->mempool, cudaMemPoolAttrReleaseThreshold, &keep);
     }
     *out = ctx;
     return SRP_OK;
@@ -324,8 +359,8 @@ srp_status srp_destroy(srp_context *ctx)
     cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->rq_ctr);
     if (ctx->rq_owned) cudaFree(ctx->rq);
     cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);
-    cudaMemPool_t pool;                                       // hand the pooled design memory back
-    if (cudaDeviceGetDefaultMemPool(&pool, ctx->device) == cudaSuccess) cudaMemPoolTrimTo(pool, 0);
+    cudaFree(ctx->rounds_total);
+    if (ctx->mempool) cudaMemPoolDestroy(ctx->mempool);       // designs not freed by now go with it
     delete ctx;
     return SRP_OK;
 }
@@ -373,6 +408,7 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
     if (D <= 0 || D > 65535) return fail(ctx, SRP_ERR_INVALID, "D must be in [1, 65535]");
     if (n_params != srp_family_n_params(family)) return fail(ctx, SRP_ERR_INVALID, "wrong n_params for this family");
     if ((long long)D * T >= (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "too many triangles in one batch");
+    if (T >= (1LL << 27) - 1) return fail(ctx, SRP_ERR_INVALID, "design too large (a ray's source triangle is a 27-bit field)");
     cudaSetDevice(ctx->device);
     srp_designs *d = new (std::nothrow) srp_designs();
     if (!d) return fail(ctx, SRP_ERR_OOM, "host allocation");
@@ -384,8 +420,9 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
     if (st != SRP_OK) { free_designs_mem(ctx, d); delete d; return st; }
     cudaError_t e = srp_launch_mesh_gen((int)family, theta, D, n_params, mesh_seed, T, d->verts_orig,
                                         d->mats_orig, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->mempool, ctx->stream);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
+    ctx->launches_total += 2 + SRP_BUILD_KERNELS(d->has_bvh);          // mesh generation: 2 kernels
     *out = d;
     return SRP_OK;
 }
@@ -403,7 +440,7 @@ srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, c
     for (int k = 0; k < D; ++k) {
         const long long t = tri_offsets[k + 1] - tri_offsets[k];
         if (t <= 0) return fail(ctx, SRP_ERR_INVALID, "tri_offsets must be strictly increasing");
-        if (t >= (1LL << 28)) return fail(ctx, SRP_ERR_INVALID, "design too large");
+        if (t >= (1LL << 27) - 1) return fail(ctx, SRP_ERR_INVALID, "design too large (a ray's source triangle is a 27-bit field)");
         if (t > maxT) maxT = t;
     }
     if (tri_offsets[D] >= (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "too many triangles in one batch");
@@ -418,8 +455,9 @@ srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, c
     cudaError_t e = cudaMemcpyAsync(d->verts_orig, verts, sizeof(float) * 9 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(d->mats_orig, mats, sizeof(float) * 3 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->stream);
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->mempool, ctx->stream);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
+    ctx->launches_total += SRP_BUILD_KERNELS(d->has_bvh);
     *out = d;
     return SRP_OK;
 }
@@ -471,7 +509,7 @@ srp_status srp_designs_set_shininess(srp_context *ctx, srp_designs *dz, const fl
         dz->shin = nullptr;
         return SRP_OK;
     }
-    if (!dz->shin) TRY_CUDA(ctx, cudaMallocAsync(&dz->shin, sizeof(float) * dz->sumT, ctx->stream), "alloc shininess");
+    if (!dz->shin) TRY_CUDA(ctx, pool_alloc(ctx, &dz->shin, sizeof(float) * dz->sumT), "alloc shininess");
     TRY_CUDA(ctx, srp_launch_gather_shininess(dz->dev(), dz->sumT, shininess, dz->shin, ctx->stream), "shininess gather");
     return SRP_OK;
 }
@@ -518,6 +556,28 @@ srp_status srp_forces_torques_pairs(srp_context *ctx, const srp_designs *dz, con
     return run_forces(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed, out_forces, x_com, out_torques);
 }
 
+srp_status srp_forces_split(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, long long N, int B,
+                            unsigned long long seed, float *out_forces, float *out_direct)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out_forces);
+    if (st != SRP_OK) return st;
+    if (!out_direct) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    cudaSetDevice(ctx->device);
+    return run_forces(ctx, dz, sun_dirs, S, nullptr, (long long)dz->D * S, N, B, seed, out_forces, nullptr, out_direct, 2);
+}
+
+srp_status srp_forces_split_pairs(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, const int *pairs,
+                                  long long n_pairs, long long N, int B, unsigned long long seed, float *out_forces,
+                                  float *out_direct)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out_forces);
+    if (st != SRP_OK) return st;
+    if (!out_direct) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    if (!pairs || n_pairs <= 0) return fail(ctx, SRP_ERR_INVALID, "bad pair list");
+    cudaSetDevice(ctx->device);
+    return run_forces(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed, out_forces, nullptr, out_direct, 2);
+}
+
 srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *dz, const float *facet_power, long long N, int B,
                               unsigned long long seed, float *out_forces)
 {
@@ -527,6 +587,7 @@ srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *dz, const flo
     if (B < 0 || B > 15) return fail(ctx, SRP_ERR_INVALID, "max_bounces must be in [0, 15]");
     if (dz->sumT >= (1LL << 31)) return fail(ctx, SRP_ERR_UNSUPPORTED, "too many triangles for the emitter list");
     cudaSetDevice(ctx->device);
+    ctx->launches_call = 0;
     srp_status st = ensure_workspace(ctx, (size_t)dz->D * 3);
     if (st != SRP_OK) return st;
     st = ensure_masks(ctx, dz, (double)N * (double)dz->sumT);
@@ -539,19 +600,25 @@ srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *dz, const flo
     a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
     a.sampler = 0; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
     a.accum = ctx->accum; a.acc_stride = 3; a.stats = ctx->stats; a.work_counter = ctx->work_counter;
+    a.rounds_total = ctx->rounds_total;
+    a.acc_scale = acc_scale_for((double)N, B + 1);             // per design: the facets' weights |W_f| / P_k sum to 1
     a.tile_rays = (int)(N < 8192 ? N : 8192);
     a.tiles_per_pair = (N + a.tile_rays - 1) / a.tile_rays;
     int *emit_list = nullptr, *n_emit = nullptr;
     float *design_power = nullptr;
-    TRY_CUDA(ctx, cudaMallocAsync(&emit_list, sizeof(int) * dz->sumT, ctx->stream), "alloc emitter list");
-    TRY_CUDA(ctx, cudaMallocAsync(&n_emit, sizeof(int), ctx->stream), "alloc emitter count");
-    TRY_CUDA(ctx, cudaMallocAsync(&design_power, sizeof(float) * dz->D, ctx->stream), "alloc design power");
-    TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * dz->D, ctx->stream), "zero accumulators");
-    TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
-    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
-    TRY_CUDA(ctx, srp_launch_thermal(a, facet_power, dz->sumT, emit_list, n_emit, design_power, out_forces, ctx->num_sms,
-                                     ctx->stream), "thermal launch");
-    cudaFreeAsync(emit_list, ctx->stream); cudaFreeAsync(n_emit, ctx->stream); cudaFreeAsync(design_power, ctx->stream);
+    cudaError_t e = pool_alloc(ctx, &emit_list, sizeof(int) * dz->sumT);
+    if (e == cudaSuccess) e = pool_alloc(ctx, &n_emit, sizeof(int));
+    if (e == cudaSuccess) e = pool_alloc(ctx, &design_power, sizeof(float) * dz->D);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * dz->D, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream);
+    if (e == cudaSuccess)
+        e = srp_launch_thermal(a, facet_power, dz->sumT, emit_list, n_emit, design_power, out_forces, ctx->num_sms, ctx->stream);
+    if (emit_list) cudaFreeAsync(emit_list, ctx->stream);      // stream-ordered: after the kernels that use them
+    if (n_emit) cudaFreeAsync(n_emit, ctx->stream);
+    if (design_power) cudaFreeAsync(design_power, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "thermal forces", e);
+    count_launches(ctx, 4);
     return SRP_OK;
 }
 
@@ -618,6 +685,7 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const fl
         st = ensure_masks(ctx, dz, (double)n_pairs * (double)N);
         if (st != SRP_OK) return st;
     }
+    ctx->launches_call = 0;
     TraceArgs a = make_args(ctx, dz, sun_dirs, S, pairs, n_pairs, N, B, seed);
     a.accum = ctx->accum;
     a.sig_out = out_sig;
@@ -641,6 +709,41 @@ srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out)
     TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
     static_assert(sizeof(DevStats) == sizeof(srp_stats), "stats layout");
     TRY_CUDA(ctx, cudaMemcpy(host_out, ctx->stats, sizeof(DevStats), cudaMemcpyDeviceToHost), "read stats");
+    // the loop's kernels: beam + bounce per round that queued rays, one more beam launch that found the tiles spent
+    // or queued nothing, and the loop-condition kernel of each round when the loop is a graph
+    host_out->kernel_launches = ctx->launches_call + host_out->loop_rounds * (ctx->opt.plain_launches ? 2ULL : 3ULL);
+    return SRP_OK;
+}
+
+srp_status srp_launch_count(srp_context *ctx, unsigned long long *n_kernels)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!n_kernels) return fail(ctx, SRP_ERR_INVALID, "null output");
+    cudaSetDevice(ctx->device);
+    unsigned long long rounds = 0;
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
+    if (ctx->rounds_total) TRY_CUDA(ctx, cudaMemcpy(&rounds, ctx->rounds_total, sizeof rounds, cudaMemcpyDeviceToHost), "read rounds");
+    *n_kernels = ctx->launches_total + rounds * (ctx->opt.plain_launches ? 2ULL : 3ULL);
+    return SRP_OK;
+}
+
+unsigned long long srp_workspace_bytes_min(const srp_context *ctx)
+{
+    if (!ctx) return 0;
+    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * 8192u;   // the largest tile (make_args)
+    return (unsigned long long)((reserve + (1u << 20)) * SRP_RQ_FIELDS_INSTR * sizeof(unsigned));
+}
+
+srp_status srp_set_workspace(srp_context *ctx, void *ptr, unsigned long long bytes)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    cudaSetDevice(ctx->device);
+    if ((ptr == nullptr) != (bytes == 0)) return fail(ctx, SRP_ERR_INVALID, "workspace pointer and size must both be given, or neither");
+    if (ptr && ((uintptr_t)ptr & 255u)) return fail(ctx, SRP_ERR_INVALID, "workspace must be 256-byte aligned");
+    if (ptr && bytes < srp_workspace_bytes_min(ctx)) return fail(ctx, SRP_ERR_INVALID, "workspace smaller than srp_workspace_bytes_min");
+    TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before the workspace changes");
+    if (ctx->rq_owned) cudaFree(ctx->rq);
+    ctx->rq = (unsigned *)ptr; ctx->rq_words = (size_t)(bytes / sizeof(unsigned)); ctx->rq_owned = false;
     return SRP_OK;
 }
 

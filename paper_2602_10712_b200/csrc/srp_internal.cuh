@@ -10,7 +10,7 @@
 
 #define SRP_BRUTE_MAX_TRIS 64      // designs with T <= this are traced without a hierarchy (one leaf)
 #define SRP_LEAF_MAX 2             // LBVH subtrees with <= this many triangles become one leaf (cfg3 -7 %, cfg5 -3 % against 3)
-#define SRP_ACC_SCALE 4294967296.0 // fixed-point scale (2^32) of the dimensionless force accumulators
+#define SRP_ACC_BITS_MAX 32        // fixed-point fraction bits of the dimensionless force accumulators, at most
 
 // Packed, BVH-sorted triangle: 3 x float4 = 48 B, fetched as three 16-byte loads.
 //   q0 = (v0.x, v0.y, v0.z, alpha)   q1 = (e1.x, e1.y, e1.z, rho_s)   q2 = (e2.x, e2.y, e2.z, rho_d)
@@ -64,6 +64,7 @@ struct DevStats {           // device mirror of srp_stats
     unsigned long long beam_tile_miss, beam_block_miss, beam_group_miss, beam_fallback;
     unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
     unsigned long long mask_escapes;
+    unsigned long long queued_rays, loop_rounds, kernel_launches;
 };
 
 struct srp_context {
@@ -79,6 +80,10 @@ struct srp_context {
     unsigned *rq = nullptr;       size_t rq_words = 0;        // ray queue between the beam and the bounce kernel
     unsigned *rq_ctr = nullptr;                               // its counters: [0] tail, [1] head, [2] warps done
     bool rq_owned = false;                                    // allocated by the library (else srp_set_workspace)
+    unsigned long long launches_total = 0;                    // kernels enqueued by the host since srp_create
+    unsigned long long launches_call = 0;                     // ... by the last srp_forces* call
+    unsigned long long *rounds_total = nullptr;               // device: loop rounds since srp_create
+    cudaMemPool_t mempool = nullptr;                          // design arrays come from this private stream-ordered pool
     cudaStream_t capture_stream = nullptr;                    // the beam / bounce loop is captured here into a graph
     struct PendingGraph { cudaGraphExec_t exec; cudaGraph_t graph; cudaEvent_t done; };
     std::vector<PendingGraph> graphs;                         // launched loops; destroyed once they have run
@@ -99,8 +104,11 @@ struct TraceArgs {
     int sampler, deposit;
     double P;
     long long *accum;        // [n_pairs*acc_stride]: force (and torque) sums in 2^-32 fixed point
-    int acc_stride;          // 3, or 6 with torque
-    int torque;              // 1: also accumulate torque about xcom
+    int acc_stride;          // 3, or 6 with a second output
+    int torque;              // second output: 0 none, 1 torque about xcom (arm in units of the design's extent, see
+                             // torque_arm_scale), 2 direct part of the force (deposits at depth 0)
+    double acc_scale;        // 2^bits: the accumulators hold sums of deposits / w_ph in this fixed point (srp_api.cu,
+                             // acc_scale_for: chosen per call so that N photons of B + 1 hits cannot overflow int64)
     const float *xcom;       // [D,3] centres of mass, or nullptr (origin)
     DevStats *stats;
     unsigned long long *work_counter;
@@ -112,6 +120,7 @@ struct TraceArgs {
     unsigned rq_cap;               // rays the queue holds
     unsigned rq_high;              // beam warps stop taking tiles once this many rays are queued
     unsigned *rq_ctr;              // [0] tail (rays queued), [1] head (rays claimed), [2] bounce warps done
+    unsigned long long *rounds_total;   // loop rounds since srp_create (srp_launch_count)
     long long max_tris;            // largest design of the batch
     int primary_mode;              // srp_options.primary_mode
 };
@@ -120,7 +129,8 @@ struct TraceArgs {
 cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_params,
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
                                 cudaStream_t stream);
-cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaStream_t stream);
+cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, cudaStream_t stream);   // 2 kernels without a BVH, 6 with
+#define SRP_BUILD_KERNELS(has_bvh) ((has_bvh) ? 6 : 2)
 cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted, cudaStream_t stream);
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream);
 cudaError_t srp_launch_escape_masks_small(const DesignsDev &dz, long long sumT, unsigned *esc, cudaStream_t stream);

@@ -86,13 +86,13 @@ bounce_trace_kernel(const TraceArgs a)
             if (fate == SHADE_CAPPED) cn.capped++;
             // S7: these hits are ~1 % of the segments; one fixed-point atomic per component and hit
             unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * (long long)p);
-            if (dep.x != 0.0f) atomicAdd(dst + 0, (unsigned long long)__double2ll_rn((double)dep.x * SRP_ACC_SCALE));
-            if (dep.y != 0.0f) atomicAdd(dst + 1, (unsigned long long)__double2ll_rn((double)dep.y * SRP_ACC_SCALE));
-            if (dep.z != 0.0f) atomicAdd(dst + 2, (unsigned long long)__double2ll_rn((double)dep.z * SRP_ACC_SCALE));
+            if (dep.x != 0.0f) atomicAdd(dst + 0, (unsigned long long)__double2ll_rn((double)dep.x * a.acc_scale));
+            if (dep.y != 0.0f) atomicAdd(dst + 1, (unsigned long long)__double2ll_rn((double)dep.y * a.acc_scale));
+            if (dep.z != 0.0f) atomicAdd(dst + 2, (unsigned long long)__double2ll_rn((double)dep.z * a.acc_scale));
             if (TORQUE) {
-                if (dep_t.x != 0.0f) atomicAdd(dst + 3, (unsigned long long)__double2ll_rn((double)dep_t.x * SRP_ACC_SCALE));
-                if (dep_t.y != 0.0f) atomicAdd(dst + 4, (unsigned long long)__double2ll_rn((double)dep_t.y * SRP_ACC_SCALE));
-                if (dep_t.z != 0.0f) atomicAdd(dst + 5, (unsigned long long)__double2ll_rn((double)dep_t.z * SRP_ACC_SCALE));
+                if (dep_t.x != 0.0f) atomicAdd(dst + 3, (unsigned long long)__double2ll_rn((double)dep_t.x * a.acc_scale));
+                if (dep_t.y != 0.0f) atomicAdd(dst + 4, (unsigned long long)__double2ll_rn((double)dep_t.y * a.acc_scale));
+                if (dep_t.z != 0.0f) atomicAdd(dst + 5, (unsigned long long)__double2ll_rn((double)dep_t.z * a.acc_scale));
             }
             if (INSTR && fate != SHADE_CONTINUE && a.sig_out) a.sig_out[(long long)p * a.N + i] = sig;
         }
@@ -220,6 +220,7 @@ bounce_trace_kernel(const TraceArgs a)
     if (lane == 0) {
         __threadfence();
         if (atomicAdd(a.rq_ctr + 2, 1u) == gridDim.x * TRACE_WARPS - 1u) {
+            if (n_queued != 0u) { a.stats->queued_rays += n_queued; a.stats->loop_rounds += 1ULL; *a.rounds_total += 1ULL; }
             a.rq_ctr[0] = 0u; a.rq_ctr[1] = 0u; a.rq_ctr[2] = 0u;
             __threadfence();
         }

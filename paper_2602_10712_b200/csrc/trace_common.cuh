@@ -110,6 +110,8 @@ struct RayGen {            // warp-uniform per work item
     int sampler;
     float inv_nx, inv_ny;
     float3 xc;             // the design's centre of mass (TORQUE kernels: Eq. 4)
+    float inv_arm;         // 1 / torque_arm_scale of the design: arms are summed in units of the design's extent
+    bool split;            // TORQUE kernels: the second sum is the direct force (depth-0 deposits), not the torque
 };
 
 // O-step 3: ray i of the pair.
@@ -343,8 +345,13 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     auto put = [&](const float3 dd) {
         acc.x += dd.x; acc.y += dd.y; acc.z += dd.z;
         if (TORQUE) {
-            const float3 r = f3(x.x - g.xc.x, x.y - g.xc.y, x.z - g.xc.z), m = cross3(r, dd);
-            acc_t.x += m.x; acc_t.y += m.y; acc_t.z += m.z;
+            if (g.split) {                                        // direct part: what sun light deposits at its first hit
+                if (depth == 0) { acc_t.x += dd.x; acc_t.y += dd.y; acc_t.z += dd.z; }
+            } else {
+                const float3 r = f3((x.x - g.xc.x) * g.inv_arm, (x.y - g.xc.y) * g.inv_arm, (x.z - g.xc.z) * g.inv_arm);
+                const float3 m = cross3(r, dd);
+                acc_t.x += m.x; acc_t.y += m.y; acc_t.z += m.z;
+            }
         }
     };
     const float al = q0.w, rs = q1.w, rd = q2.w;
@@ -407,22 +414,40 @@ __device__ __forceinline__ int shade(const float4 q0, const float4 q1, const flo
     return SHADE_CONTINUE;
 }
 
-// same for a pair index known to fit 32 bits (rays of the beam kernel's pool)
+// Pair p -> (design k, direction j).  Entries of a caller's pair list are clamped into range: a bad list gives
+// meaningless forces, never an out-of-bounds read.
+__device__ __forceinline__ void clamp_pair(const TraceArgs &a, int &k, int &j)
+{
+    k = min(max(k, 0), a.dz.D - 1); j = min(max(j, 0), a.S - 1);
+}
+// same for a pair index known to fit 32 bits (rays of the ray queue)
 __device__ __forceinline__ void pair_of32(const TraceArgs &a, uint32_t p, int &k, int &j)
 {
-    if (a.pairs) { k = a.pairs[2 * (size_t)p]; j = a.pairs[2 * (size_t)p + 1]; }
+    if (a.pairs) { k = a.pairs[2 * (size_t)p]; j = a.pairs[2 * (size_t)p + 1]; clamp_pair(a, k, j); }
     else { const uint32_t kk = p / (uint32_t)a.S; k = (int)kk; j = (int)(p - kk * (uint32_t)a.S); }
 }
 __device__ __forceinline__ void pair_of(const TraceArgs &a, long long p, int &k, int &j)
 {
-    if (a.pairs) { k = a.pairs[2 * p]; j = a.pairs[2 * p + 1]; }
+    if (a.pairs) { k = a.pairs[2 * p]; j = a.pairs[2 * p + 1]; clamp_pair(a, k, j); }
     else { k = (int)(p / a.S); j = (int)(p - (long long)k * a.S); }
+}
+
+// Torque arms |x - x_COM| are summed in units of this length (an upper bound of the arm over the design's box), so
+// that the fixed-point torque sums have the range of the force sums whatever the mesh's units; finalize_kernel
+// multiplies it back.
+__device__ __forceinline__ float torque_arm_scale(const float4 lo, const float4 hi, const float3 xc)
+{
+    const float ax = fmaxf(fabsf(lo.x - xc.x), fabsf(hi.x - xc.x)), ay = fmaxf(fabsf(lo.y - xc.y), fabsf(hi.y - xc.y)),
+                az = fmaxf(fabsf(lo.z - xc.z), fabsf(hi.z - xc.z));
+    return fmaxf(sqrtf(ax * ax + ay * ay + az * az), 1e-30f);
 }
 
 template <bool TORQUE>
 __device__ __forceinline__ void set_torque(RayGen &g, const TraceArgs &a, int k)
 {
     g.xc = (TORQUE && a.xcom) ? f3(a.xcom[3 * k], a.xcom[3 * k + 1], a.xcom[3 * k + 2]) : f3(0.f, 0.f, 0.f);
+    g.split = TORQUE && a.torque == 2;
+    g.inv_arm = (TORQUE && a.torque == 1) ? 1.0f / torque_arm_scale(a.dz.box[2 * k], a.dz.box[2 * k + 1], g.xc) : 1.0f;
 }
 
 // S7 for one work item: per-lane fp32 sums -> fp64 warp shuffle tree -> one fixed-point atomic per component.
@@ -438,7 +463,7 @@ __device__ __forceinline__ void flush_tile_acc(const TraceArgs &a, long long p, 
         for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
         if (lane == 0) {
             unsigned long long *dst = (unsigned long long *)(a.accum + a.acc_stride * p);
-            atomicAdd(dst + c, (unsigned long long)__double2ll_rn(v * SRP_ACC_SCALE));
+            atomicAdd(dst + c, (unsigned long long)__double2ll_rn(v * a.acc_scale));
         }
     }
 }

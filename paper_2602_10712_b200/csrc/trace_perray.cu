@@ -221,12 +221,19 @@ __global__ void __launch_bounds__(256) finalize_kernel(const TraceArgs a, float 
     int k, j;
     pair_of(a, p, k, j);
     const Emitter em = make_emitter(a.sun_dirs, j, a.dz.box[2 * k], a.dz.box[2 * k + 1]);
-    const double w = em.Ae > 0.0f ? a.P * (double)em.Ae / (double)a.N / SRP_ACC_SCALE : 0.0;
+    const double w = em.Ae > 0.0f ? a.P * (double)em.Ae / (double)a.N / a.acc_scale : 0.0;
 #pragma unroll
     for (int c = 0; c < 3; ++c) out[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + c] * w);
-    if (a.torque && out_torque)
+    if (a.torque && out_torque) {
+        // second output: torque (arms were summed in units of torque_arm_scale), or the direct part of the force
+        double w2 = w;
+        if (a.torque == 1) {
+            const float3 xc = a.xcom ? f3(a.xcom[3 * k], a.xcom[3 * k + 1], a.xcom[3 * k + 2]) : f3(0.f, 0.f, 0.f);
+            w2 *= (double)torque_arm_scale(a.dz.box[2 * k], a.dz.box[2 * k + 1], xc);
+        }
 #pragma unroll
-        for (int c = 0; c < 3; ++c) out_torque[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + 3 + c] * w);
+        for (int c = 0; c < 3; ++c) out_torque[3 * p + c] = (float)((double)a.accum[a.acc_stride * p + 3 + c] * w2);
+    }
 }
 
 // debug: primary-hit triangle (original index) of every ray of the listed pairs

@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(256) thermal_finalize_kernel(const TraceArgs a
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= a.dz.D) return;
-    const double w = (double)design_power[k] / (C_LIGHT * (double)a.N) / SRP_ACC_SCALE;
+    const double w = (double)design_power[k] / (C_LIGHT * (double)a.N) / a.acc_scale;
 #pragma unroll
     for (int c = 0; c < 3; ++c) out[3 * k + c] = (float)((double)a.accum[3 * k + c] * w);
 }

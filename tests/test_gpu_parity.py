@@ -771,23 +771,105 @@ def test_cfg5_full_N_properties_and_reduced_N_oracle(ctx, oracle):
 
 
 def test_force_maps_direct_and_indirect(ctx):
-    """PAPER.md:394 force maps.  A convex body has no indirect light (its map is the closed form of P3, indirect = 0
-    up to seam rays); the box-wing has some, and total = direct + indirect by construction."""
+    """PAPER.md:394 force maps from srp_forces_split.  A convex body has no indirect light (its map is the closed
+    form of P3, direct = total exactly); the box-wing has some."""
     verts = W.icosphere(2, 1.0)
     mats = W.dirichlet_materials(len(verts), 3)
     dz = ctx.srp_build_designs_from_meshes(verts, mats, [0, len(verts)])
-    total, direct, indirect = ctx.force_maps(dz, 4, 8, 1 << 14, 3, seed=1)
+    total, direct = ctx.force_maps(dz, 4, 8, 1 << 14, 3, seed=1)
     sun = W.latlong_directions(4, 8)
     t = total.cpu().numpy().reshape(-1, 3)
     for j in range(len(sun)):
         assert rel_l2(t[j], convex_polyhedron_force(verts, mats, sun[j])) < 5e-3
-    assert float(indirect.abs().max()) <= 1e-3 * float(total.abs().max())
+    assert float((total - direct).abs().max()) <= 1e-3 * float(total.abs().max())
     dz.free()
     dz = ctx.srp_build_designs(W.FAMILY_BOXWING, W.draw_params(W.FAMILY_BOXWING, 2))
-    total, direct, indirect = ctx.force_maps(dz, 4, 8, 1 << 14, 4, seed=1)
+    total, direct = ctx.force_maps(dz, 4, 8, 1 << 14, 4, seed=1)
+    indirect = total - direct
     assert tuple(total.shape) == (2, 4, 8, 3)
     assert float(indirect.abs().max()) > 1e-3 * float(total.abs().max())
     assert float(indirect.abs().max()) < float(direct.abs().max())
+    dz.free()
+
+
+@pytest.mark.parametrize("family,D,S,N,B,mode,deposit", [
+    (W.FAMILY_BOXWING, 3, 6, 1 << 14, 4, 0, 0),        # small_beam_kernel
+    (W.FAMILY_BOXWING6, 3, 6, 1 << 12, 4, 1, 1),       # trace_kernel (all triangles, every segment), analog deposit
+    (W.FAMILY_DETAILED, 2, 3, 1 << 12, 8, 1, 0),       # bvh_trace_kernel
+    (W.FAMILY_DETAILED, 2, 3, 1 << 12, 8, 2, 0),       # beam_trace_kernel (all direct) + bounce_trace_kernel
+])
+def test_direct_indirect_split_matches_oracle(ctx, oracle, family, D, S, N, B, mode, deposit):
+    """srp_forces_split against the oracle's split on the same photons: the total is srp_forces' (same photons),
+    the direct part is the B = 0 force bit for bit, and both parts match the oracle."""
+    th = W.draw_params(family, D)
+    sun = W.fibonacci_sphere(S)
+    dz = ctx.srp_build_designs(family, th)
+    ctx.srp_set_options(primary_mode=mode, deposit=deposit)
+    try:
+        F, Fd = ctx.srp_forces_split(dz, cuda(sun), N, B, seed=4)
+        F0 = ctx.srp_forces(dz, cuda(sun), N, B, 4).cpu().numpy()
+        Fnb = ctx.srp_forces(dz, cuda(sun), N, 0, 4).cpu().numpy()
+        pairs = np.array([[D - 1, 1], [0, S - 1]], np.int32)
+        Fp, Fdp = ctx.srp_forces_split_pairs(dz, cuda(sun), pairs, N, B, seed=4)
+    finally:
+        ctx.srp_set_options()
+    F, Fd = F.cpu().numpy(), Fd.cpu().numpy()
+    assert rel_l2(F.reshape(-1, 3), F0.reshape(-1, 3)).max() < 1e-6
+    # direct == "NB" (PAPER.md:340): bit for bit where a photon's lane is fixed by its index; trace_kernel hands rays
+    # to lanes as they fall free, so its per-lane fp32 partial sums group differently
+    if family == W.FAMILY_BOXWING6:
+        assert rel_l2(Fd.reshape(-1, 3), Fnb.reshape(-1, 3)).max() < 2e-6
+    else:
+        assert np.array_equal(Fd, Fnb)
+    assert np.array_equal(Fp.cpu().numpy(), F[pairs[:, 0], pairs[:, 1]])
+    assert np.array_equal(Fdp.cpu().numpy(), Fd[pairs[:, 0], pairs[:, 1]])
+    some_indirect = False
+    for k in range(D):
+        v, m = oracle.build_mesh(family, th[k], k=k)
+        r = oracle.forces_split(v, m, sun, N, B, seed=4, k=k, deposit=deposit)
+        sig = oracle.forces(v, m, sun, N, B, seed=4, k=k, deposit=deposit)["sigma"]
+        assert_parity(F[k], r["F"], sig, tol_agg=3e-3)
+        assert_parity(Fd[k], r["F_direct"], sig, tol_agg=3e-3)
+        ind_o, ind_g = r["F_indirect"], F[k].astype(float) - Fd[k].astype(float)
+        # the indirect part is a small difference of two large sums: compare it on the scale of the total
+        assert np.all(np.linalg.norm(ind_g - ind_o, axis=1) <= 4.0 * sig + 1e-4 * np.linalg.norm(r["F"], axis=1))
+        some_indirect |= bool(np.any(np.linalg.norm(ind_o, axis=1) > 1e-3 * np.linalg.norm(r["F"], axis=1)))
+    assert some_indirect
+    dz.free()
+
+
+def test_workspace_from_the_caller_and_launch_count(ctx):
+    """srp_set_workspace: the ray queue of the beam / bounce loop lives in a torch tensor; a small one means more
+    rounds of the loop and the same forces bit for bit; one below srp_workspace_bytes_min is refused.
+    srp_launch_count / srp_stats.kernel_launches count this library's kernels."""
+    import torch
+    from paper_2602_10712_b200.binding import SrpError
+    th = W.draw_params(W.FAMILY_DETAILED, 1)
+    sun = cuda(W.fibonacci_sphere(8))
+    dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    ctx.srp_set_options(primary_mode=2)
+    try:
+        n0 = ctx.srp_launch_count()
+        F0 = ctx.srp_forces(dz, sun, 1 << 18, 8, 2).cpu().numpy()
+        st0 = ctx.srp_get_stats()
+        n1 = ctx.srp_launch_count()
+        assert st0["loop_rounds"] >= 1 and st0["queued_rays"] > 0
+        assert st0["kernel_launches"] == n1 - n0 >= 3 + 3 * st0["loop_rounds"] - 1
+        need = ctx.srp_workspace_bytes_min()
+        with pytest.raises(SrpError):
+            ctx.srp_set_workspace(torch.empty(need // 2, dtype=torch.uint8, device="cuda"))
+        ws = torch.empty(need + (1 << 16), dtype=torch.uint8, device="cuda")
+        ctx.srp_set_workspace(ws)
+        F1 = ctx.srp_forces(dz, sun, 1 << 18, 8, 2).cpu().numpy()
+        st1 = ctx.srp_get_stats()
+        assert np.array_equal(F0, F1)
+        assert st1["loop_rounds"] >= st0["loop_rounds"] and st1["queued_rays"] == st0["queued_rays"]
+        ctx.srp_set_options(primary_mode=2, plain_launches=1)
+        F2 = ctx.srp_forces(dz, sun, 1 << 18, 8, 2).cpu().numpy()
+        assert np.array_equal(F0, F2)
+    finally:
+        ctx.srp_set_workspace(None)
+        ctx.srp_set_options()
     dz.free()
 
 
