@@ -48,13 +48,16 @@ typedef enum {
  *   BOXWING  n_params 2: (panel length L [m], panel angle phi [rad])             T = 16
  *   DETAILED n_params 2: (dish tilt theta_dish, panel angle phi_pan) [rad]       T = 49840
  *   BOXWING6 n_params 6: (phi1, phi2, L, bus aspect a, rho_s panel, rho_d bus)   T = 16
- *   SAIL     n_params 1: (height-field amplitude [m], 0.05 in config 5)          T = 1019698 */
+ *   SAIL     n_params 1: (height-field amplitude [m], 0.05 in config 5)          T = 1019698
+ *   BOXWING_T n_params 2: the BOXWING geometry tessellated (bus 8 x 8 cells per face,
+ *            panels 8 x 16): "a representative satellite model (1 k faces)", PAPER.md:352   T = 1280 */
 typedef enum {
     SRP_FAMILY_PLATE = 0,
     SRP_FAMILY_BOXWING = 1,
     SRP_FAMILY_DETAILED = 2,
     SRP_FAMILY_BOXWING6 = 3,
-    SRP_FAMILY_SAIL = 4
+    SRP_FAMILY_SAIL = 4,
+    SRP_FAMILY_BOXWING_T = 5
 } srp_family;
 
 typedef struct {
@@ -225,6 +228,20 @@ srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *designs, cons
 srp_status srp_forces_host(srp_context *ctx, const srp_designs *designs, const float *sun_dirs_host,
                            int S, long long rays_per_dir, int max_bounces, unsigned long long seed,
                            float *out_forces_host);
+
+/* The paper's own workload shape: a batch of M records, each with
+ * its OWN design theta_m and its OWN light direction omega_m -- "every ray effectively intersects a different world"
+ * -- and only rays_per_record photons, so no hierarchy is built: as in the paper, every ray is tested against all
+ * triangles of its record's mesh.  theta DEVICE float[M, n_params], sun_dirs DEVICE float[M,3] (body->sun),
+ * out_forces DEVICE float[M,3] newtons.  Record m is design m with direction m: its mesh, materials and photons are
+ * those of srp_build_designs + srp_forces_pairs with the pair (m, m), except that the direction index in the Philox
+ * counter is 0 (counter (ray, 0, m, depth)); M is not limited to 65535.  The family's meshes must have at most 4266
+ * triangles (one record's triangles live in a thread block's shared memory); srp_options.sampler and .deposit
+ * apply; torque, glossy lobes and escape masks do not.  The meshes are generated chunk by chunk on the way and not
+ * kept.  srp_get_stats covers the whole batch.  Enqueues only. */
+srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const float *theta, int n_params,
+                                 const float *sun_dirs, long long M, long long rays_per_record, int max_bounces,
+                                 unsigned long long seed, unsigned long long mesh_seed, float *out_forces);
 
 /* Debug: primary-hit triangle (ORIGINAL index, -1 = miss) of every ray of the listed pairs:
  * out_prim DEVICE int[n_pairs, rays_per_dir].  method 0 = BVH traversal, 1 = brute force. */

@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SOURCES = ["srp_oracle_mesh.c", "srp_oracle_trace.c"]
 _LIB_PATH = os.path.join(_HERE, "libsrp_oracle.so")
 
-FAMILY_PLATE, FAMILY_BOXWING, FAMILY_DETAILED, FAMILY_BOXWING6, FAMILY_SAIL = range(5)
+FAMILY_PLATE, FAMILY_BOXWING, FAMILY_DETAILED, FAMILY_BOXWING6, FAMILY_SAIL, FAMILY_BOXWING_T = range(6)
 SOLAR_PRESSURE = 4.56e-6  # N/m^2 at 1 AU (BASELINE.json config 1)
 
 
@@ -35,7 +35,7 @@ class Stats(ctypes.Structure):
 
 class Options(ctypes.Structure):
     _fields_ = [("solar_pressure", ctypes.c_double), ("sampler", ctypes.c_int),
-                ("deposit", ctypes.c_int)]
+                ("deposit", ctypes.c_int), ("no_caustics", ctypes.c_int)]
 
 
 def build(force=False):
@@ -83,6 +83,10 @@ def lib():
                                               ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int,
                                               ctypes.c_ulonglong, ctypes.POINTER(Options), ctypes.c_void_p, ctypes.c_void_p,
                                               ctypes.POINTER(Stats)]
+        L.srp_oracle_backward.restype = ctypes.c_int
+        L.srp_oracle_backward.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p,
+                                          ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_ulonglong,
+                                          ctypes.POINTER(Options), ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.srp_oracle_thermal.restype = ctypes.c_int
         L.srp_oracle_thermal.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p,
                                          ctypes.c_longlong, ctypes.c_int, ctypes.c_ulonglong, ctypes.POINTER(Options),
@@ -141,7 +145,7 @@ def build_mesh(family, theta, k=0, mesh_seed=2):
 
 
 def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sampler=0,
-           deposit=0, want_first_hit=False, want_path_sig=False, x_com=None, shininess=None):
+           deposit=0, want_first_hit=False, want_path_sig=False, x_com=None, shininess=None, no_caustics=0):
     """Forces of ONE design for the given sun directions.
 
     Returns dict(F f64[S,3], sumsq f64[S,3], sigma f64[S] (i.i.d. standard error of |F|,
@@ -159,7 +163,7 @@ def forces(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSURE, sam
     st = Stats()
     fh = np.empty((S, N), dtype=np.int32) if want_first_hit else None
     ps = np.empty((S, N), dtype=np.uint64) if want_path_sig else None
-    opt = Options(float(P), int(sampler), int(deposit))
+    opt = Options(float(P), int(sampler), int(deposit), int(no_caustics))
     args = (verts.ctypes.data, mats.ctypes.data, T, int(k), sun.ctypes.data,
             S, int(j0), int(N), int(B), int(seed), ctypes.byref(opt),
             F.ctypes.data, Q.ctypes.data, ctypes.byref(st),
@@ -203,13 +207,32 @@ def forces_split(verts, mats, sun_dirs, N, B, seed=0, k=0, j0=0, P=SOLAR_PRESSUR
     sh = None if shininess is None else np.ascontiguousarray(shininess, dtype=np.float32).reshape(-1)
     F = np.zeros((S, 3)); Fd = np.zeros((S, 3))
     st = Stats()
-    opt = Options(float(P), int(sampler), int(deposit))
+    opt = Options(float(P), int(sampler), int(deposit), 0)
     rc = lib().srp_oracle_forces_split(verts.ctypes.data, mats.ctypes.data, sh.ctypes.data if sh is not None else None, T,
                                        int(k), sun.ctypes.data, S, int(j0), int(N), int(B), int(seed), ctypes.byref(opt),
                                        F.ctypes.data, Fd.ctypes.data, ctypes.byref(st))
     if rc != 0:
         raise ValueError("srp_oracle_forces_split: invalid arguments")
     return {"F": F, "F_direct": Fd, "F_indirect": F - Fd, "stats": st.as_dict()}
+
+
+def backward(verts, mats, sun_dir, N, B, seed=0, k=0, j=0, P=SOLAR_PRESSURE, deposit=0):
+    """The paper's backward estimator (Eq. 5) of ONE (design, direction) pair: N surface samples,
+    paths of at most B vertices with next-event estimation.  A cross-check of `forces`.  Returns dict(F f64[3],
+    sigma (standard error of |F|), n_nee)."""
+    verts = np.ascontiguousarray(verts, dtype=np.float32).reshape(-1, 3, 3)
+    mats = np.ascontiguousarray(mats, dtype=np.float32).reshape(-1, 3)
+    w = np.ascontiguousarray(sun_dir, dtype=np.float32).reshape(3)
+    F = np.zeros(3); Q = np.zeros(3)
+    nee = ctypes.c_ulonglong()
+    opt = Options(float(P), 1, int(deposit), 0)
+    rc = lib().srp_oracle_backward(verts.ctypes.data, mats.ctypes.data, verts.shape[0], int(k), w.ctypes.data, int(j),
+                                   int(N), int(B), int(seed), ctypes.byref(opt), F.ctypes.data, Q.ctypes.data,
+                                   ctypes.byref(nee))
+    if rc != 0:
+        raise ValueError("srp_oracle_backward: invalid arguments")
+    var = np.maximum(Q / N - F * F, 0.0) / N             # variance of the mean of the per-sample totals
+    return {"F": F, "sigma": float(np.sqrt(var.sum())), "n_nee": int(nee.value)}
 
 
 def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0, shininess=None):
@@ -223,7 +246,7 @@ def thermal(verts, mats, facet_power, N, B, seed=0, k=0, deposit=0, shininess=No
     assert mats.shape[0] == T and pw.shape[0] == T
     F = np.zeros(3); Q = np.zeros(3)
     st = Stats()
-    opt = Options(float(SOLAR_PRESSURE), 0, int(deposit))
+    opt = Options(float(SOLAR_PRESSURE), 0, int(deposit), 0)
     sh = None if shininess is None else np.ascontiguousarray(shininess, dtype=np.float32).reshape(-1)
     assert sh is None or sh.shape[0] == T
     rc = lib().srp_oracle_thermal_glossy(verts.ctypes.data, mats.ctypes.data, sh.ctypes.data if sh is not None else None,

@@ -32,7 +32,7 @@
 #include <string.h>
 #include "srp_oracle_common.h"
 
-enum { FAM_PLATE = 0, FAM_BOXWING = 1, FAM_DETAILED = 2, FAM_BOXWING6 = 3, FAM_SAIL = 4 };
+enum { FAM_PLATE = 0, FAM_BOXWING = 1, FAM_DETAILED = 2, FAM_BOXWING6 = 3, FAM_SAIL = 4, FAM_BOXWING_T = 5 };
 enum { PK_PLANE = 0, PK_HFIELD = 1, PK_POLAR = 2, PK_TUBE = 3 };
 enum { MAT_DIRICHLET = 0, MAT_FIXED = 1 };
 
@@ -131,6 +131,13 @@ static int family_patches(int family, const float *theta, orc_patch *P)
         n += add_cuboid(P + n, orc_mk(0, 0, 0), 0.75, 0.75, 1.0, 1, 0);
         P[n++] = mk_panel(phi, 1.0, 1.15, L, 1, 1, 0);
         P[n++] = mk_panel(phi, -1.0, 1.15, L, 1, 1, 0);
+        break;
+    }
+    case FAM_BOXWING_T: {   /* the box-wing of FAM_BOXWING, tessellated: "a representative satellite model (1 k faces)" */
+        double L = (double)theta[0], phi = (double)theta[1];
+        n += add_cuboid(P + n, orc_mk(0, 0, 0), 0.75, 0.75, 1.0, 8, 0);
+        P[n++] = mk_panel(phi, 1.0, 1.15, L, 8, 16, 0);
+        P[n++] = mk_panel(phi, -1.0, 1.15, L, 8, 16, 0);
         break;
     }
     case FAM_BOXWING6: {
@@ -315,7 +322,7 @@ int srp_oracle_n_params(int family)
 {
     switch (family) {
     case FAM_PLATE: return 3; case FAM_BOXWING: return 2; case FAM_DETAILED: return 2;
-    case FAM_BOXWING6: return 6; case FAM_SAIL: return 1; default: return -1;
+    case FAM_BOXWING6: return 6; case FAM_SAIL: return 1; case FAM_BOXWING_T: return 2; default: return -1;
     }
 }
 

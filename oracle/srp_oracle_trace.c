@@ -46,6 +46,9 @@ typedef struct {
     double solar_pressure;   /* P, N/m^2 */
     int sampler;             /* 0 stratified-jittered Morton grid, 1 i.i.d. */
     int deposit;             /* 0 expected-value, 1 analog */
+    int no_caustics;         /* 1: a photon whose FIRST reflection is specular is not followed (its first-hit deposit
+                                stays).  That is the light a backward path tracer with a delta sun cannot find
+                                (srp_oracle_backward below); used only to cross-check the two estimators. */
 } orc_options;
 
 /* O-step 4: closest hit over ALL triangles with index != src.
@@ -151,6 +154,13 @@ static void trace_photon(const orc_geom *G, const float *mats, orc_v3 o, orc_v3 
             break;
         } else if (z0 < (double)th2 && !glossy) {
             dnew = refl;
+            if (opt->no_caustics && depth == 0) {
+                if (opt->deposit == 1) { dd[0] = wph * (d.x - dnew.x); dd[1] = wph * (d.y - dnew.y); dd[2] = wph * (d.z - dnew.z); }
+                orc_deposit(dd, x, xc, dp, dq);
+                if (dp0) { dp0[0] += dd[0]; dp0[1] += dd[1]; dp0[2] += dd[2]; }
+                st->capped++;
+                break;
+            }
         } else if (z0 < (double)th2) {
             /* Phong lobe: cos(theta) = xi^(1/(n+1)) about refl, phi uniform; attempt a = 0 uses (z1, z2) of the
              * lobe draw, attempt a >= 1 words 1 and 2 of Philox(i, j, k, (depth + 1) | cflag | a << 8).  The local
@@ -442,6 +452,163 @@ int srp_oracle_thermal_glossy(const float *verts, const float *mats, const float
     for (int c = 0; c < 3; ++c) { F[c] = Ft[c]; if (sumsq) sumsq[c] = Qt[c]; }
     if (stats) *stats = st;
     free(v0); free(e1); free(e2); free(nrm);
+    return 0;
+}
+
+/*
+ * The paper's own estimator, Eq. 5, backward from the surface -- a CROSS-CHECK of the forward
+ * tracer above (reading R25), not a second product path:
+ *   "a random triangle on the surface is chosen by sampling according to triangle area and a random point within
+ *    that triangle using uniform point picking.  Next, we pick a random incoming direction and evaluate the radiation
+ *    using a single sample of path tracing.  Finally, a random outgoing direction is selected ... We use BRDF
+ *    importance sampling to generate the incoming and outgoing direction.  We also use next-event estimation ...
+ *    at every light path vertex we check direct light from omega."
+ * One sample i (Philox ctr (i, j, k, 0x40000000 | word)):
+ *   1. facet f with probability A_f / A (inverse of the cumulative areas at xi0), x = v0 + sqrt(xi1)(1 - xi2) e1 +
+ *      sqrt(xi1) xi2 e2.  Facets are two-sided (R6): both sides s = +n, -n are evaluated and added.
+ *   2. direct light (next-event estimation at the first vertex): if n_s . w > 0 and the shadow ray x -> w (w = unit
+ *      vector to the sun) is free, the side receives the pressure P cos(theta) along d = -w.
+ *   3. indirect light: incoming direction w_in cosine-distributed about n_s (pdf cos/pi: the sampling density of a
+ *      surface's response to light, which is proportional to <n, w_in>+ in Eq. 2); the radiance arriving along it is
+ *      path-traced backwards from the surface point y the ray x + t w_in meets: at every vertex (at most B of them)
+ *      direct sun light is added by next-event estimation through the Lambertian part rho_d / pi of the BRDF (a
+ *      delta light cannot be seen through an ideal mirror), then the path goes on by BRDF importance sampling --
+ *      absorbed with probability alpha, mirrored with rho_s, cosine-distributed with rho_d -- with throughput 1.
+ *      With L in units of pressure per steradian the sample of step 3 is pi L received along d = -w_in.
+ *   4. light received along d at x on side s deposits P_received [(alpha+rho_s+rho_d) d - rho_s r - 2/3 rho_d n_s]
+ *      (expected value over the BRDF-sampled outgoing direction; opt->deposit = 1 draws w_out instead: nothing,
+ *      the mirror direction, or a cosine-distributed one), sign per reading R1, times A (the pdf of step 1).
+ * Equal in expectation to the forward tracer EXCEPT for sun light whose first reflection is specular: a backward
+ * path ends at the sun only through next-event estimation, which an ideal mirror (a delta lobe, R3) never passes.
+ * srp_oracle_forces with opt->no_caustics = 1 leaves exactly that light out.
+ * F double[3], sumsq double[3] (squared per-sample totals; may be NULL), n_nee: shadow rays cast (may be NULL).
+ */
+static int blocked(const orc_geom *G, orc_v3 o, orc_v3 d, long src)
+{
+    double t;
+    return closest_hit(G->v0, G->e1, G->e2, G->T, o, d, src, &t) >= 0;
+}
+
+static orc_v3 cosine_dir(const orc_geom *G, long f, orc_v3 nf, double u1, double u2)
+{
+    const double phi = 6.283185307179586476925286766559 * u1, rho = sqrt(u2);
+    orc_v3 tu = orc_normalize(orc_mk(G->e1[3 * f], G->e1[3 * f + 1], G->e1[3 * f + 2]));
+    orc_v3 tv = orc_cross(nf, tu);
+    return orc_add(orc_add(orc_scale(tu, rho * cos(phi)), orc_scale(tv, rho * sin(phi))), orc_scale(nf, sqrt(1.0 - u2)));
+}
+
+int srp_oracle_backward(const float *verts, const float *mats, long T, int k, const float *sun_dir, int j,
+                        long long N, int B, unsigned long long seed, const orc_options *opt,
+                        double *F, double *sumsq, unsigned long long *n_nee)
+{
+    if (!verts || !mats || !sun_dir || !F || !opt || T <= 0 || N <= 0 || B < 0 || B > 15) return -1;
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    const double P = opt->solar_pressure;
+    double *v0 = malloc(sizeof(double) * 3 * T), *e1 = malloc(sizeof(double) * 3 * T),
+           *e2 = malloc(sizeof(double) * 3 * T), *nrm = malloc(sizeof(double) * 3 * T), *cum = malloc(sizeof(double) * T);
+    double A = 0.0;
+    for (long f = 0; f < T; ++f) {
+        for (int c = 0; c < 3; ++c) {
+            double a = verts[9 * f + c], b = verts[9 * f + 3 + c], cc = verts[9 * f + 6 + c];
+            v0[3 * f + c] = a; e1[3 * f + c] = b - a; e2[3 * f + c] = cc - a;
+        }
+        orc_v3 n = orc_cross(orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]), orc_mk(e2[3 * f], e2[3 * f + 1], e2[3 * f + 2]));
+        double len = sqrt(orc_dot(n, n));
+        nrm[3 * f] = n.x / len; nrm[3 * f + 1] = n.y / len; nrm[3 * f + 2] = n.z / len;
+        A += 0.5 * len; cum[f] = A;
+    }
+    const orc_geom G = { v0, e1, e2, nrm, T, NULL };
+    const orc_v3 w = orc_normalize(orc_mk(sun_dir[0], sun_dir[1], sun_dir[2]));
+    double Ft[3] = { 0, 0, 0 }, Qt[3] = { 0, 0, 0 };
+    unsigned long long nee = 0;
+    for (long long i = 0; i < N; ++i) {
+        uint32_t c0[4] = { (uint32_t)i, (uint32_t)j, (uint32_t)k, 0x40000000u }, r[4];
+        orc_philox4x32_10(c0, key, r);
+        /* step 1 */
+        const double target = orc_uniform(r[0]) * A;
+        long lo = 0, hi = T - 1;
+        while (lo < hi) { long mid = (lo + hi) / 2; if (cum[mid] > target) hi = mid; else lo = mid + 1; }
+        const long f = lo;
+        const double su = sqrt(orc_uniform(r[1])), x2 = orc_uniform(r[2]);
+        const orc_v3 E1 = orc_mk(e1[3 * f], e1[3 * f + 1], e1[3 * f + 2]), E2 = orc_mk(e2[3 * f], e2[3 * f + 1], e2[3 * f + 2]);
+        const orc_v3 x = orc_add(orc_mk(v0[3 * f], v0[3 * f + 1], v0[3 * f + 2]),
+                                 orc_add(orc_scale(E1, su * (1.0 - x2)), orc_scale(E2, su * x2)));
+        const double al = mats[3 * f], rs = mats[3 * f + 1], rd = mats[3 * f + 2];
+        double tot[3] = { 0, 0, 0 };
+        for (int side = 0; side < 2; ++side) {
+            const orc_v3 n = orc_mk(nrm[3 * f], nrm[3 * f + 1], nrm[3 * f + 2]);
+            const orc_v3 ns = side == 0 ? n : orc_scale(n, -1.0);
+            uint32_t c1[4] = { (uint32_t)i, (uint32_t)j, (uint32_t)k, 0x40000001u + (uint32_t)side }, q[4];
+            orc_philox4x32_10(c1, key, q);
+            /* light received at x on this side: up to two arrivals (direct, indirect), each "pressure along d" */
+            orc_v3 dirs[2]; double press[2]; int n_arr = 0;
+            /* step 2: direct light */
+            const double cs = orc_dot(ns, w);
+            if (cs > 0.0) {
+                ++nee;
+                if (!blocked(&G, x, w, f)) { dirs[n_arr] = orc_scale(w, -1.0); press[n_arr] = P * cs; ++n_arr; }
+            }
+            /* step 3: indirect light */
+            if (B > 0) {
+                const orc_v3 win = cosine_dir(&G, f, ns, orc_uniform(q[0]), orc_uniform(q[1]));
+                orc_v3 o = x, dir = win; long src = f; double L = 0.0;
+                for (int depth = 1; depth <= B; ++depth) {
+                    double t;
+                    const long g = closest_hit(G.v0, G.e1, G.e2, G.T, o, dir, src, &t);
+                    if (g < 0) break;
+                    const orc_v3 y = orc_add(o, orc_scale(dir, t));
+                    orc_v3 ng = orc_mk(nrm[3 * g], nrm[3 * g + 1], nrm[3 * g + 2]);
+                    if (orc_dot(ng, dir) > 0.0) ng = orc_scale(ng, -1.0);        /* the side the path arrives on */
+                    const double cy = orc_dot(ng, w);
+                    if (cy > 0.0) {
+                        ++nee;
+                        if (!blocked(&G, y, w, g)) L += (double)mats[3 * g + 2] / 3.14159265358979323846 * P * cy;
+                    }
+                    uint32_t c2[4] = { (uint32_t)i, (uint32_t)j, (uint32_t)k, 0x40000010u + 16u * (uint32_t)side + (uint32_t)depth }, z[4];
+                    orc_philox4x32_10(c2, key, z);
+                    const double z0 = orc_uniform(z[0]);
+                    const float th1 = mats[3 * g], th2 = mats[3 * g] + mats[3 * g + 1];
+                    if (z0 < (double)th1) break;                                  /* absorbed */
+                    const orc_v3 wo = orc_scale(dir, -1.0);                      /* the direction the light leaves y in */
+                    orc_v3 nd;
+                    if (z0 < (double)th2) nd = orc_sub(orc_scale(ng, 2.0 * orc_dot(ng, wo)), wo);   /* mirror */
+                    else nd = cosine_dir(&G, g, ng, orc_uniform(z[1]), orc_uniform(z[2]));
+                    o = y; dir = nd; src = g;
+                }
+                if (L > 0.0) { dirs[n_arr] = orc_scale(win, -1.0); press[n_arr] = 3.14159265358979323846 * L; ++n_arr; }
+            }
+            /* step 4: force of what arrived */
+            for (int a = 0; a < n_arr; ++a) {
+                const orc_v3 d = dirs[a];
+                const double cost = -orc_dot(d, ns);
+                const orc_v3 refl = orc_add(d, orc_scale(ns, 2.0 * cost));
+                double dd[3];
+                if (opt->deposit == 0) {
+                    const double s3 = al + rs + rd;
+                    dd[0] = s3 * d.x - rs * refl.x - (2.0 / 3.0) * rd * ns.x;
+                    dd[1] = s3 * d.y - rs * refl.y - (2.0 / 3.0) * rd * ns.y;
+                    dd[2] = s3 * d.z - rs * refl.z - (2.0 / 3.0) * rd * ns.z;
+                } else {
+                    const double z0 = orc_uniform(q[2 + (a & 1)]);
+                    const float th1 = mats[3 * f], th2 = mats[3 * f] + mats[3 * f + 1];
+                    orc_v3 wout = orc_mk(0, 0, 0);
+                    if (z0 < (double)th1) wout = orc_mk(0, 0, 0);
+                    else if (z0 < (double)th2) wout = refl;
+                    else {
+                        uint32_t c3[4] = { (uint32_t)i, (uint32_t)j, (uint32_t)k, 0x40000004u + 2u * (uint32_t)side + (uint32_t)a }, u[4];
+                        orc_philox4x32_10(c3, key, u);
+                        wout = cosine_dir(&G, f, ns, orc_uniform(u[0]), orc_uniform(u[1]));
+                    }
+                    dd[0] = d.x - wout.x; dd[1] = d.y - wout.y; dd[2] = d.z - wout.z;
+                }
+                for (int c = 0; c < 3; ++c) tot[c] += A * press[a] * dd[c];
+            }
+        }
+        for (int c = 0; c < 3; ++c) { Ft[c] += tot[c]; Qt[c] += tot[c] * tot[c]; }
+    }
+    for (int c = 0; c < 3; ++c) { F[c] = Ft[c] / (double)N; if (sumsq) sumsq[c] = Qt[c]; }
+    if (n_nee) *n_nee = nee;
+    free(v0); free(e1); free(e2); free(nrm); free(cum);
     return 0;
 }
 

@@ -55,7 +55,7 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
            "srp_forces_torques", "srp_forces_torques_pairs", "srp_forces_split", "srp_forces_split_pairs",
-           "srp_thermal_forces", "srp_designs_set_shininess", "srp_first_hits", "srp_path_signatures", "srp_get_stats",
+           "srp_forces_per_sample", "srp_thermal_forces", "srp_designs_set_shininess", "srp_first_hits", "srp_path_signatures", "srp_get_stats",
            "srp_launch_count", "srp_set_workspace", "srp_workspace_bytes_min", "srp_probe_peaks"]
 
 _lib = None
@@ -93,6 +93,7 @@ def load_library():
     L.srp_forces_torques_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp, vp]
     L.srp_forces_split.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp]
     L.srp_forces_split_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp, vp]
+    L.srp_forces_per_sample.argtypes = [vp, ci, vp, ci, vp, ll, ll, ci, ull, ull, vp]
     L.srp_launch_count.argtypes = [vp, ctypes.POINTER(ull)]
     L.srp_set_workspace.argtypes = [vp, vp, ull]
     L.srp_workspace_bytes_min.argtypes = [vp]
@@ -331,6 +332,24 @@ class Context:
                                                     F.data_ptr(), Fd.data_ptr()))
         self.stream.synchronize()
         return F, Fd
+
+    def srp_forces_per_sample(self, family, theta, sun_dirs, rays_per_record, max_bounces, seed=0, mesh_seed=W.MESH_SEED,
+                              out=None):
+        """The paper's workload shape: record m = its own design theta[m] lit from its own
+        direction sun_dirs[m].  theta [M, n_params], sun_dirs [M, 3] (CUDA float32); returns CUDA float32 [M, 3]
+        (asynchronous on the stream)."""
+        _check_cuda_f32(theta, "theta", self.device)
+        _check_cuda_f32(sun_dirs, "sun_dirs", self.device, (3,))
+        M = theta.shape[0]
+        if theta.dim() != 2 or sun_dirs.shape[0] != M:
+            raise ValueError("theta must be [M, n_params] and sun_dirs [M, 3]")
+        if out is None:
+            out = torch.empty((M, 3), dtype=torch.float32, device=self.device)
+        elif _check_cuda_f32(out, "out", self.device).numel() != 3 * M:
+            raise ValueError("out must hold [M, 3] floats")
+        self._check(self.lib.srp_forces_per_sample(self.handle, family, theta.data_ptr(), theta.shape[1], sun_dirs.data_ptr(),
+                                                   M, rays_per_record, max_bounces, seed, mesh_seed, out.data_ptr()))
+        return out
 
     def force_maps(self, designs, n_lat, n_lon, rays_per_dir, max_bounces, seed=0):
         """The paper's force-map figures (Fig. 5): forces over a latitude-longitude image of sun

@@ -32,6 +32,7 @@ SOURCES = {
     "trace_beam.cu": [],
     "trace_bounce.cu": [],
     "trace_small.cu": [],
+    "trace_sample.cu": [],
     "trace_thermal.cu": [],
 }
 

@@ -119,6 +119,13 @@ __device__ int family_patches(int family, const float *theta, Patch *P)
         P[n++] = panel(phi, -1.0, 1.15, L, 1, 1, 0);
         break;
     }
+    case SRP_FAMILY_BOXWING_T: {          // the box-wing, tessellated to ~1 k faces
+        double L = (double)theta[0], phi = (double)theta[1];
+        n += cuboid(P + n, mk(0, 0, 0), 0.75, 0.75, 1.0, 8, 0);
+        P[n++] = panel(phi, 1.0, 1.15, L, 8, 16, 0);
+        P[n++] = panel(phi, -1.0, 1.15, L, 8, 16, 0);
+        break;
+    }
     case SRP_FAMILY_BOXWING6: {
         double phi1 = (double)theta[0], phi2 = (double)theta[1], L = (double)theta[2];
         double asp = (double)theta[3];
@@ -246,7 +253,8 @@ __global__ void patch_table_kernel(int family, const float *theta, int D, int n_
 
 __global__ void __launch_bounds__(128)
 mesh_triangles_kernel(int family, const float *theta, int D, int n_params, uint32_t k0, uint32_t k1,
-                      long long T, const Patch *patches, const int *n_patches, float *verts, float *mats)
+                      long long T, const Patch *patches, const int *n_patches, float *verts, float *mats,
+                      uint32_t k_offset /* index of design 0 in the Philox counters of the material draws */)
 {
     long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= (long long)D * T) return;
@@ -297,8 +305,8 @@ mesh_triangles_kernel(int family, const float *theta, int D, int n_params, uint3
         else                  { m0 = 0.8 * (1.0 - rd); m1 = 0.2 * (1.0 - rd); m2 = rd; }
     } else {                                   // per-facet Dirichlet(2,2,2)
         uint32_t r0[4], r1[4];
-        philox((uint32_t)f, (uint32_t)k, 0u, 0xB0u, k0, k1, r0);
-        philox((uint32_t)f, (uint32_t)k, 1u, 0xB0u, k0, k1, r1);
+        philox((uint32_t)f, (uint32_t)k + k_offset, 0u, 0xB0u, k0, k1, r0);
+        philox((uint32_t)f, (uint32_t)k + k_offset, 1u, 0xB0u, k0, k1, r1);
         double g0 = -log(uniform(r0[0]) * uniform(r0[1]));
         double g1 = -log(uniform(r0[2]) * uniform(r0[3]));
         double g2 = -log(uniform(r1[0]) * uniform(r1[1]));
@@ -319,24 +327,25 @@ long long srp_family_tris_host(int family)
     case SRP_FAMILY_DETAILED: return 6 * 2 * 24 * 24 + (128 + 2 * 47 * 128) + 4 * (2 * 64 * 16 + 2 * 64)
                                      + 8 * 2 * 32 * 40 + 12 * (2 * 6 * 10 + 2 * 6);
     case SRP_FAMILY_SAIL: return 2LL * 707 * 707 + 6 * 2 * 40 * 40 + 4 * 2 * 4 * 25;
+    case SRP_FAMILY_BOXWING_T: return 6 * 2 * 8 * 8 + 2 * 2 * 8 * 16;
     default: return -1;
     }
 }
 
 cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_params,
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
-                                cudaStream_t stream)
+                                cudaMemPool_t pool, unsigned k_offset, cudaStream_t stream)
 {
     Patch *patches = nullptr; int *n_patches = nullptr;
-    cudaError_t e = cudaMallocAsync(&patches, sizeof(Patch) * MAX_PATCHES * (size_t)D, stream);
+    cudaError_t e = cudaMallocFromPoolAsync((void **)&patches, sizeof(Patch) * MAX_PATCHES * (size_t)D, pool, stream);
     if (e != cudaSuccess) return e;
-    e = cudaMallocAsync(&n_patches, sizeof(int), stream);
-    if (e != cudaSuccess) return e;
+    e = cudaMallocFromPoolAsync((void **)&n_patches, sizeof(int), pool, stream);
+    if (e != cudaSuccess) { cudaFreeAsync(patches, stream); return e; }
     patch_table_kernel<<<(D + 63) / 64, 64, 0, stream>>>(family, theta, D, n_params, patches, n_patches);
     long long total = (long long)D * T;
     mesh_triangles_kernel<<<(unsigned)((total + 127) / 128), 128, 0, stream>>>(
         family, theta, D, n_params, (uint32_t)mesh_seed, (uint32_t)(mesh_seed >> 32), T, patches,
-        n_patches, verts, mats);
+        n_patches, verts, mats, k_offset);
     e = cudaGetLastError();
     cudaFreeAsync(patches, stream);
     cudaFreeAsync(n_patches, stream);

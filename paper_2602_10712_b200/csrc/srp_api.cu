@@ -390,7 +390,7 @@ int srp_family_n_params(srp_family family)
 {
     switch (family) {
     case SRP_FAMILY_PLATE: return 3; case SRP_FAMILY_BOXWING: return 2; case SRP_FAMILY_DETAILED: return 2;
-    case SRP_FAMILY_BOXWING6: return 6; case SRP_FAMILY_SAIL: return 1; default: return -1;
+    case SRP_FAMILY_BOXWING6: return 6; case SRP_FAMILY_SAIL: return 1; case SRP_FAMILY_BOXWING_T: return 2; default: return -1;
     }
 }
 
@@ -419,7 +419,7 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
     srp_status st = alloc_designs(ctx, d);
     if (st != SRP_OK) { free_designs_mem(ctx, d); delete d; return st; }
     cudaError_t e = srp_launch_mesh_gen((int)family, theta, D, n_params, mesh_seed, T, d->verts_orig,
-                                        d->mats_orig, ctx->stream);
+                                        d->mats_orig, ctx->mempool, 0u, ctx->stream);
     if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->mempool, ctx->stream);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     ctx->launches_total += 2 + SRP_BUILD_KERNELS(d->has_bvh);          // mesh generation: 2 kernels
@@ -654,6 +654,61 @@ srp_status srp_forces_host(srp_context *ctx, const srp_designs *dz, const float 
     if (st != SRP_OK) return st;
     TRY_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->stage_out, sizeof(float) * n_out, cudaMemcpyDeviceToHost, ctx->stream), "d2h forces");
     TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync");
+    return SRP_OK;
+}
+
+srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const float *theta, int n_params,
+                                 const float *sun_dirs, long long M, long long N, int B, unsigned long long seed,
+                                 unsigned long long mesh_seed, float *out)
+{
+    if (!ctx) return SRP_ERR_INVALID;
+    if (!theta || !sun_dirs || !out) return fail(ctx, SRP_ERR_INVALID, "null pointer argument");
+    const long long T = srp_family_tris_host((int)family);
+    if (T < 0) return fail(ctx, SRP_ERR_INVALID, "unknown family");
+    if (n_params != srp_family_n_params(family)) return fail(ctx, SRP_ERR_INVALID, "wrong n_params for this family");
+    if (T > srp_sample_max_tris()) return fail(ctx, SRP_ERR_UNSUPPORTED, "a record's mesh must fit a thread block's shared memory");
+    if (M <= 0 || M >= (1LL << 32)) return fail(ctx, SRP_ERR_INVALID, "M must be in [1, 2^32)");
+    if (N <= 0 || N > (1LL << 31)) return fail(ctx, SRP_ERR_INVALID, "rays_per_record must be in [1, 2^31]");
+    if (B < 0 || B > 15) return fail(ctx, SRP_ERR_INVALID, "max_bounces must be in [0, 15]");
+    if (ctx->opt.sampler == 0 && (N & (N - 1)) != 0)
+        return fail(ctx, SRP_ERR_INVALID, "stratified sampler needs rays_per_record to be a power of two");
+    cudaSetDevice(ctx->device);
+    ctx->launches_call = 0;
+    srp_status st = ensure_workspace(ctx, 3);
+    if (st != SRP_OK) return st;
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
+    // chunks of records: meshes for a chunk (S0), its boxes and packed triangles (S1 without a hierarchy), its photons
+    long long chunk = (256LL << 20) / (96 * T);                     // ~256 MiB of mesh per chunk
+    if (chunk > 32768) chunk = 32768;
+    if (chunk > M) chunk = M;
+    if (chunk < 1) chunk = 1;
+    srp_designs d;
+    d.D = (int)chunk; d.family = (int)family; d.sumT = chunk * T; d.maxT = T; d.has_bvh = false;
+    d.tri_off.resize(chunk + 1);
+    for (long long k = 0; k <= chunk; ++k) d.tri_off[k] = k * T;
+    st = alloc_designs(ctx, &d);
+    cudaError_t e = cudaSuccess;
+    for (long long m0 = 0; m0 < M && st == SRP_OK && e == cudaSuccess; m0 += chunk) {
+        const int Dc = (int)(M - m0 < chunk ? M - m0 : chunk);
+        d.D = Dc; d.sumT = (long long)Dc * T;
+        e = srp_launch_mesh_gen((int)family, theta + (size_t)m0 * n_params, Dc, n_params, mesh_seed, T, d.verts_orig,
+                                d.mats_orig, ctx->mempool, (unsigned)m0, ctx->stream);
+        if (e == cudaSuccess) e = srp_launch_build(&d, 0, ctx->mempool, ctx->stream);
+        if (e != cudaSuccess) break;
+        TraceArgs a;
+        memset(&a, 0, sizeof a);
+        a.dz = d.dev();
+        a.sun_dirs = sun_dirs + 3 * m0; a.n_pairs = Dc; a.S = Dc; a.N = N; a.B = B;
+        while ((1LL << a.log2N) < N) ++a.log2N;
+        a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
+        a.sampler = ctx->opt.sampler; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
+        a.stats = ctx->stats; a.max_tris = T; a.acc_scale = 1.0;
+        e = srp_launch_sample(a, out + 3 * m0, (unsigned)m0, ctx->num_sms, ctx->stream);
+        count_launches(ctx, 2 + SRP_BUILD_KERNELS(false) + 1);
+    }
+    free_designs_mem(ctx, &d);                                      // stream-ordered: after the last chunk's kernels
+    if (st != SRP_OK) return st;
+    if (e != cudaSuccess) return cuda_fail(ctx, "per-sample designs", e);
     return SRP_OK;
 }
 

@@ -128,7 +128,7 @@ struct TraceArgs {
 // ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----
 cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_params,
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
-                                cudaStream_t stream);
+                                cudaMemPool_t pool, unsigned k_offset, cudaStream_t stream);
 cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, cudaStream_t stream);   // 2 kernels without a BVH, 6 with
 #define SRP_BUILD_KERNELS(has_bvh) ((has_bvh) ? 6 : 2)
 cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted, cudaStream_t stream);
@@ -143,6 +143,8 @@ cudaError_t srp_launch_finalize(const TraceArgs &a, float *out_forces, float *ou
 cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim, cudaStream_t stream);
 cudaError_t srp_launch_thermal(const TraceArgs &a, const float *facet_power, long long sumT, int *emit_list, int *n_emit,
                                float *design_power, float *out_forces, int num_sms, cudaStream_t stream);
+long long srp_sample_max_tris();
+cudaError_t srp_launch_sample(const TraceArgs &a, float *out, unsigned k_offset, int num_sms, cudaStream_t stream);
 cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
 
 long long srp_family_tris_host(int family);

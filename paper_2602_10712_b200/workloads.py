@@ -11,11 +11,11 @@ from dataclasses import dataclass
 
 import numpy as np
 
-FAMILY_PLATE, FAMILY_BOXWING, FAMILY_DETAILED, FAMILY_BOXWING6, FAMILY_SAIL = range(5)
+FAMILY_PLATE, FAMILY_BOXWING, FAMILY_DETAILED, FAMILY_BOXWING6, FAMILY_SAIL, FAMILY_BOXWING_T = range(6)
 N_PARAMS = {FAMILY_PLATE: 3, FAMILY_BOXWING: 2, FAMILY_DETAILED: 2, FAMILY_BOXWING6: 6,
-            FAMILY_SAIL: 1}
+            FAMILY_SAIL: 1, FAMILY_BOXWING_T: 2}
 TRI_COUNT = {FAMILY_PLATE: 2, FAMILY_BOXWING: 16, FAMILY_DETAILED: 49840, FAMILY_BOXWING6: 16,
-             FAMILY_SAIL: 1019698}
+             FAMILY_SAIL: 1019698, FAMILY_BOXWING_T: 1280}
 SOLAR_PRESSURE = 4.56e-6   # N/m^2 at 1 AU
 MESH_SEED = 2
 PARAM_SEED = 1
@@ -51,7 +51,7 @@ def draw_params(family, D, seed=PARAM_SEED):
     u = rng.random((D, N_PARAMS[family]))
     if family == FAMILY_PLATE:
         th = np.tile(np.array([0.3, 0.5, 0.2]), (D, 1))                 # (alpha, rho_s, rho_d)
-    elif family == FAMILY_BOXWING:
+    elif family in (FAMILY_BOXWING, FAMILY_BOXWING_T):
         th = np.stack([2.0 + 6.0 * u[:, 0], np.pi * u[:, 1]], axis=1)   # (L, phi)
     elif family == FAMILY_DETAILED:
         th = np.pi * u                                                  # (theta_dish, phi_pan)
@@ -63,6 +63,39 @@ def draw_params(family, D, seed=PARAM_SEED):
     else:
         raise ValueError("unknown family")
     return np.ascontiguousarray(th, dtype=np.float32)
+
+
+def random_directions(M, seed=3):
+    """M unit vectors uniform on the sphere, fp64 then rounded to fp32: the light direction of each record of a
+    per-sample-design batch ("a list of pairs consisting of light directions and design
+    parameters")."""
+    rng = np.random.default_rng([seed, 77])
+    z = 2.0 * rng.random(M) - 1.0
+    phi = 2.0 * np.pi * rng.random(M)
+    r = np.sqrt(np.maximum(0.0, 1.0 - z * z))
+    return np.stack([r * np.cos(phi), r * np.sin(phi), z], axis=1).astype(np.float32)
+
+
+@dataclass(frozen=True)
+class SampleConfig:
+    """The paper's own workload shape: M records, each its own random design AND its own
+    light direction, N Monte-Carlo samples per record, a ~1 k-face mesh, every ray tested against all triangles."""
+    name: str
+    family: int
+    M: int
+    N: int
+    B: int
+    seed: int = 0
+
+    def params(self):
+        return draw_params(self.family, self.M)
+
+    def sun_dirs(self):
+        return random_directions(self.M)
+
+
+# "100 k light directions and/or designs x 1000 samples, ~1 k faces" (N = 2^10: the stratified grid)
+SAMPLE_CONFIGS = {"paper_map": SampleConfig("paper_map", FAMILY_BOXWING_T, 100_000, 1 << 10, 4)}
 
 
 @dataclass(frozen=True)

@@ -33,7 +33,7 @@ def ulp_diff(a, b):
 
 # ---------------------------------------------------------------- S0: mesh generator
 @pytest.mark.parametrize("family", [W.FAMILY_PLATE, W.FAMILY_BOXWING, W.FAMILY_DETAILED,
-                                    W.FAMILY_BOXWING6, W.FAMILY_SAIL])
+                                    W.FAMILY_BOXWING6, W.FAMILY_SAIL, W.FAMILY_BOXWING_T])
 def test_mesh_generator_matches_oracle(ctx, oracle, family):
     D = 3 if family != W.FAMILY_SAIL else 1
     th = W.draw_params(family, D)
@@ -768,6 +768,105 @@ def test_cfg5_full_N_properties_and_reduced_N_oracle(ctx, oracle):
     err = np.linalg.norm(F[pairs[:, 1]] - Fo, axis=1)
     assert np.all(err <= 4 * sig), (err, sig)
     dz.free()
+
+
+def _same_stream_parity(ctx, oracle, cfg, dz, th, sun, pairs, N, max_div_fraction, label, **opts):
+    """GPU forces (plain kernels, the launch configuration srp_forces picks for this N) against the oracle on the
+    same Philox streams, photon paths compared through the path signatures; north_star's tolerances (1e-4 per vector
+    where no photon diverged, else 4 sigma, 1e-3 aggregate).  Also: the instrumented build, which the signatures come
+    from, gives the plain build's forces bit for bit, so the divergence count describes the forces that are checked."""
+    import time
+    ctx.srp_set_options(**opts)
+    try:
+        F, st = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
+        psig = ctx.srp_path_signatures(dz, cuda(sun), pairs, N, cfg.B, cfg.seed).cpu().numpy().astype(np.uint64)
+        ctx.srp_set_options(instrumented=1, **opts)
+        Fi, sti = run_pairs(ctx, dz, sun, pairs, N, cfg.B, cfg.seed)
+    finally:
+        ctx.srp_set_options()
+    assert np.array_equal(F, Fi)
+    for key in ("launched", "primary_miss", "absorbed", "escaped", "capped", "segments", "hits_at_depth"):
+        assert st[key] == sti[key], key
+    meshes = {int(k): oracle.build_mesh(cfg.family, th[k], k=int(k)) for k in np.unique(pairs[:, 0])}
+    t0 = time.time()
+    Fo, sig, ost, osig = oracle_pairs(oracle, meshes, pairs, sun, N, cfg.B, seed=cfg.seed, want_path_sig=True)
+    n_div = (psig != osig).sum(axis=1)
+    print("%s: %d pairs x N = %d, oracle %.0f s, divergent photons per pair %s" % (label, len(pairs), N, time.time() - t0, n_div.tolist()))
+    assert n_div.sum() <= max_div_fraction * len(pairs) * N
+    bad = assert_parity(F, Fo, sig, diverged=n_div > 0)              # tol_vec 1e-4, tol_agg 1e-3: BASELINE.json
+    counters_close(st, ost, tol=4 * int(n_div.sum()) + 8)
+    return bad, n_div
+
+
+@pytest.mark.slow
+def test_cfg3_full_N_same_stream_parity(ctx, oracle):
+    """full N = 2^20, B = 8, one (design, direction) pair per host core (at most 16, the
+    designs of the batch), oracle brute force over all 49 840 triangles on the same streams (~4 min per pair and core).
+    The beam kernel and the bounce kernel run in the tile configuration of the full job, escape masks on."""
+    import os
+    cfg = W.CONFIGS["cfg3_detailed"]
+    th, sun = cfg.params(), cfg.sun_dirs()
+    n = max(4, min(16, os.cpu_count() or 4))
+    rng = np.random.default_rng(11)
+    pairs = np.stack([np.arange(n) % cfg.D, rng.integers(0, cfg.S, n)], 1).astype(np.int32)
+    dz = ctx.srp_build_designs(cfg.family, th)
+    _same_stream_parity(ctx, oracle, cfg, dz, th, sun, pairs, cfg.N, 2e-4, "cfg3 full N", escape_masks=2)
+    st = ctx.srp_get_stats()
+    assert st["beam_tile_miss"] > 0 and st["loop_rounds"] >= 1        # beams + ray queue were in play
+    dz.free()
+
+
+@pytest.mark.slow
+def test_cfg5_sail_N14_same_stream_parity(ctx, oracle):
+    """N = 2^14 on 8 directions (two grazing, two oblique, near-normal from both sides, two of
+    the workload's Fibonacci directions), B = 8, oracle brute force over all 1 019 698 triangles (~4 min per
+    direction and core)."""
+    cfg = W.CONFIGS["cfg5_sail"]
+    th = cfg.params()
+    sun = np.concatenate([np.array([[1, 0.2, 0.02], [0.3, -1, -0.03], [0.5, 0.4, 0.7], [-0.2, 0.6, -0.6],
+                                    [0.05, 0.02, 1], [0.01, -0.03, -1]], np.float32), cfg.sun_dirs()[[517, 3011]]])
+    pairs = np.stack([np.zeros(len(sun)), np.arange(len(sun))], 1).astype(np.int32)
+    dz = ctx.srp_build_designs(cfg.family, th)
+    _same_stream_parity(ctx, oracle, cfg, dz, th, sun, pairs, 1 << 14, 2e-4, "cfg5 N = 2^14")
+    dz.free()
+
+
+# ---------------------------------------------------------------- per-sample designs (PAPER.md:146, 159, 352; NEXT-3)
+@pytest.mark.parametrize("family,M,N,B,sampler,deposit", [
+    (W.FAMILY_BOXWING, 40, 1 << 10, 4, 0, 0),        # 16 triangles per record
+    (W.FAMILY_BOXWING_T, 24, 1 << 10, 4, 0, 0),      # 1280 triangles: the paper's "1 k faces"
+    (W.FAMILY_BOXWING_T, 8, 1000, 3, 1, 1),          # i.i.d. sampler (N need not be a power of two), analog deposit
+])
+def test_per_sample_designs_match_oracle(ctx, oracle, family, M, N, B, sampler, deposit):
+    """srp_forces_per_sample: every record its own design AND its own direction, brute force over all triangles.
+    Record m against the oracle's forward tracer on design m (k = m in the Philox counters, direction index 0)."""
+    import torch
+    th = W.draw_params(family, M)
+    sun = W.random_directions(M)
+    ctx.srp_set_options(sampler=sampler, deposit=deposit)
+    try:
+        F = ctx.srp_forces_per_sample(family, cuda(th), cuda(sun), N, B, seed=5).cpu().numpy()
+        st = ctx.srp_get_stats()
+    finally:
+        ctx.srp_set_options()
+    assert st["launched"] == M * N
+    assert st["launched"] == st["primary_miss"] + st["absorbed"] + st["escaped"] + st["capped"]
+    Fo, sig, tot = [], [], None
+    for m in range(M):
+        v, mt = oracle.build_mesh(family, th[m], k=m)
+        r = oracle.forces(v, mt, sun[m:m + 1], N, B, seed=5, k=m, j0=0, sampler=sampler, deposit=deposit)
+        Fo.append(r["F"][0]); sig.append(r["sigma"][0])
+        tot = r["stats"] if tot is None else {a: ([x + y for x, y in zip(tot[a], b)] if isinstance(b, list) else tot[a] + b)
+                                             for a, b in r["stats"].items()}
+    assert_parity(F, np.array(Fo), np.array(sig), tol_agg=3e-3)      # N = 2^10: one photon is ~1e-3 of a vector (R24)
+    counters_close(st, tot, tol=8)
+    # the same records through the designs + pairs interface (direction index m instead of 0: other photons, same forces)
+    if family == W.FAMILY_BOXWING and sampler == 0:
+        dz = ctx.srp_build_designs(family, th)
+        pairs = np.stack([np.arange(M), np.arange(M)], 1).astype(np.int32)
+        Fp = ctx.srp_forces_pairs(dz, cuda(sun), pairs, 1 << 16, B, 5).cpu().numpy()
+        assert np.all(np.linalg.norm(F - Fp, axis=1) <= 5.0 * np.array(sig) + 1e-3 * np.linalg.norm(Fp, axis=1))
+        dz.free()
 
 
 def test_force_maps_direct_and_indirect(ctx):
