@@ -678,7 +678,7 @@ srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const floa
     if (st != SRP_OK) return st;
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
     // chunks of records: meshes for a chunk (S0), its boxes and packed triangles (S1 without a hierarchy), its photons
-    long long chunk = (256LL << 20) / (96 * T);                     // ~256 MiB of mesh per chunk
+    long long chunk = (1LL << 30) / (96 * T);                       // ~1 GiB of mesh per chunk: many waves of blocks per launch
     if (chunk > 32768) chunk = 32768;
     if (chunk > M) chunk = M;
     if (chunk < 1) chunk = 1;
