@@ -104,7 +104,8 @@ typedef struct {
     unsigned long long beam_box_tests, tri2d_tests, tri_setups, rect_tests;
     unsigned long long mask_escapes;   /* bounce rays resolved as "escaped" by the escape masks (also counted in
                                           escaped and segments) */
-    unsigned long long queued_rays;    /* rays the beam kernel handed to the bounce kernel through the ray queue */
+    unsigned long long queued_rays;    /* slots of the ray queue the beam kernel handed to the bounce kernel (rays, plus
+                                          the few slots a beam warp reserved and did not fill) */
     unsigned long long loop_rounds;    /* rounds of the beam / bounce loop that had rays queued (counted on the device) */
     unsigned long long kernel_launches;/* kernels of this library the last srp_forces* / srp_thermal_forces call ran:
                                           those enqueued by the host plus, for the beam / bounce loop, the rounds the

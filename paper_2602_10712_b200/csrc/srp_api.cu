@@ -107,7 +107,9 @@ srp_status ensure_queue(srp_context *ctx, TraceArgs &a, bool brute, bool instrum
     a.rq = nullptr; a.rq_cap = 0; a.rq_high = 0; a.rq_ctr = nullptr;
     if (!want_beams(ctx, brute, a.max_tris, a.N, a.n_pairs)) return SRP_OK;
     const size_t fields = instrumented ? SRP_RQ_FIELDS_INSTR : SRP_RQ_FIELDS;
-    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * (size_t)a.tile_rays;
+    // slots the resident beam warps can still take after the high-water mark: a tile's rays each, in chunks of 256 of
+    // which up to 31 stay unfilled (marked dead) when a push does not fit
+    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * ((size_t)a.tile_rays + (size_t)a.tile_rays / 7 + 512);
     const size_t min_rays = reserve + (1u << 20);
     if (!ctx->rq_ctr) {
         TRY_CUDA(ctx, cudaMalloc(&ctx->rq_ctr, 4 * sizeof(unsigned)), "alloc queue counters");
@@ -785,7 +787,7 @@ srp_status srp_launch_count(srp_context *ctx, unsigned long long *n_kernels)
 unsigned long long srp_workspace_bytes_min(const srp_context *ctx)
 {
     if (!ctx) return 0;
-    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * 8192u;   // the largest tile (make_args)
+    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * (8192u + 8192u / 7 + 512u);   // the largest tile (make_args, ensure_queue)
     return (unsigned long long)((reserve + (1u << 20)) * SRP_RQ_FIELDS_INSTR * sizeof(unsigned));
 }
 

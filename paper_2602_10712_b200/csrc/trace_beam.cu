@@ -99,8 +99,14 @@ __device__ __forceinline__ bool beam_push_tris(int *cid, int &ncand, int first0,
     const int total = __shfl_sync(FULL, incl, 31);
     if (ncand + total > BEAM_CMAX) return false;
     int pos = ncand + incl - c;
-    for (int t = 0; t < cnt0; ++t) cid[pos++] = first0 + t;
-    for (int t = 0; t < cnt1; ++t) cid[pos++] = first1 + t;
+    // leaves hold <= 2 triangles by default (SRP_LEAF_MAX): two predicated stores each, then whatever is left
+    if (cnt0 > 0) cid[pos] = first0;
+    if (cnt0 > 1) cid[pos + 1] = first0 + 1;
+    for (int t = 2; t < cnt0; ++t) cid[pos + t] = first0 + t;
+    pos += cnt0;
+    if (cnt1 > 0) cid[pos] = first1;
+    if (cnt1 > 1) cid[pos + 1] = first1 + 1;
+    for (int t = 2; t < cnt1; ++t) cid[pos + t] = first1 + t;
     ncand += total;
     return true;
 }
@@ -133,19 +139,27 @@ beam_trace_kernel(const TraceArgs a)
     const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
     const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
 
-    // Appends this lane's ray (if `push`) to the ray queue; warp-wide call, one atomic per call.
+    // Appends this lane's ray (if `push`) to the ray queue; warp-wide call.  The warp reserves RQ_CHUNK slots of the
+    // queue at a time (one atomic per ~30 pushes instead of one per push); slots it has reserved and not filled when
+    // it stops are marked dead for the bounce kernel.
+    uint32_t ch_next = 0, ch_end = 0;                              // warp-uniform: the warp's reserved slots
     auto queue_push = [&](bool push, const float3 &o, const float3 &d, uint32_t i, uint32_t p, uint32_t sd,
                          unsigned long long sig) {
         const unsigned m = __ballot_sync(FULL, push);
         if (m == 0u) return;
-        uint32_t base = 0;
-        if (lane == 0) base = atomicAdd(a.rq_ctr, (unsigned)__popc(m));
-        base = __shfl_sync(FULL, base, 0);
+        const uint32_t cnt = (uint32_t)__popc(m);
+        if (ch_next + cnt > ch_end) {                              // not enough room left: give the rest up, take a new chunk
+            for (uint32_t x = ch_next + (uint32_t)lane; x < ch_end; x += 32u) rq_mark_dead(a, x);
+            uint32_t base = 0;
+            if (lane == 0) base = atomicAdd(a.rq_ctr, RQ_CHUNK);
+            ch_next = __shfl_sync(FULL, base, 0); ch_end = ch_next + RQ_CHUNK;
+        }
         if (push) {
-            const uint32_t pos = base + (uint32_t)__popc(m & lt_mask);
+            const uint32_t pos = ch_next + (uint32_t)__popc(m & lt_mask);
             SRP_CHECK(pos < a.rq_cap, "ray queue");
             rq_store<INSTR>(a, pos, o, d, i, p, sd, sig);
         }
+        ch_next += cnt;
     };
 
     // ---- S2-S5 for the primaries of one tile, as beams ----
@@ -382,6 +396,7 @@ beam_trace_kernel(const TraceArgs a)
         process_tile(tile);
         __syncwarp();
     }
+    for (uint32_t x = ch_next + (uint32_t)lane; x < ch_end; x += 32u) rq_mark_dead(a, x);   // unused slots of the last chunk
     flush_counters<INSTR>(a, cn, s_hist[warp], lane);
     flush_beam_counters(a, bc, lane);
 }

@@ -166,7 +166,7 @@ bounce_trace_kernel(const TraceArgs a)
                 const uint32_t rank = (uint32_t)__popc(idle & lt_mask);
                 if (!has && rank < navail) {
                     rq_load<INSTR>(a, gb_next + rank, o, d, ri, rp, rsd, rsig);
-                    start_ray();
+                    if (rsd != RQ_DEAD) start_ray();                 // a slot a beam warp reserved and did not fill
                 }
                 const uint32_t want = (uint32_t)__popc(idle);
                 gb_next += want < navail ? want : navail;

@@ -498,6 +498,10 @@ __device__ __forceinline__ void flush_counters(const TraceArgs &a, const LaneCou
 // plus the 64-bit path signature in the instrumented build; field-major, so that the appends of a warp and the
 // fetches of the bounce kernel coalesce.  Written with st.cg / read with ld.cg: the data crosses kernels through L2.
 constexpr uint32_t SRC_NONE = 0x07ffffffu;
+constexpr uint32_t RQ_DEAD = 0xffffffffu;        // src | depth word of a reserved slot that holds no ray (depth 31 never occurs)
+constexpr uint32_t RQ_CHUNK = 256u;              // slots a beam warp reserves at a time
+
+__device__ __forceinline__ void rq_mark_dead(const TraceArgs &a, uint32_t pos) { __stcg(a.rq + 8 * (size_t)a.rq_cap + pos, RQ_DEAD); }
 
 template <bool INSTR>
 __device__ __forceinline__ void rq_store(const TraceArgs &a, uint32_t pos, const float3 &o, const float3 &d, uint32_t i,
