@@ -77,7 +77,7 @@ srp_status ensure_workspace(srp_context *ctx, size_t accum_items)
         TRY_CUDA(ctx, cudaMalloc(&ctx->rounds_total, sizeof(unsigned long long)), "alloc round counter");
         TRY_CUDA(ctx, cudaMemsetAsync(ctx->rounds_total, 0, sizeof(unsigned long long), ctx->stream), "zero round counter");
     }
-    if (!ctx->work_counter) TRY_CUDA(ctx, cudaMalloc(&ctx->work_counter, sizeof(unsigned long long)), "alloc counter");
+    if (!ctx->work_counter) TRY_CUDA(ctx, cudaMalloc(&ctx->work_counter, SRP_PIPES * sizeof(unsigned long long)), "alloc counter");
     if (ctx->accum_items < accum_items) {
         TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before workspace growth");
         cudaFree(ctx->accum); ctx->accum = nullptr; ctx->accum_items = 0;
@@ -98,37 +98,47 @@ bool want_beams(const srp_context *ctx, bool brute, long long max_tris, long lon
     return N >= 8 * max_tris;
 }
 
-// The ray queue between the beam kernel and the bounce kernel.  The beam warps stop taking
-// tiles once rq_high rays are queued; every resident warp may still add the rays of the tile it is working on, hence
-// the reserve.  The memory is the caller's (srp_set_workspace) or, failing that, allocated here once.
-#define SRP_RQ_DEFAULT_RAYS (1u << 25)
+// The ray queues between the beam kernel and the bounce kernel.  The beam warps of a
+// pipeline stop taking tiles once rq_high rays are queued; every resident warp may still add the rays of the tile it
+// is working on, hence the reserve.  The memory is the caller's (srp_set_workspace) or, failing that, allocated here
+// once.  Sets a.rq_* for ONE queue over all of the memory; launch_trace_all shares it out among the pipelines.
+size_t queue_reserve(const srp_context *ctx, int tile_rays)
+{
+    // slots the resident beam warps can still take after the high-water mark: a tile's rays each, in chunks of 256 of
+    // which up to 31 stay unfilled (marked dead) when a push does not fit
+    return (size_t)srp_beam_warps(ctx->num_sms) * ((size_t)tile_rays + (size_t)tile_rays / 7 + 512);
+}
+
 srp_status ensure_queue(srp_context *ctx, TraceArgs &a, bool brute, bool instrumented)
 {
     a.rq = nullptr; a.rq_cap = 0; a.rq_high = 0; a.rq_ctr = nullptr;
     if (!want_beams(ctx, brute, a.max_tris, a.N, a.n_pairs)) return SRP_OK;
     const size_t fields = instrumented ? SRP_RQ_FIELDS_INSTR : SRP_RQ_FIELDS;
-    // slots the resident beam warps can still take after the high-water mark: a tile's rays each, in chunks of 256 of
-    // which up to 31 stay unfilled (marked dead) when a push does not fit
-    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * ((size_t)a.tile_rays + (size_t)a.tile_rays / 7 + 512);
+    const size_t reserve = queue_reserve(ctx, a.tile_rays);
     const size_t min_rays = reserve + (1u << 20);
     if (!ctx->rq_ctr) {
-        TRY_CUDA(ctx, cudaMalloc(&ctx->rq_ctr, 4 * sizeof(unsigned)), "alloc queue counters");
-        TRY_CUDA(ctx, cudaMemsetAsync(ctx->rq_ctr, 0, 4 * sizeof(unsigned), ctx->stream), "zero queue counters");
+        TRY_CUDA(ctx, cudaMalloc(&ctx->rq_ctr, 4 * SRP_PIPES * sizeof(unsigned)), "alloc queue counters");
+        TRY_CUDA(ctx, cudaMemsetAsync(ctx->rq_ctr, 0, 4 * SRP_PIPES * sizeof(unsigned), ctx->stream), "zero queue counters");
     }
     if (ctx->rq_words < min_rays * fields) {
         if (ctx->rq && !ctx->rq_owned)
             return fail(ctx, SRP_ERR_OOM, "the workspace given to srp_set_workspace is too small for this call's ray queue");
         TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before queue growth");
         cudaFree(ctx->rq); ctx->rq = nullptr; ctx->rq_words = 0; ctx->rq_owned = false;
-        size_t rays = SRP_RQ_DEFAULT_RAYS > 2 * min_rays ? SRP_RQ_DEFAULT_RAYS : 2 * min_rays;
-        cudaError_t e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * SRP_RQ_FIELDS_INSTR);
+        // Every round of a loop ends with a tail in which SMs idle; two pipelines hide each other's tails, and the
+        // more rays a queue holds beyond its reserve, the fewer rounds there are: 32 M slots more by default.
+#ifndef SRP_RQ_EXTRA
+#define SRP_RQ_EXTRA (32u << 20)
+#endif
+        size_t rays = SRP_PIPES * min_rays + (size_t)(SRP_RQ_EXTRA);
+        cudaError_t e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * fields);
         if (e != cudaSuccess) {                                 // less room than we would like: the smallest queue that works
             cudaGetLastError();
             rays = min_rays;
-            e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * SRP_RQ_FIELDS_INSTR);
+            e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * fields);
         }
         if (e != cudaSuccess) return cuda_fail(ctx, "alloc ray queue", e);
-        ctx->rq_words = rays * SRP_RQ_FIELDS_INSTR; ctx->rq_owned = true;
+        ctx->rq_words = rays * fields; ctx->rq_owned = true;
     }
     const size_t rays = ctx->rq_words / fields;
     a.rq = ctx->rq; a.rq_ctr = ctx->rq_ctr;
@@ -154,7 +164,10 @@ void reap_graphs(srp_context *ctx, bool all)
 // Enqueues S2-S7.  With beams: the beam kernel (primaries) and the bounce kernel (everything queued) alternate until
 // the tiles run out.  How often is known only on the device (it depends on how many photons go on), so the loop is
 // a conditional WHILE node of a CUDA graph: body = beam kernel, bounce kernel, and a one-thread kernel that sets the
-// condition from the tile counter.  Nothing is synchronised and no launch is wasted.
+// condition from the tile counter.  Nothing is synchronised and no launch is wasted.  Every round ends with a tail
+// in which SMs run out of work (the last heavy tiles, the last long photon paths); so the tiles are shared out among
+// SRP_PIPES such loops with a queue each, independent nodes of the same graph, and one loop's kernels fill the SMs
+// that the other's tail leaves idle.
 srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bool instrumented)
 {
     if (!a.rq) {
@@ -162,36 +175,63 @@ srp_status launch_trace_all(srp_context *ctx, const TraceArgs &a, bool brute, bo
         count_launches(ctx, 1);
         return SRP_OK;
     }
+    const size_t fields = instrumented ? SRP_RQ_FIELDS_INSTR : SRP_RQ_FIELDS;
+    const size_t reserve = queue_reserve(ctx, a.tile_rays);
+    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
+    int pipes = SRP_PIPES;
+    if (ctx->opt.plain_launches || total_tiles < 64 || (size_t)a.rq_cap < SRP_PIPES * (reserve + (1u << 20))) pipes = 1;
+    // Shares of the tiles and of the queue memory beyond the reserves (uneven shares, tried so that the loops' rounds
+    // would not fall into step, change nothing: 0.5 ... 0.7 all within 1 %).
+#ifndef SRP_PIPE_SHARE0
+#define SRP_PIPE_SHARE0 0.5
+#endif
+    const double share[SRP_PIPES] = { pipes == 1 ? 1.0 : SRP_PIPE_SHARE0, 1.0 - SRP_PIPE_SHARE0 };
+    const size_t extra = (size_t)a.rq_cap - (size_t)pipes * reserve;
+    TraceArgs ap[SRP_PIPES];
+    size_t ray0 = 0;
+    unsigned long long tile0 = 0;
+    for (int q = 0; q < pipes; ++q) {
+        ap[q] = a;
+        ap[q].tile_begin = tile0;
+        ap[q].tile_end = q == pipes - 1 ? total_tiles : tile0 + (unsigned long long)((double)total_tiles * share[q]);
+        tile0 = ap[q].tile_end;
+        ap[q].work_counter = a.work_counter + q;
+        ap[q].rq_ctr = a.rq_ctr + 4 * q;
+        ap[q].rq_cap = (unsigned)(reserve + (size_t)((double)extra * share[q]));
+        ap[q].rq = a.rq + ray0 * fields;
+        ray0 += ap[q].rq_cap;
+        ap[q].rq_high = (unsigned)(ap[q].rq_cap - reserve);
+    }
+    count_launches(ctx, pipes);                               // at least one beam launch each; the rounds are counted on the device
     if (ctx->opt.plain_launches) {                          // a sufficient number of rounds; surplus ones find nothing to do
-        count_launches(ctx, 1);
-        const long long rounds = (long long)((double)a.n_pairs * (double)a.N / (double)a.rq_high) + 1;
+        const long long rounds = (long long)((double)a.n_pairs * (double)a.N / (double)ap[0].rq_high) + 1;
         for (long long r = 0; r < rounds; ++r) {
-            TRY_CUDA(ctx, srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->stream), "beam launch");
-            TRY_CUDA(ctx, srp_launch_bounce(a, instrumented, ctx->num_sms, ctx->stream), "bounce launch");
+            TRY_CUDA(ctx, srp_launch_trace(ap[0], brute, instrumented, ctx->num_sms, ctx->stream), "beam launch");
+            TRY_CUDA(ctx, srp_launch_bounce(ap[0], instrumented, ctx->num_sms, ctx->stream), "bounce launch");
         }
         return SRP_OK;
     }
-    count_launches(ctx, 1);                                 // at least one beam launch; the rounds are counted on the device
     reap_graphs(ctx, false);
-    if (!ctx->capture_stream)
-        TRY_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "create capture stream");
     srp_context::PendingGraph g = { nullptr, nullptr, nullptr };
     cudaError_t e = cudaGraphCreate(&g.graph, 0);
-    cudaGraphConditionalHandle handle;
-    if (e == cudaSuccess) e = cudaGraphConditionalHandleCreate(&handle, g.graph, 1, cudaGraphCondAssignDefault);
-    cudaGraphNodeParams cp = { cudaGraphNodeTypeConditional };
-    cp.conditional.handle = handle; cp.conditional.type = cudaGraphCondTypeWhile; cp.conditional.size = 1;
-    cudaGraphNode_t cnode;
-    if (e == cudaSuccess) e = cudaGraphAddNode(&cnode, g.graph, nullptr, 0, &cp);
-    if (e == cudaSuccess) {
+    for (int q = 0; q < pipes && e == cudaSuccess; ++q) {
+        if (!ctx->capture_stream[q]) e = cudaStreamCreateWithFlags(&ctx->capture_stream[q], cudaStreamNonBlocking);
+        cudaGraphConditionalHandle handle;
+        if (e == cudaSuccess) e = cudaGraphConditionalHandleCreate(&handle, g.graph, 1, cudaGraphCondAssignDefault);
+        cudaGraphNodeParams cp = { cudaGraphNodeTypeConditional };
+        cp.conditional.handle = handle; cp.conditional.type = cudaGraphCondTypeWhile; cp.conditional.size = 1;
+        cudaGraphNode_t cnode;
+        if (e == cudaSuccess) e = cudaGraphAddNode(&cnode, g.graph, nullptr, 0, &cp);      // no dependencies: the loops run side by side
+        if (e != cudaSuccess) break;
         cudaGraph_t body = cp.conditional.phGraph_out[0];
-        e = cudaStreamBeginCaptureToGraph(ctx->capture_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+        cudaStream_t cs = ctx->capture_stream[q];
+        e = cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
         if (e == cudaSuccess) {
-            cudaError_t e1 = srp_launch_trace(a, brute, instrumented, ctx->num_sms, ctx->capture_stream);
-            if (e1 == cudaSuccess) e1 = srp_launch_bounce(a, instrumented, ctx->num_sms, ctx->capture_stream);
-            if (e1 == cudaSuccess) e1 = srp_launch_loop_cond(handle, a, ctx->capture_stream);
+            cudaError_t e1 = srp_launch_trace(ap[q], brute, instrumented, ctx->num_sms, cs);
+            if (e1 == cudaSuccess) e1 = srp_launch_bounce(ap[q], instrumented, ctx->num_sms, cs);
+            if (e1 == cudaSuccess) e1 = srp_launch_loop_cond(handle, ap[q], cs);
             cudaGraph_t same = nullptr;
-            e = cudaStreamEndCapture(ctx->capture_stream, &same);
+            e = cudaStreamEndCapture(cs, &same);
             if (e1 != cudaSuccess) e = e1;
         }
     }
@@ -276,11 +316,15 @@ TraceArgs make_args(srp_context *ctx, const srp_designs *dz, const float *sun_di
     const bool beam = brute ? (ctx->opt.sampler == 0 && ctx->opt.primary_mode != 1)
                             : want_beams(ctx, ctx->opt.force_brute != 0, a.max_tris, N, n_pairs);
     const long long warps = (long long)ctx->num_sms * srp_trace_blocks_per_sm(brute, beam);
-    long long tile = 8192;
+#ifndef SRP_BEAM_TILE_MAX
+#define SRP_BEAM_TILE_MAX 4096     // beam tiles: half the reserve of the ray queues (there is one per pipeline); same speed as 8192
+#endif
+    long long tile = (beam && !brute) ? SRP_BEAM_TILE_MAX : 8192;
     if (tile > N) tile = N;
     while (tile > 256 && n_pairs * ((N + tile - 1) / tile) < 8 * warps) tile >>= 1;
     a.tile_rays = (int)tile;
     a.tiles_per_pair = (N + tile - 1) / tile;
+    a.tile_begin = 0; a.tile_end = (unsigned long long)n_pairs * a.tiles_per_pair;
     return a;
 }
 
@@ -306,7 +350,7 @@ srp_status run_forces(srp_context *ctx, const srp_designs *dz, const float *sun_
     if (ctx->opt.escape_masks == 0) a.dz.esc = nullptr;        // masks an earlier call built stay unused
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * stride * n_pairs, ctx->stream), "zero accumulators");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
-    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, SRP_PIPES * sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
     st = ensure_queue(ctx, a, brute, ctx->opt.instrumented != 0);
     if (st != SRP_OK) return st;
@@ -357,7 +401,8 @@ srp_status srp_destroy(srp_context *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     reap_graphs(ctx, true);
-    if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
+    for (cudaStream_t cs : ctx->capture_stream)
+        if (cs) cudaStreamDestroy(cs);
     cudaFree(ctx->accum); cudaFree(ctx->stats); cudaFree(ctx->work_counter); cudaFree(ctx->rq_ctr);
     if (ctx->rq_owned) cudaFree(ctx->rq);
     cudaFree(ctx->stage_dirs); cudaFree(ctx->stage_out);
@@ -613,7 +658,7 @@ srp_status srp_thermal_forces(srp_context *ctx, const srp_designs *dz, const flo
     if (e == cudaSuccess) e = pool_alloc(ctx, &design_power, sizeof(float) * dz->D);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * dz->D, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->work_counter, 0, SRP_PIPES * sizeof(unsigned long long), ctx->stream);
     if (e == cudaSuccess)
         e = srp_launch_thermal(a, facet_power, dz->sumT, emit_list, n_emit, design_power, out_forces, ctx->num_sms, ctx->stream);
     if (emit_list) cudaFreeAsync(emit_list, ctx->stream);      // stream-ordered: after the kernels that use them
@@ -750,7 +795,7 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *dz, const fl
     TRY_CUDA(ctx, cudaMemsetAsync(out_sig, 0, sizeof(unsigned long long) * n_pairs * N, ctx->stream), "zero signatures");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->accum, 0, sizeof(long long) * 3 * n_pairs, ctx->stream), "zero accumulators");
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
-    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, sizeof(unsigned long long), ctx->stream), "zero counter");
+    TRY_CUDA(ctx, cudaMemsetAsync(ctx->work_counter, 0, SRP_PIPES * sizeof(unsigned long long), ctx->stream), "zero counter");
     const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
     st = ensure_queue(ctx, a, brute, true);
     if (st != SRP_OK) return st;
@@ -787,8 +832,7 @@ srp_status srp_launch_count(srp_context *ctx, unsigned long long *n_kernels)
 unsigned long long srp_workspace_bytes_min(const srp_context *ctx)
 {
     if (!ctx) return 0;
-    const size_t reserve = (size_t)srp_beam_warps(ctx->num_sms) * (8192u + 8192u / 7 + 512u);   // the largest tile (make_args, ensure_queue)
-    return (unsigned long long)((reserve + (1u << 20)) * SRP_RQ_FIELDS_INSTR * sizeof(unsigned));
+    return (unsigned long long)((queue_reserve(ctx, SRP_BEAM_TILE_MAX) + (1u << 20)) * SRP_RQ_FIELDS_INSTR * sizeof(unsigned));
 }
 
 srp_status srp_set_workspace(srp_context *ctx, void *ptr, unsigned long long bytes)

@@ -8,6 +8,7 @@
 #include <vector>
 #include "srp.h"
 
+#define SRP_PIPES 2                // beam / bounce loops that run side by side, each on its share of the tiles
 #define SRP_BRUTE_MAX_TRIS 64      // designs with T <= this are traced without a hierarchy (one leaf)
 #define SRP_LEAF_MAX 2             // LBVH subtrees with <= this many triangles become one leaf (cfg3 -7 %, cfg5 -3 % against 3)
 #define SRP_ACC_BITS_MAX 32        // fixed-point fraction bits of the dimensionless force accumulators, at most
@@ -84,7 +85,7 @@ struct srp_context {
     unsigned long long launches_call = 0;                     // ... by the last srp_forces* call
     unsigned long long *rounds_total = nullptr;               // device: loop rounds since srp_create
     cudaMemPool_t mempool = nullptr;                          // design arrays come from this private stream-ordered pool
-    cudaStream_t capture_stream = nullptr;                    // the beam / bounce loop is captured here into a graph
+    cudaStream_t capture_stream[SRP_PIPES] = { nullptr, nullptr };   // the beam / bounce loops are captured here into a graph
     struct PendingGraph { cudaGraphExec_t exec; cudaGraph_t graph; cudaEvent_t done; };
     std::vector<PendingGraph> graphs;                         // launched loops; destroyed once they have run
     float *stage_dirs = nullptr;  size_t stage_dirs_items = 0; // srp_forces_host staging
@@ -113,6 +114,7 @@ struct TraceArgs {
     DevStats *stats;
     unsigned long long *work_counter;
     long long tiles_per_pair;
+    unsigned long long tile_begin, tile_end;   // beam kernel: this launch works on tiles [tile_begin, tile_end) (a pipeline's share)
     int tile_rays;
     unsigned long long *sig_out;   // debug (instrumented kernels): [n_pairs, N] path signatures, or nullptr
     // ray queue (trace_beam.cu -> trace_bounce.cu): continuing photons the beam kernel hands to the bounce kernel

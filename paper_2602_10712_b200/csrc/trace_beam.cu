@@ -135,7 +135,6 @@ beam_trace_kernel(const TraceArgs a)
     BeamSmem &W = s_w[warp];
     LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
     BeamCounters bc = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
     const uint32_t ldx = compact_even_bits((uint32_t)lane), ldy = compact_even_bits((uint32_t)lane >> 1);
     const float inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1)), inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
 
@@ -390,9 +389,9 @@ beam_trace_kernel(const TraceArgs a)
     // to take over (the host then launches this kernel again; the tile counter carries on) ----
     for (;;) {
         unsigned long long tile = ~0ULL;
-        if (lane == 0 && *(volatile unsigned *)a.rq_ctr < a.rq_high) tile = atomicAdd(a.work_counter, 1ULL);
+        if (lane == 0 && *(volatile unsigned *)a.rq_ctr < a.rq_high) tile = a.tile_begin + atomicAdd(a.work_counter, 1ULL);
         tile = __shfl_sync(FULL, tile, 0);
-        if (tile >= total_tiles) break;
+        if (tile >= a.tile_end) break;
         process_tile(tile);
         __syncwarp();
     }

@@ -220,7 +220,11 @@ bounce_trace_kernel(const TraceArgs a)
     if (lane == 0) {
         __threadfence();
         if (atomicAdd(a.rq_ctr + 2, 1u) == gridDim.x * TRACE_WARPS - 1u) {
-            if (n_queued != 0u) { a.stats->queued_rays += n_queued; a.stats->loop_rounds += 1ULL; *a.rounds_total += 1ULL; }
+            if (n_queued != 0u) {                                   // atomics: the pipelines' bounce kernels may run side by side
+                atomicAdd((unsigned long long *)&a.stats->queued_rays, (unsigned long long)n_queued);
+                atomicAdd((unsigned long long *)&a.stats->loop_rounds, 1ULL);
+                atomicAdd(a.rounds_total, 1ULL);
+            }
             a.rq_ctr[0] = 0u; a.rq_ctr[1] = 0u; a.rq_ctr[2] = 0u;
             __threadfence();
         }
@@ -230,9 +234,9 @@ bounce_trace_kernel(const TraceArgs a)
 // Loop condition of the beam / bounce loop (a conditional WHILE node of a CUDA graph): go round again while tiles
 // are left.  Runs after the bounce kernel, which has emptied the queue.
 __global__ void loop_cond_kernel(cudaGraphConditionalHandle handle, const unsigned long long *work_counter,
-                                 unsigned long long total_tiles)
+                                 unsigned long long n_tiles)
 {
-    cudaGraphSetConditional(handle, *work_counter < total_tiles ? 1u : 0u);
+    cudaGraphSetConditional(handle, *work_counter < n_tiles ? 1u : 0u);
 }
 
 template <typename K>
@@ -254,7 +258,7 @@ cudaError_t launch_bounce(K kernel, const TraceArgs &a, int num_sms, cudaStream_
 
 cudaError_t srp_launch_loop_cond(cudaGraphConditionalHandle handle, const TraceArgs &a, cudaStream_t stream)
 {
-    loop_cond_kernel<<<1, 1, 0, stream>>>(handle, a.work_counter, (unsigned long long)a.n_pairs * a.tiles_per_pair);
+    loop_cond_kernel<<<1, 1, 0, stream>>>(handle, a.work_counter, a.tile_end - a.tile_begin);
     return cudaGetLastError();
 }
 

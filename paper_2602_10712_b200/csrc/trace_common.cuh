@@ -589,7 +589,7 @@ cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStr
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    const unsigned long long total_tiles = (unsigned long long)a.n_pairs * a.tiles_per_pair;
+    const unsigned long long total_tiles = a.tile_end - a.tile_begin;
     unsigned long long blocks = (unsigned long long)num_sms * per_sm;       // persistent: fill the machine once
     const unsigned long long needed = (total_tiles + TRACE_WARPS - 1) / TRACE_WARPS;
     if (blocks > needed) blocks = needed;
