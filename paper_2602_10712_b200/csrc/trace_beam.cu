@@ -26,18 +26,18 @@ namespace {
 // along an edge-on panel, a bundle of thin facets) sends its 32 primaries to the queue as well, so
 // any input is handled.
 #ifndef BEAM_BLOCKS_PER_SM
-#define BEAM_BLOCKS_PER_SM 5
+#define BEAM_BLOCKS_PER_SM 4        // 4 blocks with 240-candidate lists beat 5 with 160 (-4 %), 6 with 144 (+7 %), 8 with 96 (+35 %)
 #endif
 #ifndef BEAM_SB_DEF
 #define BEAM_SB_DEF 256
 #endif
 constexpr int BEAM_SB = BEAM_SB_DEF;        // rays per sub-block
 #ifndef BEAM_CMAX_DEF
-#define BEAM_CMAX_DEF 160
+#define BEAM_CMAX_DEF 240
 #endif
 constexpr int BEAM_CMAX = BEAM_CMAX_DEF;      // candidate triangles per sub-block
 #ifndef BEAM_QN_DEF
-#define BEAM_QN_DEF 192
+#define BEAM_QN_DEF 160
 #endif
 constexpr int BEAM_QN = BEAM_QN_DEF;        // node queue of the sub-block descent
 constexpr int BEAM_EN = 64;         // tile entry list: internal nodes
@@ -125,7 +125,8 @@ template <bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
 __global__ void __launch_bounds__(TRACE_THREADS, BEAM_BLOCKS_PER_SM)
 beam_trace_kernel(const TraceArgs a)
 {
-    __shared__ BeamSmem s_w[TRACE_WARPS];
+    extern __shared__ __align__(16) unsigned char s_dyn[];     // BeamSmem per warp: more than the 48 KB a static array may have
+    BeamSmem *s_w = reinterpret_cast<BeamSmem *>(s_dyn);
     __shared__ unsigned s_hist[TRACE_WARPS][16];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -402,16 +403,19 @@ beam_trace_kernel(const TraceArgs a)
 
 } // namespace
 
-int srp_beam_blocks_per_sm() { return blocks_per_sm(beam_trace_kernel<false, false, false, false>); }
+constexpr size_t BEAM_SMEM_BYTES = sizeof(BeamSmem) * TRACE_WARPS;
+
+int srp_beam_blocks_per_sm() { return blocks_per_sm(beam_trace_kernel<false, false, false, false>, BEAM_SMEM_BYTES); }
 
 // Resident warps of the beam kernel at most (any build): each may add one tile's rays to the queue after the
 // high-water mark is reached.
 int srp_beam_warps(int num_sms)
 {
     int per_sm = 0;
-    const int occ[6] = { blocks_per_sm(beam_trace_kernel<true, false, false, false>), blocks_per_sm(beam_trace_kernel<true, false, true, false>),
-                         blocks_per_sm(beam_trace_kernel<false, false, false, false>), blocks_per_sm(beam_trace_kernel<false, false, true, false>),
-                         blocks_per_sm(beam_trace_kernel<false, true, false, false>), blocks_per_sm(beam_trace_kernel<false, true, true, false>) };
+    const size_t sm = BEAM_SMEM_BYTES;
+    const int occ[6] = { blocks_per_sm(beam_trace_kernel<true, false, false, false>, sm), blocks_per_sm(beam_trace_kernel<true, false, true, false>, sm),
+                         blocks_per_sm(beam_trace_kernel<false, false, false, false>, sm), blocks_per_sm(beam_trace_kernel<false, false, true, false>, sm),
+                         blocks_per_sm(beam_trace_kernel<false, true, false, false>, sm), blocks_per_sm(beam_trace_kernel<false, true, true, false>, sm) };
     for (int v = 0; v < 6; ++v) if (occ[v] > per_sm) per_sm = occ[v];
     if (per_sm < 1) per_sm = 1;
     return num_sms * per_sm * TRACE_WARPS;
@@ -419,5 +423,6 @@ int srp_beam_warps(int num_sms)
 
 cudaError_t srp_launch_beam(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream)
 {
+    const size_t dyn_smem = BEAM_SMEM_BYTES;
     return SRP_LAUNCH3(beam_trace_kernel);
 }

@@ -583,10 +583,13 @@ __device__ __forceinline__ void beam_setup(const float4 q0, const float4 q1, con
 
 // Launches a persistent trace kernel: as many blocks as fit the machine once, or fewer if there is less work.
 template <typename K>
-cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStream_t stream)
+cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStream_t stream, size_t dyn_smem = 0)
 {
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, 0);
+    cudaError_t e = cudaSuccess;
+    if (dyn_smem > 0) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, dyn_smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     const unsigned long long total_tiles = a.tile_end - a.tile_begin;
@@ -594,15 +597,16 @@ cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStr
     const unsigned long long needed = (total_tiles + TRACE_WARPS - 1) / TRACE_WARPS;
     if (blocks > needed) blocks = needed;
     if (blocks < 1) blocks = 1;
-    kernel<<<(unsigned)blocks, TRACE_THREADS, 0, stream>>>(a);
+    kernel<<<(unsigned)blocks, TRACE_THREADS, dyn_smem, stream>>>(a);
     return cudaGetLastError();
 }
 
 template <typename K>
-int blocks_per_sm(K kernel)
+int blocks_per_sm(K kernel, size_t dyn_smem = 0)
 {
     int per_sm = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, 0);
+    if (dyn_smem > 0) cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, dyn_smem);
     return per_sm;
 }
 
@@ -610,8 +614,8 @@ int blocks_per_sm(K kernel)
 // accumulation -- each also with glossy specular lobes (R23), used when the designs carry
 // shininess, and each of those for the expected-value and for the analog deposit rule.  Instrumented torque runs are refused by the caller (srp_api.cu).
 #define SRP_LAUNCH_A(K_, I_, T_, G_, ...)                                                                 \
-    (a.deposit ? launch_persistent(K_<__VA_ARGS__ I_, T_, G_, true>, a, num_sms, stream)                  \
-               : launch_persistent(K_<__VA_ARGS__ I_, T_, G_, false>, a, num_sms, stream))
+    (a.deposit ? launch_persistent(K_<__VA_ARGS__ I_, T_, G_, true>, a, num_sms, stream, dyn_smem)        \
+               : launch_persistent(K_<__VA_ARGS__ I_, T_, G_, false>, a, num_sms, stream, dyn_smem))
 #define SRP_LAUNCH_G(K_, I_, T_, ...)                                                                     \
     (a.dz.shin ? SRP_LAUNCH_A(K_, I_, T_, true, __VA_ARGS__) : SRP_LAUNCH_A(K_, I_, T_, false, __VA_ARGS__))
 #define SRP_LAUNCH3(K_, ...)                                                                              \

@@ -283,6 +283,7 @@ int srp_perray_blocks_per_sm(bool brute)
 // mode: MODE_BVH (0 is BRUTE_SMEM, 1 BVH, 2 BRUTE_GLOBAL -- the enum of trace_common.cuh)
 cudaError_t srp_launch_perray(const TraceArgs &a, int mode, bool instrumented, int num_sms, cudaStream_t stream)
 {
+    const size_t dyn_smem = 0;
     if (mode == MODE_BRUTE_GLOBAL) return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_GLOBAL,);
     if (mode == MODE_BRUTE_SMEM) return SRP_LAUNCH3(trace_kernel, MODE_BRUTE_SMEM,);
     return a.dz.esc ? SRP_LAUNCH3(bvh_trace_kernel, true,) : SRP_LAUNCH3(bvh_trace_kernel, false,);

@@ -295,5 +295,6 @@ int srp_small_blocks_per_sm() { return blocks_per_sm(small_beam_kernel<false, fa
 
 cudaError_t srp_launch_small(const TraceArgs &a, bool instrumented, int num_sms, cudaStream_t stream)
 {
+    const size_t dyn_smem = 0;
     return a.dz.esc ? SRP_LAUNCH3(small_beam_kernel, true,) : SRP_LAUNCH3(small_beam_kernel, false,);
 }
