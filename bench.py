@@ -58,10 +58,10 @@ def kernel_source_hash():
     return h.hexdigest()[:16]
 
 
-def measured_traffic(workload, segments):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the trace kernels from the committed `ncu --set full` capture of
-    this workload (profiles/r2_traffic.json: bytes per segment, the command, the source hash), scaled to this
-    launch's segments -- or None when there is no capture of THIS build."""
+def ncu_figures(workload):
+    """Figures of the trace kernels from the committed `ncu` captures of this workload (profiles/r2_traffic.json:
+    DRAM and L2 bytes per segment, FMA-pipe utilisation, issue slots, lanes, the commands, and a hash of csrc/) --
+    or (None, why) when there is no capture of THIS build of the kernels."""
     try:
         t = json.load(open(TRAFFIC_FILE))
     except (OSError, ValueError):
@@ -71,7 +71,7 @@ def measured_traffic(workload, segments):
         return None, "no ncu capture of this workload on file"
     if e.get("source_hash") != kernel_source_hash():
         return None, "the ncu capture on file (%s) is of another build of the kernels" % e.get("capture")
-    return e["dram_bytes_per_segment"] * segments, "%s: %s" % (e.get("capture"), e.get("command"))
+    return e, "%s: %s" % (e.get("capture"), e.get("command"))
 
 
 def parse():
@@ -339,13 +339,25 @@ def run_ours(args, rank, world, local_rank):
     else:
         kernel = "small_beam_kernel" if beams else "trace_kernel"
     frac_alu, frac_l2 = ach_tflops / FP32_PEAK_TFLOPS, l2_gbs / peaks["l2_read_gbs"]
-    traffic, traffic_source = measured_traffic(args.workload, st_k["segments"])
-    # the higher of the FP32 and the L2 fraction is the binding roofline
-    alu_binds = frac_alu >= frac_l2
+    # "ncu decides which bound applies: the higher of sm__inst_executed_pipe_fma utilisation and
+    # lts__t_bytes / probed L2 peak".  With a capture of this build on file that rule is applied to its figures (the L2
+    # bytes per segment scaled to this launch); without one, to the algorithmic fractions.
+    ncu, ncu_source = ncu_figures(args.workload)
+    traffic = ncu["dram_bytes_per_segment"] * st_k["segments"] if ncu else None
+    if ncu and ncu.get("lts_bytes_per_segment") is not None:
+        l2_measured = ncu["lts_bytes_per_segment"] * st_k["segments"] / t_kernel / 1e9
+        alu_binds = ncu["fma_pipe_pct"] / 100.0 >= l2_measured / peaks["l2_read_gbs"]
+    else:
+        l2_measured = None
+        alu_binds = frac_alu >= frac_l2
     roofline = {"bound": "alu" if alu_binds else "l2", "kernel": kernel,
                 "achieved": ach_tflops if alu_binds else l2_gbs, "peak": FP32_PEAK_TFLOPS if alu_binds else peaks["l2_read_gbs"],
-                "unit": "TFLOP/s" if alu_binds else "GB/s", "frac": max(frac_alu, frac_l2),
-                "traffic": traffic, "traffic_source": traffic_source,
+                "unit": "TFLOP/s" if alu_binds else "GB/s", "frac": frac_alu if alu_binds else frac_l2,
+                "traffic": traffic, "traffic_source": ncu_source,
+                "ncu": ({"fma_pipe_pct": ncu["fma_pipe_pct"], "alu_pipe_pct": ncu.get("alu_pipe_pct"), "issue_pct": ncu.get("issue_pct"),
+                         "lanes_of_32": ncu.get("lanes"), "l2_gbs_this_launch": l2_measured,
+                         "l2_frac_of_probed_peak": (l2_measured / peaks["l2_read_gbs"]) if l2_measured is not None else None}
+                        if ncu else None),
                 "alu": {"achieved_tflops": ach_tflops, "peak_tflops": FP32_PEAK_TFLOPS, "frac": frac_alu,
                         "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz; probed FMA chain %.1f TFLOP/s" % peaks["fp32_tflops"],
                         "flop_per_segment": flop_ps},
