@@ -325,6 +325,10 @@ def run_ours(args, rank, world, local_rank):
     # per-sample kernel reads its triangles from shared memory: one 48-byte fetch per triangle and record)
     if per_sample:
         bytes_ps = BYTES_TRI * W.TRI_COUNT[cfg.family] * n_forces / max(st_k["segments"], 1)
+    elif W.TRI_COUNT[cfg.family] <= 64:
+        # designs without a hierarchy: a warp stages its design's <= 64 triangles in shared memory once per design and
+        # tests from there -- 3 KB per (warp, design), nothing per segment
+        bytes_ps = 0.0
     else:
         bytes_ps = (BYTES_NODE * (per["box_tests"] + per["beam_box_tests"]) / 2.0 +
                     BYTES_TRI * (per["tri_tests"] + per["tri_setups"]))
@@ -350,9 +354,15 @@ def run_ours(args, rank, world, local_rank):
     else:
         l2_measured = None
         alu_binds = frac_alu >= frac_l2
+    # an L2-bound line quotes the MEASURED L2 bytes when a capture of this build is on file: the algorithmic count
+    # (roofline.l2: 64 B per node visit and lane) is what the lanes ask for, and lanes of a warp share node fetches
+    l2_quote = l2_measured if l2_measured is not None else l2_gbs
     roofline = {"bound": "alu" if alu_binds else "l2", "kernel": kernel,
-                "achieved": ach_tflops if alu_binds else l2_gbs, "peak": FP32_PEAK_TFLOPS if alu_binds else peaks["l2_read_gbs"],
-                "unit": "TFLOP/s" if alu_binds else "GB/s", "frac": frac_alu if alu_binds else frac_l2,
+                "achieved": ach_tflops if alu_binds else l2_quote, "peak": FP32_PEAK_TFLOPS if alu_binds else peaks["l2_read_gbs"],
+                "unit": "TFLOP/s" if alu_binds else "GB/s", "frac": frac_alu if alu_binds else l2_quote / peaks["l2_read_gbs"],
+                "frac_source": ("algorithmic flops of the counted tests" if alu_binds else
+                                ("lts__t_bytes of the ncu capture, per segment, x this launch's segments" if l2_measured is not None
+                                 else "algorithmic node + triangle bytes of the counted tests")),
                 "traffic": traffic, "traffic_source": ncu_source,
                 "ncu": ({"fma_pipe_pct": ncu["fma_pipe_pct"], "alu_pipe_pct": ncu.get("alu_pipe_pct"), "issue_pct": ncu.get("issue_pct"),
                          "lanes_of_32": ncu.get("lanes"), "l2_gbs_this_launch": l2_measured,

@@ -869,6 +869,74 @@ def test_per_sample_designs_match_oracle(ctx, oracle, family, M, N, B, sampler, 
         dz.free()
 
 
+def test_new_entry_points_reject_bad_arguments(ctx):
+    """SRP_ERR_INVALID / SRP_ERR_UNSUPPORTED before any launch: per-sample records, split, workspace."""
+    import ctypes
+    import torch
+    from paper_2602_10712_b200.binding import SrpError
+    L, h = ctx.lib, ctx.handle
+    th = cuda(W.draw_params(W.FAMILY_BOXWING_T, 4))
+    sun = cuda(W.random_directions(4))
+    out = torch.empty((4, 3), dtype=torch.float32, device="cuda")
+    ok = lambda *a: L.srp_forces_per_sample(h, *a)
+    assert ok(W.FAMILY_BOXWING_T, th.data_ptr(), 2, sun.data_ptr(), 4, 1 << 10, 4, 0, 2, out.data_ptr()) == 0
+    assert ok(W.FAMILY_BOXWING_T, th.data_ptr(), 3, sun.data_ptr(), 4, 1 << 10, 4, 0, 2, out.data_ptr()) == -1     # n_params
+    assert ok(W.FAMILY_BOXWING_T, th.data_ptr(), 2, sun.data_ptr(), 0, 1 << 10, 4, 0, 2, out.data_ptr()) == -1     # M
+    assert ok(W.FAMILY_BOXWING_T, th.data_ptr(), 2, sun.data_ptr(), 4, 1000, 4, 0, 2, out.data_ptr()) == -1        # stratified: 2^m
+    assert ok(W.FAMILY_BOXWING_T, th.data_ptr(), 2, sun.data_ptr(), 4, 1 << 10, 16, 0, 2, out.data_ptr()) == -1    # B
+    assert ok(W.FAMILY_BOXWING_T, None, 2, sun.data_ptr(), 4, 1 << 10, 4, 0, 2, out.data_ptr()) == -1              # null
+    assert ok(W.FAMILY_DETAILED, th.data_ptr(), 2, sun.data_ptr(), 4, 1 << 10, 4, 0, 2, out.data_ptr()) == -4      # 49 840 triangles
+    assert ok(9, th.data_ptr(), 2, sun.data_ptr(), 4, 1 << 10, 4, 0, 2, out.data_ptr()) == -1                      # family
+    torch.cuda.synchronize()
+    dz = ctx.srp_build_designs(W.FAMILY_BOXWING, W.draw_params(W.FAMILY_BOXWING, 2))
+    assert L.srp_forces_split(h, dz.handle, sun.data_ptr(), 4, 1 << 10, 2, 0, out.data_ptr(), None) == -1
+    assert L.srp_forces_split_pairs(h, dz.handle, sun.data_ptr(), 4, None, 2, 1 << 10, 2, 0, out.data_ptr(), out.data_ptr()) == -1
+    buf = torch.empty(ctx.srp_workspace_bytes_min() + 4096, dtype=torch.uint8, device="cuda")
+    assert L.srp_set_workspace(h, ctypes.c_void_p(buf.data_ptr() + 8), buf.numel() - 8) == -1                     # alignment
+    assert L.srp_set_workspace(h, None, 4096) == -1 and L.srp_set_workspace(h, ctypes.c_void_p(buf.data_ptr()), 0) == -1
+    assert L.srp_set_workspace(h, None, 0) == 0
+    assert L.srp_launch_count(h, None) == -1
+    with pytest.raises(ValueError):
+        ctx.srp_forces_pairs(dz, sun, np.array([[0, 0], [2, 1]], np.int32), 1 << 10, 2)                           # design 2 of 2
+    with pytest.raises(ValueError):
+        ctx.srp_forces(dz, sun.cpu(), 1 << 10, 2)                                                                  # a CPU tensor is no device pointer
+    with pytest.raises(ValueError):
+        ctx.srp_build_designs_from_meshes(W.icosphere(0), np.full((20, 3), 0.5, np.float32), [0, 20])              # materials sum to 1.5
+    # a pair list the binding did not see: out-of-range entries are clamped on the device, nothing is read out of bounds
+    bad = torch.tensor([[7, 9], [-3, 0]], dtype=torch.int32, device="cuda")
+    assert L.srp_forces_pairs(h, dz.handle, sun.data_ptr(), 4, bad.data_ptr(), 2, 1 << 10, 2, 0, out.data_ptr()) == 0
+    torch.cuda.synchronize()
+    assert torch.isfinite(out[:2]).all()
+    # a zero sun direction gives a zero force, not NaN
+    z = cuda(np.array([[0, 0, 0], [0, 0, 1]], np.float32))
+    F = ctx.srp_forces(dz, z, 1 << 10, 2).cpu().numpy()
+    assert np.all(F[:, 0] == 0.0) and np.all(np.isfinite(F)) and np.linalg.norm(F[0, 1]) > 0
+    dz.free()
+
+
+def test_large_accumulations_do_not_wrap(ctx):
+    """The fixed-point scale is chosen per call (R21): a mirror plate deposits 2 per photon, which wrapped the 2^-32
+    accumulators at N = 2^30 photons per direction.  And torque arms are summed in units of the design's extent, so a
+    mesh given in millimetres gives 1e6 times the force and 1e9 times the torque of the same mesh in metres (area x arm)
+    instead of wrapping (arms of ~1e3 mesh units times 2^20 photons used to exceed the accumulators' range)."""
+    plate = quad([-0.5, -0.5, 0.0], [1, 0, 0], [0, 1, 0])
+    dz = ctx.srp_build_designs_from_meshes(plate, const_mats(2, 0.0, 1.0, 0.0), [0, 2])
+    sun = cuda(np.array([[0, 0, 1]], np.float32))
+    F = ctx.srp_forces(dz, sun, 1 << 30, 1, 0).cpu().numpy()[0, 0]
+    np.testing.assert_allclose(F, [0, 0, -2 * P0], rtol=1e-5, atol=1e-12)
+    dz.free()
+    # the same off-centre plate in metres and in millimetres: torque scales with length^3 (area x arm)
+    res = []
+    for s in (1.0, 1000.0):
+        v = quad([1.5 * s, -1.75 * s, 0.5 * s], [1.0 * s, 0, 0], [0, 1.5 * s, 0.3 * s])
+        d = ctx.srp_build_designs_from_meshes(v, const_mats(2, 0.3, 0.5, 0.2), [0, 2])
+        Fm, Tm = ctx.srp_forces_torques(d, cuda(np.array([[0.3, 0.2, 0.8]], np.float32)), 1 << 20, 1, seed=3)
+        res.append((Fm.cpu().numpy()[0, 0], Tm.cpu().numpy()[0, 0]))
+        d.free()
+    assert np.allclose(res[1][0], res[0][0] * 1e6, rtol=2e-4)
+    assert np.allclose(res[1][1], res[0][1] * 1e9, rtol=2e-4)
+
+
 def test_force_maps_direct_and_indirect(ctx):
     """PAPER.md:394 force maps from srp_forces_split.  A convex body has no indirect light (its map is the closed
     form of P3, direct = total exactly); the box-wing has some."""
