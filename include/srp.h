@@ -83,8 +83,12 @@ typedef struct {
                                conditional WHILE node of a CUDA graph; 1 = the same kernels as plain launches, a fixed
                                sufficient number of rounds (surplus rounds find nothing to do) -- for profilers that do
                                not list kernels inside conditional graph nodes.  Results are identical.            */
-    int leaf_max;           /* LBVH: subtrees with at most this many triangles become one leaf, 1..8; 0 = default (2).
+    int leaf_max;           /* subtrees with at most this many triangles become one leaf, 1..8; 0 = default (2).
                                Read by srp_build_designs*; test and tuning use                                       */
+    int bvh_builder;        /* the hierarchy of designs with more than 64 triangles: 0 (default) = top-down binned
+                               surface-area heuristic over the Morton order (bvh_sah.cu), 1 = linear BVH (Karras
+                               hierarchy of the Morton codes, lbvh.cu; the structure of PAPER.md:366).  Same node
+                               layout, same results up to the order of summation.  Read by srp_build_designs*      */
 } srp_options;
 
 /* Photon bookkeeping of the last srp_forces call (DESIGN.md "Pins" P8).

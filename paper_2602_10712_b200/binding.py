@@ -28,7 +28,8 @@ class SrpError(RuntimeError):
 class srp_options(ctypes.Structure):
     _fields_ = [("solar_pressure", ctypes.c_double), ("sampler", ctypes.c_int), ("deposit", ctypes.c_int),
                 ("force_brute", ctypes.c_int), ("instrumented", ctypes.c_int), ("primary_mode", ctypes.c_int), ("escape_masks", ctypes.c_int),
-                ("plain_launches", ctypes.c_int), ("leaf_max", ctypes.c_int)]
+                ("plain_launches", ctypes.c_int), ("leaf_max", ctypes.c_int),
+                ("bvh_builder", ctypes.c_int)]
 
 
 class srp_stats(ctypes.Structure):
@@ -193,9 +194,9 @@ class Context:
             self.handle = None
 
     def srp_set_options(self, solar_pressure=W.SOLAR_PRESSURE, sampler=0, deposit=0, force_brute=0, instrumented=0,
-                        primary_mode=0, escape_masks=1, plain_launches=0, leaf_max=0):
+                        primary_mode=0, escape_masks=1, plain_launches=0, leaf_max=0, bvh_builder=0):
         o = srp_options(solar_pressure, sampler, deposit, force_brute, instrumented, primary_mode, escape_masks,
-                        plain_launches, leaf_max)
+                        plain_launches, leaf_max, bvh_builder)
         self._check(self.lib.srp_set_options(self.handle, ctypes.byref(o)))
 
     def srp_build_designs(self, family, theta, mesh_seed=W.MESH_SEED):

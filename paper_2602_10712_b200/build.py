@@ -26,6 +26,7 @@ SOURCES = {
     "srp_api.cu": [],
     "mesh_gen.cu": ["--fmad=false"],
     "lbvh.cu": [],
+    "bvh_sah.cu": [],
     "escape_mask.cu": [],
     "trace.cu": [],
     "trace_perray.cu": [],

@@ -301,7 +301,7 @@ node_plane_kernel(const DesignsDev dz, long long sumT, float4 *nplane)
 
 // Builds box / tri / perm (and nodes when the batch has a design above the brute-force limit) from
 // verts_orig / mats_orig.  All device arrays of `dz` are already allocated.
-cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, cudaStream_t stream)
+cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, int builder, cudaMemPool_t pool, cudaStream_t stream, int *launches)
 {
     const long long sumT = dz->sumT;
     const int D = dz->D;
@@ -310,6 +310,7 @@ cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, 
     if (!dz->has_bvh) {
         pack_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->mats_orig, dz->tri_off_dev, D, sumT,
                                                 nullptr, dz->tri, dz->perm);
+        *launches = 2;
         return cudaGetLastError();
     }
     // scratch of the build, from the context's pool; freed (stream-ordered) whether or not the build succeeds
@@ -324,9 +325,11 @@ cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, 
         CK(cudaMallocFromPoolAsync((void **)&keys_out, sizeof(u64) * sumT, pool, stream));
         CK(cudaMallocFromPoolAsync((void **)&vals, sizeof(unsigned) * sumT, pool, stream));
         CK(cudaMallocFromPoolAsync((void **)&vals_out, sizeof(unsigned) * sumT, pool, stream));
-        CK(cudaMallocFromPoolAsync((void **)&ibuf, sizeof(int) * 7 * sumT, pool, stream));
-        CK(cudaMallocFromPoolAsync((void **)&lbox, sizeof(float4) * 2 * sumT, pool, stream));
-        CK(cudaMallocFromPoolAsync((void **)&nbox, sizeof(float4) * 2 * sumT, pool, stream));
+        if (builder == 1) {
+            CK(cudaMallocFromPoolAsync((void **)&ibuf, sizeof(int) * 7 * sumT, pool, stream));
+            CK(cudaMallocFromPoolAsync((void **)&lbox, sizeof(float4) * 2 * sumT, pool, stream));
+            CK(cudaMallocFromPoolAsync((void **)&nbox, sizeof(float4) * 2 * sumT, pool, stream));
+        }
         int end_bit = 48;
         while ((1LL << (end_bit - 48)) < D) ++end_bit;
         CK(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys_out, vals, vals_out, (int)sumT, 0,
@@ -335,8 +338,18 @@ cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, 
         morton_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->tri_off_dev, D, sumT, dz->box, keys, vals);
         CK(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys_out, vals, vals_out, (int)sumT, 0,
                                            end_bit, stream));
+        *launches = 2 + 4;                     // box, codes; the sort: histogram, exclusive sum, 2 onesweep passes or more
+        if (builder != 1) {                    // binned SAH over the Morton order (bvh_sah.cu); `vals` is free again
+            int n = 0;
+            CK(srp_launch_sah_build(dz, vals_out, vals, leaf_max, pool, stream, &n));
+            pack_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->mats_orig, dz->tri_off_dev, D, sumT,
+                                                    vals, dz->tri, dz->perm);
+            *launches += n + 1;
+            return cudaGetLastError();
+        }
         pack_kernel<<<blocks, 256, 0, stream>>>(dz->verts_orig, dz->mats_orig, dz->tri_off_dev, D, sumT,
                                                 vals_out, dz->tri, dz->perm);
+        *launches += 5;
         int *left = ibuf, *right = ibuf + sumT, *pnode = ibuf + 2 * sumT, *pleaf = ibuf + 3 * sumT,
             *rfirst = ibuf + 4 * sumT, *rcount = ibuf + 5 * sumT, *flags = ibuf + 6 * sumT;
         CK(cudaMemsetAsync(flags, 0, sizeof(int) * sumT, stream));

@@ -379,7 +379,7 @@ srp_status srp_create(srp_context **out, int cuda_device, void *cuda_stream)
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt.solar_pressure = 4.56e-6; ctx->opt.sampler = 0; ctx->opt.deposit = 0;
     ctx->opt.force_brute = 0; ctx->opt.instrumented = 0; ctx->opt.primary_mode = 0; ctx->opt.escape_masks = 1;
-    ctx->opt.plain_launches = 0; ctx->opt.leaf_max = 0;
+    ctx->opt.plain_launches = 0; ctx->opt.leaf_max = 0; ctx->opt.bvh_builder = 0;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) ctx->num_sms = prop.multiProcessorCount;
     {   // a pool of the context's own that keeps freed blocks: builds reuse them instead of going back to the driver
@@ -418,7 +418,8 @@ srp_status srp_set_options(srp_context *ctx, const srp_options *opt)
     if (!opt) return fail(ctx, SRP_ERR_INVALID, "null options");
     if (!(opt->solar_pressure > 0.0) || opt->sampler < 0 || opt->sampler > 1 || opt->deposit < 0 || opt->deposit > 1 ||
         opt->primary_mode < 0 || opt->primary_mode > 2 || opt->escape_masks < 0 || opt->escape_masks > 2 ||
-        opt->plain_launches < 0 || opt->plain_launches > 1 || opt->leaf_max < 0 || opt->leaf_max > 8)
+        opt->plain_launches < 0 || opt->plain_launches > 1 || opt->leaf_max < 0 || opt->leaf_max > 8 ||
+        opt->bvh_builder < 0 || opt->bvh_builder > 1)
         return fail(ctx, SRP_ERR_INVALID, "option out of range");
     ctx->opt = *opt;
     return SRP_OK;
@@ -467,9 +468,10 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
     if (st != SRP_OK) { free_designs_mem(ctx, d); delete d; return st; }
     cudaError_t e = srp_launch_mesh_gen((int)family, theta, D, n_params, mesh_seed, T, d->verts_orig,
                                         d->mats_orig, ctx->mempool, 0u, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->mempool, ctx->stream);
+    int build_launches = 0;
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->opt.bvh_builder, ctx->mempool, ctx->stream, &build_launches);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
-    ctx->launches_total += 2 + SRP_BUILD_KERNELS(d->has_bvh);          // mesh generation: 2 kernels
+    ctx->launches_total += 2 + build_launches;                         // mesh generation: 2 kernels
     *out = d;
     return SRP_OK;
 }
@@ -502,9 +504,10 @@ srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, c
     cudaError_t e = cudaMemcpyAsync(d->verts_orig, verts, sizeof(float) * 9 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(d->mats_orig, mats, sizeof(float) * 3 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
-    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->mempool, ctx->stream);
+    int build_launches = 0;
+    if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->opt.bvh_builder, ctx->mempool, ctx->stream, &build_launches);
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
-    ctx->launches_total += SRP_BUILD_KERNELS(d->has_bvh);
+    ctx->launches_total += build_launches;
     *out = d;
     return SRP_OK;
 }
@@ -740,7 +743,8 @@ srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const floa
         d.D = Dc; d.sumT = (long long)Dc * T;
         e = srp_launch_mesh_gen((int)family, theta + (size_t)m0 * n_params, Dc, n_params, mesh_seed, T, d.verts_orig,
                                 d.mats_orig, ctx->mempool, (unsigned)m0, ctx->stream);
-        if (e == cudaSuccess) e = srp_launch_build(&d, 0, ctx->mempool, ctx->stream);
+        int build_launches = 0;
+        if (e == cudaSuccess) e = srp_launch_build(&d, 0, 0, ctx->mempool, ctx->stream, &build_launches);
         if (e != cudaSuccess) break;
         TraceArgs a;
         memset(&a, 0, sizeof a);
@@ -751,7 +755,7 @@ srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const floa
         a.sampler = ctx->opt.sampler; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
         a.stats = ctx->stats; a.max_tris = T; a.acc_scale = 1.0;
         e = srp_launch_sample(a, out + 3 * m0, (unsigned)m0, ctx->num_sms, ctx->stream);
-        count_launches(ctx, 2 + SRP_BUILD_KERNELS(false) + 1);
+        count_launches(ctx, 2 + build_launches + 1);
     }
     free_designs_mem(ctx, &d);                                      // stream-ordered: after the last chunk's kernels
     if (st != SRP_OK) return st;

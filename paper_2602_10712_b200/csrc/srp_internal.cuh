@@ -10,7 +10,7 @@
 
 #define SRP_PIPES 2                // beam / bounce loops that run side by side, each on its share of the tiles
 #define SRP_BRUTE_MAX_TRIS 64      // designs with T <= this are traced without a hierarchy (one leaf)
-#define SRP_LEAF_MAX 2             // LBVH subtrees with <= this many triangles become one leaf (cfg3 -7 %, cfg5 -3 % against 3)
+#define SRP_LEAF_MAX 2             // subtrees with <= this many triangles become one leaf (cfg3 -7 %, cfg5 -3 % against 3)
 #define SRP_ACC_BITS_MAX 32        // fixed-point fraction bits of the dimensionless force accumulators, at most
 
 // Packed, BVH-sorted triangle: 3 x float4 = 48 B, fetched as three 16-byte loads.
@@ -131,8 +131,10 @@ struct TraceArgs {
 cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_params,
                                 unsigned long long mesh_seed, long long T, float *verts, float *mats,
                                 cudaMemPool_t pool, unsigned k_offset, cudaStream_t stream);
-cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, cudaMemPool_t pool, cudaStream_t stream);   // 2 kernels without a BVH, 6 with
-#define SRP_BUILD_KERNELS(has_bvh) ((has_bvh) ? 6 : 2)
+// builder: srp_options.bvh_builder; *launches = kernels enqueued
+cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, int builder, cudaMemPool_t pool, cudaStream_t stream, int *launches);
+cudaError_t srp_launch_sah_build(srp_designs *dz, const unsigned *vals, unsigned *vals_final, int leaf_max,
+                                 cudaMemPool_t pool, cudaStream_t stream, int *launches);
 cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted, cudaStream_t stream);
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream);
 cudaError_t srp_launch_escape_masks_small(const DesignsDev &dz, long long sumT, unsigned *esc, cudaStream_t stream);

@@ -78,7 +78,8 @@ __device__ inline Emitter make_emitter(const float *sun_dirs, int j, float4 lo, 
     Emitter e;
     const float wx = sun_dirs[3 * j], wy = sun_dirs[3 * j + 1], wz = sun_dirs[3 * j + 2];
     const float len = sqrtf(wx * wx + wy * wy + wz * wz);
-    e.s = f3(-wx / len, -wy / len, -wz / len);
+    const bool usable = len > 0.f && len <= FLT_MAX;      // a zero or non-finite direction: A_e = 0, F = 0 (srp.h)
+    e.s = usable ? f3(-wx / len, -wy / len, -wz / len) : f3(0.f, 0.f, -1.f);
     basis3(e.s, e.u, e.v);
     float u0 = FLT_MAX, u1 = -FLT_MAX, v0 = FLT_MAX, v1 = -FLT_MAX, w0 = FLT_MAX;
 #pragma unroll
@@ -91,7 +92,7 @@ __device__ inline Emitter make_emitter(const float *sun_dirs, int j, float4 lo, 
     }
     e.u0 = u0; e.v0 = v0; e.du = u1 - u0; e.dv = v1 - v0;
     e.worg = w0 - 1.0f;
-    e.Ae = e.du * e.dv;
+    e.Ae = usable ? e.du * e.dv : 0.f;
     return e;
 }
 

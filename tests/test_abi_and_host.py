@@ -36,8 +36,8 @@ def test_library_exports_every_declared_symbol(libpath):
 def test_struct_layouts_match_header():
     from paper_2602_10712_b200 import binding
     assert ctypes.sizeof(binding.srp_stats) == 8 * (6 + 16 + 2 + 4 + 4 + 1 + 3)
-    assert ctypes.sizeof(binding.srp_options) == 40
-    assert binding.srp_options.leaf_max.offset == 36
+    assert ctypes.sizeof(binding.srp_options) == 48
+    assert binding.srp_options.leaf_max.offset == 36 and binding.srp_options.bvh_builder.offset == 40
     assert binding.srp_options.primary_mode.offset == 24
     assert binding.srp_options.sampler.offset == 8
 
