@@ -6,9 +6,9 @@
 // the Morton order and every level partitions each range in place (stably), so the final order is a depth-first order
 // of the leaves and every node's triangles stay contiguous -- the layout lbvh.cu emits and every trace kernel reads.
 // One level =
-//   bin      every triangle of an open node adds its box to 3 axes x 8 bins of its node (integer atomics on
+//   bin      every triangle of an open node adds its box to 3 axes x 16 bins of its node (integer atomics on
 //            order-preserving codes of the floats: the result does not depend on the order of arrival)
-//   split    one warp per open node: 21 candidate planes, cost = area(L) n(L) + area(R) n(R); the node takes its
+//   split    one warp per open node: 45 candidate planes, cost = area(L) n(L) + area(R) n(R); the node takes its
 //            number (head + n(L) - 1: the position it splits after, unique like Karras's), links itself to its parent,
 //            opens its children or writes them as leaves (<= leaf_max triangles)
 //   flag / scan / scatter   stable partition by an exclusive sum over "goes right"
@@ -22,7 +22,10 @@
 
 namespace {
 
-constexpr int NB = 8;                   // bins per axis
+#ifndef SAH_BINS_DEF
+#define SAH_BINS_DEF 16
+#endif
+constexpr int NB = SAH_BINS_DEF;        // bins per axis
 constexpr int BIN_WORDS = 3 * NB * 7;   // per open node: [axis][bin]{lo.xyz, hi.xyz as codes, count}
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -212,13 +215,13 @@ sah_split_kernel(Sah s, int cur, int by_position)
         const int h = (int)(g - lane) + (__ffs(m) - 1);
         const int count = s.count[cur][h];
         const unsigned *b = s.bins + slot_of(s, h) * BIN_WORDS;
-        float cost = FLT_MAX;
-        int nl = 0;
-        if (lane < 3 * (NB - 1) && !by_position) {
-            const int a = lane / (NB - 1), sp = lane % (NB - 1);       // left = bins 0..sp of axis a
+        float best = FLT_MAX;                        // this lane's cheapest candidate plane, then the warp's
+        int who = 3 * (NB - 1), nl_best = 0;
+        for (int cand = lane; cand < 3 * (NB - 1) && !by_position; cand += 32) {
+            const int a = cand / (NB - 1), sp = cand % (NB - 1);       // left = bins 0..sp of axis a
             float llo[3] = { FLT_MAX, FLT_MAX, FLT_MAX }, lhi[3] = { -FLT_MAX, -FLT_MAX, -FLT_MAX };
             float rlo[3] = { FLT_MAX, FLT_MAX, FLT_MAX }, rhi[3] = { -FLT_MAX, -FLT_MAX, -FLT_MAX };
-            int nr = 0;
+            int nl = 0, nr = 0;
             for (int i = 0; i < NB; ++i) {
                 const unsigned *w = b + (a * NB + i) * 7;
                 const int n = (int)w[6];
@@ -233,17 +236,20 @@ sah_split_kernel(Sah s, int cur, int by_position)
                     for (int c = 0; c < 3; ++c) { rlo[c] = fminf(rlo[c], o2f(w[c])); rhi[c] = fmaxf(rhi[c], o2f(w[3 + c])); }
                 }
             }
-            if (nl > 0 && nr > 0) cost = half_area(llo, lhi) * (float)nl + half_area(rlo, rhi) * (float)nr;
+            if (nl > 0 && nr > 0) {
+                const float cost = half_area(llo, lhi) * (float)nl + half_area(rlo, rhi) * (float)nr;
+                if (cost < best) { best = cost; who = cand; nl_best = nl; }
+            }
         }
-        // the cheapest candidate, the lowest lane among equals
-        float best = cost; int who = lane;
+        // the cheapest candidate of the warp, the lowest-numbered among equals
         for (int o = 16; o > 0; o >>= 1) {
             const float oc = __shfl_xor_sync(FULL, best, o);
             const int ow = __shfl_xor_sync(FULL, who, o);
-            if (oc < best || (oc == best && ow < who)) { best = oc; who = ow; }
+            const int on = __shfl_xor_sync(FULL, nl_best, o);
+            if (oc < best || (oc == best && ow < who)) { best = oc; who = ow; nl_best = on; }
         }
         const bool positional = !(best < FLT_MAX);
-        const int n_left = positional ? count / 2 : __shfl_sync(FULL, nl, who);
+        const int n_left = positional ? count / 2 : nl_best;
         __syncwarp();
         if (lane == 0) {
             const int k = find_design(s.off, s.D, h);
@@ -254,7 +260,7 @@ sah_split_kernel(Sah s, int cur, int by_position)
             if (par < 0) { id = 0; s.rootnat[k] = nat; }
             else id = nat == 0 ? s.rootnat[k] : nat;
             const long long gid = (long long)base + id;
-            s.dec[h] = make_int4(who / (NB - 1), who % (NB - 1), n_left, positional ? 1 : 0);
+            s.dec[h] = make_int4(positional ? 0 : who / (NB - 1), positional ? 0 : who % (NB - 1), n_left, positional ? 1 : 0);
             s.parent_of[gid] = par;
             int *rec = (int *)(s.nodes + 4 * gid + 3);
             rec[2] = h - base; rec[3] = count;

@@ -15,8 +15,9 @@ namespace {
 #define BOUNCE_STACK_DEF 12
 #endif
 constexpr int BOUNCE_STACK = BOUNCE_STACK_DEF;   // per-thread stack entries in shared memory; deeper ones in local memory
-constexpr int HITQ = 64;                 // queued hits per warp (shaded 32 at a time, converged)
-constexpr int LQ = 64;                   // photons that go on after such a hit, waiting for a free lane
+constexpr int HITQ = 64;                 // queued hits per warp (shaded 32 at a time, converged) and photons that go on after
+                                         // such a hit, waiting for a free lane, in one array: hits from the front, photons
+                                         // from the back (a warp holds <= 63 photons in lanes and queues together)
 #ifndef BOUNCE_BATCH_DEF
 #define BOUNCE_BATCH_DEF 256
 #endif
@@ -29,9 +30,10 @@ constexpr int DRAIN_ACTIVE_MIN = DRAIN_ACTIVE_MIN_DEF;   // leave the traversal 
 template <bool INSTR>
 struct BounceSmem {                 // per warp
     int stack[BOUNCE_STACK * 32];   // per-thread traversal stacks, thread-interleaved
-    uint32_t hq[11][HITQ];          // queued hits: o, d, i, p, sd, triangle, t
-    uint32_t lq[9][LQ];             // photons that go on: o, d, i, p, sd
-    unsigned long long hsig[INSTR ? HITQ : 1], lsig[INSTR ? LQ : 1];
+    uint32_t hq[11][HITQ];          // queued hits [0, nhit): o, d, i, p, sd, triangle, t; photons that go on
+                                    // [HITQ - nlq, HITQ), last one first: o, d, i, p, sd.  Less shared memory = more L1
+                                    // for the nodes: 8 blocks leave 92 KB instead of 28 KB
+    unsigned long long hsig[INSTR ? HITQ : 1];
 };
 
 template <bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
@@ -98,13 +100,14 @@ bounce_trace_kernel(const TraceArgs a)
         }
         nhit -= take;
         const unsigned mc = __ballot_sync(FULL, fate == SHADE_CONTINUE);
-        SRP_CHECK(nlq + __popc(mc) <= LQ, "photon queue");
+        SRP_CHECK(nhit + nlq + __popc(mc) <= HITQ, "photon queue");
+        __syncwarp();                                                // the hits of this batch have been read: their slots are free
         if (fate == SHADE_CONTINUE) {
-            const int e = nlq + __popc(mc & lt_mask);
-            W.lq[0][e] = __float_as_uint(o.x); W.lq[1][e] = __float_as_uint(o.y); W.lq[2][e] = __float_as_uint(o.z);
-            W.lq[3][e] = __float_as_uint(d.x); W.lq[4][e] = __float_as_uint(d.y); W.lq[5][e] = __float_as_uint(d.z);
-            W.lq[6][e] = i; W.lq[7][e] = p; W.lq[8][e] = ((uint32_t)depth << 27) | (uint32_t)src;
-            if (INSTR) W.lsig[e] = sig;
+            const int e = HITQ - 1 - (nlq + __popc(mc & lt_mask));
+            W.hq[0][e] = __float_as_uint(o.x); W.hq[1][e] = __float_as_uint(o.y); W.hq[2][e] = __float_as_uint(o.z);
+            W.hq[3][e] = __float_as_uint(d.x); W.hq[4][e] = __float_as_uint(d.y); W.hq[5][e] = __float_as_uint(d.z);
+            W.hq[6][e] = i; W.hq[7][e] = p; W.hq[8][e] = ((uint32_t)depth << 27) | (uint32_t)src;
+            if (INSTR) W.hsig[e] = sig;
         }
         nlq += __popc(mc);
         __syncwarp();
@@ -142,11 +145,11 @@ bounce_trace_kernel(const TraceArgs a)
             const int nidle = __popc(idle), take = nidle < nlq ? nidle : nlq;
             const int rank = __popc(idle & lt_mask);
             if (!has && rank < take) {
-                const int e = nlq - take + rank;
-                o = f3(__uint_as_float(W.lq[0][e]), __uint_as_float(W.lq[1][e]), __uint_as_float(W.lq[2][e]));
-                d = f3(__uint_as_float(W.lq[3][e]), __uint_as_float(W.lq[4][e]), __uint_as_float(W.lq[5][e]));
-                ri = W.lq[6][e]; rp = W.lq[7][e]; rsd = W.lq[8][e];
-                if (INSTR) rsig = W.lsig[e];
+                const int e = HITQ - 1 - (nlq - take + rank);
+                o = f3(__uint_as_float(W.hq[0][e]), __uint_as_float(W.hq[1][e]), __uint_as_float(W.hq[2][e]));
+                d = f3(__uint_as_float(W.hq[3][e]), __uint_as_float(W.hq[4][e]), __uint_as_float(W.hq[5][e]));
+                ri = W.hq[6][e]; rp = W.hq[7][e]; rsd = W.hq[8][e];
+                if (INSTR) rsig = W.hsig[e];
                 start_ray();
             }
             nlq -= take;
@@ -197,7 +200,7 @@ bounce_trace_kernel(const TraceArgs a)
             if (INSTR && a.sig_out) a.sig_out[(long long)rp * a.N + ri] = rsig;
         }
         const unsigned mh = __ballot_sync(FULL, hit);
-        SRP_CHECK(nhit + __popc(mh) <= HITQ, "hit queue");
+        SRP_CHECK(nhit + nlq + __popc(mh) <= HITQ, "hit queue");
         if (hit) {
             const int e = nhit + __popc(mh & lt_mask);
             W.hq[0][e] = __float_as_uint(o.x); W.hq[1][e] = __float_as_uint(o.y); W.hq[2][e] = __float_as_uint(o.z);
@@ -209,8 +212,8 @@ bounce_trace_kernel(const TraceArgs a)
         nhit += __popc(mh);
         if (fin) has = false;
         __syncwarp();
-        // A warp holds at most 63 photons (new ones enter only into free lanes, with lq empty and < 32 hits queued),
-        // so neither queue can overflow.
+        // A warp holds at most 63 photons (new ones enter only into free lanes, with no photon waiting and < 32 hits
+        // queued), so the two ends of the queue cannot meet.
         if (nhit >= 32) shade_batch();
     }
     if (INSTR) cn.n_tri += nt;
@@ -246,6 +249,8 @@ cudaError_t launch_bounce(K kernel, const TraceArgs &a, int num_sms, cudaStream_
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
+    e = prefer_l1(kernel, per_sm, 0);
+    if (e != cudaSuccess) return e;
     kernel<<<(unsigned)(num_sms * per_sm), TRACE_THREADS, 0, stream>>>(a);
     return cudaGetLastError();
 }

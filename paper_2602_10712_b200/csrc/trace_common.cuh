@@ -582,6 +582,24 @@ __device__ __forceinline__ void beam_setup(const float4 q0, const float4 q1, con
 }
 
 
+// Shared-memory carve-out: no more than the resident blocks of the kernel use; the rest of the SM's 256 KB is L1
+// for nodes and triangles (bounce kernel: 92 KB instead of 28 KB, cfg3 -3.7 %).
+#ifndef SRP_NO_CARVE
+template <typename K>
+cudaError_t prefer_l1(K kernel, int per_sm, size_t dyn_smem)
+{
+    cudaFuncAttributes fa;
+    const cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
+    if (e != cudaSuccess) return e;
+    const size_t need = (size_t)per_sm * (fa.sharedSizeBytes + dyn_smem + 1024);
+    int pct = (int)((need * 100 + 228 * 1024 - 1) / (228 * 1024));
+    if (pct > 100) pct = 100;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct);
+}
+#else
+template <typename K> cudaError_t prefer_l1(K, int, size_t) { return cudaSuccess; }
+#endif
+
 // Launches a persistent trace kernel: as many blocks as fit the machine once, or fewer if there is less work.
 template <typename K>
 cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStream_t stream, size_t dyn_smem = 0)
@@ -593,6 +611,8 @@ cudaError_t launch_persistent(K kernel, const TraceArgs &a, int num_sms, cudaStr
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TRACE_THREADS, dyn_smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
+    e = prefer_l1(kernel, per_sm, dyn_smem);
+    if (e != cudaSuccess) return e;
     const unsigned long long total_tiles = a.tile_end - a.tile_begin;
     unsigned long long blocks = (unsigned long long)num_sms * per_sm;       // persistent: fill the machine once
     const unsigned long long needed = (total_tiles + TRACE_WARPS - 1) / TRACE_WARPS;
