@@ -46,6 +46,7 @@ constexpr int BEAM_EL = 96;         // tile entry list: leaf links (<= 32 when a
 struct BeamFrame {                  // warp-uniform per pair
     float3 uh, vh, auh, avh;        // u/2, v/2 and their absolute values
     float csu, csv;                 // cell size along u and v
+    float icsu, icsv;               // and their reciprocals
     float margin;                   // bound of the fp32 projection error of a box
 };
 
@@ -115,11 +116,15 @@ __device__ __forceinline__ bool beam_push_tris(int *cid, int &ncand, int first0,
 struct BeamSmem {                   // per warp
     float4 eq[3 * BEAM_CMAX];       // (A0,B0,C0,Wu) (A1,B1,C1,Wv) (A2,B2,C2,Wc) per candidate
     int cid[BEAM_CMAX];             // candidate -> sorted triangle index
+    unsigned short cbox[BEAM_CMAX]; // the cells of the 16 x 16 sub-block its projection can touch, 4 bits each:
+                                    // x0 | x1 << 4 | y0 << 8 | y1 << 12 (x0 = 15, x1 = 0: none)
     int enode[BEAM_EN];
     int eleaf[BEAM_EL];
-    int nq[BEAM_QN];
-    unsigned char glist[BEAM_CMAX];
+    int nq[BEAM_QN];                // node queue of the sub-block descent; afterwards the groups' candidate lists
+                                    // (one byte per entry) live here
 };
+static_assert(BEAM_SB <= 256, "cbox holds 4-bit cell coordinates");
+static_assert(BEAM_QN * 4 >= BEAM_CMAX, "the group list lives in the node queue");
 
 template <bool INSTR, bool TORQUE, bool GLOSSY, bool ANALOG>
 __global__ void __launch_bounds__(TRACE_THREADS, BEAM_BLOCKS_PER_SM)
@@ -183,6 +188,7 @@ beam_trace_kernel(const TraceArgs a)
         bf.auh = f3(fabsf(bf.uh.x), fabsf(bf.uh.y), fabsf(bf.uh.z));
         bf.avh = f3(fabsf(bf.vh.x), fabsf(bf.vh.y), fabsf(bf.vh.z));
         bf.csu = em.du * inv_nx; bf.csv = em.dv * inv_ny;
+        bf.icsu = 1.0f / bf.csu; bf.icsv = 1.0f / bf.csv;
         {   // fp32 projections of points of this design are off by < 1e-6 of this scale; 10x that
             const float L = fmaxf(fabsf(blo.x), fabsf(bhi.x)) + fmaxf(fabsf(blo.y), fabsf(bhi.y)) +
                             fmaxf(fabsf(blo.z), fabsf(bhi.z));
@@ -283,8 +289,17 @@ beam_trace_kernel(const TraceArgs a)
                     for (int c = lane; c < ncand; c += 32) {
                         const int f = W.cid[c];
                         if (INSTR) bc.setups++;
+                        float4 bb;
                         beam_setup(__ldg(gtri + 3 * f), __ldg(gtri + 3 * f + 1), __ldg(gtri + 3 * f + 2), em, s_offu, s_offv,
-                                   W.eq + 3 * c);
+                                   W.eq + 3 * c, &bb);
+                        // cells of the sub-block (16 x 16) the triangle's bounding rectangle touches, widened by the
+                        // projection error bound: a ray outside them is outside the triangle
+                        const float x0 = floorf((bb.x - bf.margin) * bf.icsu), x1 = floorf((bb.y + bf.margin) * bf.icsu);
+                        const float y0 = floorf((bb.z - bf.margin) * bf.icsv), y1 = floorf((bb.w + bf.margin) * bf.icsv);
+                        const bool none = !(bb.x <= bb.y) || x1 < 0.f || y1 < 0.f || x0 > 15.f || y0 > 15.f;
+                        W.cbox[c] = none ? (unsigned short)0x000f
+                                         : (unsigned short)((unsigned)fmaxf(x0, 0.f) | ((unsigned)fminf(x1, 15.f) << 4) |
+                                                            ((unsigned)fmaxf(y0, 0.f) << 8) | ((unsigned)fminf(y1, 15.f) << 12));
                     }
                     __syncwarp();
                 }
@@ -294,13 +309,15 @@ beam_trace_kernel(const TraceArgs a)
             for (uint32_t gs = sb; gs < sb + nb; gs += 32) {
                 const uint32_t gcx = compact_even_bits(gs) - scx0, gcy = compact_even_bits(gs >> 1) - scy0;
                 int ng = 0;
+                unsigned char *glist = reinterpret_cast<unsigned char *>(W.nq);
                 if (!ovf) {
                     const float gu0 = (float)gcx * bf.csu, gu1 = (float)(gcx + g_wx) * bf.csu;
                     const float gv0 = (float)gcy * bf.csv, gv1 = (float)(gcy + g_wy) * bf.csv;
                     for (int base = 0; base < ncand; base += 32) {
                         const int c = base + lane;
                         bool keep = false;
-                        if (c < ncand) {
+                        const unsigned cb = c < ncand ? W.cbox[c] : 0x000fu;
+                        if ((cb & 15u) < gcx + g_wx && ((cb >> 4) & 15u) >= gcx && ((cb >> 8) & 15u) < gcy + g_wy && (cb >> 12) >= gcy) {
                             if (INSTR) bc.rect++;
                             const float4 E0 = W.eq[3 * c], E1 = W.eq[3 * c + 1], E2 = W.eq[3 * c + 2];
                             // largest value of each edge function over the rectangle (monotone in fp32 too)
@@ -311,7 +328,7 @@ beam_trace_kernel(const TraceArgs a)
                         }
                         const unsigned m = __ballot_sync(FULL, keep);
                         SRP_CHECK(ng + __popc(m) <= BEAM_CMAX, "group list");
-                        if (keep) W.glist[ng + __popc(m & lt_mask)] = (unsigned char)c;
+                        if (keep) glist[ng + __popc(m & lt_mask)] = (unsigned char)c;
                         ng += __popc(m);
                     }
                     __syncwarp();
@@ -350,7 +367,7 @@ beam_trace_kernel(const TraceArgs a)
                 float tbest = FLT_MAX;
                 int best = -1;
                 for (int e = 0; e < ng; ++e) {
-                    const int c = W.glist[e];
+                    const int c = glist[e];
                     const float4 E0 = W.eq[3 * c], E1 = W.eq[3 * c + 1], E2 = W.eq[3 * c + 2];
                     const float e0 = fmaf(E0.x, lu, fmaf(E0.y, lv, E0.z));
                     const float e1 = fmaf(E1.x, lu, fmaf(E1.y, lv, E1.z));

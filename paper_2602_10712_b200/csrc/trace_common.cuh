@@ -553,8 +553,10 @@ __device__ __forceinline__ void flush_beam_counters(const TraceArgs &a, const Be
 // Candidate set-up: triangle -> sign-normalised edge functions E_i(x) = A_i x_u + B_i x_v + C_i
 // (inside <=> all >= 0) and the depth plane t(x) = Wu x_u + Wv x_v + Wc, in the sub-block's local
 // emitter frame (origin at the sub-block's corner, t measured from the ray-origin plane).
+// bbox (optional): the projected triangle's extent (umin, umax, vmin, vmax) in the same frame; empty (min > max) for a
+// triangle that is never hit.
 __device__ __forceinline__ void beam_setup(const float4 q0, const float4 q1, const float4 q2, const Emitter &em,
-                                           float offu, float offv, float4 *eq)
+                                           float offu, float offv, float4 *eq, float4 *bbox = nullptr)
 {
     const float3 a = f3(q0.x, q0.y, q0.z);
     const float3 b = f3(q0.x + q1.x, q0.y + q1.y, q0.z + q1.z);
@@ -569,8 +571,10 @@ __device__ __forceinline__ void beam_setup(const float4 q0, const float4 q1, con
     const float area2 = fmaf(A0, cu, fmaf(B0, cv, C0));                     // E_ab(c)
     if (area2 == 0.0f || !(fabsf(area2) < FLT_MAX)) {                       // edge-on or degenerate: never hit
         eq[0] = make_float4(0.f, 0.f, -1.f, 0.f); eq[1] = eq[0]; eq[2] = eq[0];
+        if (bbox) *bbox = make_float4(1.f, 0.f, 1.f, 0.f);
         return;
     }
+    if (bbox) *bbox = make_float4(fminf(au, fminf(bu, cu)), fmaxf(au, fmaxf(bu, cu)), fminf(av, fminf(bv, cv)), fmaxf(av, fmaxf(bv, cv)));
     if (area2 < 0.0f) { A0 = -A0; B0 = -B0; C0 = -C0; A1 = -A1; B1 = -B1; C1 = -C1; A2 = -A2; B2 = -B2; C2 = -C2; }
     const float ia = 1.0f / area2;
     const float Wu = ((cv - av) * (bw - aw) - (bv - av) * (cw - aw)) * ia;
