@@ -79,9 +79,37 @@ def check_bvh(nodes, perm, verts):
     return n_visited
 
 
-def test_lbvh_structure_detailed(ctx):
+def sah_cost(nodes):
+    """Surface-area-heuristic cost of the tree: sum over reachable inner children of their box area plus, over leaf
+    children, box area x triangles, in units of the root box's area."""
+    link = nodes[:, 12:14].copy().view(np.int32)
+    def area(lo, hi):
+        d = np.maximum(hi - lo, 0.0)
+        return d[0] * d[1] + d[1] * d[2] + d[0] * d[2]
+    root = area(np.minimum(nodes[0, 0:3], nodes[0, 6:9]), np.maximum(nodes[0, 3:6], nodes[0, 9:12]))
+    cost, stack = root, [0]
+    while stack:
+        n = stack.pop()
+        for side in range(2):
+            a = area(nodes[n, 6 * side:6 * side + 3], nodes[n, 6 * side + 3:6 * side + 6])
+            l = int(link[n, side])
+            if l >= 0:
+                cost += a; stack.append(l)
+            else:
+                cost += a * (((~l) & 7) + 1)
+    return cost / root
+
+
+@pytest.mark.parametrize("builder", [0, 1])
+def test_bvh_structure_detailed(ctx, builder):
+    """Both builders (srp_options.bvh_builder: binned SAH, linear BVH): a permutation of the triangles, every triangle in
+    exactly one leaf, every box inside its parent's and around its triangles."""
     th = W.draw_params(W.FAMILY_DETAILED, 2)
-    dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    ctx.srp_set_options(bvh_builder=builder)
+    try:
+        dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+    finally:
+        ctx.srp_set_options()
     for k in range(2):
         nodes, perm = dz.read_bvh(k)
         v, _ = dz.read_mesh(k)
@@ -91,6 +119,31 @@ def test_lbvh_structure_detailed(ctx):
     dz.free()
 
 
+def test_sah_builder_is_reproducible_and_cheaper_than_lbvh(ctx):
+    """Two builds give the same bytes (integer atomics and a scan: no dependence on arrival order); the SAH cost of
+    the binned builder's tree is well below the linear BVH's on the detailed design; both give the same forces up to
+    the photons whose closest hit is a tie."""
+    th = W.draw_params(W.FAMILY_DETAILED, 1)
+    sun = cuda(W.fibonacci_sphere(4))
+    out = {}
+    for builder in (0, 0, 1):
+        ctx.srp_set_options(bvh_builder=builder)
+        try:
+            dz = ctx.srp_build_designs(W.FAMILY_DETAILED, th)
+        finally:
+            ctx.srp_set_options()
+        nodes, perm = dz.read_bvh(0)
+        F = ctx.srp_forces(dz, sun, 1 << 16, 4, 0).cpu().numpy()
+        out.setdefault(builder, []).append((nodes, perm, F))
+        dz.free()
+    (n0, p0, F0), (n1, p1, F1) = out[0]
+    assert np.array_equal(n0.view(np.uint32), n1.view(np.uint32)) and np.array_equal(p0, p1) and np.array_equal(F0, F1)
+    nl, pl, Fl = out[1][0]
+    c_sah, c_lbvh = sah_cost(n0), sah_cost(nl)
+    assert c_sah < 0.8 * c_lbvh, (c_sah, c_lbvh)
+    assert np.linalg.norm(F0 - Fl) <= 5e-4 * np.linalg.norm(Fl)          # a photon is 1e-4 of a force here
+
+
 def test_small_designs_have_no_hierarchy(ctx):
     dz = ctx.srp_build_designs(W.FAMILY_BOXWING, W.draw_params(W.FAMILY_BOXWING, 4))
     nodes, perm = dz.read_bvh(2)
@@ -98,19 +151,25 @@ def test_small_designs_have_no_hierarchy(ctx):
     dz.free()
 
 
-def test_lbvh_mixed_sizes_and_duplicates(ctx):
-    """from_meshes with 1, 3, 70 and 500 triangles in one batch; the 70 are 70 copies of one triangle
-    (identical Morton keys -> index tie-break)."""
+@pytest.mark.parametrize("builder", [0, 1])
+def test_bvh_mixed_sizes_and_duplicates(ctx, builder):
+    """from_meshes with 1, 2, 3, 70 and 500 triangles in one batch; the 70 are 70 copies of one triangle
+    (identical Morton keys -> index tie-break; identical centroids -> the SAH builder halves them by position)."""
     rng = np.random.default_rng(0)
     one = quad([0, 0, 0], [1, 0, 0], [0, 1, 0])[:1]
     three = rng.normal(size=(3, 3, 3)).astype(np.float32)
     dup = np.repeat(one, 70, axis=0)
     big = (rng.normal(size=(500, 1, 3)) + 0.1 * rng.normal(size=(500, 3, 3))).astype(np.float32)
-    verts = np.concatenate([one, three, dup, big])
+    two = rng.normal(size=(2, 3, 3)).astype(np.float32)
+    verts = np.concatenate([one, two, three, dup, big])
     mats = W.dirichlet_materials(len(verts), 1)
-    off = np.cumsum([0, 1, 3, 70, 500])
-    dz = ctx.srp_build_designs_from_meshes(verts, mats, off)
-    for k in range(4):
+    off = np.cumsum([0, 1, 2, 3, 70, 500])
+    ctx.srp_set_options(bvh_builder=builder)
+    try:
+        dz = ctx.srp_build_designs_from_meshes(verts, mats, off)
+    finally:
+        ctx.srp_set_options()
+    for k in range(5):
         nodes, perm = dz.read_bvh(k)
         check_bvh(nodes, perm, verts[off[k]:off[k + 1]])
     dz.free()
