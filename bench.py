@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3_detailed] [--impl ours|reference]
 
 A step = one pass of the whole hot path over one batch of synthetic input: srp_build_designs
-(mesh generation + LBVH build, S0-S1) followed by srp_forces (S2-S7) for every (design, direction)
+(mesh generation + BVH build, S0-S1) followed by srp_forces (S2-S7) for every (design, direction)
 pair of the workload.  metric = photon-bounce segments per second (BASELINE.json; every ray cast, hit or
 miss, INCLUDING primaries that a beam test resolves as misses without generating them), whole job.  Read
 `forces_per_s`, `hits_per_s` and `traced_segments_per_s` first: they cannot be inflated by empty emitter area.

@@ -8,8 +8,9 @@
  * tracing with multiple bounces (Sec. 3.2 "Estimation"), the reading of the paper
  * written out in DESIGN.md ("O-steps", R1-R17).  "takes design parameters and the light direction,
  * returns 3-D force": srp_build_designs is the "design parameters -> triangle mesh
- * with per-face material" map of PAPER.md:148 plus a per-design LBVH (Karras-style linear BVH, the
- * structure the paper builds for its Fig. 8); srp_forces is the estimator.
+ * with per-face material" map of PAPER.md:148 plus a per-design bounding-volume hierarchy (a binned-SAH
+ * BVH2 by default; srp_options.bvh_builder = 1 gives the Karras-style linear BVH, the structure the
+ * paper builds for its Fig. 8); srp_forces is the estimator.
  *
  * Conventions
  *  - Every function returns srp_status; outputs are untouched unless SRP_OK.  No exceptions cross
@@ -129,7 +130,7 @@ int srp_family_n_params(srp_family family);
 long long srp_family_tri_count(srp_family family);
 
 /* S0 + S1: theta DEVICE float[D, n_params] row-major -> meshes (fp64 evaluation rounded once to fp32)
- * and per-design LBVHs.  mesh_seed keys the per-facet Dirichlet(2,2,2) material draws and the sail's
+ * and per-design BVHs.  mesh_seed keys the per-facet Dirichlet(2,2,2) material draws and the sail's
  * noise.  n_params must equal srp_family_n_params(family).  Enqueues only. */
 srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *theta, int D,
                              int n_params, unsigned long long mesh_seed, srp_designs **out);
