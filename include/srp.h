@@ -263,6 +263,22 @@ srp_status srp_path_signatures(srp_context *ctx, const srp_designs *designs, con
                                const int *pairs, long long n_pairs, long long rays_per_dir,
                                int max_bounces, unsigned long long seed, unsigned long long *out_sig);
 
+/* srp_forces for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same results (S2-S7), but this call allocates nothing and
+ * frees nothing -- no cudaMalloc / cudaFree, no stream-ordered pool, no escape-mask build (masks that an earlier
+ * call built with these designs are used).  Its scratch (device counters and the int64 accumulators, 24 bytes per
+ * (design, direction) pair) is a static device array of SRP_NOALLOC_MAX_PAIRS pairs = 1.5 MiB that every GPU which
+ * loads the library holds until the process exits.  Limits: designs x directions <= SRP_NOALLOC_MAX_PAIRS, else
+ * SRP_ERR_INVALID; calls that srp_forces would trace as beams through a ray queue (designs with more than 64
+ * triangles and rays_per_dir >= 8 x the largest triangle count, unless srp_options.primary_mode = 1) and the
+ * instrumented kernels give SRP_ERR_UNSUPPORTED.  All contexts and streams of a process on one GPU share the array:
+ * calls that overlap on the GPU race (enqueue them on one stream, or order them with events); the array keeps the
+ * last call's contents and every call clears what it uses.  srp_get_stats does not cover this call.  sun_dirs and
+ * out_forces are DEVICE pointers as in srp_forces.  Enqueues only. */
+#define SRP_NOALLOC_MAX_PAIRS 65536
+srp_status srp_forces_noalloc(srp_context *ctx, const srp_designs *designs, const float *sun_dirs, int S,
+                              long long rays_per_dir, int max_bounces, unsigned long long seed, float *out_forces);
+
 /* Counters of the last srp_forces* call on this context.  Syncs. */
 srp_status srp_get_stats(srp_context *ctx, srp_stats *host_out);
 

@@ -56,7 +56,7 @@ EXPORTS = ["srp_create", "srp_destroy", "srp_set_options", "srp_get_options", "s
            "srp_build_designs_from_meshes", "srp_designs_info", "srp_designs_read_mesh",
            "srp_designs_read_bvh", "srp_free_designs", "srp_forces", "srp_forces_pairs", "srp_forces_host",
            "srp_forces_torques", "srp_forces_torques_pairs", "srp_forces_split", "srp_forces_split_pairs",
-           "srp_forces_per_sample", "srp_thermal_forces", "srp_designs_set_shininess", "srp_first_hits", "srp_path_signatures", "srp_get_stats",
+           "srp_forces_per_sample", "srp_forces_noalloc", "srp_thermal_forces", "srp_designs_set_shininess", "srp_first_hits", "srp_path_signatures", "srp_get_stats",
            "srp_launch_count", "srp_set_workspace", "srp_workspace_bytes_min", "srp_probe_peaks"]
 
 _lib = None
@@ -88,6 +88,7 @@ def load_library():
     L.srp_designs_read_bvh.argtypes = [vp, vp, ci, ctypes.POINTER(ll), vp, vp]
     L.srp_free_designs.argtypes = [vp, vp]
     L.srp_forces.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
+    L.srp_forces_noalloc.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
     L.srp_forces_pairs.argtypes = [vp, vp, vp, ci, vp, ll, ll, ci, ull, vp]
     L.srp_forces_host.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp]
     L.srp_forces_torques.argtypes = [vp, vp, vp, ci, ll, ci, ull, vp, vp, vp]
@@ -223,6 +224,17 @@ class Context:
                                                            off.ctypes.data, len(off) - 1, ctypes.byref(h)))
         self.stream.synchronize()
         return Designs(self, h)
+
+    def srp_forces_noalloc(self, designs, sun_dirs, rays_per_dir, max_bounces, seed, out):
+        """srp_forces through the library's static scratch: allocates nothing (the caller brings `out`, CUDA float32
+        [D,S,3]); at most NOALLOC_MAX_PAIRS (design, direction) pairs, no beam-traced calls (include/srp.h)."""
+        _check_cuda_f32(sun_dirs, "sun_dirs", self.device, (3,))
+        S = sun_dirs.shape[0]
+        if _check_cuda_f32(out, "out", self.device).numel() != designs.D * S * 3:
+            raise ValueError("out must hold [D, S, 3] floats")
+        self._check(self.lib.srp_forces_noalloc(self.handle, designs.handle, sun_dirs.data_ptr(), S, rays_per_dir,
+                                                max_bounces, seed, out.data_ptr()))
+        return out
 
     def srp_forces(self, designs, sun_dirs, rays_per_dir, max_bounces, seed=0, out=None):
         """sun_dirs: CUDA float32 [S,3]; returns CUDA float32 [D,S,3] (asynchronous on the stream)."""

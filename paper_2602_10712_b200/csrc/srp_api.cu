@@ -861,4 +861,63 @@ srp_status srp_probe_peaks(srp_context *ctx, double *fp32_tflops, double *l2_rea
     return SRP_OK;
 }
 
+// ---- srp_forces_noalloc: the forces call for callers that must not allocate (include/srp.h) ----
+// Its scratch -- the device counters every trace kernel updates and the fixed-point accumulators of the pairs --
+// lives in this file-scope array instead of the context's cudaMalloc'ed workspace: every GPU that loads the
+// library holds SRP_NOALLOC_SCRATCH_BYTES (1.5 MiB + 1 KiB) until the process exits.  In host code the array's
+// name is only a handle; its device address comes from cudaGetSymbolAddress, once per device, with that device current.
+#define SRP_NOALLOC_HEADER_BYTES 1024
+#define SRP_NOALLOC_SCRATCH_BYTES (SRP_NOALLOC_HEADER_BYTES + (size_t)SRP_NOALLOC_MAX_PAIRS * 3 * sizeof(long long))
+static __device__ __align__(256) unsigned char srp_noalloc_scratch[SRP_NOALLOC_SCRATCH_BYTES];
+static_assert(sizeof(DevStats) <= 512 && (SRP_PIPES + 1) * sizeof(unsigned long long) <= 256, "header layout");
+
+static cudaError_t noalloc_scratch_address(int device, unsigned char **out)
+{
+    static unsigned char *addr[64];                    // per device; written once, the same value from any thread
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    if (!addr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, srp_noalloc_scratch);     // the caller made `device` current
+        if (e != cudaSuccess) return e;
+        addr[device] = (unsigned char *)p;
+    }
+    *out = addr[device];
+    return cudaSuccess;
+}
+
+srp_status srp_forces_noalloc(srp_context *ctx, const srp_designs *dz, const float *sun_dirs, int S, long long N, int B,
+                              unsigned long long seed, float *out)
+{
+    srp_status st = check_trace_args(ctx, dz, sun_dirs, S, N, B, out);
+    if (st != SRP_OK) return st;
+    const long long n_pairs = (long long)dz->D * S;
+    if (n_pairs > SRP_NOALLOC_MAX_PAIRS)
+        return fail(ctx, SRP_ERR_INVALID, "srp_forces_noalloc: designs x directions exceeds SRP_NOALLOC_MAX_PAIRS (65536)");
+    if (ctx->opt.instrumented) return fail(ctx, SRP_ERR_UNSUPPORTED, "srp_forces_noalloc: not with the instrumented kernels");
+    const bool brute = !dz->has_bvh || ctx->opt.force_brute != 0;
+    if (want_beams(ctx, brute, dz->maxT, N, n_pairs))
+        return fail(ctx, SRP_ERR_UNSUPPORTED, "srp_forces_noalloc: this call would trace beams through a ray queue "
+                                             "(designs with a BVH and rays_per_dir >= 8 x triangles); use srp_forces");
+    cudaSetDevice(ctx->device);
+    unsigned char *scratch = nullptr;
+    TRY_CUDA(ctx, noalloc_scratch_address(ctx->device, &scratch), "address of the static scratch");
+    ctx->launches_call = 0;
+    TraceArgs a = make_args(ctx, dz, sun_dirs, S, nullptr, n_pairs, N, B, seed);
+    a.stats = (DevStats *)scratch;                                             // [0, 512): counters
+    a.work_counter = (unsigned long long *)(scratch + 512);                    // [512, 768): tile counters, loop rounds
+    a.rounds_total = a.work_counter + SRP_PIPES;
+    a.accum = (long long *)(scratch + SRP_NOALLOC_HEADER_BYTES);               // [1024, ...): 3 int64 per pair
+    a.acc_stride = 3; a.torque = 0; a.xcom = nullptr;
+    a.rq = nullptr; a.rq_cap = 0; a.rq_high = 0; a.rq_ctr = nullptr;
+    // escape masks an earlier call built with these designs are used; none is built here (results do not depend on them)
+    if (ctx->opt.escape_masks == 0 || ctx->opt.force_brute != 0) a.dz.esc = nullptr;
+    // the array keeps the last call's contents: everything this call reads before writing starts at zero
+    TRY_CUDA(ctx, cudaMemsetAsync(scratch, 0, SRP_NOALLOC_HEADER_BYTES + sizeof(long long) * 3 * (size_t)n_pairs, ctx->stream),
+             "zero the static scratch");
+    TRY_CUDA(ctx, srp_launch_trace(a, brute, false, ctx->num_sms, ctx->stream), "trace launch");
+    TRY_CUDA(ctx, srp_launch_finalize(a, out, nullptr, ctx->stream), "finalize launch");
+    count_launches(ctx, 2);
+    return SRP_OK;
+}
+
 } // extern "C"
