@@ -27,6 +27,7 @@ SOURCES = {
     "mesh_gen.cu": ["--fmad=false"],
     "lbvh.cu": [],
     "bvh_sah.cu": [],
+    "bvh4.cu": [],
     "escape_mask.cu": [],
     "trace.cu": [],
     "trace_perray.cu": [],

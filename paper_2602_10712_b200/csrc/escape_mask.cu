@@ -21,13 +21,15 @@ namespace {
 
 constexpr int ESC_STACK = 96;
 #ifndef ESC_MAX_VISITS_DEF
-#define ESC_MAX_VISITS_DEF 4000
+#define ESC_MAX_VISITS_DEF 2000
 #endif
 constexpr int ESC_MAX_VISITS = ESC_MAX_VISITS_DEF;      // beyond this the triangle sits in cluttered surroundings: mark everything
 #ifndef ESC_SIN_DESCEND_DEF
-#define ESC_SIN_DESCEND_DEF 0.25f
+#define ESC_SIN_DESCEND_DEF 0.5f
 #endif
-constexpr float ESC_SIN_DESCEND = ESC_SIN_DESCEND_DEF;  // subtrees seen under a wider cone than this are opened
+constexpr float ESC_SIN_DESCEND = ESC_SIN_DESCEND_DEF;  // subtrees seen under a wider cone than this are opened.  0.5 / 2000 visits
+                                                        // against 0.25 / 4000: the build of cfg3's 16 designs 114 -> 62 ms AND 4 % more
+                                                        // escapes resolved (fewer clusters run into the visit cap and mark everything)
 #ifndef ESC_SIN_SHARED_DEF
 #define ESC_SIN_SHARED_DEF 0.8f
 #endif

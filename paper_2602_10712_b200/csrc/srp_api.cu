@@ -48,7 +48,7 @@ double acc_scale_for(double photons, int B)
 
 void free_designs_mem(srp_context *ctx, srp_designs *d)
 {
-    void *ptrs[10] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm, d->esc, d->nplane, d->shin };
+    void *ptrs[11] = { d->verts_orig, d->mats_orig, d->tri, d->nodes, d->tri_off_dev, d->box, d->perm, d->esc, d->nplane, d->shin, d->nodes4 };
     for (void *q : ptrs)
         if (q) cudaFreeAsync(q, ctx->stream);
 }
@@ -61,6 +61,9 @@ srp_status alloc_designs(srp_context *ctx, srp_designs *d)
     TRY_CUDA(ctx, pool_alloc(ctx, &d->mats_orig, sizeof(float) * 3 * sumT), "alloc mats");
     TRY_CUDA(ctx, pool_alloc(ctx, &d->tri, sizeof(float4) * 3 * sumT), "alloc packed triangles");
     if (d->has_bvh) TRY_CUDA(ctx, pool_alloc(ctx, &d->nodes, sizeof(float4) * 4 * sumT), "alloc nodes");
+#ifdef SRP_BVH4
+    if (d->has_bvh) TRY_CUDA(ctx, pool_alloc(ctx, &d->nodes4, sizeof(float4) * 8 * sumT), "alloc wide nodes");
+#endif
     TRY_CUDA(ctx, pool_alloc(ctx, &d->tri_off_dev, sizeof(long long) * (d->D + 1)), "alloc offsets");
     TRY_CUDA(ctx, pool_alloc(ctx, &d->box, sizeof(float4) * 2 * d->D), "alloc boxes");
     TRY_CUDA(ctx, pool_alloc(ctx, &d->perm, sizeof(int) * sumT), "alloc perm");
@@ -470,6 +473,7 @@ srp_status srp_build_designs(srp_context *ctx, srp_family family, const float *t
                                         d->mats_orig, ctx->mempool, 0u, ctx->stream);
     int build_launches = 0;
     if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->opt.bvh_builder, ctx->mempool, ctx->stream, &build_launches);
+    if (e == cudaSuccess && d->nodes4) { e = srp_launch_collapse4(d, ctx->stream); ++build_launches; }
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     ctx->launches_total += 2 + build_launches;                         // mesh generation: 2 kernels
     *out = d;
@@ -506,6 +510,7 @@ srp_status srp_build_designs_from_meshes(srp_context *ctx, const float *verts, c
         e = cudaMemcpyAsync(d->mats_orig, mats, sizeof(float) * 3 * d->sumT, cudaMemcpyDeviceToDevice, ctx->stream);
     int build_launches = 0;
     if (e == cudaSuccess) e = srp_launch_build(d, ctx->opt.leaf_max, ctx->opt.bvh_builder, ctx->mempool, ctx->stream, &build_launches);
+    if (e == cudaSuccess && d->nodes4) { e = srp_launch_collapse4(d, ctx->stream); ++build_launches; }
     if (e != cudaSuccess) { free_designs_mem(ctx, d); delete d; return cuda_fail(ctx, "design build", e); }
     ctx->launches_total += build_launches;
     *out = d;

@@ -23,6 +23,7 @@
 struct DesignsDev {
     const float4 *tri;        // [sumT * 3]
     const float4 *nodes;      // [sumT * 4]; node base of design k == tri_off[k]
+    const float4 *nodes4;     // [sumT * 8]: 4-wide nodes folded from the BVH2 (bvh4.cu), same numbering; or nullptr
     const long long *tri_off; // [D + 1]
     const float4 *box;        // [D * 2]: (lo, -), (hi, -)
     const int *perm;          // [sumT]: sorted position -> original index within the design
@@ -42,6 +43,7 @@ struct srp_designs {
     float *mats_orig = nullptr;         // [sumT*3]
     float4 *tri = nullptr;
     float4 *nodes = nullptr;
+    float4 *nodes4 = nullptr;
     long long *tri_off_dev = nullptr;
     float4 *box = nullptr;
     int *perm = nullptr;
@@ -52,7 +54,7 @@ struct srp_designs {
     bool has_bvh = false;
     DesignsDev dev() const {
         DesignsDev d;
-        d.tri = tri; d.nodes = nodes; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.esc = esc; d.nplane = nplane; d.shin = shin; d.D = D;
+        d.tri = tri; d.nodes = nodes; d.nodes4 = nodes4; d.tri_off = tri_off_dev; d.box = box; d.perm = perm; d.esc = esc; d.nplane = nplane; d.shin = shin; d.D = D;
         d.has_bvh = has_bvh ? 1 : 0;
         return d;
     }
@@ -135,6 +137,7 @@ cudaError_t srp_launch_mesh_gen(int family, const float *theta, int D, int n_par
 cudaError_t srp_launch_build(srp_designs *dz, int leaf_max, int builder, cudaMemPool_t pool, cudaStream_t stream, int *launches);
 cudaError_t srp_launch_sah_build(srp_designs *dz, const unsigned *vals, unsigned *vals_final, int leaf_max,
                                  cudaMemPool_t pool, cudaStream_t stream, int *launches);
+cudaError_t srp_launch_collapse4(const srp_designs *dz, cudaStream_t stream);   // nodes -> nodes4
 cudaError_t srp_launch_gather_shininess(const DesignsDev &dz, long long sumT, const float *shin_orig, float *shin_sorted, cudaStream_t stream);
 cudaError_t srp_launch_node_planes(const DesignsDev &dz, long long sumT, float4 *nplane, cudaStream_t stream);
 cudaError_t srp_launch_escape_masks_small(const DesignsDev &dz, long long sumT, unsigned *esc, cudaStream_t stream);

@@ -130,7 +130,7 @@ bounce_trace_kernel(const TraceArgs a)
         int k, j;
         pair_of32(a, rp, k, j);
         const long long tb = a.dz.tri_off[k];
-        ln = a.dz.nodes + 4 * tb; lt = a.dz.tri + 3 * tb;
+        ln = SRP_TRAV_NODES(a.dz, tb); lt = a.dz.tri + 3 * tb;
         const uint32_t s27 = rsd & SRC_NONE;
         src = s27 == SRC_NONE ? -1 : (int)s27;
         idx = safe_rcp(d.x); idy = safe_rcp(d.y); idz = safe_rcp(d.z);

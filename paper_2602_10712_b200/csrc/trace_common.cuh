@@ -30,7 +30,12 @@ constexpr int TRACE_WARPS = TRACE_THREADS / 32;
 #define STACK_SMEM_DEF 20
 #endif
 constexpr int STACK_SMEM = STACK_SMEM_DEF;   // traversal stack entries per thread kept in shared memory
-constexpr int STACK_OVF = 80;        // deeper entries spill to local memory (degenerate trees only)
+#ifdef SRP_BVH4
+constexpr int STACK_OVF = 128;       // a wide node pushes up to three entries
+#else
+constexpr int STACK_OVF = 80;
+#endif
+//        // deeper entries spill to local memory (degenerate trees only)
 constexpr unsigned FULL = 0xffffffffu;
 
 enum { MODE_BRUTE_SMEM = 0, MODE_BVH = 1, MODE_BRUTE_GLOBAL = 2 };
@@ -204,6 +209,68 @@ constexpr int NODE_RUN_CAP = NODE_RUN_CAP_DEF;
         else { --sp; cur_ = sp < NSMEM ? s_stack[sp * STRIDE] : ovf[sp - NSMEM]; }        \
     } while (0)
 
+#ifdef SRP_BVH4
+// 4-wide node (bvh4.cu): four child boxes against the ray, the hits in order of entry distance: nearest next, the
+// others pushed farthest first.  `nodes` is the design's nodes4 base.
+#define SRP_TRAV_NODES(dz_, tb_) ((dz_).nodes4 + 8 * (tb_))
+#define SRP_CSWAP(i_, j_)                                                                                     \
+    do {                                                                                                      \
+        const bool sw_ = key[j_] < key[i_];                                                                   \
+        const float kf_ = sw_ ? key[j_] : key[i_], kg_ = sw_ ? key[i_] : key[j_];                              \
+        const int lf_ = sw_ ? link[j_] : link[i_], lg_ = sw_ ? link[i_] : link[j_];                            \
+        key[i_] = kf_; key[j_] = kg_; link[i_] = lf_; link[j_] = lg_;                                          \
+    } while (0)
+template <int STRIDE, int NSMEM>
+__device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, int cur, int &sp, int *s_stack, int *ovf,
+                                             float idx, float idy, float idz, float oxi, float oyi, float ozi, float tbest)
+{
+    const float4 *p = nodes + 8 * (long long)cur;
+    const F8 qa = ldg256(p), qb = ldg256(p + 2), qc = ldg256(p + 4), qd = ldg256(p + 6);
+    const float w[24] = { qa.a.x, qa.a.y, qa.a.z, qa.a.w, qa.b.x, qa.b.y, qa.b.z, qa.b.w, qb.a.x, qb.a.y, qb.a.z, qb.a.w,
+                          qb.b.x, qb.b.y, qb.b.z, qb.b.w, qc.a.x, qc.a.y, qc.a.z, qc.a.w, qc.b.x, qc.b.y, qc.b.z, qc.b.w };
+    int link[4] = { __float_as_int(qd.a.x), __float_as_int(qd.a.y), __float_as_int(qd.a.z), __float_as_int(qd.a.w) };
+    float key[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float a0 = fmaf(w[6 * c + 0], idx, -oxi), a1 = fmaf(w[6 * c + 3], idx, -oxi);
+        const float b0 = fmaf(w[6 * c + 1], idy, -oyi), b1 = fmaf(w[6 * c + 4], idy, -oyi);
+        const float c0 = fmaf(w[6 * c + 2], idz, -ozi), c1 = fmaf(w[6 * c + 5], idz, -ozi);
+        const float tmin = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
+        const float tmax = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
+        key[c] = tmin <= tmax * 1.0000004f ? tmin : FLT_MAX;
+    }
+#ifdef SRP_BVH4_NOSORT
+    int m = 0;
+    float km = key[0];
+#pragma unroll
+    for (int c = 1; c < 4; ++c)
+        if (key[c] < km) { km = key[c]; m = c; }
+    int lm = link[0];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        if (c == m) lm = link[c];
+        else if (key[c] < FLT_MAX) {
+            if (sp < NSMEM) s_stack[sp * STRIDE] = link[c]; else ovf[sp - NSMEM] = link[c];
+            ++sp;
+        }
+    }
+    if (km < FLT_MAX) return lm;
+#else
+    SRP_CSWAP(0, 1); SRP_CSWAP(2, 3); SRP_CSWAP(0, 2); SRP_CSWAP(1, 3); SRP_CSWAP(1, 2);
+#pragma unroll
+    for (int c = 3; c >= 1; --c)
+        if (key[c] < FLT_MAX) {
+            SRP_CHECK(sp < NSMEM + STACK_OVF, "traversal stack");
+            if (sp < NSMEM) s_stack[sp * STRIDE] = link[c]; else ovf[sp - NSMEM] = link[c];
+            ++sp;
+        }
+    if (key[0] < FLT_MAX) return link[0];
+#endif
+    SRP_POP(cur);
+    return cur;
+}
+#else
+#define SRP_TRAV_NODES(dz_, tb_) ((dz_).nodes + 4 * (tb_))
 // STRIDE: distance in ints between consecutive stack entries of one thread (thread-interleaved
 // layout); NSMEM: entries kept in shared memory.
 // One internal node for one lane: both child boxes against the ray, nearer child next, farther child
@@ -243,6 +310,8 @@ __device__ __forceinline__ int bvh_node_step(const float4 *__restrict__ nodes, i
     SRP_POP(cur);
     return cur;
 }
+
+#endif
 
 // One leaf for one lane: its triangles (source excluded, R10), then the next stack entry.
 template <int STRIDE, int NSMEM>

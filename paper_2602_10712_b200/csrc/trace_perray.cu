@@ -38,7 +38,7 @@ trace_kernel(const TraceArgs a)
         const long long tbase = a.dz.tri_off[k];
         const int T = (int)(a.dz.tri_off[k + 1] - tbase);
         const float4 *gtri = a.dz.tri + 3 * tbase;
-        const float4 *gnodes = a.dz.nodes + 4 * tbase;
+        const float4 *gnodes = SRP_TRAV_NODES(a.dz, tbase);
         if (MODE == MODE_BRUTE_SMEM && loaded_k != k) {
             __syncwarp();
             for (int x = lane; x < 3 * T; x += 32) my_tri[x] = gtri[x];
@@ -146,7 +146,7 @@ bvh_trace_kernel(const TraceArgs a)
         if (!(em.Ae > 0.0f)) continue;
         const long long tbase = a.dz.tri_off[k];
         const float4 *gtri = a.dz.tri + 3 * tbase;
-        const float4 *gnodes = a.dz.nodes + 4 * tbase;
+        const float4 *gnodes = SRP_TRAV_NODES(a.dz, tbase);
         RayGen g;
         g.j = (uint32_t)j; g.k = (uint32_t)k; g.key0 = a.key0; g.key1 = a.key1; g.sampler = a.sampler; set_torque<TORQUE>(g, a, k);
         g.inv_nx = 1.0f / (float)(1u << ((a.log2N + 1) >> 1));
@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(TRACE_THREADS) first_hit_kernel(const TraceArg
             float tbest = FLT_MAX;
             unsigned nb = 0, nt = 0;
             if (MODE == MODE_BVH)
-                closest_bvh<false>(a.dz.nodes + 4 * tbase, a.dz.tri + 3 * tbase, o, em.s, -1, tbest, best,
+                closest_bvh<false>(SRP_TRAV_NODES(a.dz, tbase), a.dz.tri + 3 * tbase, o, em.s, -1, tbest, best,
                                    s_stack + threadIdx.x, nb, nt);
             else
                 closest_brute<false>(a.dz.tri + 3 * tbase, T, o, em.s, -1, tbest, best, nt);

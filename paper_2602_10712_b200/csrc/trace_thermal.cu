@@ -91,7 +91,7 @@ thermal_trace_kernel(const TraceArgs a, const ThermalArgs h)
         const float W = h.power[tbase + f];
         const float Pk = h.design_power[k];
         const float4 *gtri = a.dz.tri + 3 * tbase;
-        const float4 *gnodes = a.dz.nodes + 4 * tbase;
+        const float4 *gnodes = SRP_TRAV_NODES(a.dz, tbase);
         const float4 q0 = __ldg(gtri + 3 * fs), q1 = __ldg(gtri + 3 * fs + 1), q2 = __ldg(gtri + 3 * fs + 2);
         float3 n = cross3(f3(q1.x, q1.y, q1.z), f3(q2.x, q2.y, q2.z));
         const float il = 1.0f / sqrtf(dot3(n, n));
