@@ -129,9 +129,11 @@ srp_status ensure_queue(srp_context *ctx, TraceArgs &a, bool brute, bool instrum
         TRY_CUDA(ctx, cudaStreamSynchronize(ctx->stream), "sync before queue growth");
         cudaFree(ctx->rq); ctx->rq = nullptr; ctx->rq_words = 0; ctx->rq_owned = false;
         // Every round of a loop ends with a tail in which SMs idle; two pipelines hide each other's tails, and the
-        // more rays a queue holds beyond its reserve, the fewer rounds there are: 32 M slots more by default.
+        // more rays a queue holds beyond its reserve, the fewer rounds there are: 128 M slots more by default
+        // (4.6 GB; cfg3 against 32 M / 64 M / 256 M slots: +3.5 % / +1.2 % / -1.1 % time).  A caller who wants
+        // another trade gives the workspace (srp_set_workspace).
 #ifndef SRP_RQ_EXTRA
-#define SRP_RQ_EXTRA (32u << 20)
+#define SRP_RQ_EXTRA (128u << 20)
 #endif
         size_t rays = SRP_PIPES * min_rays + (size_t)(SRP_RQ_EXTRA);
         cudaError_t e = cudaMalloc(&ctx->rq, sizeof(unsigned) * rays * fields);
