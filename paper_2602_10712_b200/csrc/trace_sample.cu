@@ -16,6 +16,13 @@ namespace {
 
 constexpr int SAMPLE_THREADS = 512;
 constexpr int SAMPLE_WARPS = SAMPLE_THREADS / 32;
+// Primaries of the stratified sampler sit one per cell of the emitter grid, so the closest primary hits of a record
+// are found triangle by triangle: a triangle is tested against the rays of the cells its bounding rectangle touches
+// (a few) instead of every ray against every triangle -- the same test on the same operands, ~100 x fewer of them.
+constexpr int SAMPLE_CLUSTER = 32;                    // triangles per cluster box (bounce rays)
+constexpr int RASTER_MIN_TRIS = 256;                  // below: testing all triangles costs nothing
+constexpr int RASTER_MAX_RAYS = 2048;                 // 16 bytes of shared memory per ray
+constexpr int RASTER_BIG = 32, RASTER_BIGCAP = 128;   // a triangle over more cells goes to a warp (the first 128 of them)
 
 // O-step 4 for a primary in the emitter frame: origin (pu, pv, worg), direction (0, 0, 1), all triangles.
 __device__ __forceinline__ void closest_primary(const float4 *__restrict__ tp, const int T, const float pu, const float pv,
@@ -43,30 +50,117 @@ __device__ __forceinline__ void closest_primary(const float4 *__restrict__ tp, c
     }
 }
 
-// O-step 4 for the bounce rays of a pass.  n <= 32 rays wait in the warp's queue; with fewer than 17 the lanes are
-// shared out: g = 32 / n' lanes per ray (n' = n rounded up to a power of two), each testing every g-th triangle,
-// then a minimum over the group (smallest t, ties to the smallest index as in the definition) -- so that the few
-// photons of the deep bounces, of which a record with ~10^3 photons has only a handful, still fill the warp.
-__device__ __forceinline__ void closest_shared(const float4 *__restrict__ tp, const int T, const float3 o, const float3 d,
-                                               const int src, const int g, const int sub, float &tbest, int &best, unsigned &n_tri)
+// The same test for ONE triangle and the primary of ONE cell of the emitter grid (rasterised primaries, below): the
+// hit goes into the cell's key -- depth in the high word, triangle in the low word, so that a 64-bit minimum keeps the
+// smallest t and, among equal t, the smallest index (the definition's tie rule).
+__device__ __forceinline__ void raster_test(const float4 q0, const float4 q1, const float4 q2, const int f, const float2 p,
+                                            const float worg, unsigned long long *key)
 {
-    for (int f = sub; f < T; f += g) {
-        if (f == src) continue;
-        tri_test(tp[3 * f], tp[3 * f + 1], tp[3 * f + 2], o, d, f, tbest, best);
+    const float det = fmaf(q1.y, q2.x, -q1.x * q2.y);
+    const float tx = p.x - q0.x, ty = p.y - q0.y;
+    const uint32_t sb = __float_as_uint(det) & 0x80000000u;
+    const float U = __uint_as_float(__float_as_uint(fmaf(ty, q2.x, -tx * q2.y)) ^ sb);
+    const float V = __uint_as_float(__float_as_uint(fmaf(tx, q1.y, -ty * q1.x)) ^ sb);
+    const float adet = fabsf(det);
+    if (U >= 0.0f && V >= 0.0f && U + V <= adet && adet > 0.0f) {
+        const float tz = worg - q0.z;
+        const float3 qv = f3(fmaf(ty, q1.z, -tz * q1.y), fmaf(tz, q1.x, -tx * q1.z), fmaf(tx, q1.y, -ty * q1.x));
+        const float Tn = __uint_as_float(__float_as_uint(fmaf(q2.x, qv.x, fmaf(q2.y, qv.y, q2.z * qv.z))) ^ sb);
+        if (Tn > 0.0f) {
+            const float t = Tn / adet;
+            atomicMin(key, ((unsigned long long)__float_as_uint(t) << 32) | (unsigned long long)(unsigned)f);
+        }
     }
-    n_tri += (unsigned)((T - sub + g - 1) / g);
-    for (int off = 1; off < g; off <<= 1) {           // the g lanes of a ray are consecutive
-        const float t2 = __shfl_xor_sync(FULL, tbest, off);
-        const int b2 = __shfl_xor_sync(FULL, best, off);
-        if (b2 >= 0 && (t2 < tbest || (t2 == tbest && b2 < best) || best < 0)) { tbest = t2; best = b2; }
+}
+
+__device__ __forceinline__ uint32_t spread_even_bits(uint32_t x)     // inverse of compact_even_bits, 16 bits
+{
+    x &= 0x0000FFFFu;
+    x = (x | (x << 8)) & 0x00FF00FFu;
+    x = (x | (x << 4)) & 0x0F0F0F0Fu;
+    x = (x | (x << 2)) & 0x33333333u;
+    x = (x | (x << 1)) & 0x55555555u;
+    return x;
+}
+
+// The cells of the nx x ny emitter grid that a triangle's bounding rectangle touches (widened by `marg`, the bound of
+// the fp32 projection error: a ray outside them fails the test above).  false: none.
+__device__ __forceinline__ bool raster_cells(const float4 q0, const float4 q1, const float4 q2, const Emitter &em, const float sx,
+                                             const float sy, const float marg, const int nx, const int ny, int &cx0, int &cx1, int &cy0, int &cy1)
+{
+    const float ua = q0.x, ub = q0.x + q1.x, uc = q0.x + q2.x, va = q0.y, vb = q0.y + q1.y, vc = q0.y + q2.y;
+    const float x0 = floorf((fminf(ua, fminf(ub, uc)) - em.u0 - marg) * sx), x1 = floorf((fmaxf(ua, fmaxf(ub, uc)) - em.u0 + marg) * sx);
+    const float y0 = floorf((fminf(va, fminf(vb, vc)) - em.v0 - marg) * sy), y1 = floorf((fmaxf(va, fmaxf(vb, vc)) - em.v0 + marg) * sy);
+    if (!(x1 >= 0.f && y1 >= 0.f && x0 <= (float)(nx - 1) && y0 <= (float)(ny - 1))) return false;      // also NaN
+    cx0 = (int)fmaxf(x0, 0.f); cx1 = (int)fminf(x1, (float)(nx - 1)); cy0 = (int)fmaxf(y0, 0.f); cy1 = (int)fminf(y1, (float)(ny - 1));
+    return true;
+}
+
+// O-step 4 for the bounce rays of a pass.  n <= 32 rays wait in the warp's queue; with fewer than 17 the lanes are
+// shared out: g = 32 / n' lanes per ray (n' = n rounded up to a power of two).  The triangles sit in clusters of 32
+// consecutive ones (neighbours on their patch) behind a box each.  The lanes of a ray test its boxes, every g-th each;
+// for every box that a ray meets the WHOLE warp then tests the cluster's 32 triangles against that ray, a lane per
+// triangle, and reduces to the closest (smallest t, ties to the smallest index as in the definition) -- so both
+// steps run with full warps however few photons the deep bounces of a record with ~10^3 photons have left.
+__device__ __forceinline__ void closest_shared(const float4 *__restrict__ tp, const float4 *__restrict__ cl, const int T, const bool has_ray,
+                                               const float3 o, const float3 d, const int src, const int g, const int sub, float &tbest,
+                                               int &best, unsigned &n_tri, unsigned &n_box)
+{
+    const int lane = threadIdx.x & 31;
+    const float idx = safe_rcp(d.x), idy = safe_rcp(d.y), idz = safe_rcp(d.z);
+    const float oxi = o.x * idx, oyi = o.y * idy, ozi = o.z * idz;
+    const int ncl = (T + SAMPLE_CLUSTER - 1) / SAMPLE_CLUSTER;
+    const int iters = (ncl + g - 1) / g;                                   // warp-uniform
+    for (int k = 0; k < iters; ++k) {
+        const int c = sub + k * g;
+        bool hit = false;
+        if (has_ray && c < ncl) {
+            const float4 lo = cl[2 * c], hi = cl[2 * c + 1];
+            const float a0 = fmaf(lo.x, idx, -oxi), a1 = fmaf(hi.x, idx, -oxi);
+            const float b0 = fmaf(lo.y, idy, -oyi), b1 = fmaf(hi.y, idy, -oyi);
+            const float c0 = fmaf(lo.z, idz, -ozi), c1 = fmaf(hi.z, idz, -ozi);
+            const float tmin = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), 0.0f));
+            const float tmax = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), tbest));
+            ++n_box;
+            hit = tmin <= tmax * 1.0000004f;
+        }
+        unsigned m = __ballot_sync(FULL, hit);
+        while (m != 0u) {                                                  // one (ray, cluster) pair at a time, all lanes
+            const int L = __ffs(m) - 1;
+            m &= m - 1u;
+            const float3 ro = f3(__shfl_sync(FULL, o.x, L), __shfl_sync(FULL, o.y, L), __shfl_sync(FULL, o.z, L));
+            const float3 rd = f3(__shfl_sync(FULL, d.x, L), __shfl_sync(FULL, d.y, L), __shfl_sync(FULL, d.z, L));
+            const int rsrc = __shfl_sync(FULL, src, L);
+            const int f = __shfl_sync(FULL, c, L) * SAMPLE_CLUSTER + lane;
+            float tt = FLT_MAX;
+            int bb = -1;
+            if (f < T && f != rsrc) {
+                tri_test(tp[3 * f], tp[3 * f + 1], tp[3 * f + 2], ro, rd, f, tt, bb);
+                ++n_tri;
+            }
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                const float t2 = __shfl_xor_sync(FULL, tt, off);
+                const int b2 = __shfl_xor_sync(FULL, bb, off);
+                if (b2 >= 0 && (bb < 0 || t2 < tt || (t2 == tt && b2 < bb))) { tt = t2; bb = b2; }
+            }
+            // every lane of the ray's group keeps the result, so that its later boxes are tested against it
+            if (lane / g == L / g && bb >= 0 && (best < 0 || tt < tbest || (tt == tbest && bb < best))) { tbest = tt; best = bb; }
+        }
     }
 }
 
 template <bool ANALOG>
 __global__ void __launch_bounds__(SAMPLE_THREADS, 2)
-sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t k_offset)
+sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t k_offset, const uint32_t raster_n)
 {
     extern __shared__ float4 s_tri[];                 // 3 x float4 per triangle of the record being traced
+    // rasterised primaries (raster_n = N, else 0): per cell of the emitter grid the ray's position and its closest hit
+    float4 *s_cl = s_tri + 3 * a.max_tris;            // 2 x float4 per cluster of 32 triangles: its box (lo, hi)
+    float2 *s_puv = reinterpret_cast<float2 *>(s_cl + 2 * ((a.max_tris + SAMPLE_CLUSTER - 1) / SAMPLE_CLUSTER));
+    unsigned long long *s_key = reinterpret_cast<unsigned long long *>(s_puv + raster_n);
+    __shared__ int s_big[RASTER_BIGCAP];              // triangles over many cells: rasterised by a warp, not a thread
+    __shared__ int s_nbig;
     __shared__ WarpQueue s_q[SAMPLE_WARPS];           // photons that go on, per warp
     __shared__ double s_part[SAMPLE_WARPS][3];
     __shared__ unsigned s_hist[SAMPLE_WARPS][16];
@@ -77,7 +171,8 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
     if (lane < 16) s_hist[warp][lane] = 0;
     WarpQueue &Q = s_q[warp];
     LaneCounters cn = { 0, 0, 0, 0, 0, 0, 0, 0 };
-    unsigned long long n_tri64 = 0, n_2d64 = 0;       // every test is counted (32-bit lane counters are folded in per record)
+    unsigned long long n_tri64 = 0, n_2d64 = 0, n_cl64 = 0;
+    unsigned n_cl = 0;                                // cluster-box tests of the record       // every test is counted (32-bit lane counters are folded in per record)
 
     for (long long m = blockIdx.x; m < a.n_pairs; m += gridDim.x) {
         const long long tbase = a.dz.tri_off[m];
@@ -91,6 +186,28 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
             s_tri[x] = make_float4(dot3(p, em.u), dot3(p, em.v), dot3(p, em.s), q.w);
         }
         __syncthreads();
+        for (int c = warp; c < (T + SAMPLE_CLUSTER - 1) / SAMPLE_CLUSTER; c += SAMPLE_WARPS) {      // cluster boxes: a lane per triangle
+            const int f = c * SAMPLE_CLUSTER + lane;
+            float lo[3] = { FLT_MAX, FLT_MAX, FLT_MAX }, hi[3] = { -FLT_MAX, -FLT_MAX, -FLT_MAX };
+            if (f < T) {
+                const float4 q0 = s_tri[3 * f], q1 = s_tri[3 * f + 1], q2 = s_tri[3 * f + 2];
+                const float v[3][3] = { { q0.x, q0.x + q1.x, q0.x + q2.x }, { q0.y, q0.y + q1.y, q0.y + q2.y }, { q0.z, q0.z + q1.z, q0.z + q2.z } };
+#pragma unroll
+                for (int x = 0; x < 3; ++x) { lo[x] = fminf(v[x][0], fminf(v[x][1], v[x][2])); hi[x] = fmaxf(v[x][0], fmaxf(v[x][1], v[x][2])); }
+            }
+#pragma unroll
+            for (int x = 0; x < 3; ++x)
+                for (int off = 16; off > 0; off >>= 1) {
+                    lo[x] = fminf(lo[x], __shfl_xor_sync(FULL, lo[x], off)); hi[x] = fmaxf(hi[x], __shfl_xor_sync(FULL, hi[x], off));
+                }
+            if (lane == 0) {
+                // widened by the rounding of the vertex sums (the test works on v0, e1, e2)
+                const float m = 1.0e-6f * (fabsf(lo[0]) + fabsf(hi[0]) + fabsf(lo[1]) + fabsf(hi[1]) + fabsf(lo[2]) + fabsf(hi[2]));
+                s_cl[2 * c] = make_float4(lo[0] - m, lo[1] - m, lo[2] - m, 0.f);
+                s_cl[2 * c + 1] = make_float4(hi[0] + m, hi[1] + m, hi[2] + m, 0.f);
+            }
+        }
+        __syncthreads();
         float3 acc = f3(0, 0, 0), acc_t = f3(0, 0, 0);
         if (em.Ae > 0.0f) {                           // else: edge-on flat design, F = 0, nothing launched
             RayGen g;
@@ -100,6 +217,52 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
             g.inv_ny = 1.0f / (float)(1u << (a.log2N >> 1));
             const uint32_t end = (uint32_t)a.N;
             const float3 sdir = f3(0.f, 0.f, 1.f);    // the photons' travel direction in the emitter frame
+            const bool raster = raster_n != 0u && T >= RASTER_MIN_TRIS;          // block-uniform
+            if (raster) {
+                for (uint32_t i = threadIdx.x; i < end; i += SAMPLE_THREADS) {   // O-step 3 for every ray of the record
+                    uint32_t r0, r1, r2, r3;
+                    philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
+                    const float fu = ((float)compact_even_bits(i) + uniform23(r0)) * g.inv_nx;
+                    const float fv = ((float)compact_even_bits(i >> 1) + uniform23(r1)) * g.inv_ny;
+                    s_puv[i] = make_float2(fmaf(fu, em.du, em.u0), fmaf(fv, em.dv, em.v0));
+                    s_key[i] = ~0ULL;
+                }
+                if (threadIdx.x == 0) s_nbig = 0;
+                __syncthreads();
+                const int nx = 1 << ((a.log2N + 1) >> 1), ny = 1 << (a.log2N >> 1);
+                const float sx = (float)nx / em.du, sy = (float)ny / em.dv;
+                const float marg = 1.0e-5f * (fabsf(em.u0) + fabsf(em.v0) + em.du + em.dv);
+                for (int f = threadIdx.x; f < T; f += SAMPLE_THREADS) {
+                    const float4 q0 = s_tri[3 * f], q1 = s_tri[3 * f + 1], q2 = s_tri[3 * f + 2];
+                    int cx0, cx1, cy0, cy1;
+                    if (!raster_cells(q0, q1, q2, em, sx, sy, marg, nx, ny, cx0, cx1, cy0, cy1)) continue;
+                    if ((cx1 - cx0 + 1) * (cy1 - cy0 + 1) > RASTER_BIG) {
+                        const int slot = atomicAdd(&s_nbig, 1);
+                        if (slot < RASTER_BIGCAP) { s_big[slot] = f; continue; }
+                    }
+                    for (int cy = cy0; cy <= cy1; ++cy)
+                        for (int cx = cx0; cx <= cx1; ++cx) {
+                            const uint32_t i = spread_even_bits((uint32_t)cx) | (spread_even_bits((uint32_t)cy) << 1);
+                            raster_test(q0, q1, q2, f, s_puv[i], em.worg, s_key + i);
+                            ++n_2d64;
+                        }
+                }
+                __syncthreads();
+                const int nbig = s_nbig < RASTER_BIGCAP ? s_nbig : RASTER_BIGCAP;
+                for (int b = warp; b < nbig; b += SAMPLE_WARPS) {
+                    const int f = s_big[b];
+                    const float4 q0 = s_tri[3 * f], q1 = s_tri[3 * f + 1], q2 = s_tri[3 * f + 2];
+                    int cx0 = 0, cx1 = -1, cy0 = 0, cy1 = -1;
+                    raster_cells(q0, q1, q2, em, sx, sy, marg, nx, ny, cx0, cx1, cy0, cy1);
+                    const int w = cx1 - cx0 + 1, n = w * (cy1 - cy0 + 1);
+                    for (int x = lane; x < n; x += 32) {
+                        const uint32_t i = spread_even_bits((uint32_t)(cx0 + x % w)) | (spread_even_bits((uint32_t)(cy0 + x / w)) << 1);
+                        raster_test(q0, q1, q2, f, s_puv[i], em.worg, s_key + i);
+                        ++n_2d64;
+                    }
+                }
+                __syncthreads();
+            }
             bool more = true;                         // the record still has rays nobody has taken
             int qcount = 0;                           // warp-uniform
             for (;;) {
@@ -122,7 +285,7 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
                     }
                     qcount -= take;
                     __syncwarp();
-                    closest_shared(s_tri, alive ? T : 0, o, d, src, share, lane % share, tbest, best, cn.n_tri);   // all lanes: it shuffles
+                    closest_shared(s_tri, s_cl, T, alive, o, d, src, share, lane % share, tbest, best, cn.n_tri, n_cl);   // all lanes: it shuffles
                     alive = alive && (lane % share) == 0;                 // one lane per ray goes on to shade
                     if (alive) cn.segments++;
                 } else if (more) {                                        // a pass of primaries (O-step 3 in the emitter frame)
@@ -130,8 +293,16 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
                     if (lane == 0) next = atomicAdd(&s_next, 32u);
                     next = __shfl_sync(FULL, next, 0);
                     more = next + 32u < end;
-                    i = next + (uint32_t)lane;
-                    if (i < end) {
+                    // rasterised: a warp's 32 rays are spread over the grid, so that the warps share the hits evenly
+                    i = raster ? (uint32_t)lane * (end >> 5) + (next >> 5) : next + (uint32_t)lane;
+                    if (raster && next < end) {
+                        const float2 p = s_puv[i];
+                        const unsigned long long key = s_key[i];
+                        o = f3(p.x, p.y, em.worg);
+                        alive = true;
+                        cn.launched++; cn.segments++;
+                        if (key != ~0ULL) { tbest = __uint_as_float((uint32_t)(key >> 32)); best = (int)(uint32_t)key; }
+                    } else if (!raster && i < end) {
                         uint32_t r0, r1, r2, r3;
                         philox4(i, g.j, g.k, 0u, g.key0, g.key1, r0, r1, r2, r3);
                         float fu, fv;
@@ -170,7 +341,7 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
                 __syncwarp();
             }
         }
-        n_tri64 += cn.n_tri; cn.n_tri = 0; n_2d64 += cn.n_box; cn.n_box = 0;
+        n_tri64 += cn.n_tri; cn.n_tri = 0; n_2d64 += cn.n_box; cn.n_box = 0; n_cl64 += n_cl; n_cl = 0;
         // S7: lane fp32 sums -> fp64 warp shuffle tree -> the block's warps in index order -> back to the body frame
         double s[3] = { acc.x, acc.y, acc.z };
 #pragma unroll
@@ -196,8 +367,10 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
         n_tri64 += __shfl_xor_sync(FULL, n_tri64, off); n2d += __shfl_xor_sync(FULL, n2d, off);
+        n_cl64 += __shfl_xor_sync(FULL, n_cl64, off);
     }
     if (lane == 0) {
+        atomicAdd((unsigned long long *)&a.stats->box_tests, n_cl64);
         atomicAdd((unsigned long long *)&a.stats->tri_tests, n_tri64);
         atomicAdd((unsigned long long *)&a.stats->tri2d_tests, n2d);
     }
@@ -209,13 +382,18 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
 // records the kernel can take: the triangles of one record must fit the block's shared memory
 long long srp_sample_max_tris()
 {
-    return (200 * 1024) / 48;
+    return (190 * 1024) / 49;                    // 48 bytes per triangle and 32 per cluster of 32, beside 36 KB of queues
 }
 
 // a.n_pairs records; record m = design m of a.dz (no hierarchy) lit from a.sun_dirs[m]; out DEVICE float[n_pairs,3].
 cudaError_t srp_launch_sample(const TraceArgs &a, float *out, unsigned k_offset, int num_sms, cudaStream_t stream)
 {
-    const size_t smem = (size_t)a.max_tris * 48;
+    size_t smem = (size_t)a.max_tris * 48 + 32 * (size_t)((a.max_tris + SAMPLE_CLUSTER - 1) / SAMPLE_CLUSTER);
+    uint32_t raster_n = 0;                       // rasterised primaries: stratified sampler, a grid of 32 .. 2048 cells that fits
+    if (a.sampler == 0 && a.N >= 32 && a.N <= RASTER_MAX_RAYS && a.max_tris >= RASTER_MIN_TRIS && smem + 16 * (size_t)a.N <= 190 * 1024) {
+        raster_n = (uint32_t)a.N;
+        smem += 16 * (size_t)a.N;
+    }
     auto kernel = a.deposit ? sample_design_kernel<true> : sample_design_kernel<false>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -225,6 +403,6 @@ cudaError_t srp_launch_sample(const TraceArgs &a, float *out, unsigned k_offset,
     if (per_sm < 1) per_sm = 1;
     long long blocks = (long long)num_sms * per_sm;
     if (blocks > a.n_pairs) blocks = a.n_pairs;
-    kernel<<<(unsigned)blocks, SAMPLE_THREADS, smem, stream>>>(a, out, k_offset);
+    kernel<<<(unsigned)blocks, SAMPLE_THREADS, smem, stream>>>(a, out, k_offset, raster_n);
     return cudaGetLastError();
 }
