@@ -20,7 +20,7 @@ constexpr int SAMPLE_WARPS = SAMPLE_THREADS / 32;
 // are found triangle by triangle: a triangle is tested against the rays of the cells its bounding rectangle touches
 // (a few) instead of every ray against every triangle -- the same test on the same operands, ~100 x fewer of them.
 constexpr int SAMPLE_CLUSTER = 32;                    // triangles per cluster box (bounce rays)
-constexpr int RASTER_MIN_TRIS = 256;                  // below: testing all triangles costs nothing
+constexpr int RASTER_MIN_TRIS = 1;                    // (a threshold below which all triangles would be tested per ray: none)
 constexpr int RASTER_MAX_RAYS = 2048;                 // 16 bytes of shared memory per ray
 constexpr int RASTER_BIG = 32, RASTER_BIGCAP = 128;   // a triangle over more cells goes to a warp (the first 128 of them)
 
@@ -138,12 +138,11 @@ __device__ __forceinline__ void closest_shared(const float4 *__restrict__ tp, co
                 tri_test(tp[3 * f], tp[3 * f + 1], tp[3 * f + 2], ro, rd, f, tt, bb);
                 ++n_tri;
             }
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-                const float t2 = __shfl_xor_sync(FULL, tt, off);
-                const int b2 = __shfl_xor_sync(FULL, bb, off);
-                if (b2 >= 0 && (bb < 0 || t2 < tt || (t2 == tt && b2 < bb))) { tt = t2; bb = b2; }
-            }
+            // closest of the 32: t > 0, so its bits order like the value; among equal t the lowest lane has the smallest index
+            const unsigned tmin = __reduce_min_sync(FULL, __float_as_uint(tt));
+            const unsigned who = __ballot_sync(FULL, bb >= 0 && __float_as_uint(tt) == tmin);
+            tt = __uint_as_float(tmin);
+            bb = who != 0u ? f - lane + (__ffs(who) - 1) : -1;
             // every lane of the ray's group keeps the result, so that its later boxes are tested against it
             if (lane / g == L / g && bb >= 0 && (best < 0 || tt < tbest || (tt == tbest && bb < best))) { tbest = tt; best = bb; }
         }

@@ -892,8 +892,11 @@ def test_cfg5_sail_N14_same_stream_parity(ctx, oracle):
 
 # ---------------------------------------------------------------- per-sample designs (NEXT-3)
 @pytest.mark.parametrize("family,M,N,B,sampler,deposit", [
-    (W.FAMILY_BOXWING, 40, 1 << 10, 4, 0, 0),        # 16 triangles per record
-    (W.FAMILY_BOXWING_T, 24, 1 << 10, 4, 0, 0),      # 1280 triangles: the paper's "1 k faces"
+    (W.FAMILY_BOXWING, 40, 1 << 10, 4, 0, 0),        # 16 triangles per record, each over hundreds of grid cells (rasterised by a warp)
+    (W.FAMILY_BOXWING_T, 24, 1 << 10, 4, 0, 0),      # 1280 triangles: the paper's "1 k faces" (rasterised by a thread each)
+    (W.FAMILY_BOXWING_T, 6, 1 << 11, 4, 0, 0),       # a 64 x 32 grid
+    (W.FAMILY_BOXWING_T, 4, 1 << 12, 3, 0, 0),       # more rays than the rasteriser takes: every primary against every triangle
+    (W.FAMILY_PLATE, 16, 1 << 7, 2, 0, 0),           # 2 triangles, 16 x 8 cells
     (W.FAMILY_BOXWING_T, 8, 1000, 3, 1, 1),          # i.i.d. sampler (N need not be a power of two), analog deposit
 ])
 def test_per_sample_designs_match_oracle(ctx, oracle, family, M, N, B, sampler, deposit):
