@@ -237,11 +237,12 @@ srp_status srp_forces_host(srp_context *ctx, const srp_designs *designs, const f
 
 /* The paper's own workload shape: a batch of M records, each with
  * its OWN design theta_m and its OWN light direction omega_m -- "every ray effectively intersects a different world"
- * -- and only rays_per_record photons, so no hierarchy is built: as in the paper, every ray is tested against all
- * triangles of its record's mesh.  theta DEVICE float[M, n_params], sun_dirs DEVICE float[M,3] (body->sun),
+ * -- and only rays_per_record photons, so no hierarchy is built: the closest hit is that of the paper's test of every
+ * ray against all triangles of its record's mesh (found with fewer tests: primaries rasterised into the emitter grid,
+ * bounce rays through boxes around clusters of 32 triangles).  theta DEVICE float[M, n_params], sun_dirs DEVICE float[M,3] (body->sun),
  * out_forces DEVICE float[M,3] newtons.  Record m is design m with direction m: its mesh, materials and photons are
  * those of srp_build_designs + srp_forces_pairs with the pair (m, m), except that the direction index in the Philox
- * counter is 0 (counter (ray, 0, m, depth)); M is not limited to 65535.  The family's meshes must have at most 4266
+ * counter is 0 (counter (ray, 0, m, depth)); M is not limited to 65535.  The family's meshes must have at most 3970
  * triangles (one record's triangles live in a thread block's shared memory); srp_options.sampler and .deposit
  * apply; torque, glossy lobes and escape masks do not.  The meshes are generated chunk by chunk on the way and not
  * kept.  srp_get_stats covers the whole batch.  Enqueues only. */
