@@ -77,7 +77,8 @@ def ncu_figures(workload):
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="timed steps; default 3, 20 for the short steps of paper_map (so that the clocks are sampled under load)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_detailed", choices=sorted(W.CONFIGS) + sorted(W.SAMPLE_CONFIGS))
@@ -85,7 +86,10 @@ def parse():
                     help="beam / bounce loop as plain launches (for ncu); a little slower, same results")
     ap.add_argument("--scale", type=float, default=1.0,
                     help="fraction of the workload's sun directions (debug; < 1 marks the line invalid)")
-    return ap.parse_args()
+    args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 20 if args.workload in W.SAMPLE_CONFIGS else 3
+    return args
 
 
 class ClockSampler:
