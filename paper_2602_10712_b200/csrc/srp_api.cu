@@ -734,7 +734,7 @@ srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const floa
     srp_status st = ensure_workspace(ctx, 3);
     if (st != SRP_OK) return st;
     TRY_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), ctx->stream), "zero stats");
-    // chunks of records: meshes for a chunk (S0), its boxes and packed triangles (S1 without a hierarchy), its photons
+    // chunks of records: meshes for a chunk (S0), then its photons (the kernel boxes and packs each record on the way in)
     long long chunk = (1LL << 30) / (96 * T);                       // ~1 GiB of mesh per chunk: many waves of blocks per launch
     if (chunk > 32768) chunk = 32768;
     if (chunk > M) chunk = M;
@@ -750,10 +750,8 @@ srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const floa
         d.D = Dc; d.sumT = (long long)Dc * T;
         e = srp_launch_mesh_gen((int)family, theta + (size_t)m0 * n_params, Dc, n_params, mesh_seed, T, d.verts_orig,
                                 d.mats_orig, ctx->mempool, (unsigned)m0, ctx->stream);
-        int build_launches = 0;
-        if (e == cudaSuccess) e = srp_launch_build(&d, 0, 0, ctx->mempool, ctx->stream, &build_launches);
         if (e != cudaSuccess) break;
-        TraceArgs a;
+        TraceArgs a;                                                // the sample kernel boxes and packs a record itself (S1 without a hierarchy)
         memset(&a, 0, sizeof a);
         a.dz = d.dev();
         a.sun_dirs = sun_dirs + 3 * m0; a.n_pairs = Dc; a.S = Dc; a.N = N; a.B = B;
@@ -761,8 +759,8 @@ srp_status srp_forces_per_sample(srp_context *ctx, srp_family family, const floa
         a.key0 = (uint32_t)seed; a.key1 = (uint32_t)(seed >> 32);
         a.sampler = ctx->opt.sampler; a.deposit = ctx->opt.deposit; a.P = ctx->opt.solar_pressure;
         a.stats = ctx->stats; a.max_tris = T; a.acc_scale = 1.0;
-        e = srp_launch_sample(a, out + 3 * m0, (unsigned)m0, ctx->num_sms, ctx->stream);
-        count_launches(ctx, 2 + build_launches + 1);
+        e = srp_launch_sample(a, d.verts_orig, d.mats_orig, out + 3 * m0, (unsigned)m0, ctx->num_sms, ctx->stream);
+        count_launches(ctx, 2 + 1);
     }
     free_designs_mem(ctx, &d);                                      // stream-ordered: after the last chunk's kernels
     if (st != SRP_OK) return st;

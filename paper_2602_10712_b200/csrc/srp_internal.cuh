@@ -151,7 +151,8 @@ cudaError_t srp_launch_first_hits(const TraceArgs &a, int method, int *out_prim,
 cudaError_t srp_launch_thermal(const TraceArgs &a, const float *facet_power, long long sumT, int *emit_list, int *n_emit,
                                float *design_power, float *out_forces, int num_sms, cudaStream_t stream);
 long long srp_sample_max_tris();
-cudaError_t srp_launch_sample(const TraceArgs &a, float *out, unsigned k_offset, int num_sms, cudaStream_t stream);
+cudaError_t srp_launch_sample(const TraceArgs &a, const float *verts, const float *mats, float *out, unsigned k_offset, int num_sms,
+                              cudaStream_t stream);
 cudaError_t srp_run_probes(int num_sms, cudaStream_t stream, double *fp32_tflops, double *l2_gbs);
 
 long long srp_family_tris_host(int family);

@@ -21,7 +21,7 @@ constexpr int SAMPLE_WARPS = SAMPLE_THREADS / 32;
 // (a few) instead of every ray against every triangle -- the same test on the same operands, ~100 x fewer of them.
 constexpr int SAMPLE_CLUSTER = 32;                    // triangles per cluster box (bounce rays)
 constexpr int RASTER_MIN_TRIS = 1;                    // (a threshold below which all triangles would be tested per ray: none)
-constexpr int RASTER_MAX_RAYS = 2048;                 // 16 bytes of shared memory per ray
+constexpr int RASTER_MAX_RAYS = 8192;                 // 16 bytes of shared memory per ray, if they fit beside the triangles
 constexpr int RASTER_BIG = 32, RASTER_BIGCAP = 128;   // a triangle over more cells goes to a warp (the first 128 of them)
 
 // O-step 4 for a primary in the emitter frame: origin (pu, pv, worg), direction (0, 0, 1), all triangles.
@@ -151,7 +151,8 @@ __device__ __forceinline__ void closest_shared(const float4 *__restrict__ tp, co
 
 template <bool ANALOG>
 __global__ void __launch_bounds__(SAMPLE_THREADS, 2)
-sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t k_offset, const uint32_t raster_n)
+sample_design_kernel(const TraceArgs a, const float *__restrict__ verts, const float *__restrict__ mats, float *__restrict__ out,
+                     const uint32_t k_offset, const uint32_t raster_n)
 {
     extern __shared__ float4 s_tri[];                 // 3 x float4 per triangle of the record being traced
     // rasterised primaries (raster_n = N, else 0): per cell of the emitter grid the ray's position and its closest hit
@@ -176,11 +177,37 @@ sample_design_kernel(const TraceArgs a, float *__restrict__ out, const uint32_t 
     for (long long m = blockIdx.x; m < a.n_pairs; m += gridDim.x) {
         const long long tbase = a.dz.tri_off[m];
         const int T = (int)(a.dz.tri_off[m + 1] - tbase);
-        const Emitter em = make_emitter(a.sun_dirs, (int)m, a.dz.box[2 * m], a.dz.box[2 * m + 1]);
         __syncthreads();                              // the previous record's photons are done with s_tri / s_part
         if (threadIdx.x == 0) s_next = 0u;
+        // S1 for a record without a hierarchy, on the way into shared memory: the generator's vertices (verts: 9 floats per
+        // triangle, mats: 3) become (v0, alpha) (e1, rho_s) (e2, rho_d), and the block finds the design's box
+        float blo[3] = { FLT_MAX, FLT_MAX, FLT_MAX }, bhi[3] = { -FLT_MAX, -FLT_MAX, -FLT_MAX };
+        for (int f = threadIdx.x; f < T; f += SAMPLE_THREADS) {
+            const float *v = verts + 9 * (tbase + f), *mt = mats + 3 * (tbase + f);
+            float p[9];
+#pragma unroll
+            for (int x = 0; x < 9; ++x) p[x] = __ldg(v + x);
+            s_tri[3 * f] = make_float4(p[0], p[1], p[2], __ldg(mt));
+            s_tri[3 * f + 1] = make_float4(p[3] - p[0], p[4] - p[1], p[5] - p[2], __ldg(mt + 1));
+            s_tri[3 * f + 2] = make_float4(p[6] - p[0], p[7] - p[1], p[8] - p[2], __ldg(mt + 2));
+#pragma unroll
+            for (int x = 0; x < 9; ++x) { blo[x % 3] = fminf(blo[x % 3], p[x]); bhi[x % 3] = fmaxf(bhi[x % 3], p[x]); }
+        }
+        float *s_box = reinterpret_cast<float *>(&s_part[0][0]);          // [warp][6]: free until the record's reduction
+#pragma unroll
+        for (int x = 0; x < 3; ++x) {
+            for (int off = 16; off > 0; off >>= 1) {
+                blo[x] = fminf(blo[x], __shfl_xor_sync(FULL, blo[x], off)); bhi[x] = fmaxf(bhi[x], __shfl_xor_sync(FULL, bhi[x], off));
+            }
+            if (lane == 0) { s_box[6 * warp + x] = blo[x]; s_box[6 * warp + 3 + x] = bhi[x]; }
+        }
+        __syncthreads();
+        for (int w = 0; w < SAMPLE_WARPS; ++w)
+#pragma unroll
+            for (int x = 0; x < 3; ++x) { blo[x] = fminf(blo[x], s_box[6 * w + x]); bhi[x] = fmaxf(bhi[x], s_box[6 * w + 3 + x]); }
+        const Emitter em = make_emitter(a.sun_dirs, (int)m, make_float4(blo[0], blo[1], blo[2], 0.f), make_float4(bhi[0], bhi[1], bhi[2], 0.f));
         for (int x = threadIdx.x; x < 3 * T; x += SAMPLE_THREADS) {      // into the emitter frame; materials ride along
-            const float4 q = __ldg(a.dz.tri + 3 * tbase + x);
+            const float4 q = s_tri[x];
             const float3 p = f3(q.x, q.y, q.z);
             s_tri[x] = make_float4(dot3(p, em.u), dot3(p, em.v), dot3(p, em.s), q.w);
         }
@@ -384,8 +411,10 @@ long long srp_sample_max_tris()
     return (190 * 1024) / 49;                    // 48 bytes per triangle and 32 per cluster of 32, beside 36 KB of queues
 }
 
-// a.n_pairs records; record m = design m of a.dz (no hierarchy) lit from a.sun_dirs[m]; out DEVICE float[n_pairs,3].
-cudaError_t srp_launch_sample(const TraceArgs &a, float *out, unsigned k_offset, int num_sms, cudaStream_t stream)
+// a.n_pairs records; record m = the triangles [a.dz.tri_off[m], a.dz.tri_off[m + 1]) of verts / mats (the mesh generator's
+// output: no box, no packing, no hierarchy) lit from a.sun_dirs[m]; out DEVICE float[n_pairs,3].
+cudaError_t srp_launch_sample(const TraceArgs &a, const float *verts, const float *mats, float *out, unsigned k_offset, int num_sms,
+                              cudaStream_t stream)
 {
     size_t smem = (size_t)a.max_tris * 48 + 32 * (size_t)((a.max_tris + SAMPLE_CLUSTER - 1) / SAMPLE_CLUSTER);
     uint32_t raster_n = 0;                       // rasterised primaries: stratified sampler, a grid of 32 .. 2048 cells that fits
@@ -402,6 +431,6 @@ cudaError_t srp_launch_sample(const TraceArgs &a, float *out, unsigned k_offset,
     if (per_sm < 1) per_sm = 1;
     long long blocks = (long long)num_sms * per_sm;
     if (blocks > a.n_pairs) blocks = a.n_pairs;
-    kernel<<<(unsigned)blocks, SAMPLE_THREADS, smem, stream>>>(a, out, k_offset, raster_n);
+    kernel<<<(unsigned)blocks, SAMPLE_THREADS, smem, stream>>>(a, verts, mats, out, k_offset, raster_n);
     return cudaGetLastError();
 }

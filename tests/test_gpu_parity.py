@@ -895,7 +895,8 @@ def test_cfg5_sail_N14_same_stream_parity(ctx, oracle):
     (W.FAMILY_BOXWING, 40, 1 << 10, 4, 0, 0),        # 16 triangles per record, each over hundreds of grid cells (rasterised by a warp)
     (W.FAMILY_BOXWING_T, 24, 1 << 10, 4, 0, 0),      # 1280 triangles: the paper's "1 k faces" (rasterised by a thread each)
     (W.FAMILY_BOXWING_T, 6, 1 << 11, 4, 0, 0),       # a 64 x 32 grid
-    (W.FAMILY_BOXWING_T, 4, 1 << 12, 3, 0, 0),       # more rays than the rasteriser takes: every primary against every triangle
+    (W.FAMILY_BOXWING_T, 4, 1 << 12, 3, 0, 0),       # 64 KB of grid beside the triangles: one block per SM
+    (W.FAMILY_BOXWING_T, 2, 1 << 13, 2, 0, 0),       # a grid that does not fit: every primary against every triangle
     (W.FAMILY_PLATE, 16, 1 << 7, 2, 0, 0),           # 2 triangles, 16 x 8 cells
     (W.FAMILY_BOXWING_T, 8, 1000, 3, 1, 1),          # i.i.d. sampler (N need not be a power of two), analog deposit
 ])
